@@ -1,0 +1,171 @@
+"""ctypes wrapper of oracle/tpcca_oracle.cpp (argument marshalling only)."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "tpcca_oracle.cpp")
+
+# DESIGN.md Table A defaults (the oracle keeps its own copy; the product's live in binding.py)
+DEFAULT_PARAMS = dict(
+    sigma_y=0.1, sigma_z=0.15,
+    nbr_dydx=1.5, nbr_dzdx=1.5, nbr_margin_y=0.5, nbr_margin_z=0.75, triplet_cut=18.0,
+    cov0=(1.0, 1.0, 0.25, 1.0, 100.0),
+    pick_cut=16.0, reject_cut=25.0, max_gap=5, edge_margin=3.0, max_sinphi=0.95,
+    min_seed_hits=4, min_tracklet_hits=10, min_track_hits=10, qual_scale=1000.0,
+    tan_half_angle=float(np.tan(np.deg2rad(10.0))),
+)
+
+
+class _Params(C.Structure):
+    _fields_ = [
+        ("sigma_y", C.c_float), ("sigma_z", C.c_float),
+        ("nbr_dydx", C.c_float), ("nbr_dzdx", C.c_float), ("nbr_margin_y", C.c_float), ("nbr_margin_z", C.c_float),
+        ("triplet_cut", C.c_float), ("cov0", C.c_float * 5),
+        ("pick_cut", C.c_float), ("reject_cut", C.c_float), ("max_gap", C.c_int32),
+        ("edge_margin", C.c_float), ("max_sinphi", C.c_float),
+        ("min_seed_hits", C.c_int32), ("min_tracklet_hits", C.c_int32), ("min_track_hits", C.c_int32),
+        ("qual_scale", C.c_float), ("tan_half_angle", C.c_float),
+    ]
+
+
+TRACK_DTYPE = np.dtype([
+    ("sector", "<i4"), ("first_row", "<i4"), ("last_row", "<i4"), ("n_hits", "<i4"),
+    ("x", "<f4"), ("y", "<f4"), ("z", "<f4"), ("sinphi", "<f4"), ("dzds", "<f4"), ("qpt", "<f4"),
+    ("cov", "<f4", (15,)), ("chi2", "<f4"), ("ndf", "<i4"), ("pad", "<i4", (5,)),
+])
+assert TRACK_DTYPE.itemsize == 128
+
+
+def build(opt: str = "-O2", force: bool = False) -> str:
+    so = os.path.join(_HERE, f"libtpcca_oracle{opt.replace('-', '_')}.so")
+    if force or not os.path.exists(so) or os.path.getmtime(so) < os.path.getmtime(_SRC):
+        subprocess.check_call(["g++", opt, "-std=c++17", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC",
+                               "-o", so, _SRC])
+    return so
+
+
+_libs: dict = {}
+
+
+def _load(opt: str = "-O2"):
+    if opt not in _libs:
+        lib = C.CDLL(build(opt))
+        lib.orc_track.restype = C.c_void_p
+        lib.orc_track.argtypes = [C.c_int32, C.c_int32, C.c_void_p, C.c_float, C.POINTER(_Params), C.c_void_p,
+                                  C.c_int64, C.c_void_p, C.c_int32]
+        lib.orc_free.argtypes = [C.c_void_p]
+        for name in ("orc_n_start", "orc_n_tracks"):
+            getattr(lib, name).restype = C.c_int64
+            getattr(lib, name).argtypes = [C.c_void_p]
+        for name in ("orc_link_up_raw", "orc_link_down_raw", "orc_link_up", "orc_link_down", "orc_start_hits",
+                     "orc_row_hit", "orc_assignment", "orc_tracks", "orc_track_tracklet"):
+            getattr(lib, name).restype = C.c_void_p
+            getattr(lib, name).argtypes = [C.c_void_p]
+        lib.orc_tracklets.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.orc_kf_transport.restype = C.c_int32
+        lib.orc_kf_transport.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_float]
+        lib.orc_kf_update.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_float]
+        lib.orc_refit_hits.restype = C.c_int32
+        lib.orc_refit_hits.argtypes = [C.c_int32, C.c_void_p, C.c_float, C.c_float, C.POINTER(_Params), C.c_void_p]
+        _libs[opt] = lib
+    return _libs[opt]
+
+
+def _params(p: dict | None) -> _Params:
+    d = dict(DEFAULT_PARAMS)
+    if p:
+        d.update(p)
+    cp = _Params()
+    for k, v in d.items():
+        if k == "cov0":
+            cp.cov0 = (C.c_float * 5)(*v)
+        else:
+            setattr(cp, k, v)
+    return cp
+
+
+@dataclass
+class OracleResult:
+    link_up_raw: np.ndarray
+    link_down_raw: np.ndarray
+    link_up: np.ndarray
+    link_down: np.ndarray
+    start_hits: np.ndarray
+    row_hit: np.ndarray          # (n_tracklets, n_rows) input indices or -1
+    tracklet_ints: np.ndarray    # (n_tracklets, 4): valid, first_row, last_row, n_hits
+    tracklet_floats: np.ndarray  # (n_tracklets, 23): x, p5, C15, chi2, z_ref
+    assignment: np.ndarray
+    tracks: np.ndarray           # TRACK_DTYPE
+    track_tracklet: np.ndarray
+
+
+def _arr(ptr, n, dtype):
+    if n == 0 or not ptr:
+        return np.zeros(0, dtype=dtype)
+    buf = (C.c_char * (n * np.dtype(dtype).itemsize)).from_address(ptr)
+    return np.frombuffer(buf, dtype=dtype).copy()
+
+
+def track(clusters: np.ndarray, sector_offsets: np.ndarray, row_x: np.ndarray, bz: float = 0.5,
+          params: dict | None = None, brute: bool = False, opt: str = "-O2") -> OracleResult:
+    """Steps O1-O7 on one frame.  `clusters`: structured (x,y,z f32,row i32); returns input-index-space results."""
+    lib = _load(opt)
+    cl = np.ascontiguousarray(clusters)
+    assert cl.dtype.itemsize == 16
+    so = np.ascontiguousarray(sector_offsets, dtype=np.int32)
+    rx = np.ascontiguousarray(row_x, dtype=np.float32)
+    n, ns, nr = cl.shape[0], so.shape[0] - 1, rx.shape[0]
+    cp = _params(params)
+    h = lib.orc_track(ns, nr, rx.ctypes.data, bz, C.byref(cp), cl.ctypes.data, n, so.ctypes.data, int(brute))
+    try:
+        nt, ntr = lib.orc_n_start(h), lib.orc_n_tracks(h)
+        ti = np.zeros((nt, 4), np.int32)
+        tf = np.zeros((nt, 23), np.float32)
+        if nt:
+            lib.orc_tracklets(h, ti.ctypes.data, tf.ctypes.data)
+        return OracleResult(
+            _arr(lib.orc_link_up_raw(h), n, np.int32), _arr(lib.orc_link_down_raw(h), n, np.int32),
+            _arr(lib.orc_link_up(h), n, np.int32), _arr(lib.orc_link_down(h), n, np.int32),
+            _arr(lib.orc_start_hits(h), nt, np.int32),
+            _arr(lib.orc_row_hit(h), nt * nr, np.int32).reshape(nt, nr),
+            ti, tf,
+            _arr(lib.orc_assignment(h), n, np.int32),
+            _arr(lib.orc_tracks(h), ntr, TRACK_DTYPE), _arr(lib.orc_track_tracklet(h), ntr, np.int32))
+    finally:
+        lib.orc_free(h)
+
+
+def kf_transport(x, p5, cov15, xnew, bz=0.5, max_sinphi=0.95, opt="-O2"):
+    lib = _load(opt)
+    xx = np.array([x], np.float32)
+    p = np.array(p5, np.float32)
+    c = np.array(cov15, np.float32)
+    ok = lib.orc_kf_transport(xx.ctypes.data, p.ctypes.data, c.ctypes.data, xnew, bz, max_sinphi)
+    return bool(ok), float(xx[0]), p, c
+
+
+def kf_update(p5, cov15, chi2, ym, zm, sy2, sz2, opt="-O2"):
+    lib = _load(opt)
+    p = np.array(p5, np.float32)
+    c = np.array(cov15, np.float32)
+    ch = np.array([chi2], np.float32)
+    lib.orc_kf_update(p.ctypes.data, c.ctypes.data, ch.ctypes.data, ym, zm, sy2, sz2)
+    return p, c, float(ch[0])
+
+
+def refit_hits(x, y, z, q0=0.0, bz=0.5, params=None, opt="-O2"):
+    """O7 three-pass refit of a free-standing hit list (increasing x).  Returns (ok, out22)."""
+    lib = _load(opt)
+    n = len(x)
+    cl = np.zeros(n, dtype=[("x", "<f4"), ("y", "<f4"), ("z", "<f4"), ("row", "<i4")])
+    cl["x"], cl["y"], cl["z"] = x, y, z
+    out = np.zeros(22, np.float32)
+    cp = _params(params)
+    ok = lib.orc_refit_hits(n, cl.ctypes.data, q0, bz, C.byref(cp), out.ctypes.data)
+    return bool(ok), out

@@ -1,0 +1,565 @@
+// tpcca_oracle.cpp -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+//
+// Plain, single-threaded CPU oracle for the per-sector cellular-automaton track finder and
+// Kalman fit of arXiv 1811.11481 (PAPER.md:49-51 phase 1; :65-68 outward then inward through
+// the seed with outlier rejection; :71 three-pass refit; :98/:104 no vertex constraint, window
+// centred on the hit; :121 fp32, z kept relative).  It follows the algorithm step by step in
+// the order of DESIGN.md section "Arithmetic" (steps O1-O7) and shares no code with the CUDA path.
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+// load it.  Build: g++ -O2 -ffp-contract=off (no fast-math): every decision is fp32, no FMA.
+//
+// Pins (tests/test_oracle_pins.py): brute-force all-triplet search (P1), noiseless helix (P2),
+// mutual links (P3), exclusive assignment (P4), permutation invariance (P5), transport closed
+// form (P6), straight-line least squares (P7), pulls (P8), -O0 == -O2 (P10).
+// Parity unpinned: the numeric defaults of DESIGN.md Table A (cuts, windows, cov0) -- the paper
+// prints no value for them.
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+namespace {
+
+struct Params {  // mirrors DESIGN.md Table A; filled field by field from Python
+  float sigma_y, sigma_z;
+  float nbr_dydx, nbr_dzdx, nbr_margin_y, nbr_margin_z, triplet_cut;
+  float cov0[5];
+  float pick_cut, reject_cut;
+  int32_t max_gap;
+  float edge_margin, max_sinphi;
+  int32_t min_seed_hits, min_tracklet_hits, min_track_hits;
+  float qual_scale;
+  float tan_half_angle;
+};
+
+struct Cl { float x, y, z; int32_t row; };
+
+struct TrackRec {  // 128 bytes, same field order as the product's record (declared independently)
+  int32_t sector, first_row, last_row, n_hits;
+  float x, y, z, sinphi, dzds, qpt;
+  float cov[15];
+  float chi2;
+  int32_t ndf;
+  int32_t pad[5];
+};
+
+struct KF {
+  float x;
+  float p[5];   // y, z~ (relative to z_ref), sin(phi), dz/ds, q/pT
+  float C[15];  // lower triangle, row major: C[i*(i+1)/2+j], i>=j
+  float chi2;
+};
+
+inline uint32_t ordf(float f) {  // monotone float -> uint map
+  uint32_t b;
+  std::memcpy(&b, &f, 4);
+  return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+
+// ---- O5 model: transport x -> xnew ----
+bool transport(KF& k, float xnew, float kq, float max_sinphi) {
+  const float dx = xnew - k.x;
+  if (dx == 0.0f) return true;
+  const float s = k.p[2], t = k.p[3], q = k.p[4];
+  const float kk = q * kq;
+  const float s1 = s + dx * kk;
+  if (!(std::fabs(s) <= max_sinphi) || !(std::fabs(s1) <= max_sinphi)) return false;
+  const float c0 = std::sqrt(1.0f - s * s);
+  const float c1 = std::sqrt(1.0f - s1 * s1);
+  const float cc = c0 + c1;
+  const float f = (s + s1) / cc;
+  const float dy = dx * f;
+  float L = std::sqrt(dx * dx + dy * dy);
+  if (dx < 0.0f) L = -L;
+  const float u = (0.5f * kk) * L;
+  const float u2 = u * u;
+  const float g = 1.0f + u2 * (0.16666667f + u2 * 0.075f);  // asin(u)/u series
+  const float dS = L * g;
+  const float fs0 = (1.0f + (f * s) / c0) / cc;
+  const float fs1 = (1.0f + (f * s1) / c1) / cc;
+  const float h = dx * kq;
+  const float fss = fs0 + fs1;
+  const float a02 = dx * fss;
+  const float a04 = (dx * fs1) * h;
+  const float w = (t * g) * ((dx * dy) / L);
+  const float a12 = w * fss;
+  const float a13 = dS;
+  const float a14 = (w * fs1) * h;
+  const float a24 = h;
+  k.p[0] = k.p[0] + dy;
+  k.p[1] = k.p[1] + t * dS;
+  k.p[2] = s1;
+  k.x = xnew;
+  float* C = k.C;
+  const float c00 = C[0], c10 = C[1], c11 = C[2], c20 = C[3], c21 = C[4], c22 = C[5], c30 = C[6], c31 = C[7],
+              c32 = C[8], c33 = C[9], c40 = C[10], c41 = C[11], c42 = C[12], c43 = C[13], c44 = C[14];
+  const float m00 = (c00 + a02 * c20) + a04 * c40;
+  const float m02 = (c20 + a02 * c22) + a04 * c42;
+  const float m04 = (c40 + a02 * c42) + a04 * c44;
+  const float m10 = ((c10 + a12 * c20) + a13 * c30) + a14 * c40;
+  const float m11 = ((c11 + a12 * c21) + a13 * c31) + a14 * c41;
+  const float m12 = ((c21 + a12 * c22) + a13 * c32) + a14 * c42;
+  const float m13 = ((c31 + a12 * c32) + a13 * c33) + a14 * c43;
+  const float m14 = ((c41 + a12 * c42) + a13 * c43) + a14 * c44;
+  const float m20 = c20 + a24 * c40;
+  const float m21 = c21 + a24 * c41;
+  const float m22 = c22 + a24 * c42;
+  const float m23 = c32 + a24 * c43;
+  const float m24 = c42 + a24 * c44;
+  C[0] = (m00 + a02 * m02) + a04 * m04;
+  C[1] = (m10 + a02 * m12) + a04 * m14;
+  C[2] = ((m11 + a12 * m12) + a13 * m13) + a14 * m14;
+  C[3] = (m20 + a02 * m22) + a04 * m24;
+  C[4] = ((m21 + a12 * m22) + a13 * m23) + a14 * m24;
+  C[5] = m22 + a24 * m24;
+  C[6] = (c30 + a02 * c32) + a04 * c43;
+  C[7] = ((c31 + a12 * c32) + a13 * c33) + a14 * c43;
+  C[8] = c32 + a24 * c43;
+  C[9] = c33;
+  C[10] = (c40 + a02 * c42) + a04 * c44;
+  C[11] = ((c41 + a12 * c42) + a13 * c43) + a14 * c44;
+  C[12] = c42 + a24 * c44;
+  C[13] = c43;
+  C[14] = c44;
+  return true;
+}
+
+inline int tri(int i, int j) { return i >= j ? i * (i + 1) / 2 + j : j * (j + 1) / 2 + i; }
+
+// ---- O5 model: scalar measurement update of component i (0: y, 1: z~) ----
+void update1(KF& k, int i, float m, float v) {
+  float ci[5];
+  for (int j = 0; j < 5; j++) ci[j] = k.C[tri(j, i)];
+  const float r = m - k.p[i];
+  const float S = ci[i] + v;
+  const float w = 1.0f / S;
+  float K[5];
+  for (int j = 0; j < 5; j++) K[j] = ci[j] * w;
+  for (int j = 0; j < 5; j++) k.p[j] = k.p[j] + K[j] * r;
+  for (int j = 0; j < 5; j++)
+    for (int l = 0; l <= j; l++) k.C[tri(j, l)] = k.C[tri(j, l)] - K[j] * ci[l];
+  k.chi2 = k.chi2 + (r * r) * w;
+}
+
+void update(KF& k, float ym, float zm_rel, float sy2, float sz2) {
+  update1(k, 0, ym, sy2);
+  update1(k, 1, zm_rel, sz2);
+}
+
+void reset_cov(KF& k, const Params& P) {
+  for (int i = 0; i < 15; i++) k.C[i] = 0.0f;
+  for (int i = 0; i < 5; i++) k.C[tri(i, i)] = P.cov0[i];
+  k.chi2 = 0.0f;
+}
+
+struct Tracklet {
+  int32_t sector, start_hit;  // start_hit: input index
+  int32_t valid, first_row, last_row, n_hits;
+  float x, p[5], C[15], chi2, z_ref;
+  uint64_t W;
+};
+
+struct Result {
+  int64_t n = 0;
+  int32_t n_sectors = 0, n_rows = 0;
+  std::vector<int32_t> link_up_raw, link_down_raw, link_up, link_down;  // input-index space
+  std::vector<int32_t> start_hits;                                       // input indices, canonical order
+  std::vector<Tracklet> tracklets;
+  std::vector<int32_t> row_hit;  // n_tracklets * n_rows, input indices or -1
+  std::vector<int32_t> assignment;
+  std::vector<TrackRec> tracks;
+  std::vector<int32_t> track_tracklet;
+};
+
+struct Sector {
+  const Cl* cl;                              // all clusters (input order)
+  std::vector<std::vector<int32_t>> rows;    // per row: input indices sorted by key (z, y, idx)
+};
+
+struct Ctx {
+  const Cl* cl;
+  const float* row_x;
+  int n_rows;
+  Params P;
+  float kq, sy2, sz2, inv_sy2, inv_sz2;
+  bool brute;
+};
+
+inline bool key_less(const Cl* cl, int32_t a, int32_t b) {  // same-row key: (ord z, ord y, input index)
+  const uint32_t za = ordf(cl[a].z), zb = ordf(cl[b].z);
+  if (za != zb) return za < zb;
+  const uint32_t ya = ordf(cl[a].y), yb = ordf(cl[b].y);
+  if (ya != yb) return ya < yb;
+  return a < b;
+}
+
+// Candidates of a row with z in [zlo, zhi] (a superset is fine; exact predicates are applied by the caller).
+inline void z_range(const Ctx& c, const std::vector<int32_t>& row, double zlo, double zhi, size_t& b, size_t& e) {
+  if (c.brute) { b = 0; e = row.size(); return; }
+  const Cl* cl = c.cl;
+  b = std::lower_bound(row.begin(), row.end(), zlo, [cl](int32_t i, double z) { return (double)cl[i].z < z; }) - row.begin();
+  e = std::upper_bound(row.begin(), row.end(), zhi, [cl](double z, int32_t i) { return z < (double)cl[i].z; }) - row.begin();
+  if (!(zlo <= zhi)) { b = 0; e = 0; }  // NaN window: nothing can pass the exact predicate
+}
+
+// ---- O2 neighbours finder for one sector ----
+void find_neighbours(const Ctx& c, const Sector& S, std::vector<int32_t>& up, std::vector<int32_t>& down) {
+  const int R = c.n_rows;
+  const Cl* cl = c.cl;
+  const Params& P = c.P;
+  std::vector<int32_t> U, D;
+  for (int r = 0; r < R; r++) {
+    int ru = -1, rd = -1;
+    if (r + 1 < R && !S.rows[r + 1].empty()) ru = r + 1;
+    else if (r + 2 < R && !S.rows[r + 2].empty()) ru = r + 2;
+    if (r - 1 >= 0 && !S.rows[r - 1].empty()) rd = r - 1;
+    else if (r - 2 >= 0 && !S.rows[r - 2].empty()) rd = r - 2;
+    if (ru < 0 || rd < 0) continue;  // links stay -1
+    const float dxu = c.row_x[ru] - c.row_x[r];
+    const float dxd = c.row_x[r] - c.row_x[rd];
+    const float t = dxd / (dxu + dxd);
+    const float wyu = dxu * P.nbr_dydx + P.nbr_margin_y;
+    const float wzu = dxu * P.nbr_dzdx + P.nbr_margin_z;
+    const float wyd = dxd * P.nbr_dydx + P.nbr_margin_y;
+    const float wzd = dxd * P.nbr_dzdx + P.nbr_margin_z;
+    for (int32_t h : S.rows[r]) {
+      const float y0 = cl[h].y, z0 = cl[h].z;
+      U.clear(); D.clear();
+      size_t b, e;
+      z_range(c, S.rows[ru], (double)z0 - wzu - 0.01, (double)z0 + wzu + 0.01, b, e);
+      for (size_t i = b; i < e; i++) {
+        const int32_t u = S.rows[ru][i];
+        if (std::fabs(cl[u].y - y0) <= wyu && std::fabs(cl[u].z - z0) <= wzu) U.push_back(u);
+      }
+      z_range(c, S.rows[rd], (double)z0 - wzd - 0.01, (double)z0 + wzd + 0.01, b, e);
+      for (size_t i = b; i < e; i++) {
+        const int32_t d = S.rows[rd][i];
+        if (std::fabs(cl[d].y - y0) <= wyd && std::fabs(cl[d].z - z0) <= wzd) D.push_back(d);
+      }
+      int32_t bu = -1, bd = -1;
+      float bc = 0.0f;
+      for (int32_t u : U)
+        for (int32_t d : D) {
+          const float yu = cl[u].y, zu = cl[u].z, yd = cl[d].y, zd = cl[d].z;
+          const float ey = y0 - (yd + t * (yu - yd));
+          const float ez = z0 - (zd + t * (zu - zd));
+          const float cost = (ey * ey) * c.inv_sy2 + (ez * ez) * c.inv_sz2;
+          if (!(cost <= P.triplet_cut)) continue;
+          bool better;
+          if (bu < 0) better = true;
+          else if (cost != bc) better = cost < bc;
+          else if (u != bu) better = key_less(cl, u, bu);
+          else better = key_less(cl, d, bd);
+          if (better) { bu = u; bd = d; bc = cost; }
+        }
+      up[h] = bu;
+      down[h] = bd;
+    }
+  }
+}
+
+// Best pick-up candidate in a row for the predicted state (O5 "search"); returns input index or -1.
+int32_t search_row(const Ctx& c, const std::vector<int32_t>& row, const KF& k, float z_ref, float cut) {
+  if (row.empty()) return -1;
+  const Cl* cl = c.cl;
+  const float vy = k.C[0] + c.sy2, vz = k.C[2] + c.sz2;
+  const float iy = 1.0f / vy, iz = 1.0f / vz;
+  const float wy = std::sqrt(cut * vy), wz = std::sqrt(cut * vz);
+  const double zc = (double)z_ref + (double)k.p[1];
+  size_t b, e;
+  const double m = 0.01 + 1e-6 * std::fabs(zc);
+  z_range(c, row, zc - (double)wz - m, zc + (double)wz + m, b, e);
+  int32_t best = -1;
+  float bd = 0.0f;
+  for (size_t i = b; i < e; i++) {
+    const int32_t h = row[i];
+    const float dy = cl[h].y - k.p[0];
+    const float dz = (cl[h].z - z_ref) - k.p[1];
+    if (!(std::fabs(dy) <= wy) || !(std::fabs(dz) <= wz)) continue;
+    const float d = (dy * dy) * iy + (dz * dz) * iz;
+    if (!(d <= cut)) continue;
+    bool better;
+    if (best < 0) better = true;
+    else if (d != bd) better = d < bd;
+    else better = key_less(cl, h, best);
+    if (better) { best = h; bd = d; }
+  }
+  return best;
+}
+
+inline float hit_dist(const Ctx& c, const KF& k, const Cl& h, float z_ref) {
+  const float iy = 1.0f / (k.C[0] + c.sy2), iz = 1.0f / (k.C[2] + c.sz2);
+  const float dy = h.y - k.p[0];
+  const float dz = (h.z - z_ref) - k.p[1];
+  return (dy * dy) * iy + (dz * dz) * iz;
+}
+
+// ---- O5 tracklet construction for one start hit ----
+void build_tracklet(const Ctx& c, const Sector& S, const std::vector<int32_t>& link_up, int32_t h0, Tracklet& T,
+                    int32_t* row_hit /* n_rows, preset to -1 */) {
+  const Params& P = c.P;
+  const Cl* cl = c.cl;
+  const int R = c.n_rows;
+  T.valid = 0; T.first_row = T.last_row = -1; T.n_hits = 0; T.W = 0; T.chi2 = 0; T.x = 0;
+  for (int i = 0; i < 5; i++) T.p[i] = 0;
+  for (int i = 0; i < 15; i++) T.C[i] = 0;
+  const float z_ref = cl[h0].z;
+  T.z_ref = z_ref;
+  // E1: seed fit outward along the links
+  const int32_t h1 = link_up[h0];
+  KF k;
+  {
+    const float dx = cl[h1].x - cl[h0].x, dy = cl[h1].y - cl[h0].y, dz = cl[h1].z - cl[h0].z;
+    const float ds = std::sqrt(dx * dx + dy * dy);
+    k.x = cl[h0].x;
+    k.p[0] = cl[h0].y; k.p[1] = 0.0f; k.p[2] = dy / ds; k.p[3] = dz / ds; k.p[4] = 0.0f;
+    reset_cov(k, P);
+  }
+  update(k, cl[h0].y, cl[h0].z - z_ref, c.sy2, c.sz2);
+  row_hit[cl[h0].row] = h0;
+  int n_chain = 1, last_row = cl[h0].row;
+  for (int32_t h = h1; h >= 0; h = link_up[h]) {
+    if (!transport(k, cl[h].x, c.kq, P.max_sinphi)) return;  // void
+    update(k, cl[h].y, cl[h].z - z_ref, c.sy2, c.sz2);
+    row_hit[cl[h].row] = h;
+    last_row = cl[h].row;
+    n_chain++;
+  }
+  if (n_chain < P.min_seed_hits) return;  // void
+  const int r_low = cl[h0].row;
+  // E2: outward extrapolation, one best cluster per row
+  KF snap = k;  // state at the outermost hit
+  int top_row = last_row, gap = 0;
+  for (int r = last_row + 1; r < R; r++) {
+    if (!transport(k, c.row_x[r], c.kq, P.max_sinphi)) break;
+    if (std::fabs(k.p[0]) > c.row_x[r] * P.tan_half_angle + P.edge_margin) break;
+    const int32_t hb = search_row(c, S.rows[r], k, z_ref, P.pick_cut);
+    if (hb >= 0) {
+      update(k, cl[hb].y, cl[hb].z - z_ref, c.sy2, c.sz2);
+      row_hit[r] = hb; gap = 0; snap = k; top_row = r;
+    } else {
+      gap++;
+      if (gap > P.max_gap) break;
+    }
+  }
+  // E3: inward pass through the seed with outlier rejection, then pick-up below it
+  k = snap;
+  reset_cov(k, P);
+  KF inner = k;
+  int inner_row = -1;
+  gap = 0;
+  int r = top_row;
+  for (; r >= 0; r--) {
+    if (!transport(k, c.row_x[r], c.kq, P.max_sinphi)) break;
+    if (std::fabs(k.p[0]) > c.row_x[r] * P.tan_half_angle + P.edge_margin) break;
+    bool hit = false;
+    if (row_hit[r] >= 0) {
+      const Cl& hc = cl[row_hit[r]];
+      const float d = hit_dist(c, k, hc, z_ref);
+      if (d <= P.reject_cut) { update(k, hc.y, hc.z - z_ref, c.sy2, c.sz2); hit = true; }
+      else row_hit[r] = -1;
+    } else {
+      const int32_t hb = search_row(c, S.rows[r], k, z_ref, P.pick_cut);
+      if (hb >= 0) { update(k, cl[hb].y, cl[hb].z - z_ref, c.sy2, c.sz2); row_hit[r] = hb; hit = true; }
+    }
+    if (hit) { gap = 0; inner = k; inner_row = r; }
+    else { gap++; if (r < r_low && gap > P.max_gap) { r--; break; } }
+  }
+  for (int rr = r; rr >= 0; rr--) row_hit[rr] = -1;  // rows the pass never reached (or stopped on)
+  if (inner_row < 0) return;
+  int n_hits = 0, first = -1, last = -1;
+  for (int rr = 0; rr < R; rr++)
+    if (row_hit[rr] >= 0) { n_hits++; if (first < 0) first = rr; last = rr; }
+  if (n_hits < P.min_tracklet_hits) return;
+  T.valid = 1; T.first_row = first; T.last_row = last; T.n_hits = n_hits;
+  T.x = inner.x; T.chi2 = inner.chi2;
+  for (int i = 0; i < 5; i++) T.p[i] = inner.p[i];
+  for (int i = 0; i < 15; i++) T.C[i] = inner.C[i];
+}
+
+inline uint64_t pack_weight(const Params& P, int n_hits, float chi2, uint32_t tid) {
+  float qf = (P.qual_scale * chi2) / (float)(2 * n_hits);
+  qf = std::fmin(65535.0f, qf);
+  qf = std::fmax(0.0f, qf);
+  const int qi = (int)qf;
+  const uint32_t qual = (uint32_t)(65535 - qi);
+  return ((uint64_t)(uint32_t)n_hits << 48) | ((uint64_t)qual << 32) | (uint64_t)(0xFFFFFFFFu - tid);
+}
+
+// ---- O7 refit: inward, outward, inward over the track's hits ----
+// hits: input indices in increasing row order.  Returns false if a transport failed.
+bool refit(const Ctx& c, const std::vector<int32_t>& hits, float q0, KF& k, float& z_ref) {
+  const Cl* cl = c.cl;
+  const int n = (int)hits.size();
+  const Cl& hN = cl[hits[n - 1]];
+  const Cl& hM = cl[hits[n - 2]];
+  z_ref = hN.z;
+  const float dx = hN.x - hM.x, dy = hN.y - hM.y, dz = hN.z - hM.z;
+  const float ds = std::sqrt(dx * dx + dy * dy);
+  k.x = hN.x;
+  k.p[0] = hN.y; k.p[1] = 0.0f; k.p[2] = dy / ds; k.p[3] = dz / ds; k.p[4] = q0;
+  for (int pass = 0; pass < 3; pass++) {
+    reset_cov(k, c.P);
+    for (int j = 0; j < n; j++) {
+      const Cl& h = cl[hits[(pass == 1) ? j : n - 1 - j]];
+      if (!transport(k, h.x, c.kq, c.P.max_sinphi)) return false;
+      update(k, h.y, h.z - z_ref, c.sy2, c.sz2);
+    }
+  }
+  return true;
+}
+
+Ctx make_ctx(const Cl* cl, const float* row_x, int n_rows, const Params& P, float bz, bool brute) {
+  Ctx c;
+  c.cl = cl; c.row_x = row_x; c.n_rows = n_rows; c.P = P; c.brute = brute;
+  c.kq = -((0.000299792458f * 10.0f) * bz);
+  c.sy2 = P.sigma_y * P.sigma_y;
+  c.sz2 = P.sigma_z * P.sigma_z;
+  c.inv_sy2 = 1.0f / c.sy2;
+  c.inv_sz2 = 1.0f / c.sz2;
+  return c;
+}
+
+}  // namespace
+
+extern "C" {
+
+// Whole path O1-O7.  Returns an opaque result handle (free with orc_free).
+void* orc_track(int32_t n_sectors, int32_t n_rows, const float* row_x, float bz, const Params* P, const Cl* cl,
+                int64_t n, const int32_t* sector_offsets, int32_t brute) {
+  Result* R = new Result;
+  R->n = n; R->n_sectors = n_sectors; R->n_rows = n_rows;
+  R->link_up_raw.assign(n, -1); R->link_down_raw.assign(n, -1);
+  R->assignment.assign(n, -1);
+  Ctx c = make_ctx(cl, row_x, n_rows, *P, bz, brute != 0);
+  std::vector<Sector> secs(n_sectors);
+  // O1: group by sector and row; canonical order inside a row slice
+  for (int s = 0; s < n_sectors; s++) {
+    Sector& S = secs[s];
+    S.cl = cl;
+    S.rows.assign(n_rows, {});
+    for (int32_t i = sector_offsets[s]; i < sector_offsets[s + 1]; i++)
+      if (cl[i].row >= 0 && cl[i].row < n_rows) S.rows[cl[i].row].push_back(i);
+    for (auto& row : S.rows) std::sort(row.begin(), row.end(), [cl](int32_t a, int32_t b) { return key_less(cl, a, b); });
+    find_neighbours(c, S, R->link_up_raw, R->link_down_raw);  // O2
+  }
+  // O3: keep mutual links only
+  R->link_up = R->link_up_raw; R->link_down = R->link_down_raw;
+  for (int64_t h = 0; h < n; h++) {
+    const int32_t u = R->link_up_raw[h], d = R->link_down_raw[h];
+    if (u >= 0 && R->link_down_raw[u] != h) R->link_up[h] = -1;
+    if (d >= 0 && R->link_up_raw[d] != h) R->link_down[h] = -1;
+  }
+  // O4: start hits in (sector, key) order
+  std::vector<int32_t> start_sector;
+  for (int s = 0; s < n_sectors; s++)
+    for (int r = 0; r < n_rows; r++)
+      for (int32_t h : secs[s].rows[r])
+        if (R->link_down[h] < 0 && R->link_up[h] >= 0) { R->start_hits.push_back(h); start_sector.push_back(s); }
+  // O5: tracklets
+  const size_t nt = R->start_hits.size();
+  R->tracklets.resize(nt);
+  R->row_hit.assign(nt * (size_t)n_rows, -1);
+  std::vector<uint64_t> weight(n, 0);
+  for (size_t t = 0; t < nt; t++) {
+    Tracklet& T = R->tracklets[t];
+    T.sector = start_sector[t]; T.start_hit = R->start_hits[t];
+    int32_t* rh = &R->row_hit[t * (size_t)n_rows];
+    build_tracklet(c, secs[T.sector], R->link_up, T.start_hit, T, rh);
+    if (!T.valid) { for (int r = 0; r < n_rows; r++) rh[r] = -1; continue; }
+    T.W = pack_weight(*P, T.n_hits, T.chi2, (uint32_t)t);
+    for (int r = 0; r < n_rows; r++)
+      if (rh[r] >= 0) weight[rh[r]] = std::max(weight[rh[r]], T.W);
+  }
+  // O6: selection by exclusive ownership; O7: refit
+  std::vector<int32_t> hits;
+  for (size_t t = 0; t < nt; t++) {
+    const Tracklet& T = R->tracklets[t];
+    if (!T.valid) continue;
+    const int32_t* rh = &R->row_hit[t * (size_t)n_rows];
+    hits.clear();
+    for (int r = 0; r < n_rows; r++)
+      if (rh[r] >= 0 && weight[rh[r]] == T.W) hits.push_back(rh[r]);
+    if ((int)hits.size() < P->min_track_hits) continue;
+    const int32_t id = (int32_t)R->tracks.size();
+    for (int32_t h : hits) R->assignment[h] = id;
+    TrackRec tr;
+    std::memset(&tr, 0, sizeof(tr));
+    tr.sector = T.sector; tr.first_row = cl[hits.front()].row; tr.last_row = cl[hits.back()].row;
+    tr.n_hits = (int32_t)hits.size();
+    KF k; float z_ref = 0;
+    const bool ok = refit(c, hits, T.p[4], k, z_ref);
+    tr.x = k.x; tr.y = k.p[0]; tr.z = k.p[1] + z_ref; tr.sinphi = k.p[2]; tr.dzds = k.p[3]; tr.qpt = k.p[4];
+    for (int i = 0; i < 15; i++) tr.cov[i] = k.C[i];
+    tr.chi2 = k.chi2;
+    tr.ndf = ok ? 2 * tr.n_hits - 5 : -1;
+    R->tracks.push_back(tr);
+    R->track_tracklet.push_back((int32_t)t);
+  }
+  return R;
+}
+
+void orc_free(void* r) { delete (Result*)r; }
+int64_t orc_n_start(void* r) { return (int64_t)((Result*)r)->start_hits.size(); }
+int64_t orc_n_tracks(void* r) { return (int64_t)((Result*)r)->tracks.size(); }
+const int32_t* orc_link_up_raw(void* r) { return ((Result*)r)->link_up_raw.data(); }
+const int32_t* orc_link_down_raw(void* r) { return ((Result*)r)->link_down_raw.data(); }
+const int32_t* orc_link_up(void* r) { return ((Result*)r)->link_up.data(); }
+const int32_t* orc_link_down(void* r) { return ((Result*)r)->link_down.data(); }
+const int32_t* orc_start_hits(void* r) { return ((Result*)r)->start_hits.data(); }
+const int32_t* orc_row_hit(void* r) { return ((Result*)r)->row_hit.data(); }
+const int32_t* orc_assignment(void* r) { return ((Result*)r)->assignment.data(); }
+const TrackRec* orc_tracks(void* r) { return ((Result*)r)->tracks.data(); }
+const int32_t* orc_track_tracklet(void* r) { return ((Result*)r)->track_tracklet.data(); }
+// tracklet table as flat arrays: ints (valid, first_row, last_row, n_hits) and floats (x, p5, C15, chi2, z_ref)
+void orc_tracklets(void* r, int32_t* ints4, float* floats23) {
+  Result* R = (Result*)r;
+  for (size_t t = 0; t < R->tracklets.size(); t++) {
+    const Tracklet& T = R->tracklets[t];
+    ints4[4 * t + 0] = T.valid; ints4[4 * t + 1] = T.first_row; ints4[4 * t + 2] = T.last_row; ints4[4 * t + 3] = T.n_hits;
+    float* f = floats23 + 23 * t;
+    f[0] = T.x;
+    for (int i = 0; i < 5; i++) f[1 + i] = T.p[i];
+    for (int i = 0; i < 15; i++) f[6 + i] = T.C[i];
+    f[21] = T.chi2; f[22] = T.z_ref;
+  }
+}
+
+// ---- single-step entry points for the pins (P6-P8) ----
+// state9: x, p[5]; cov15; returns 1 on success
+int32_t orc_kf_transport(float* x, float* p5, float* cov15, float xnew, float bz, float max_sinphi) {
+  KF k; k.x = *x; k.chi2 = 0;
+  for (int i = 0; i < 5; i++) k.p[i] = p5[i];
+  for (int i = 0; i < 15; i++) k.C[i] = cov15[i];
+  const float kq = -((0.000299792458f * 10.0f) * bz);
+  const bool ok = transport(k, xnew, kq, max_sinphi);
+  *x = k.x;
+  for (int i = 0; i < 5; i++) p5[i] = k.p[i];
+  for (int i = 0; i < 15; i++) cov15[i] = k.C[i];
+  return ok ? 1 : 0;
+}
+void orc_kf_update(float* p5, float* cov15, float* chi2, float ym, float zm, float sy2, float sz2) {
+  KF k; k.x = 0; k.chi2 = *chi2;
+  for (int i = 0; i < 5; i++) k.p[i] = p5[i];
+  for (int i = 0; i < 15; i++) k.C[i] = cov15[i];
+  update(k, ym, zm, sy2, sz2);
+  for (int i = 0; i < 5; i++) p5[i] = k.p[i];
+  for (int i = 0; i < 15; i++) cov15[i] = k.C[i];
+  *chi2 = k.chi2;
+}
+// O7 on a free-standing hit list (hits in increasing x).  out: x, y, z, sinphi, dzds, qpt, cov15, chi2 (22 floats)
+int32_t orc_refit_hits(int32_t n, const Cl* hits, float q0, float bz, const Params* P, float* out22) {
+  std::vector<float> rx(1, 0.0f);
+  Ctx c = make_ctx(hits, rx.data(), 1, *P, bz, true);
+  std::vector<int32_t> idx(n);
+  for (int i = 0; i < n; i++) idx[i] = i;
+  KF k; float z_ref = 0;
+  const bool ok = refit(c, idx, q0, k, z_ref);
+  out22[0] = k.x; out22[1] = k.p[0]; out22[2] = k.p[1] + z_ref; out22[3] = k.p[2]; out22[4] = k.p[3]; out22[5] = k.p[4];
+  for (int i = 0; i < 15; i++) out22[6 + i] = k.C[i];
+  out22[21] = k.chi2;
+  return ok ? 1 : 0;
+}
+
+}  // extern "C"
