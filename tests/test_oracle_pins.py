@@ -1,0 +1,387 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (P1-P11).
+
+None of these call the CUDA path.  Each pin is chosen so that a plausible mistake in the oracle
+(dropped Jacobian term, wrong curvature sign, transposed covariance index, non-mutual link,
+grid search missing a candidate) fails it.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1811_11481_b200 import score, synth
+from tests.helix import KAPPA_PER_T, helix_points
+
+CL = synth.CLUSTER_DTYPE
+
+
+def _mk(rows, y, z, rx):
+    cl = np.zeros(len(rows), CL)
+    cl["row"] = rows
+    cl["x"] = rx[rows]
+    cl["y"] = y
+    cl["z"] = z
+    return cl
+
+
+def _same(a, b):
+    for f in ("link_up_raw", "link_down_raw", "link_up", "link_down", "start_hits", "row_hit", "assignment",
+              "tracklet_ints", "track_tracklet"):
+        assert np.array_equal(getattr(a, f), getattr(b, f)), f
+    assert a.tracks.tobytes() == b.tracks.tobytes()
+    assert a.tracklet_floats.tobytes() == b.tracklet_floats.tobytes()
+
+
+# ---------------------------------------------------------------- P1
+def _brute_links_py(cl, rx, P):
+    """All-triplet search, no acceleration structure, numpy float32 scalars (O2)."""
+    f = np.float32
+    n = len(cl)
+    up, dn = np.full(n, -1, np.int32), np.full(n, -1, np.int32)
+    rows = cl["row"]
+    R = len(rx)
+    occupied = [np.flatnonzero(rows == r) for r in range(R)]
+    inv_sy2 = f(1) / (f(P["sigma_y"]) * f(P["sigma_y"]))
+    inv_sz2 = f(1) / (f(P["sigma_z"]) * f(P["sigma_z"]))
+
+    def key(i):
+        return (float(cl["z"][i]), float(cl["y"][i]), int(i))
+
+    for r in range(R):
+        ru = r + 1 if r + 1 < R and len(occupied[r + 1]) else (r + 2 if r + 2 < R and len(occupied[r + 2]) else -1)
+        rd = r - 1 if r - 1 >= 0 and len(occupied[r - 1]) else (r - 2 if r - 2 >= 0 and len(occupied[r - 2]) else -1)
+        if ru < 0 or rd < 0:
+            continue
+        dxu, dxd = f(rx[ru]) - f(rx[r]), f(rx[r]) - f(rx[rd])
+        t = dxd / (dxu + dxd)
+        wyu, wzu = dxu * f(P["nbr_dydx"]) + f(P["nbr_margin_y"]), dxu * f(P["nbr_dzdx"]) + f(P["nbr_margin_z"])
+        wyd, wzd = dxd * f(P["nbr_dydx"]) + f(P["nbr_margin_y"]), dxd * f(P["nbr_dzdx"]) + f(P["nbr_margin_z"])
+        for h in occupied[r]:
+            y0, z0 = cl["y"][h], cl["z"][h]
+            best = None
+            for u in occupied[ru]:
+                yu, zu = cl["y"][u], cl["z"][u]
+                if not (abs(yu - y0) <= wyu and abs(zu - z0) <= wzu):
+                    continue
+                for d in occupied[rd]:
+                    yd, zd = cl["y"][d], cl["z"][d]
+                    if not (abs(yd - y0) <= wyd and abs(zd - z0) <= wzd):
+                        continue
+                    ey = y0 - (yd + t * (yu - yd))
+                    ez = z0 - (zd + t * (zu - zd))
+                    cost = (ey * ey) * inv_sy2 + (ez * ez) * inv_sz2
+                    if not cost <= f(P["triplet_cut"]):
+                        continue
+                    cand = (float(cost), key(u), key(d), u, d)
+                    if best is None or cand[:3] < best[:3]:
+                        best = cand
+            if best is not None:
+                up[h], dn[h] = best[3], best[4]
+    return up, dn
+
+
+@pytest.mark.parametrize("seed", [11, 12])
+def test_p1_brute_force_triplets_tiny(row_x, seed):
+    fr = synth.generate(synth.config(1, scale=0.02, seed=seed), noise_frac=0.4)  # 4 tracks + heavy noise
+    assert 100 < fr.n <= 700
+    with np.errstate(over="ignore"):
+        up, dn = _brute_links_py(fr.clusters, row_x, oracle.DEFAULT_PARAMS)
+    r = oracle.track(fr.clusters, fr.sector_offsets, row_x)
+    assert np.array_equal(r.link_up_raw, up)
+    assert np.array_equal(r.link_down_raw, dn)
+    assert (up >= 0).sum() > 50
+
+
+@pytest.mark.parametrize("cfg,scale", [(1, 0.05), (2, 0.01), (3, 0.01)])
+def test_p1_structure_free_mode_equals_sorted_mode(row_x, cfg, scale):
+    """The oracle's z-sorted search and its no-structure mode (every cluster of the row is a candidate)
+    give identical results for every step (links, tracklets, assignment, tracks)."""
+    fr = synth.generate(synth.config(cfg, scale=scale, seed=5))
+    a = oracle.track(fr.clusters, fr.sector_offsets, row_x, brute=False)
+    b = oracle.track(fr.clusters, fr.sector_offsets, row_x, brute=True)
+    _same(a, b)
+    assert len(a.tracks) > 0
+
+
+# ---------------------------------------------------------------- P2
+@pytest.mark.parametrize("pt,q,tanl,sinphi0", [(0.35, -1, 0.5, -0.33), (0.4, 1, 0.6, 0.3), (0.5, -1, -0.8, -0.1), (1.0, 1, 0.3, 0.12),
+                                                (2.0, -1, 1.0, 0.0), (8.0, 1, -0.2, 0.02)])
+def test_p2_noiseless_helix(row_x, pt, q, tanl, sinphi0):
+    """A noiseless helix: links follow the true hits, one chain rows 1..R-2, one start hit, one track with all
+    hits, and q/pT and tan(lambda) recovered (curvature sign DESIGN.md A15)."""
+    R = len(row_x)
+    qpt = q / pt
+    y, z, s = helix_points(row_x.astype(np.float64), 85.0, 1.0, 30.0, sinphi0, tanl, qpt, 0.5)
+    ok = np.abs(y) < row_x * np.tan(np.deg2rad(10))
+    assert ok.all()
+    cl = _mk(np.arange(R), y, z, row_x)
+    r = oracle.track(cl, np.array([0, R], np.int32), row_x)
+    idx = np.arange(R)
+    exp_up = np.where((idx >= 1) & (idx <= R - 2), idx + 1, -1)
+    exp_dn = np.where((idx >= 1) & (idx <= R - 2), idx - 1, -1)
+    assert np.array_equal(r.link_up_raw, exp_up) and np.array_equal(r.link_down_raw, exp_dn)
+    # cleaning cuts the links of the two end triplet centres whose partner is an end hit (A6)
+    assert np.array_equal(r.link_up, np.where((idx >= 1) & (idx <= R - 3), idx + 1, -1))
+    assert np.array_equal(r.link_down, np.where((idx >= 2) & (idx <= R - 2), idx - 1, -1))
+    assert list(r.start_hits) == [1]
+    assert len(r.tracks) == 1 and r.tracks["n_hits"][0] == R and (r.assignment == 0).all()
+    t = r.tracks[0]
+    assert t["x"] == row_x[0]
+    assert abs(t["qpt"] - qpt) <= 2e-3 * abs(qpt) + 1e-4, (t["qpt"], qpt)
+    assert abs(t["dzds"] - tanl) <= 1e-4 * max(1, abs(tanl)), (t["dzds"], tanl)
+    assert abs(t["sinphi"] - sinphi0) <= 2e-4
+    assert abs(t["y"] - 1.0) < 2e-3 and abs(t["z"] - 30.0) < 2e-3
+    assert t["chi2"] < 1.0  # noiseless: residuals are fp32 rounding only
+
+
+def test_p2_curvature_sign(row_x):
+    """Positive charge in +z field bends towards -y for a track along +x (d sinphi/dx = -0.003*B*q/pT < 0)."""
+    R = len(row_x)
+    y, z, s = helix_points(row_x.astype(np.float64), 85.0, 0.0, 0.0, 0.0, 0.1, +1.0 / 0.5, 0.5)
+    assert y[-1] < -1.0
+    cl = _mk(np.arange(R), y, z, row_x)
+    r = oracle.track(cl, np.array([0, R], np.int32), row_x)
+    assert len(r.tracks) == 1 and r.tracks["qpt"][0] > 1.9
+
+
+# ---------------------------------------------------------------- P3-P5
+@pytest.fixture(scope="module")
+def cfg2_small(row_x):
+    fr = synth.generate(synth.config(2, scale=0.05, seed=2))
+    return fr, oracle.track(fr.clusters, fr.sector_offsets, row_x)
+
+
+def test_p3_links_mutual_after_cleaning(cfg2_small):
+    fr, r = cfg2_small
+    h = np.flatnonzero(r.link_up >= 0)
+    assert len(h) > 1000
+    assert np.array_equal(r.link_down[r.link_up[h]], h)
+    h = np.flatnonzero(r.link_down >= 0)
+    assert np.array_equal(r.link_up[r.link_down[h]], h)
+    # cleaning only removes
+    assert ((r.link_up == r.link_up_raw) | (r.link_up == -1)).all()
+    # start hits are exactly the chain heads
+    sh = np.flatnonzero((r.link_down < 0) & (r.link_up >= 0))
+    assert np.array_equal(np.sort(r.start_hits), sh)
+
+
+def test_p4_exclusive_assignment(cfg2_small):
+    fr, r = cfg2_small
+    nt = len(r.tracks)
+    assert nt > 100
+    cnt = np.bincount(r.assignment[r.assignment >= 0], minlength=nt)
+    assert np.array_equal(cnt, r.tracks["n_hits"])
+    assert cnt.min() >= oracle.DEFAULT_PARAMS["min_track_hits"]
+    sec = score.sector_of_cluster(fr.sector_offsets, fr.n)
+    for t in range(0, nt, 7):
+        h = np.flatnonzero(r.assignment == t)
+        assert len(np.unique(fr.clusters["row"][h])) == len(h)  # one hit per row
+        assert (sec[h] == r.tracks["sector"][t]).all()
+        assert fr.clusters["row"][h].min() == r.tracks["first_row"][t]
+        assert fr.clusters["row"][h].max() == r.tracks["last_row"][t]
+    # every hit of a track comes from its tracklet's row table
+    for t in range(0, nt, 11):
+        rh = r.row_hit[r.track_tracklet[t]]
+        assert set(np.flatnonzero(r.assignment == t)) <= set(rh[rh >= 0])
+
+
+def test_p5_permutation_invariance(cfg2_small, row_x):
+    fr, r = cfg2_small
+    fp, p = synth.permute_within_sectors(fr, seed=99)
+    rp = oracle.track(fp.clusters, fp.sector_offsets, row_x)
+    assert len(rp.tracks) == len(r.tracks)
+    # new[i] = old[p[i]]: assignment equal up to the permutation, track ids included (canonical order)
+    assert np.array_equal(rp.assignment, r.assignment[p])
+    inv = np.empty_like(p)
+    inv[p] = np.arange(len(p))
+    lu = np.where(r.link_up >= 0, inv[np.maximum(r.link_up, 0)], -1)
+    assert np.array_equal(rp.link_up, lu[p])
+    assert np.array_equal(rp.start_hits, inv[r.start_hits])
+    assert np.array_equal(rp.tracks["n_hits"], r.tracks["n_hits"])
+    assert rp.tracks.tobytes() == r.tracks.tobytes()
+
+
+# ---------------------------------------------------------------- P6
+@pytest.mark.parametrize("qpt,s0,tanl", [(2.0, 0.1, 0.7), (-4.0, -0.3, -1.2), (0.1, 0.6, 0.2), (0.0, 0.2, 0.5)])
+def test_p6_transport_closed_form(qpt, s0, tanl):
+    """sin(phi) linear in x, y on the circle, z = tan(lambda) * arc: one 100 cm step, 100 one-cm steps and the
+    float64 helix agree."""
+    x0, y0 = 90.0, 3.0
+    p = [y0, 0.0, s0, tanl, qpt]
+    C0 = np.zeros(15, np.float32)
+    ok, x1, p1, _ = oracle.kf_transport(x0, p, C0, x0 + 40.0)
+    assert ok
+    y, z, s = helix_points([x0 + 40.0], x0, y0, 0.0, s0, tanl, qpt, 0.5)
+    assert abs(p1[2] - s[0]) < 2e-6
+    assert abs(p1[0] - y[0]) < 2e-5 * max(1, abs(y[0]))
+    # the arc series is truncated after u^4: a single long step is slightly short at high curvature
+    assert abs(p1[1] - z[0]) < 2e-3 * max(1, abs(z[0]))
+    x, pp, C = x0, np.array(p, np.float32), C0
+    for i in range(40):
+        ok, x, pp, C = oracle.kf_transport(x, pp, C, x0 + (i + 1))
+        assert ok
+    assert abs(pp[2] - s[0]) < 5e-6
+    assert abs(pp[0] - y[0]) < 1e-4
+    assert abs(pp[1] - z[0]) < 1e-4 * max(1, abs(z[0]))
+    # and back again: transport is reversible
+    for i in range(40):
+        ok, x, pp, C = oracle.kf_transport(x, pp, C, x0 + 39 - i)
+    assert abs(pp[0] - y0) < 2e-4 and abs(pp[1]) < 2e-4 and abs(pp[2] - s0) < 1e-5
+
+
+def test_p6_transport_fails_beyond_max_sinphi():
+    ok, *_ = oracle.kf_transport(100.0, [0, 0, 0.9, 0, -10.0], np.zeros(15, np.float32), 110.0)
+    assert not ok  # 0.9 + 10*0.015 > 0.95
+    ok, *_ = oracle.kf_transport(100.0, [0, 0, 0.99, 0, 0.0], np.zeros(15, np.float32), 101.0)
+    assert not ok
+
+
+def test_p6_jacobian_matches_finite_differences():
+    """C <- F C F^T with F from the transport: compare the propagated covariance with a float64
+    finite-difference Jacobian of the closed-form helix map (catches a dropped or transposed term)."""
+    x0, dx, bz = 100.0, 12.0, 0.5
+    p0 = np.array([2.0, 5.0, 0.25, 0.8, 1.5])
+
+    def fmap(p):
+        y, z, s = helix_points([x0 + dx], x0, p[0], p[1], p[2], p[3], p[4], bz)
+        return np.array([y[0], z[0], s[0], p[3], p[4]])
+
+    F = np.zeros((5, 5))
+    for j in range(5):
+        e = np.zeros(5)
+        e[j] = 1e-6 * max(1.0, abs(p0[j]))
+        F[:, j] = (fmap(p0 + e) - fmap(p0 - e)) / (2 * e[j])
+    rng = np.random.default_rng(0)
+    A = rng.normal(size=(5, 5)) * np.array([0.1, 0.1, 0.01, 0.01, 0.1])[:, None]
+    Cm = A @ A.T
+    tri = [Cm[i, j] for i in range(5) for j in range(i + 1)]
+    ok, x1, p1, C1 = oracle.kf_transport(x0, p0, tri, x0 + dx)
+    exp = F @ Cm @ F.T
+    got = np.zeros((5, 5))
+    k = 0
+    for i in range(5):
+        for j in range(i + 1):
+            got[i, j] = got[j, i] = C1[k]
+            k += 1
+    scale = np.sqrt(np.outer(np.diag(exp), np.diag(exp)))
+    assert np.max(np.abs(got - exp) / scale) < 2e-3  # the neglected d(g) term is O(u^2) ~ 1e-5 here
+
+
+# ---------------------------------------------------------------- P7
+def test_p7_zero_field_is_linear_least_squares():
+    """Bz = 0: the three-pass filter equals the weighted straight-line least-squares fit of y(x) and z(x) with the
+    diagonal prior cov0 (textbook normal equations in float64).  sin(phi)=0 track so the model is exactly linear
+    in (y, sinphi) to first order; compare value and covariance."""
+    rng = np.random.default_rng(3)
+    x = np.linspace(85, 245, 60)
+    sy, sz = 0.1, 0.15
+    ytrue = 1.0 + 0.02 * (x - 85)
+    ztrue = -4.0 + 0.5 * (x - 85)
+    y = ytrue + rng.normal(0, sy, x.size)
+    z = ztrue + rng.normal(0, sz, x.size)
+    ok, out = oracle.refit_hits(x, y, z, q0=0.0, bz=0.0)
+    assert ok
+    # float64 weighted LSQ on y = a + b (x - x0): params at x0 = innermost hit
+    A = np.stack([np.ones_like(x), x - x[0]], 1)
+
+    def lsq(v, sig, prior_var):
+        N = A.T @ A / sig**2 + np.diag(1.0 / np.asarray(prior_var))
+        return np.linalg.solve(N, A.T @ v / sig**2), np.linalg.inv(N)
+
+    (a, b), covy = lsq(y, sy, [1e12, 1e12])
+    (az, bz_), covz = lsq(z, sz, [1e12, 1e12])
+    sinphi = b / np.sqrt(1 + b * b)
+    dzds = bz_ / np.sqrt(1 + b * b)
+    assert abs(out[1] - a) < 3e-3          # y at x0
+    assert abs(out[3] - sinphi) < 1e-4     # sin(phi)
+    assert abs(out[2] - az) < 5e-3         # z at x0
+    assert abs(out[4] - dzds) < 2e-4       # dz/ds
+    # covariance of y: (A^T W A)^-1 up to the prior (cov0 = 1 cm^2 vs 1e-4 information per hit: < 1 %)
+    assert abs(out[6] - covy[0, 0]) / covy[0, 0] < 0.03
+    assert abs(out[6 + 2] - covz[0, 0]) / covz[0, 0] < 0.03
+    # q/pT unobservable at B = 0: stays at its start value, variance stays at the prior
+    assert out[5] == 0.0 and abs(out[6 + 14] - 100.0) < 1e-3
+
+
+def test_p7_single_update_is_textbook_gain():
+    """One scalar update equals K = C H^T (H C H^T + v)^-1 in float64 for a full random covariance."""
+    rng = np.random.default_rng(1)
+    A = rng.normal(size=(5, 5))
+    Cm = A @ A.T
+    p = rng.normal(size=5)
+    tri = [Cm[i, j] for i in range(5) for j in range(i + 1)]
+    ym, zm, vy, vz = 0.3, -0.2, 0.01, 0.0225
+    p1, C1, chi2 = oracle.kf_update(p, tri, 0.0, ym, zm, vy, vz)
+    H = np.zeros((2, 5))
+    H[0, 0] = H[1, 1] = 1
+    V = np.diag([vy, vz])
+    S = H @ Cm @ H.T + V
+    K = Cm @ H.T @ np.linalg.inv(S)
+    r = np.array([ym, zm]) - H @ p
+    pe = p + K @ r
+    Ce = (np.eye(5) - K @ H) @ Cm
+    assert np.allclose(p1, pe, rtol=2e-4, atol=2e-5)
+    got = np.zeros((5, 5))
+    k = 0
+    for i in range(5):
+        for j in range(i + 1):
+            got[i, j] = got[j, i] = C1[k]
+            k += 1
+    assert np.allclose(got, Ce, rtol=2e-3, atol=2e-4)
+    assert abs(chi2 - r @ np.linalg.inv(S) @ r) < 1e-3 * max(1, chi2)
+
+
+# ---------------------------------------------------------------- P8
+def test_p8_pulls_and_chi2(row_x):
+    """Smeared single helices: pulls of (y, z, sinphi, dzds, qpt) ~ N(0,1) and <chi2/ndf> ~ 1."""
+    rng = np.random.default_rng(8)
+    pulls, red = [], []
+    xs = row_x.astype(np.float64)
+    for i in range(400):
+        pt = np.exp(rng.uniform(np.log(0.4), np.log(5)))
+        q = rng.choice([-1.0, 1.0])
+        s0, tl, y0, z0 = rng.uniform(-0.1, 0.1), rng.uniform(-1, 1), rng.uniform(-5, 5), rng.uniform(-100, 100)
+        y, z, s = helix_points(xs, 85.0, y0, z0, s0, tl, q / pt, 0.5)
+        ok, out = oracle.refit_hits(xs, y + rng.normal(0, 0.1, xs.size), z + rng.normal(0, 0.15, xs.size), 0.0, 0.5)
+        assert ok
+        true = np.array([y0, z0, s0, tl, q / pt])
+        var = np.array([out[6 + k] for k in (0, 2, 5, 9, 14)])
+        pulls.append((out[1:6] - true) / np.sqrt(var))
+        red.append(out[21] / (2 * xs.size - 5))
+    pulls = np.array(pulls)
+    assert np.all(np.abs(pulls.mean(0)) < 0.2), pulls.mean(0)
+    assert np.all(np.abs(pulls.std(0) - 1) < 0.15), pulls.std(0)
+    assert abs(np.mean(red) - 1) < 0.05
+
+
+# ---------------------------------------------------------------- P10 / P11
+def test_p10_optimisation_level_independent(row_x):
+    fr = synth.generate(synth.config(2, scale=0.02, seed=10))
+    a = oracle.track(fr.clusters, fr.sector_offsets, row_x, opt="-O2")
+    b = oracle.track(fr.clusters, fr.sector_offsets, row_x, opt="-O0")
+    _same(a, b)
+    c = oracle.track(fr.clusters, fr.sector_offsets, row_x, opt="-O2")
+    _same(a, c)
+
+
+def test_p11_config1_efficiency(row_x):
+    fr = synth.generate(1)
+    r = oracle.track(fr.clusters, fr.sector_offsets, row_x)
+    sc = score.score(r.assignment, fr.truth, score.sector_of_cluster(fr.sector_offsets, fr.n), len(r.tracks))
+    assert sc["efficiency"] > 0.98 and sc["fake_rate"] < 0.01, sc
+
+
+def test_edge_cases(row_x):
+    e = oracle.track(np.zeros(0, CL), np.zeros(37, np.int32), row_x)
+    assert len(e.tracks) == 0 and len(e.start_hits) == 0
+    # a sector with rows r and r+2 only (row skipping, A5): chain through every second row still links
+    rows = np.arange(0, 152, 2)
+    y, z, s = helix_points(row_x[rows].astype(np.float64), 85.0, 0.0, 10.0, 0.05, 0.4, 1.0, 0.5)
+    cl = _mk(rows, y, z, row_x)
+    r = oracle.track(cl, np.array([0, len(rows)], np.int32), row_x)
+    assert (r.link_up_raw[1:-1] == np.arange(2, len(rows))).all()
+    assert len(r.tracks) == 1 and r.tracks["n_hits"][0] == len(rows)
+    # every third row only: no links at all (one skip at most)
+    rows = np.arange(0, 152, 3)
+    y, z, s = helix_points(row_x[rows].astype(np.float64), 85.0, 0.0, 10.0, 0.05, 0.4, 1.0, 0.5)
+    r = oracle.track(_mk(rows, y, z, row_x), np.array([0, len(rows)], np.int32), row_x)
+    assert (r.link_up_raw == -1).all() and len(r.tracks) == 0
