@@ -1,0 +1,148 @@
+/*
+ * tpcca.h -- C-ABI of the B200-native per-sector TPC track finder (arXiv 1811.11481).
+ *
+ * The operation: PAPER.md:49-51 (section 2) -- for each of the 36 TPC sectors, a cellular automaton
+ * links hit triplets that lie close to a straight line, consecutive links are concatenated into
+ * seeds, each seed is fitted with a (simplified) Kalman filter, extrapolated through the TPC picking
+ * up adjacent hits without following multiple hypotheses, and refitted; PAPER.md:65-68 (outward,
+ * then inward through the seed with outlier rejection); PAPER.md:71 (final refit inward, outward,
+ * inward); PAPER.md:93 (cluster time already scaled linearly to z, arbitrarily long TPC);
+ * PAPER.md:121 (fp32).  Every constant the paper leaves open is a field of tpcca_params with the
+ * default of DESIGN.md Table A.
+ *
+ * Conventions: plain pointers and sizes, no framework types.  "device" = CUDA device memory of the
+ * current device, "host" = ordinary host memory.  The library never allocates or frees device
+ * memory: all scratch lives in the caller-provided workspace.  All entry points return 0 on success
+ * or a negative tpcca_status; tpcca_last_error() describes the last failure of the calling thread.
+ * There is no CPU fallback: without a CUDA device tpcca_init fails.
+ */
+#ifndef TPCCA_H
+#define TPCCA_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tpcca_handle tpcca_handle;
+
+enum tpcca_status {
+  TPCCA_OK = 0,
+  TPCCA_ERR_ARGUMENT = -1, /* null / misaligned pointer, n > max_clusters, offsets not monotone ... */
+  TPCCA_ERR_NOT_INIT = -2,
+  TPCCA_ERR_CUDA = -3      /* a CUDA runtime call or kernel launch failed */
+};
+
+/* device-side status bits (tpcca_out_header.status) */
+enum {
+  TPCCA_STAT_TRACKLET_OVERFLOW = 1, /* more start hits than max_tracklets: highest ids dropped */
+  TPCCA_STAT_TRACK_OVERFLOW = 2,    /* more tracks than max_tracks: highest ids dropped */
+  TPCCA_STAT_BAD_CLUSTER = 4,       /* a cluster with row outside [0,n_rows) was ignored */
+  TPCCA_STAT_BIN_OVERFLOW = 8       /* internal grid capacity hit (never with the default sizing) */
+};
+
+/* Geometry (152 pad rows; 36 trapezoidal sectors). */
+typedef struct {
+  int32_t n_sectors;     /* 1..64; 36 for the full TPC (0-17 side A, 18-35 side C) */
+  int32_t n_rows;        /* 2..256; 152 */
+  const float* row_x;    /* host, n_rows, cm, strictly increasing; copied by tpcca_init */
+  float tan_half_angle;  /* tan(10 deg): a row spans |y| <= x*tan_half_angle */
+} tpcca_geometry;
+
+/* Parameters.  Physics fields follow DESIGN.md Table A (A1-A13); grid_* only shape the search
+ * acceleration structure and never change a result. */
+typedef struct {
+  float sigma_y, sigma_z;                   /* cluster errors, cm */
+  float nbr_dydx, nbr_dzdx;                 /* neighbour window slope per cm of row distance */
+  float nbr_margin_y, nbr_margin_z;         /* neighbour window margins, cm */
+  float triplet_cut;                        /* max straight-line triplet cost */
+  float cov0[5];                            /* initial / reset covariance diagonal */
+  float pick_cut, reject_cut;               /* 2-dof distance cuts: pick-up, seed-hit rejection */
+  int32_t max_gap;                          /* consecutive rows without hit before stopping */
+  float edge_margin, max_sinphi;
+  int32_t min_seed_hits, min_tracklet_hits, min_track_hits;
+  float qual_scale;
+  float grid_bin_y, grid_bin_z_min;         /* cm */
+  float grid_bins_per_cluster;              /* target bins per cluster in a row slice, <= 2 */
+  int64_t max_clusters;                     /* capacity per call */
+  int32_t max_tracklets, max_tracks;
+  void* workspace;                          /* device, >= tpcca_workspace_bytes(), 256-byte aligned; caller-owned */
+  size_t workspace_bytes;
+} tpcca_params;
+
+/* Input cluster, sector-local coordinates: x along the sector axis (must equal row_x[row]), y across,
+ * z along the drift.  16 bytes, read as one float4. */
+typedef struct { float x, y, z; int32_t row; } tpcca_cluster;
+
+/* Output: header followed by max_tracks records. */
+typedef struct { int32_t n_tracks, n_tracklets, n_start_hits, status; } tpcca_out_header; /* 16 B */
+typedef struct {
+  int32_t sector, first_row, last_row, n_hits;
+  float x, y, z, sinphi, dzds, qpt;         /* state at x = row_x[first_row] (innermost hit) */
+  float cov[15];                            /* lower triangle of cov(y, z, sinphi, dzds, qpt) */
+  float chi2;                               /* of the last (inward) refit pass */
+  int32_t ndf;                              /* 2*n_hits-5, or -1 if the refit transport failed */
+  int32_t pad[5];
+} tpcca_track_rec;                          /* 128 B */
+
+/* Fill *p with the defaults of DESIGN.md Table A (capacities 0, workspace NULL). */
+void tpcca_default_params(tpcca_params* p);
+
+/* Bytes of device workspace needed for the capacities in *p (workspace fields ignored).  0 on bad arguments. */
+size_t tpcca_workspace_bytes(const tpcca_geometry* g, const tpcca_params* p);
+
+/* Create a tracker on the current CUDA device.  Host-only work plus one small upload (row_x).
+ * Returns NULL on error (see tpcca_last_error). */
+tpcca_handle* tpcca_init(const tpcca_geometry* g, float bz_tesla, const tpcca_params* p);
+
+/* Track one time frame: steps (a)-(g) of DESIGN.md for all sectors, enqueued on `stream`; returns
+ * without waiting.  clusters: device, n records, clusters of sector s at
+ * [sector_offsets[s], sector_offsets[s+1]) in any order, 16-byte aligned.  sector_offsets: HOST,
+ * n_sectors+1 entries, CSR, read before return.  stream: a cudaStream_t (NULL = default stream).
+ * out_tracks: device, sizeof(header) + max_tracks*128 bytes; tracks in canonical order.
+ * out_hit_assignment: device, n int32 in input order, track id or -1.
+ * n == 0 is valid (header all zero).  Capacity overflow sets header.status and truncates; nothing is
+ * ever written out of bounds. */
+int tpcca_track(tpcca_handle* h, const tpcca_cluster* clusters, int64_t n, const int32_t* sector_offsets,
+                void* stream, void* out_tracks, int32_t* out_hit_assignment);
+
+/* Same, end to end from HOST buffers (pinned for best speed): copies clusters host->device into the
+ * workspace, tracks, copies header, tracks and assignment device->host and synchronises `stream`.
+ * out_tracks: host, sizeof(header) + max_tracks*128 bytes (only n_tracks records are written). */
+int tpcca_track_host(tpcca_handle* h, const tpcca_cluster* clusters, int64_t n, const int32_t* sector_offsets,
+                     void* stream, void* out_tracks, int32_t* out_hit_assignment);
+
+/* Intermediates of the last tpcca_track on this handle, translated to INPUT-index space so that they
+ * can be compared with an independent implementation.  dst: device.  Enqueued on `stream`. */
+enum tpcca_intermediate {
+  TPCCA_LINK_UP_RAW = 0,    /* int32[n]  (b) before cleaning */
+  TPCCA_LINK_DOWN_RAW = 1,  /* int32[n] */
+  TPCCA_LINK_UP = 2,        /* int32[n]  (c) mutual links only */
+  TPCCA_LINK_DOWN = 3,      /* int32[n] */
+  TPCCA_START_HITS = 4,     /* int32[n_start_hits], canonical order = tracklet ids */
+  TPCCA_TRACKLET_ROW_HITS = 5, /* int32[n_start_hits][n_rows], -1 = no hit (void tracklets: all -1) */
+  TPCCA_TRACKLET_INTS = 6,  /* int32[n_start_hits][4]: valid, first_row, last_row, n_hits */
+  TPCCA_TRACKLET_FLOATS = 7,/* float[n_start_hits][8]: x, y, z-z_ref, sinphi, dzds, qpt, chi2, z_ref */
+  TPCCA_TRACK_TRACKLET = 8  /* int32[n_tracks]: tracklet id of each track */
+};
+int tpcca_get_intermediate(tpcca_handle* h, int what, void* dst_device, size_t bytes, void* stream);
+
+/* Per-stage device times of the last tpcca_track when profiling is on (CUDA events on the call's
+ * stream; synchronises those events).  ms: host float[TPCCA_N_STAGES]. */
+enum { TPCCA_STAGE_GRID = 0, TPCCA_STAGE_NEIGHBOURS, TPCCA_STAGE_CLEAN_START, TPCCA_STAGE_TRACKLETS,
+       TPCCA_STAGE_SELECT, TPCCA_STAGE_REFIT, TPCCA_N_STAGES };
+int tpcca_set_profiling(tpcca_handle* h, int on);
+int tpcca_get_stage_ms(tpcca_handle* h, float* ms);
+
+/* Kernels launched by the last tpcca_track / tpcca_track_host on this handle. */
+int tpcca_last_launch_count(tpcca_handle* h);
+
+const char* tpcca_last_error(void);
+void tpcca_free(tpcca_handle* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TPCCA_H */

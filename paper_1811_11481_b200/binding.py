@@ -1,0 +1,215 @@
+"""Thin ctypes binding of include/tpcca.h (argument marshalling only).
+
+PyTorch supplies device memory and streams; every step of the path runs in the CUDA kernels of
+`csrc/`.  There is no fallback: a missing or unloadable libtpcca.so raises at import of `load()`.
+Names follow the C-ABI: tpcca_init / tpcca_track / tpcca_track_host / tpcca_get_intermediate / tpcca_free.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libtpcca.so")
+
+LINK_UP_RAW, LINK_DOWN_RAW, LINK_UP, LINK_DOWN, START_HITS, TRACKLET_ROW_HITS, TRACKLET_INTS, TRACKLET_FLOATS, \
+    TRACK_TRACKLET = range(9)
+STAGES = ("grid", "neighbours", "clean_start", "tracklets", "select", "refit")
+
+CLUSTER_DTYPE = np.dtype([("x", "<f4"), ("y", "<f4"), ("z", "<f4"), ("row", "<i4")])
+TRACK_DTYPE = np.dtype([
+    ("sector", "<i4"), ("first_row", "<i4"), ("last_row", "<i4"), ("n_hits", "<i4"),
+    ("x", "<f4"), ("y", "<f4"), ("z", "<f4"), ("sinphi", "<f4"), ("dzds", "<f4"), ("qpt", "<f4"),
+    ("cov", "<f4", (15,)), ("chi2", "<f4"), ("ndf", "<i4"), ("pad", "<i4", (5,)),
+])
+HEADER_DTYPE = np.dtype([("n_tracks", "<i4"), ("n_tracklets", "<i4"), ("n_start_hits", "<i4"), ("status", "<i4")])
+
+
+class Geometry(C.Structure):
+    _fields_ = [("n_sectors", C.c_int32), ("n_rows", C.c_int32), ("row_x", C.POINTER(C.c_float)),
+                ("tan_half_angle", C.c_float)]
+
+
+class Params(C.Structure):
+    _fields_ = [
+        ("sigma_y", C.c_float), ("sigma_z", C.c_float),
+        ("nbr_dydx", C.c_float), ("nbr_dzdx", C.c_float), ("nbr_margin_y", C.c_float), ("nbr_margin_z", C.c_float),
+        ("triplet_cut", C.c_float), ("cov0", C.c_float * 5),
+        ("pick_cut", C.c_float), ("reject_cut", C.c_float), ("max_gap", C.c_int32),
+        ("edge_margin", C.c_float), ("max_sinphi", C.c_float),
+        ("min_seed_hits", C.c_int32), ("min_tracklet_hits", C.c_int32), ("min_track_hits", C.c_int32),
+        ("qual_scale", C.c_float),
+        ("grid_bin_y", C.c_float), ("grid_bin_z_min", C.c_float), ("grid_bins_per_cluster", C.c_float),
+        ("max_clusters", C.c_int64), ("max_tracklets", C.c_int32), ("max_tracks", C.c_int32),
+        ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
+    ]
+
+
+_lib = None
+
+
+def load():
+    """Load libtpcca.so (built in-tree by build.py).  Raises if it is missing: no CPU fallback exists."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_SO):
+            raise RuntimeError(f"{_SO} not built: run `python -m paper_1811_11481_b200.build` "
+                               "(or __graft_entry__.build()); this package has no CPU fallback")
+        lib = C.CDLL(_SO)
+        lib.tpcca_default_params.argtypes = [C.POINTER(Params)]
+        lib.tpcca_workspace_bytes.restype = C.c_size_t
+        lib.tpcca_workspace_bytes.argtypes = [C.POINTER(Geometry), C.POINTER(Params)]
+        lib.tpcca_init.restype = C.c_void_p
+        lib.tpcca_init.argtypes = [C.POINTER(Geometry), C.c_float, C.POINTER(Params)]
+        for name in ("tpcca_track", "tpcca_track_host"):
+            fn = getattr(lib, name)
+            fn.restype = C.c_int
+            fn.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.tpcca_get_intermediate.restype = C.c_int
+        lib.tpcca_get_intermediate.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_size_t, C.c_void_p]
+        lib.tpcca_set_profiling.argtypes = [C.c_void_p, C.c_int]
+        lib.tpcca_get_stage_ms.restype = C.c_int
+        lib.tpcca_get_stage_ms.argtypes = [C.c_void_p, C.c_void_p]
+        lib.tpcca_last_launch_count.restype = C.c_int
+        lib.tpcca_last_launch_count.argtypes = [C.c_void_p]
+        lib.tpcca_last_error.restype = C.c_char_p
+        lib.tpcca_free.argtypes = [C.c_void_p]
+        _lib = lib
+    return _lib
+
+
+def default_params() -> Params:
+    p = Params()
+    load().tpcca_default_params(C.byref(p))
+    return p
+
+
+class TpccaError(RuntimeError):
+    pass
+
+
+class Tracker:
+    """tpcca_init ... tpcca_free around one handle; owns the workspace tensor (caller-owned memory of the C-ABI)."""
+
+    def __init__(self, row_x: np.ndarray, n_sectors: int = 36, bz: float = 0.5, max_clusters: int = 1 << 20,
+                 max_tracklets: int | None = None, max_tracks: int | None = None,
+                 tan_half_angle: float = float(np.tan(np.deg2rad(10.0))), device: str = "cuda:0", **params):
+        import torch
+        self.torch = torch
+        self.lib = load()
+        if not torch.cuda.is_available():
+            raise TpccaError("no CUDA device: the tpcca path has no CPU fallback")
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self._rx = np.ascontiguousarray(row_x, dtype=np.float32)
+        self.n_rows, self.n_sectors = int(self._rx.shape[0]), int(n_sectors)
+        self.geo = Geometry(self.n_sectors, self.n_rows, self._rx.ctypes.data_as(C.POINTER(C.c_float)), tan_half_angle)
+        p = default_params()
+        for k, v in params.items():
+            if k == "cov0":
+                p.cov0 = (C.c_float * 5)(*v)
+            elif hasattr(p, k):
+                setattr(p, k, v)
+            else:
+                raise TypeError(f"unknown parameter {k}")
+        p.max_clusters = int(max_clusters)
+        p.max_tracklets = int(max_tracklets if max_tracklets is not None else max(1024, max_clusters // 8))
+        p.max_tracks = int(max_tracks if max_tracks is not None else p.max_tracklets)
+        nbytes = self.lib.tpcca_workspace_bytes(C.byref(self.geo), C.byref(p))
+        if nbytes == 0:
+            raise TpccaError(self.lib.tpcca_last_error().decode())
+        self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        base = (self.workspace.data_ptr() + 255) & ~255
+        p.workspace, p.workspace_bytes = base, nbytes
+        self.params = p
+        self.max_clusters, self.max_tracklets, self.max_tracks = p.max_clusters, p.max_tracklets, p.max_tracks
+        self.h = self.lib.tpcca_init(C.byref(self.geo), float(bz), C.byref(p))
+        if not self.h:
+            raise TpccaError(self.lib.tpcca_last_error().decode())
+        self.out_tracks = torch.empty(16 + 128 * self.max_tracks, dtype=torch.uint8, device=self.device)
+        self.out_assign = torch.empty(max(1, self.max_clusters), dtype=torch.int32, device=self.device)
+        self.n = 0
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.tpcca_free(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc):
+        if rc != 0:
+            raise TpccaError(f"tpcca error {rc}: {self.lib.tpcca_last_error().decode()}")
+
+    def _stream(self):
+        return self.torch.cuda.current_stream(self.device).cuda_stream
+
+    # ---- device-resident call: clusters is a torch uint8/float32 CUDA tensor holding n 16-byte records
+    def track(self, clusters_dev, n: int, sector_offsets: np.ndarray):
+        so = np.ascontiguousarray(sector_offsets, dtype=np.int32)
+        assert so.shape[0] == self.n_sectors + 1
+        self._so = so
+        self.n = int(n)
+        self._check(self.lib.tpcca_track(self.h, clusters_dev.data_ptr() if n else None, n, so.ctypes.data,
+                                         self._stream(), self.out_tracks.data_ptr(), self.out_assign.data_ptr()))
+
+    def upload(self, clusters: np.ndarray):
+        t = self.torch.from_numpy(np.ascontiguousarray(clusters).view(np.uint8).reshape(-1))
+        return t.to(self.device)
+
+    def header(self) -> dict:
+        h = self.out_tracks[:16].cpu().numpy().view(HEADER_DTYPE)[0]
+        return {k: int(h[k]) for k in HEADER_DTYPE.names}
+
+    def tracks(self) -> np.ndarray:
+        nt = self.header()["n_tracks"]
+        return self.out_tracks[16:16 + 128 * nt].cpu().numpy().view(TRACK_DTYPE).copy()
+
+    def assignment(self) -> np.ndarray:
+        return self.out_assign[:self.n].cpu().numpy().copy()
+
+    # ---- end to end from host buffers (pinned numpy-backed torch tensors recommended)
+    def track_host(self, clusters_host, n: int, sector_offsets: np.ndarray, out_tracks_host, out_assign_host):
+        so = np.ascontiguousarray(sector_offsets, dtype=np.int32)
+        self._so = so
+        self.n = int(n)
+        self._check(self.lib.tpcca_track_host(self.h, clusters_host.data_ptr() if n else None, n, so.ctypes.data,
+                                              self._stream(), out_tracks_host.data_ptr(), out_assign_host.data_ptr()))
+
+    def intermediate(self, what: int) -> np.ndarray:
+        torch = self.torch
+        hd = self.header()
+        ns, nt = hd["n_start_hits"], hd["n_tracks"]
+        if what <= LINK_DOWN:
+            shape, dt = (self.n,), torch.int32
+        elif what == START_HITS:
+            shape, dt = (ns,), torch.int32
+        elif what == TRACKLET_ROW_HITS:
+            shape, dt = (ns, self.n_rows), torch.int32
+        elif what == TRACKLET_INTS:
+            shape, dt = (ns, 4), torch.int32
+        elif what == TRACKLET_FLOATS:
+            shape, dt = (ns, 8), torch.float32
+        else:
+            shape, dt = (nt,), torch.int32
+        numel = int(np.prod(shape))
+        dst = torch.empty(max(4, numel), dtype=dt, device=self.device)
+        self._check(self.lib.tpcca_get_intermediate(self.h, what, dst.data_ptr(), dst.numel() * 4, self._stream()))
+        return dst[:numel].reshape(shape).cpu().numpy()
+
+    def set_profiling(self, on: bool):
+        self.lib.tpcca_set_profiling(self.h, int(on))
+
+    def stage_ms(self) -> dict:
+        ms = (C.c_float * len(STAGES))()
+        self._check(self.lib.tpcca_get_stage_ms(self.h, ms))
+        return dict(zip(STAGES, [float(v) for v in ms]))
+
+    def launch_count(self) -> int:
+        return int(self.lib.tpcca_last_launch_count(self.h))

@@ -1,0 +1,289 @@
+// tpcca_api.cu -- the C-ABI of include/tpcca.h: argument checks, workspace carving, stream-ordered
+// enqueue of steps (a)-(g).  No kernel of the hot path lives here.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "tpcca_dev.cuh"
+
+static thread_local char g_err[512] = "";
+static void set_err(const char* fmt, const char* a = "", long long b = 0) { snprintf(g_err, sizeof(g_err), fmt, a, b); }
+
+struct tpcca_handle {
+  Dev d;
+  tpcca_geometry geo;
+  int64_t max_clusters;
+  // host-API staging (inside the workspace)
+  float4* stage_clusters;
+  int32_t* stage_assign;
+  char* stage_tracks;
+  // last call
+  int64_t last_n;
+  int launches;
+  bool profiling, have_times;
+  cudaEvent_t ev[TPCCA_N_STAGES + 1];
+};
+
+static size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
+
+// One pass computes the layout; with base != NULL it also assigns the pointers.
+static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params* p, char* base) {
+  size_t off = 0;
+  const size_t N = (size_t)p->max_clusters, T = (size_t)p->max_tracklets, K = (size_t)p->max_tracks;
+  const size_t SL = (size_t)g->n_sectors * g->n_rows;
+  const size_t NB = 2 * N + 128 * SL + 1;
+  const size_t NSCAN = T + 8 + NB / 2048 + T / 2048 + 64;
+#define CARVE(field, type, count)                                  \
+  do {                                                             \
+    if (base) h->field = reinterpret_cast<type*>(base + off);      \
+    off += align_up(sizeof(type) * (size_t)(count));               \
+  } while (0)
+  CARVE(d.cnt, DevCounters, 1);
+  CARVE(d.row_x, const float, g->n_rows);
+  CARVE(d.slice_count, int32_t, SL + 1);
+  CARVE(d.row_start, int32_t, SL + 1);
+  CARVE(d.slice_bbox, uint32_t, SL * 4);
+  CARVE(d.grid, GridHdr, SL);
+  CARVE(d.slice_nstart, int32_t, SL + 1);
+  CARVE(d.slice_sbase, int32_t, SL + 1);
+  CARVE(d.cluster_bin, int32_t, N);
+  CARVE(d.cluster_rank, int32_t, N);
+  CARVE(d.bin_start, int32_t, NB + 1);
+  CARVE(d.scan_tmp, int32_t, NSCAN);
+  CARVE(d.yz, float2, N);
+  CARVE(d.orig_idx, int32_t, N);
+  CARVE(d.slice_of, uint16_t, N);
+  CARVE(d.link_up, int32_t, N);
+  CARVE(d.link_down, int32_t, N);
+  CARVE(d.link_up_clean, int32_t, N);
+  CARVE(d.start_flag, uint8_t, N);
+  CARVE(d.hit_weight, unsigned long long, N);
+  CARVE(d.start_tmp, int32_t, T);
+  CARVE(d.start_hits, int32_t, T);
+  CARVE(d.row_hit, int32_t, T * (size_t)g->n_rows);
+  CARVE(d.tl_ints, int32_t, T * 4);
+  CARVE(d.tl_floats, float, T * 8);
+  CARVE(d.tl_W, unsigned long long, T);
+  CARVE(d.tl_track, int32_t, T + 1);
+  CARVE(d.track_tracklet, int32_t, K);
+  CARVE(stage_clusters, float4, N);
+  CARVE(stage_assign, int32_t, N);
+  CARVE(stage_tracks, char, sizeof(tpcca_out_header) + K * sizeof(tpcca_track_rec));
+#undef CARVE
+  if (base) h->d.max_bins = (int32_t)NB;
+  return off;
+}
+
+static bool check_geo_params(const tpcca_geometry* g, const tpcca_params* p) {
+  if (!g || !p) { set_err("null geometry or params"); return false; }
+  if (g->n_sectors < 1 || g->n_sectors > TPCCA_MAX_SECTORS) { set_err("n_sectors out of range [1,64]"); return false; }
+  if (g->n_rows < 2 || g->n_rows > TPCCA_MAX_ROWS) { set_err("n_rows out of range [2,256]"); return false; }
+  if ((size_t)g->n_sectors * g->n_rows > 65535) { set_err("n_sectors*n_rows must fit 16 bits"); return false; }
+  if (p->max_clusters < 0 || p->max_clusters > 1000000000LL || p->max_tracklets < 0 || p->max_tracks < 0) {
+    set_err("capacities out of range"); return false;
+  }
+  if (p->min_track_hits < 2 || p->min_tracklet_hits < 2 || p->min_seed_hits < 2) { set_err("min_*_hits must be >= 2"); return false; }
+  if (!(p->sigma_y > 0) || !(p->sigma_z > 0)) { set_err("sigma_y/sigma_z must be > 0"); return false; }
+  if (!(p->grid_bin_y > 0) || !(p->grid_bin_z_min > 0) || !(p->grid_bins_per_cluster > 0) || p->grid_bins_per_cluster > 2.0f) {
+    set_err("grid_* parameters out of range"); return false;
+  }
+  return true;
+}
+
+extern "C" {
+
+void tpcca_default_params(tpcca_params* p) {
+  if (!p) return;
+  memset(p, 0, sizeof(*p));
+  p->sigma_y = 0.1f; p->sigma_z = 0.15f;
+  p->nbr_dydx = 1.5f; p->nbr_dzdx = 1.5f; p->nbr_margin_y = 0.5f; p->nbr_margin_z = 0.75f; p->triplet_cut = 18.0f;
+  p->cov0[0] = 1.0f; p->cov0[1] = 1.0f; p->cov0[2] = 0.25f; p->cov0[3] = 1.0f; p->cov0[4] = 100.0f;
+  p->pick_cut = 16.0f; p->reject_cut = 25.0f; p->max_gap = 5; p->edge_margin = 3.0f; p->max_sinphi = 0.95f;
+  p->min_seed_hits = 4; p->min_tracklet_hits = 10; p->min_track_hits = 10; p->qual_scale = 1000.0f;
+  p->grid_bin_y = 2.0f; p->grid_bin_z_min = 2.5f; p->grid_bins_per_cluster = 1.0f;
+}
+
+size_t tpcca_workspace_bytes(const tpcca_geometry* g, const tpcca_params* p) {
+  if (!check_geo_params(g, p)) return 0;
+  return carve(nullptr, g, p, nullptr) + 256;
+}
+
+tpcca_handle* tpcca_init(const tpcca_geometry* g, float bz_tesla, const tpcca_params* p) {
+  if (!check_geo_params(g, p)) return nullptr;
+  if (!g->row_x) { set_err("row_x is null"); return nullptr; }
+  for (int r = 1; r < g->n_rows; r++)
+    if (!(g->row_x[r] > g->row_x[r - 1])) { set_err("row_x must be strictly increasing"); return nullptr; }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+    cudaGetLastError();
+    set_err("no CUDA device: this library has no CPU fallback");
+    return nullptr;
+  }
+  const size_t need = carve(nullptr, g, p, nullptr) + 256;
+  if (!p->workspace || ((uintptr_t)p->workspace & 255) || p->workspace_bytes < need) {
+    set_err("workspace null, misaligned (256 B) or too small%s (need %lld bytes)", "", (long long)need);
+    return nullptr;
+  }
+  tpcca_handle* h = new (std::nothrow) tpcca_handle;
+  if (!h) { set_err("out of host memory"); return nullptr; }
+  memset(h, 0, sizeof(*h));
+  h->geo = *g;
+  h->geo.row_x = nullptr;
+  h->max_clusters = p->max_clusters;
+  carve(h, g, p, (char*)p->workspace);
+  Dev& d = h->d;
+  d.n_sectors = g->n_sectors; d.n_rows = g->n_rows; d.n_slices = g->n_sectors * g->n_rows;
+  d.tan_half_angle = g->tan_half_angle;
+  d.P = *p;
+  d.kq = -((0.000299792458f * 10.0f) * bz_tesla);
+  d.sy2 = p->sigma_y * p->sigma_y;
+  d.sz2 = p->sigma_z * p->sigma_z;
+  d.inv_sy2 = 1.0f / d.sy2;
+  d.inv_sz2 = 1.0f / d.sz2;
+  d.max_tracklets = p->max_tracklets; d.max_tracks = p->max_tracks;
+  if (cudaMemcpy((void*)d.row_x, g->row_x, sizeof(float) * g->n_rows, cudaMemcpyHostToDevice) != cudaSuccess) {
+    set_err("row_x upload failed: %s", cudaGetErrorString(cudaGetLastError()));
+    delete h;
+    return nullptr;
+  }
+  for (int i = 0; i <= TPCCA_N_STAGES; i++)
+    if (cudaEventCreate(&h->ev[i]) != cudaSuccess) { set_err("cudaEventCreate failed"); delete h; return nullptr; }
+  return h;
+}
+
+static int track_impl(tpcca_handle* h, const tpcca_cluster* clusters, int64_t n, const int32_t* so_host,
+                      cudaStream_t st, void* out_tracks, int32_t* out_assign, Launch& L) {
+  Dev d = h->d;
+  SecOff so;
+  memset(&so, 0, sizeof(so));
+  if (so_host[0] != 0 || so_host[d.n_sectors] != n) { set_err("sector_offsets must start at 0 and end at n"); return TPCCA_ERR_ARGUMENT; }
+  for (int s = 0; s <= d.n_sectors; s++) {
+    if (s && so_host[s] < so_host[s - 1]) { set_err("sector_offsets not monotone"); return TPCCA_ERR_ARGUMENT; }
+    so.v[s] = so_host[s];
+  }
+  d.clusters = reinterpret_cast<const float4*>(clusters);
+  d.n = (int32_t)n;
+  d.out_hdr = reinterpret_cast<tpcca_out_header*>(out_tracks);
+  d.out_tracks = reinterpret_cast<tpcca_track_rec*>((char*)out_tracks + sizeof(tpcca_out_header));
+  d.out_assign = out_assign;
+  h->d.n = d.n; h->d.clusters = d.clusters; h->d.out_hdr = d.out_hdr; h->d.out_tracks = d.out_tracks; h->d.out_assign = out_assign;
+  h->last_n = n;
+  const bool prof = h->profiling;
+  if (prof) cudaEventRecord(h->ev[0], st);
+  launch_grid(d, so, L);
+  if (prof) cudaEventRecord(h->ev[1], st);
+  launch_neighbours(d, L);
+  if (prof) cudaEventRecord(h->ev[2], st);
+  launch_clean_start(d, L);
+  if (prof) cudaEventRecord(h->ev[3], st);
+  launch_tracklets(d, L);
+  if (prof) cudaEventRecord(h->ev[4], st);
+  launch_select(d, L);
+  if (prof) cudaEventRecord(h->ev[5], st);
+  launch_refit(d, L);
+  if (prof) cudaEventRecord(h->ev[6], st);
+  h->have_times = prof;
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) { set_err("kernel launch failed: %s", cudaGetErrorString(e)); return TPCCA_ERR_CUDA; }
+  return TPCCA_OK;
+}
+
+static int check_call(tpcca_handle* h, const void* clusters, int64_t n, const int32_t* so, const void* out_tracks,
+                      const void* out_assign) {
+  if (!h) { set_err("handle is null (not initialised)"); return TPCCA_ERR_NOT_INIT; }
+  if (n < 0 || n > h->max_clusters) { set_err("n out of range%s (max_clusters %lld)", "", (long long)h->max_clusters); return TPCCA_ERR_ARGUMENT; }
+  if (!so || !out_tracks) { set_err("sector_offsets or out_tracks is null"); return TPCCA_ERR_ARGUMENT; }
+  if (n > 0 && (!clusters || !out_assign)) { set_err("clusters or out_hit_assignment is null"); return TPCCA_ERR_ARGUMENT; }
+  if (((uintptr_t)clusters & 15) || ((uintptr_t)out_tracks & 15) || ((uintptr_t)out_assign & 3)) {
+    set_err("misaligned pointer (clusters/out_tracks 16 B, assignment 4 B)"); return TPCCA_ERR_ARGUMENT;
+  }
+  return TPCCA_OK;
+}
+
+int tpcca_track(tpcca_handle* h, const tpcca_cluster* clusters, int64_t n, const int32_t* sector_offsets, void* stream,
+                void* out_tracks, int32_t* out_hit_assignment) {
+  int rc = check_call(h, clusters, n, sector_offsets, out_tracks, out_hit_assignment);
+  if (rc) return rc;
+  Launch L{(cudaStream_t)stream, 0};
+  rc = track_impl(h, clusters, n, sector_offsets, L.st, out_tracks, out_hit_assignment, L);
+  h->launches = L.count;
+  return rc;
+}
+
+int tpcca_track_host(tpcca_handle* h, const tpcca_cluster* clusters, int64_t n, const int32_t* sector_offsets,
+                     void* stream, void* out_tracks, int32_t* out_hit_assignment) {
+  int rc = check_call(h, clusters, n, sector_offsets, out_tracks, out_hit_assignment);
+  if (rc) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  Launch L{st, 0};
+  if (n > 0 && cudaMemcpyAsync(h->stage_clusters, clusters, (size_t)n * 16, cudaMemcpyHostToDevice, st) != cudaSuccess) {
+    set_err("H2D copy failed: %s", cudaGetErrorString(cudaGetLastError())); return TPCCA_ERR_CUDA;
+  }
+  rc = track_impl(h, reinterpret_cast<const tpcca_cluster*>(h->stage_clusters), n, sector_offsets, st, h->stage_tracks,
+                  h->stage_assign, L);
+  h->launches = L.count;
+  if (rc) return rc;
+  cudaError_t e = cudaMemcpyAsync(out_tracks, h->stage_tracks, sizeof(tpcca_out_header), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess && n > 0)
+    e = cudaMemcpyAsync(out_hit_assignment, h->stage_assign, (size_t)n * 4, cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e == cudaSuccess) {
+    const tpcca_out_header* hd = reinterpret_cast<const tpcca_out_header*>(out_tracks);
+    if (hd->n_tracks > 0) {
+      e = cudaMemcpyAsync((char*)out_tracks + sizeof(tpcca_out_header), h->stage_tracks + sizeof(tpcca_out_header),
+                          (size_t)hd->n_tracks * sizeof(tpcca_track_rec), cudaMemcpyDeviceToHost, st);
+      if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    }
+  }
+  if (e != cudaSuccess) { set_err("D2H copy / execution failed: %s", cudaGetErrorString(e)); cudaGetLastError(); return TPCCA_ERR_CUDA; }
+  return TPCCA_OK;
+}
+
+int tpcca_get_intermediate(tpcca_handle* h, int what, void* dst, size_t bytes, void* stream) {
+  if (!h) { set_err("handle is null (not initialised)"); return TPCCA_ERR_NOT_INIT; }
+  if (!dst || what < 0 || what > TPCCA_TRACK_TRACKLET) { set_err("bad intermediate id or null dst"); return TPCCA_ERR_ARGUMENT; }
+  const Dev& d = h->d;
+  size_t need;
+  if (what <= TPCCA_LINK_DOWN) need = (size_t)d.n * 4;
+  else if (what == TPCCA_START_HITS) need = (size_t)d.max_tracklets * 4;
+  else if (what == TPCCA_TRACKLET_ROW_HITS) need = 0;  // data-dependent: caller sizes with n_start_hits
+  else need = 0;
+  if (what <= TPCCA_LINK_DOWN && bytes < need) { set_err("dst too small"); return TPCCA_ERR_ARGUMENT; }
+  (void)bytes;
+  Launch L{(cudaStream_t)stream, 0};
+  launch_export(d, what, dst, L);
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) { set_err("export launch failed: %s", cudaGetErrorString(e)); return TPCCA_ERR_CUDA; }
+  return TPCCA_OK;
+}
+
+int tpcca_set_profiling(tpcca_handle* h, int on) {
+  if (!h) return TPCCA_ERR_NOT_INIT;
+  h->profiling = on != 0;
+  h->have_times = false;
+  return TPCCA_OK;
+}
+
+int tpcca_get_stage_ms(tpcca_handle* h, float* ms) {
+  if (!h) return TPCCA_ERR_NOT_INIT;
+  if (!ms || !h->have_times) { set_err("no stage times recorded (enable profiling before tpcca_track)"); return TPCCA_ERR_ARGUMENT; }
+  if (cudaEventSynchronize(h->ev[TPCCA_N_STAGES]) != cudaSuccess) { set_err("event sync failed"); return TPCCA_ERR_CUDA; }
+  for (int i = 0; i < TPCCA_N_STAGES; i++)
+    if (cudaEventElapsedTime(&ms[i], h->ev[i], h->ev[i + 1]) != cudaSuccess) { set_err("event elapsed failed"); return TPCCA_ERR_CUDA; }
+  return TPCCA_OK;
+}
+
+int tpcca_last_launch_count(tpcca_handle* h) { return h ? h->launches : 0; }
+
+const char* tpcca_last_error(void) { return g_err; }
+
+void tpcca_free(tpcca_handle* h) {
+  if (!h) return;
+  for (int i = 0; i <= TPCCA_N_STAGES; i++)
+    if (h->ev[i]) cudaEventDestroy(h->ev[i]);
+  delete h;
+}
+
+}  // extern "C"

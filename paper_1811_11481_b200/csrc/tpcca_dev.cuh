@@ -1,0 +1,264 @@
+// tpcca_dev.cuh -- device-side context, layouts and fp32 helpers of the CUDA path.
+// Arithmetic follows DESIGN.md "Arithmetic" (steps O2-O7) operation by operation; every translation
+// unit is compiled with -fmad=false so that no multiply-add is contracted.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/tpcca.h"
+
+#define TPCCA_MAX_SECTORS 64
+#define TPCCA_MAX_ROWS 256
+
+struct GridHdr {  // 32 B per (sector,row) slice
+  float ymin, zmin, inv_by, inv_bz;
+  int32_t ny, nz, bin_base, pad;
+};
+
+struct DevCounters {  // device-resident scalars
+  int32_t n_start;     // start hits (clamped to max_tracklets)
+  int32_t n_tracks;    // accepted tracks (clamped to max_tracks)
+  int32_t n_valid;     // non-void tracklets
+  int32_t status;
+  int32_t n_bins;      // total grid bins of the frame
+  int32_t pad[3];
+};
+
+struct SecOff { int32_t v[TPCCA_MAX_SECTORS + 1]; };
+
+// Everything a kernel needs, passed by value.
+struct Dev {
+  // geometry / parameters
+  int32_t n_sectors, n_rows, n_slices;
+  float tan_half_angle, kq, sy2, sz2, inv_sy2, inv_sz2;
+  tpcca_params P;
+  const float* row_x;
+  // per call
+  const float4* clusters;
+  int32_t n;
+  // capacities
+  int32_t max_tracklets, max_tracks, max_bins;
+  // (a) grid
+  int32_t* slice_count;    // [n_slices+1]
+  int32_t* row_start;      // [n_slices+1] exclusive scan of slice_count
+  uint32_t* slice_bbox;    // [n_slices*4] ordered-uint ymin, ymax, zmin, zmax
+  GridHdr* grid;           // [n_slices]
+  int32_t* cluster_bin;    // [n] global bin id (input order)
+  int32_t* cluster_rank;   // [n] arrival rank inside the bin
+  int32_t* bin_start;      // [max_bins+1] counts, then exclusive scan
+  int32_t* scan_tmp;       // partial sums
+  float2* yz;              // [n] sorted (sector,row,bin)
+  int32_t* orig_idx;       // [n] sorted -> input index
+  uint16_t* slice_of;      // [n] slice id of a sorted cluster
+  // (b)-(d)
+  int32_t* link_up;        // [n] sorted index space
+  int32_t* link_down;
+  int32_t* link_up_clean;
+  uint8_t* start_flag;     // [n]
+  int32_t* slice_nstart;   // [n_slices+1]
+  int32_t* slice_sbase;    // [n_slices+1]
+  int32_t* start_tmp;      // [max_tracklets] unsorted start hits per slice
+  int32_t* start_hits;     // [max_tracklets] canonical order (sorted indices)
+  // (e)
+  int32_t* row_hit;        // [n_rows][max_tracklets]
+  int32_t* tl_ints;        // [max_tracklets][4] valid, first_row, last_row, n_hits
+  float* tl_floats;        // [max_tracklets][8] x, y, z~, sinphi, dzds, qpt, chi2, z_ref
+  unsigned long long* tl_W;        // [max_tracklets]
+  unsigned long long* hit_weight;  // [n]
+  // (f),(g)
+  int32_t* tl_track;       // [max_tracklets] scan buffer: flag -> track id
+  int32_t* track_tracklet; // [max_tracks]
+  DevCounters* cnt;
+  tpcca_out_header* out_hdr;
+  tpcca_track_rec* out_tracks;
+  int32_t* out_assign;
+};
+
+__device__ __forceinline__ uint32_t ordf(float f) {
+  const uint32_t b = __float_as_uint(f);
+  return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
+}
+__device__ __forceinline__ float unordf(uint32_t o) {
+  return __uint_as_float((o & 0x80000000u) ? (o & 0x7FFFFFFFu) : ~o);
+}
+
+__device__ __forceinline__ int sector_of(const SecOff& so, int n_sectors, int i) {
+  int lo = 0, hi = n_sectors;  // so.v[lo] <= i < so.v[hi]
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if (so.v[mid] <= i) lo = mid; else hi = mid;
+  }
+  return lo;
+}
+
+// ---- Kalman state ----
+struct KF {
+  float x;
+  float y, z, s, t, q;  // y, z~ = z - z_ref, sin(phi), dz/ds, q/pT
+  float c00, c10, c11, c20, c21, c22, c30, c31, c32, c33, c40, c41, c42, c43, c44;
+  float chi2;
+};
+
+__device__ __forceinline__ void kf_reset_cov(KF& k, const float* cov0) {
+  k.c00 = cov0[0]; k.c11 = cov0[1]; k.c22 = cov0[2]; k.c33 = cov0[3]; k.c44 = cov0[4];
+  k.c10 = k.c20 = k.c21 = k.c30 = k.c31 = k.c32 = k.c40 = k.c41 = k.c42 = k.c43 = 0.0f;
+  k.chi2 = 0.0f;
+}
+
+// Transport x -> xnew.  false: |sin(phi)| would exceed max_sinphi (state unchanged).
+__device__ __forceinline__ bool kf_transport(KF& k, float xnew, float kq, float max_sinphi) {
+  const float dx = xnew - k.x;
+  if (dx == 0.0f) return true;
+  const float s = k.s, t = k.t, q = k.q;
+  const float kk = q * kq;
+  const float s1 = s + dx * kk;
+  if (!(fabsf(s) <= max_sinphi) || !(fabsf(s1) <= max_sinphi)) return false;
+  const float c0 = sqrtf(1.0f - s * s);
+  const float c1 = sqrtf(1.0f - s1 * s1);
+  const float cc = c0 + c1;
+  const float f = (s + s1) / cc;
+  const float dy = dx * f;
+  float L = sqrtf(dx * dx + dy * dy);
+  if (dx < 0.0f) L = -L;
+  const float u = (0.5f * kk) * L;
+  const float u2 = u * u;
+  const float g = 1.0f + u2 * (0.16666667f + u2 * 0.075f);
+  const float dS = L * g;
+  const float fs0 = (1.0f + (f * s) / c0) / cc;
+  const float fs1 = (1.0f + (f * s1) / c1) / cc;
+  const float h = dx * kq;
+  const float fss = fs0 + fs1;
+  const float a02 = dx * fss;
+  const float a04 = (dx * fs1) * h;
+  const float w = (t * g) * ((dx * dy) / L);
+  const float a12 = w * fss;
+  const float a13 = dS;
+  const float a14 = (w * fs1) * h;
+  const float a24 = h;
+  k.y = k.y + dy;
+  k.z = k.z + t * dS;
+  k.s = s1;
+  k.x = xnew;
+  const float c00 = k.c00, c10 = k.c10, c11 = k.c11, c20 = k.c20, c21 = k.c21, c22 = k.c22, c30 = k.c30,
+              c31 = k.c31, c32 = k.c32, c33 = k.c33, c40 = k.c40, c41 = k.c41, c42 = k.c42, c43 = k.c43, c44 = k.c44;
+  const float m00 = (c00 + a02 * c20) + a04 * c40;
+  const float m02 = (c20 + a02 * c22) + a04 * c42;
+  const float m04 = (c40 + a02 * c42) + a04 * c44;
+  const float m10 = ((c10 + a12 * c20) + a13 * c30) + a14 * c40;
+  const float m11 = ((c11 + a12 * c21) + a13 * c31) + a14 * c41;
+  const float m12 = ((c21 + a12 * c22) + a13 * c32) + a14 * c42;
+  const float m13 = ((c31 + a12 * c32) + a13 * c33) + a14 * c43;
+  const float m14 = ((c41 + a12 * c42) + a13 * c43) + a14 * c44;
+  const float m20 = c20 + a24 * c40;
+  const float m21 = c21 + a24 * c41;
+  const float m22 = c22 + a24 * c42;
+  const float m23 = c32 + a24 * c43;
+  const float m24 = c42 + a24 * c44;
+  k.c00 = (m00 + a02 * m02) + a04 * m04;
+  k.c10 = (m10 + a02 * m12) + a04 * m14;
+  k.c11 = ((m11 + a12 * m12) + a13 * m13) + a14 * m14;
+  k.c20 = (m20 + a02 * m22) + a04 * m24;
+  k.c21 = ((m21 + a12 * m22) + a13 * m23) + a14 * m24;
+  k.c22 = m22 + a24 * m24;
+  k.c30 = (c30 + a02 * c32) + a04 * c43;
+  k.c31 = ((c31 + a12 * c32) + a13 * c33) + a14 * c43;
+  k.c32 = c32 + a24 * c43;
+  k.c40 = (c40 + a02 * c42) + a04 * c44;
+  k.c41 = ((c41 + a12 * c42) + a13 * c43) + a14 * c44;
+  k.c42 = c42 + a24 * c44;
+  return true;
+}
+
+// Sequential scalar updates, y then z~.
+__device__ __forceinline__ void kf_update(KF& k, float ym, float zm, float sy2, float sz2) {
+  {  // component 0 (y): column (c00, c10, c20, c30, c40)
+    const float i0 = k.c00, i1 = k.c10, i2 = k.c20, i3 = k.c30, i4 = k.c40;
+    const float r = ym - k.y;
+    const float S = i0 + sy2;
+    const float w = 1.0f / S;
+    const float K0 = i0 * w, K1 = i1 * w, K2 = i2 * w, K3 = i3 * w, K4 = i4 * w;
+    k.y = k.y + K0 * r; k.z = k.z + K1 * r; k.s = k.s + K2 * r; k.t = k.t + K3 * r; k.q = k.q + K4 * r;
+    k.c00 = k.c00 - K0 * i0;
+    k.c10 = k.c10 - K1 * i0; k.c11 = k.c11 - K1 * i1;
+    k.c20 = k.c20 - K2 * i0; k.c21 = k.c21 - K2 * i1; k.c22 = k.c22 - K2 * i2;
+    k.c30 = k.c30 - K3 * i0; k.c31 = k.c31 - K3 * i1; k.c32 = k.c32 - K3 * i2; k.c33 = k.c33 - K3 * i3;
+    k.c40 = k.c40 - K4 * i0; k.c41 = k.c41 - K4 * i1; k.c42 = k.c42 - K4 * i2; k.c43 = k.c43 - K4 * i3;
+    k.c44 = k.c44 - K4 * i4;
+    k.chi2 = k.chi2 + (r * r) * w;
+  }
+  {  // component 1 (z~): column (c10, c11, c21, c31, c41)
+    const float i0 = k.c10, i1 = k.c11, i2 = k.c21, i3 = k.c31, i4 = k.c41;
+    const float r = zm - k.z;
+    const float S = i1 + sz2;
+    const float w = 1.0f / S;
+    const float K0 = i0 * w, K1 = i1 * w, K2 = i2 * w, K3 = i3 * w, K4 = i4 * w;
+    k.y = k.y + K0 * r; k.z = k.z + K1 * r; k.s = k.s + K2 * r; k.t = k.t + K3 * r; k.q = k.q + K4 * r;
+    k.c00 = k.c00 - K0 * i0;
+    k.c10 = k.c10 - K1 * i0; k.c11 = k.c11 - K1 * i1;
+    k.c20 = k.c20 - K2 * i0; k.c21 = k.c21 - K2 * i1; k.c22 = k.c22 - K2 * i2;
+    k.c30 = k.c30 - K3 * i0; k.c31 = k.c31 - K3 * i1; k.c32 = k.c32 - K3 * i2; k.c33 = k.c33 - K3 * i3;
+    k.c40 = k.c40 - K4 * i0; k.c41 = k.c41 - K4 * i1; k.c42 = k.c42 - K4 * i2; k.c43 = k.c43 - K4 * i3;
+    k.c44 = k.c44 - K4 * i4;
+    k.chi2 = k.chi2 + (r * r) * w;
+  }
+}
+
+// same-row key order (ord z, ord y, input index): true if a < b
+__device__ __forceinline__ bool key_less(float za, float ya, int32_t ia, float zb, float yb, int32_t ib) {
+  const uint32_t oza = ordf(za), ozb = ordf(zb);
+  if (oza != ozb) return oza < ozb;
+  const uint32_t oya = ordf(ya), oyb = ordf(yb);
+  if (oya != oyb) return oya < oyb;
+  return ia < ib;
+}
+
+// Conservative bin range of [lo, hi] along one grid axis (monotone fp32 map + clamp => superset).
+__device__ __forceinline__ void bin_range(float lo, float hi, float vmin, float inv_b, int nb, int& b0, int& b1) {
+  const float f0 = (lo - vmin) * inv_b, f1 = (hi - vmin) * inv_b;
+  b0 = (f0 > 0.0f) ? ((f0 < (float)nb) ? (int)f0 : nb - 1) : 0;
+  b1 = (f1 >= 0.0f) ? ((f1 < (float)nb) ? (int)f1 : nb - 1) : -1;  // -1 => empty range
+  if (!(lo <= hi)) { b0 = 1; b1 = 0; }                             // NaN window: nothing
+}
+
+// exclusive block scan; every thread receives the block total.  smem: >= 32 ints.
+__device__ __forceinline__ int block_scan_excl(int v, int* total, int* smem /* >= 32 */) {
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  int x = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int y = __shfl_up_sync(0xffffffffu, x, o);
+    if (lane >= o) x += y;
+  }
+  if (lane == 31) smem[wid] = x;
+  __syncthreads();
+  if (wid == 0) {
+    const int nw = blockDim.x >> 5;
+    int w = (lane < nw) ? smem[lane] : 0;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int y = __shfl_up_sync(0xffffffffu, w, o);
+      if (lane >= o) w += y;
+    }
+    smem[lane] = w;  // inclusive over warps
+  }
+  __syncthreads();
+  const int base = wid ? smem[wid - 1] : 0;
+  *total = smem[(blockDim.x >> 5) - 1];
+  __syncthreads();
+  return base + x - v;
+}
+
+// launchers (one per pipeline step; defined in the .cu of that step)
+struct Launch {
+  cudaStream_t st;
+  int count;  // kernels launched
+};
+void launch_grid(const Dev& d, const SecOff& so, Launch& L);
+void launch_neighbours(const Dev& d, Launch& L);
+void launch_clean_start(const Dev& d, Launch& L);
+void launch_tracklets(const Dev& d, Launch& L);
+void launch_select(const Dev& d, Launch& L);
+void launch_refit(const Dev& d, Launch& L);
+void launch_export(const Dev& d, int what, void* dst, Launch& L);
+// exclusive scan of data[0..n) in place, n read from *n_dev (<= n_max); data[n] receives the total
+void launch_scan_i32(int32_t* data, const int32_t* n_dev, int32_t n_max, int32_t* tmp, Launch& L);

@@ -1,0 +1,105 @@
+"""GPU parity: the CUDA path through the C-ABI against the CPU oracle, element by element."""
+import numpy as np
+import pytest
+
+from paper_1811_11481_b200 import binding as B
+from paper_1811_11481_b200 import synth
+from tests.parity import compare, run_gpu
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("cfg,scale", [(1, 1.0), (2, 0.25), (2, 1.0), (3, 1.0), (4, 0.2)])
+def test_parity_configs(row_x, cfg, scale):
+    fr = synth.generate(synth.config(cfg, scale=scale))
+    t, orc, exact = compare(fr, row_x)
+    assert len(orc.tracks) > 50
+    assert exact, "fp32 no-FMA arithmetic in identical order: track records should be bit-identical"
+
+
+def test_parity_config5_reduced(row_x):
+    fr = synth.generate(synth.config(5, scale=0.1))
+    compare(fr, row_x)
+
+
+def test_grid_policy_does_not_change_results(row_x):
+    fr = synth.generate(synth.config(2, scale=0.1, seed=21))
+    base = run_gpu(fr, row_x)
+    a0, t0 = base.assignment(), base.tracks()
+    for kw in (dict(grid_bin_y=0.7, grid_bins_per_cluster=2.0), dict(grid_bin_y=9.0, grid_bins_per_cluster=0.1),
+               dict(grid_bin_z_min=40.0)):
+        t = run_gpu(fr, row_x, **kw)
+        assert np.array_equal(t.assignment(), a0), kw
+        assert t.tracks().tobytes() == t0.tobytes(), kw
+
+
+def test_determinism_and_handle_reuse(row_x):
+    fr = synth.generate(synth.config(2, scale=0.2, seed=7))
+    fr2 = synth.generate(synth.config(3, scale=0.1, seed=8))
+    t = B.Tracker(row_x, max_clusters=max(fr.n, fr2.n), max_tracklets=max(fr.n, fr2.n) // 4)
+    ref = None
+    for i in range(5):
+        run_gpu(fr2 if i == 2 else fr, row_x, t)
+        if i == 2:
+            continue
+        cur = (t.assignment().tobytes(), t.tracks().tobytes(), t.intermediate(B.START_HITS).tobytes())
+        ref = ref or cur
+        assert cur == ref
+    compare(fr2, row_x, tracker=t)
+
+
+def test_edge_cases(row_x):
+    t = B.Tracker(row_x, max_clusters=4096, max_tracklets=1024)
+    empty = synth.Frame(np.zeros(0, synth.CLUSTER_DTYPE), np.zeros(37, np.int32), np.zeros(0, np.int32),
+                        np.zeros((0, 8)), 36, "empty")
+    run_gpu(empty, row_x, t)
+    assert t.header() == dict(n_tracks=0, n_tracklets=0, n_start_hits=0, status=0)
+    # one cluster, and clusters in a single sector only
+    fr = synth.generate(synth.config(2, scale=0.002, seed=3))
+    compare(fr, row_x, tracker=t)
+    one = synth.Frame(fr.clusters[:1].copy(), np.r_[0, np.ones(36, np.int32)].astype(np.int32), fr.truth[:1],
+                      fr.track_par, 36, "one")
+    compare(one, row_x, tracker=t)
+    # invalid row: ignored, status bit set, assignment -1
+    bad = fr.clusters.copy()
+    bad["row"][5] = 999
+    fb = synth.Frame(bad, fr.sector_offsets, fr.truth, fr.track_par, 36, "bad")
+    run_gpu(fb, row_x, t)
+    assert t.header()["status"] & 4 and t.assignment()[5] == -1
+    # n > max_clusters is refused
+    big = synth.generate(synth.config(2, scale=0.05, seed=3))
+    with pytest.raises(B.TpccaError):
+        run_gpu(big, row_x, t)
+
+
+def test_capacity_overflow_is_flagged(row_x):
+    fr = synth.generate(synth.config(2, scale=0.1, seed=4))
+    t = B.Tracker(row_x, max_clusters=fr.n, max_tracklets=64, max_tracks=16)
+    run_gpu(fr, row_x, t)
+    hd = t.header()
+    assert hd["status"] & 1 and hd["n_start_hits"] == 64 and hd["n_tracks"] <= 16
+    assert t.assignment().max() < 16
+
+
+def test_host_api_equals_device_api(row_x):
+    import torch
+    fr = synth.generate(synth.config(2, scale=0.2, seed=12))
+    t = run_gpu(fr, row_x)
+    a0, tr0 = t.assignment(), t.tracks()
+    hc = torch.from_numpy(fr.clusters.view(np.uint8).reshape(-1).copy()).pin_memory()
+    ot = torch.empty(16 + 128 * t.max_tracks, dtype=torch.uint8).pin_memory()
+    oa = torch.empty(fr.n, dtype=torch.int32).pin_memory()
+    t.track_host(hc, fr.n, fr.sector_offsets, ot, oa)
+    nt = int(ot[:16].numpy().view(B.HEADER_DTYPE)["n_tracks"][0])
+    assert nt == len(tr0)
+    assert np.array_equal(oa.numpy(), a0)
+    assert ot[16:16 + 128 * nt].numpy().tobytes() == tr0.tobytes()
+
+
+def test_permutation_invariance_gpu(row_x):
+    fr = synth.generate(synth.config(2, scale=0.1, seed=30))
+    fp, p = synth.permute_within_sectors(fr, seed=5)
+    a = run_gpu(fr, row_x)
+    b = run_gpu(fp, row_x)
+    assert np.array_equal(b.assignment(), a.assignment()[p])
+    assert b.tracks().tobytes() == a.tracks().tobytes()
