@@ -129,12 +129,20 @@ enum tpcca_intermediate {
 };
 int tpcca_get_intermediate(tpcca_handle* h, int what, void* dst_device, size_t bytes, void* stream);
 
-/* Per-stage device times of the last tpcca_track when profiling is on (CUDA events on the call's
- * stream; synchronises those events).  ms: host float[TPCCA_N_STAGES]. */
+/* Per-stage device times, averaged over the tpcca_track calls (at most the last 32) made since profiling
+ * was switched on (CUDA events recorded on each call's stream; synchronises those events).  ms: host float[TPCCA_N_STAGES]. */
 enum { TPCCA_STAGE_GRID = 0, TPCCA_STAGE_NEIGHBOURS, TPCCA_STAGE_CLEAN_START, TPCCA_STAGE_TRACKLETS,
        TPCCA_STAGE_SELECT, TPCCA_STAGE_REFIT, TPCCA_N_STAGES };
 int tpcca_set_profiling(tpcca_handle* h, int on);
 int tpcca_get_stage_ms(tpcca_handle* h, float* ms);
+
+/* Device-side work counters of the last tpcca_track (synchronises `stream`): host int64[TPCCA_N_WORK]. */
+enum { TPCCA_WORK_N_BINS = 0,      /* grid bins of the frame */
+       TPCCA_WORK_ROW_STEPS,       /* Kalman row steps (transport attempts) taken by the tracklet constructor */
+       TPCCA_WORK_SEARCHES,        /* pick-up searches (grid look-ups) by the tracklet constructor */
+       TPCCA_WORK_TRACK_HITS,      /* hits owned by accepted tracks */
+       TPCCA_N_WORK };
+int tpcca_get_stats(tpcca_handle* h, int64_t* stats, void* stream);
 
 /* Kernels launched by the last tpcca_track / tpcca_track_host on this handle. */
 int tpcca_last_launch_count(tpcca_handle* h);

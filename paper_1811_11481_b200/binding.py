@@ -72,6 +72,8 @@ def load():
         lib.tpcca_set_profiling.argtypes = [C.c_void_p, C.c_int]
         lib.tpcca_get_stage_ms.restype = C.c_int
         lib.tpcca_get_stage_ms.argtypes = [C.c_void_p, C.c_void_p]
+        lib.tpcca_get_stats.restype = C.c_int
+        lib.tpcca_get_stats.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         lib.tpcca_last_launch_count.restype = C.c_int
         lib.tpcca_last_launch_count.argtypes = [C.c_void_p]
         lib.tpcca_last_error.restype = C.c_char_p
@@ -210,6 +212,11 @@ class Tracker:
         ms = (C.c_float * len(STAGES))()
         self._check(self.lib.tpcca_get_stage_ms(self.h, ms))
         return dict(zip(STAGES, [float(v) for v in ms]))
+
+    def stats(self) -> dict:
+        st = (C.c_int64 * 4)()
+        self._check(self.lib.tpcca_get_stats(self.h, st, self._stream()))
+        return dict(n_bins=int(st[0]), row_steps=int(st[1]), searches=int(st[2]), track_hits=int(st[3]))
 
     def launch_count(self) -> int:
         return int(self.lib.tpcca_last_launch_count(self.h))

@@ -11,6 +11,7 @@
 static thread_local char g_err[512] = "";
 static void set_err(const char* fmt, const char* a = "", long long b = 0) { snprintf(g_err, sizeof(g_err), fmt, a, b); }
 
+#define PROF_RING 32
 struct tpcca_handle {
   Dev d;
   tpcca_geometry geo;
@@ -23,7 +24,8 @@ struct tpcca_handle {
   int64_t last_n;
   int launches;
   bool profiling, have_times;
-  cudaEvent_t ev[TPCCA_N_STAGES + 1];
+  int prof_calls;
+  cudaEvent_t ev[PROF_RING][TPCCA_N_STAGES + 1];
 };
 
 static size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
@@ -148,8 +150,9 @@ tpcca_handle* tpcca_init(const tpcca_geometry* g, float bz_tesla, const tpcca_pa
     delete h;
     return nullptr;
   }
-  for (int i = 0; i <= TPCCA_N_STAGES; i++)
-    if (cudaEventCreate(&h->ev[i]) != cudaSuccess) { set_err("cudaEventCreate failed"); delete h; return nullptr; }
+  for (int k = 0; k < PROF_RING; k++)
+    for (int i = 0; i <= TPCCA_N_STAGES; i++)
+      if (cudaEventCreate(&h->ev[k][i]) != cudaSuccess) { set_err("cudaEventCreate failed"); delete h; return nullptr; }
   return h;
 }
 
@@ -171,20 +174,22 @@ static int track_impl(tpcca_handle* h, const tpcca_cluster* clusters, int64_t n,
   h->d.n = d.n; h->d.clusters = d.clusters; h->d.out_hdr = d.out_hdr; h->d.out_tracks = d.out_tracks; h->d.out_assign = out_assign;
   h->last_n = n;
   const bool prof = h->profiling;
-  if (prof) cudaEventRecord(h->ev[0], st);
+  cudaEvent_t* ev = h->ev[h->prof_calls % PROF_RING];
+  if (prof) cudaEventRecord(ev[0], st);
   launch_grid(d, so, L);
-  if (prof) cudaEventRecord(h->ev[1], st);
+  if (prof) cudaEventRecord(ev[1], st);
   launch_neighbours(d, L);
-  if (prof) cudaEventRecord(h->ev[2], st);
+  if (prof) cudaEventRecord(ev[2], st);
   launch_clean_start(d, L);
-  if (prof) cudaEventRecord(h->ev[3], st);
+  if (prof) cudaEventRecord(ev[3], st);
   launch_tracklets(d, L);
-  if (prof) cudaEventRecord(h->ev[4], st);
+  if (prof) cudaEventRecord(ev[4], st);
   launch_select(d, L);
-  if (prof) cudaEventRecord(h->ev[5], st);
+  if (prof) cudaEventRecord(ev[5], st);
   launch_refit(d, L);
-  if (prof) cudaEventRecord(h->ev[6], st);
-  h->have_times = prof;
+  if (prof) cudaEventRecord(ev[6], st);
+  if (prof) h->prof_calls++;
+  h->have_times = prof && h->prof_calls > 0;
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) { set_err("kernel launch failed: %s", cudaGetErrorString(e)); return TPCCA_ERR_CUDA; }
   return TPCCA_OK;
@@ -262,16 +267,38 @@ int tpcca_get_intermediate(tpcca_handle* h, int what, void* dst, size_t bytes, v
 int tpcca_set_profiling(tpcca_handle* h, int on) {
   if (!h) return TPCCA_ERR_NOT_INIT;
   h->profiling = on != 0;
-  h->have_times = false;
+  if (on) { h->have_times = false; h->prof_calls = 0; }
   return TPCCA_OK;
 }
 
 int tpcca_get_stage_ms(tpcca_handle* h, float* ms) {
   if (!h) return TPCCA_ERR_NOT_INIT;
   if (!ms || !h->have_times) { set_err("no stage times recorded (enable profiling before tpcca_track)"); return TPCCA_ERR_ARGUMENT; }
-  if (cudaEventSynchronize(h->ev[TPCCA_N_STAGES]) != cudaSuccess) { set_err("event sync failed"); return TPCCA_ERR_CUDA; }
-  for (int i = 0; i < TPCCA_N_STAGES; i++)
-    if (cudaEventElapsedTime(&ms[i], h->ev[i], h->ev[i + 1]) != cudaSuccess) { set_err("event elapsed failed"); return TPCCA_ERR_CUDA; }
+  const int nc = h->prof_calls < PROF_RING ? h->prof_calls : PROF_RING;
+  for (int i = 0; i < TPCCA_N_STAGES; i++) ms[i] = 0.0f;
+  for (int c = 0; c < nc; c++) {
+    cudaEvent_t* ev = h->ev[(h->prof_calls - 1 - c) % PROF_RING];
+    if (cudaEventSynchronize(ev[TPCCA_N_STAGES]) != cudaSuccess) { set_err("event sync failed"); return TPCCA_ERR_CUDA; }
+    for (int i = 0; i < TPCCA_N_STAGES; i++) {
+      float t = 0.0f;
+      if (cudaEventElapsedTime(&t, ev[i], ev[i + 1]) != cudaSuccess) { set_err("event elapsed failed"); return TPCCA_ERR_CUDA; }
+      ms[i] += t / (float)nc;
+    }
+  }
+  return TPCCA_OK;
+}
+
+int tpcca_get_stats(tpcca_handle* h, int64_t* stats, void* stream) {
+  if (!h) { set_err("handle is null (not initialised)"); return TPCCA_ERR_NOT_INIT; }
+  if (!stats) { set_err("stats is null"); return TPCCA_ERR_ARGUMENT; }
+  DevCounters c;
+  cudaError_t e = cudaMemcpyAsync(&c, h->d.cnt, sizeof(c), cudaMemcpyDeviceToHost, (cudaStream_t)stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);
+  if (e != cudaSuccess) { set_err("stats copy failed: %s", cudaGetErrorString(e)); cudaGetLastError(); return TPCCA_ERR_CUDA; }
+  stats[TPCCA_WORK_N_BINS] = c.n_bins;
+  stats[TPCCA_WORK_ROW_STEPS] = (int64_t)c.row_steps;
+  stats[TPCCA_WORK_SEARCHES] = (int64_t)c.searches;
+  stats[TPCCA_WORK_TRACK_HITS] = (int64_t)c.track_hits;
   return TPCCA_OK;
 }
 
@@ -281,8 +308,9 @@ const char* tpcca_last_error(void) { return g_err; }
 
 void tpcca_free(tpcca_handle* h) {
   if (!h) return;
-  for (int i = 0; i <= TPCCA_N_STAGES; i++)
-    if (h->ev[i]) cudaEventDestroy(h->ev[i]);
+  for (int k = 0; k < PROF_RING; k++)
+    for (int i = 0; i <= TPCCA_N_STAGES; i++)
+      if (h->ev[k][i]) cudaEventDestroy(h->ev[k][i]);
   delete h;
 }
 

@@ -22,6 +22,8 @@ struct DevCounters {  // device-resident scalars
   int32_t status;
   int32_t n_bins;      // total grid bins of the frame
   int32_t pad[3];
+  unsigned long long row_steps, searches, track_hits;  // work counters (roofline units)
+  unsigned long long pad2;
 };
 
 struct SecOff { int32_t v[TPCCA_MAX_SECTORS + 1]; };

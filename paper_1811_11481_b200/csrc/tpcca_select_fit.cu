@@ -22,6 +22,7 @@ __global__ void __launch_bounds__(128) k_select_flag(Dev d) {
       else d.row_hit[(size_t)r * T + t] = -2 - h;
     }
     flag = owned >= d.P.min_track_hits ? 1 : 0;
+    if (flag) atomicAdd(&d.cnt->track_hits, (unsigned long long)owned);
   }
   d.tl_track[t] = flag;
 }

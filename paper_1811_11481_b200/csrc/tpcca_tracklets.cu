@@ -66,6 +66,7 @@ __global__ void __launch_bounds__(E_THREADS) k_tracklets(Dev d) {
   int4 ti = make_int4(0, -1, -1, 0);
   float4 tf0 = make_float4(0.f, 0.f, 0.f, 0.f), tf1 = make_float4(0.f, 0.f, 0.f, 0.f);
   unsigned long long W = 0ull;
+  int n_steps = 0, n_search = 0;  // work counters (roofline units)
 
   const float2 p0 = d.yz[h0];
   const float z_ref = p0.y;
@@ -86,6 +87,7 @@ __global__ void __launch_bounds__(E_THREADS) k_tracklets(Dev d) {
     rh[(size_t)r0 * T] = h0;
     while (h >= 0) {
       const float2 p = d.yz[h];
+      n_steps++;
       if (!kf_transport(k, d.row_x[r], d.kq, d.P.max_sinphi)) { ok = false; break; }
       kf_update(k, p.x, p.y - z_ref, d.sy2, d.sz2);
       if (r == last_row + 2) rh[(size_t)(r - 1) * T] = -1;  // skipped (empty) row
@@ -102,8 +104,10 @@ __global__ void __launch_bounds__(E_THREADS) k_tracklets(Dev d) {
     float sx = k.x, sy = k.y, sz = k.z, ss = k.s, st = k.t, sq = k.q;  // snapshot at the outermost hit
     int top_row = last_row, gap = 0;
     for (int r = last_row + 1; r < R; r++) {
+      n_steps++;
       if (!kf_transport(k, d.row_x[r], d.kq, d.P.max_sinphi)) break;
       if (fabsf(k.y) > d.row_x[r] * d.tan_half_angle + d.P.edge_margin) break;
+      n_search++;
       const int hb = search_row(d, sbase + r, k, z_ref, d.P.pick_cut);
       rh[(size_t)r * T] = hb;
       if (hb >= 0) {
@@ -123,6 +127,7 @@ __global__ void __launch_bounds__(E_THREADS) k_tracklets(Dev d) {
     int inner_row = -1, n_hits = 0, outer_row = -1;
     gap = 0;
     for (int r = top_row; r >= 0; r--) {
+      n_steps++;
       if (!kf_transport(k, d.row_x[r], d.kq, d.P.max_sinphi)) break;
       if (fabsf(k.y) > d.row_x[r] * d.tan_half_angle + d.P.edge_margin) break;
       bool hit = false;
@@ -136,6 +141,7 @@ __global__ void __launch_bounds__(E_THREADS) k_tracklets(Dev d) {
         if (dist <= d.P.reject_cut) { kf_update(k, p.x, p.y - z_ref, d.sy2, d.sz2); hit = true; }
         else rh[(size_t)r * T] = -1;
       } else {
+        n_search++;
         const int hb = search_row(d, sbase + r, k, z_ref, d.P.pick_cut);
         rh[(size_t)r * T] = hb;
         if (hb >= 0) {
@@ -163,6 +169,14 @@ __global__ void __launch_bounds__(E_THREADS) k_tracklets(Dev d) {
         if (h >= 0) atomicMax(&d.hit_weight[h], W);
       }
       atomicAdd(&d.cnt->n_valid, 1);
+    }
+  }
+  {
+    const unsigned m = __activemask();
+    const int ws = __reduce_add_sync(m, n_steps), wq = __reduce_add_sync(m, n_search);
+    if ((threadIdx.x & 31) == (__ffs(m) - 1)) {
+      atomicAdd(&d.cnt->row_steps, (unsigned long long)ws);
+      atomicAdd(&d.cnt->searches, (unsigned long long)wq);
     }
   }
   reinterpret_cast<int4*>(d.tl_ints)[t] = ti;
