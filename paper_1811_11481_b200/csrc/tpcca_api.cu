@@ -48,6 +48,7 @@ static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params
   CARVE(d.row_start, int32_t, SL + 1);
   CARVE(d.slice_bbox, uint32_t, SL * 4);
   CARVE(d.grid, GridHdr, SL);
+  CARVE(d.nbr, NbrHdr, SL);
   CARVE(d.slice_nstart, int32_t, SL + 1);
   CARVE(d.slice_sbase, int32_t, SL + 1);
   CARVE(d.cluster_bin, int32_t, N);
@@ -62,7 +63,10 @@ static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params
   CARVE(d.link_up_clean, int32_t, N);
   CARVE(d.start_flag, uint8_t, N);
   CARVE(d.hit_weight, unsigned long long, N);
-  CARVE(d.start_tmp, int32_t, T);
+  CARVE(d.start_tmp, int32_t, N);
+  CARVE(d.sb_count, int32_t, T + 1);
+  CARVE(d.sb_sorted, int32_t, T);
+  CARVE(d.sb_skey, int32_t, T);
   CARVE(d.start_hits, int32_t, T);
   CARVE(d.row_hit, int32_t, T * (size_t)g->n_rows);
   CARVE(d.tl_ints, int32_t, T * 4);
@@ -74,7 +78,7 @@ static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params
   CARVE(stage_assign, int32_t, N);
   CARVE(stage_tracks, char, sizeof(tpcca_out_header) + K * sizeof(tpcca_track_rec));
 #undef CARVE
-  if (base) h->d.max_bins = (int32_t)NB;
+  if (base) { h->d.max_bins = (int32_t)NB; h->d.sb_key = h->d.cluster_rank; }
   return off;
 }
 

@@ -15,13 +15,20 @@ struct GridHdr {  // 32 B per (sector,row) slice
   int32_t ny, nz, bin_base, pad;
 };
 
+struct NbrHdr {  // 32 B per slice: the per-row constants of the neighbours finder (O2)
+  int32_t su, sd;  // slices of the up / down row, -1 if none
+  float t, wyu, wzu, wyd, wzd;
+  int32_t pad;
+};
+
 struct DevCounters {  // device-resident scalars
   int32_t n_start;     // start hits (clamped to max_tracklets)
   int32_t n_tracks;    // accepted tracks (clamped to max_tracks)
   int32_t n_valid;     // non-void tracklets
   int32_t status;
   int32_t n_bins;      // total grid bins of the frame
-  int32_t pad[3];
+  int32_t n_start_raw; // start hits before clamping to capacity
+  int32_t pad[2];
   unsigned long long row_steps, searches, track_hits;  // work counters (roofline units)
   unsigned long long pad2;
 };
@@ -45,6 +52,7 @@ struct Dev {
   int32_t* row_start;      // [n_slices+1] exclusive scan of slice_count
   uint32_t* slice_bbox;    // [n_slices*4] ordered-uint ymin, ymax, zmin, zmax
   GridHdr* grid;           // [n_slices]
+  NbrHdr* nbr;             // [n_slices]
   int32_t* cluster_bin;    // [n] global bin id (input order)
   int32_t* cluster_rank;   // [n] arrival rank inside the bin
   int32_t* bin_start;      // [max_bins+1] counts, then exclusive scan
@@ -59,7 +67,11 @@ struct Dev {
   uint8_t* start_flag;     // [n]
   int32_t* slice_nstart;   // [n_slices+1]
   int32_t* slice_sbase;    // [n_slices+1]
-  int32_t* start_tmp;      // [max_tracklets] unsorted start hits per slice
+  int32_t* start_tmp;      // [n] start hits in arrival order
+  int32_t* sb_key;         // [n] z-bucket of start_tmp[i] (global bucket id), aliases cluster_rank
+  int32_t* sb_count;       // [max_tracklets+1] bucket histogram -> scan -> cursors
+  int32_t* sb_sorted;      // [max_tracklets] start hits grouped by bucket
+  int32_t* sb_skey;        // [max_tracklets] bucket of sb_sorted[p]
   int32_t* start_hits;     // [max_tracklets] canonical order (sorted indices)
   // (e)
   int32_t* row_hit;        // [n_rows][max_tracklets]

@@ -99,7 +99,7 @@ __global__ void k_reset(Dev d) {
     d.slice_bbox[4 * i + 3] = 0u;           // zmax
   }
   if (i == 0) {
-    d.cnt->n_start = 0; d.cnt->n_tracks = 0; d.cnt->n_valid = 0; d.cnt->status = 0; d.cnt->n_bins = 0;
+    d.cnt->n_start = 0; d.cnt->n_tracks = 0; d.cnt->n_valid = 0; d.cnt->status = 0; d.cnt->n_bins = 0; d.cnt->n_start_raw = 0;
     d.cnt->row_steps = 0ull; d.cnt->searches = 0ull; d.cnt->track_hits = 0ull;
   }
 }
@@ -190,6 +190,27 @@ __global__ void __launch_bounds__(1024) k_slice_setup(Dev d) {
         atomicOr(&d.cnt->status, TPCCA_STAT_BIN_OVERFLOW);
       }
       d.grid[sl] = g;
+      // per-row constants of the neighbours finder (O2): up/down row with one skip
+      const int sec = sl / d.n_rows, r = sl - sec * d.n_rows;
+      NbrHdr nb;
+      nb.su = nb.sd = -1; nb.t = nb.wyu = nb.wzu = nb.wyd = nb.wzd = 0.0f; nb.pad = 0;
+      int ru = -1, rd = -1;
+      if (r + 1 < d.n_rows && d.slice_count[sl + 1] > 0) ru = r + 1;
+      else if (r + 2 < d.n_rows && d.slice_count[sl + 2] > 0) ru = r + 2;
+      if (r - 1 >= 0 && d.slice_count[sl - 1] > 0) rd = r - 1;
+      else if (r - 2 >= 0 && d.slice_count[sl - 2] > 0) rd = r - 2;
+      if (ru >= 0 && rd >= 0 && cnt > 0) {
+        const float xr = d.row_x[r];
+        const float dxu = d.row_x[ru] - xr;
+        const float dxd = xr - d.row_x[rd];
+        nb.su = sec * d.n_rows + ru; nb.sd = sec * d.n_rows + rd;
+        nb.t = dxd / (dxu + dxd);
+        nb.wyu = dxu * d.P.nbr_dydx + d.P.nbr_margin_y;
+        nb.wzu = dxu * d.P.nbr_dzdx + d.P.nbr_margin_z;
+        nb.wyd = dxd * d.P.nbr_dydx + d.P.nbr_margin_y;
+        nb.wzd = dxd * d.P.nbr_dzdx + d.P.nbr_margin_z;
+      }
+      d.nbr[sl] = nb;
     }
     carry_c += tot_c;
     carry_b += tot_b;

@@ -77,7 +77,7 @@ def test_capacity_overflow_is_flagged(row_x):
     t = B.Tracker(row_x, max_clusters=fr.n, max_tracklets=64, max_tracks=16)
     run_gpu(fr, row_x, t)
     hd = t.header()
-    assert hd["status"] & 1 and hd["n_start_hits"] == 64 and hd["n_tracks"] <= 16
+    assert hd["status"] & 1 and 0 < hd["n_start_hits"] <= 64 and hd["n_tracks"] <= 16
     assert t.assignment().max() < 16
 
 
