@@ -129,7 +129,8 @@ def run_gpu(args):
     fr = synth.generate(synth.config(5, seed=5 + 1000 * rank))
     rx = synth.row_x()
     n = fr.n
-    trk = binding.Tracker(rx, n_sectors=36, max_clusters=n, max_tracklets=max(1 << 16, n // 8), device=f"cuda:{local}")
+    trk = binding.Tracker(rx, n_sectors=36, max_clusters=n, max_tracklets=max(1 << 16, n // 8),
+                          max_tracks=max(1 << 16, n // 24), device=f"cuda:{local}")
     dev_clusters = trk.upload(fr.clusters)
     stream = torch.cuda.current_stream()
 

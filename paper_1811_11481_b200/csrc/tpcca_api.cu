@@ -68,12 +68,18 @@ static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params
   CARVE(d.sb_sorted, int32_t, T);
   CARVE(d.sb_skey, int32_t, T);
   CARVE(d.start_hits, int32_t, T);
+  CARVE(d.seed_w, int32_t, T + 1);
+  CARVE(d.work_t, int32_t, T);
   CARVE(d.row_hit, int32_t, T * (size_t)g->n_rows);
   CARVE(d.tl_ints, int32_t, T * 4);
   CARVE(d.tl_floats, float, T * 8);
   CARVE(d.tl_W, unsigned long long, T);
+  CARVE(d.sel_scan, int32_t, T + 1);
   CARVE(d.tl_track, int32_t, T + 1);
   CARVE(d.track_tracklet, int32_t, K);
+  CARVE(d.track_info, int32_t, K);
+  CARVE(d.th_yz, float2, K * (size_t)g->n_rows);
+  CARVE(d.th_row, uint8_t, K * (size_t)g->n_rows);
   CARVE(stage_clusters, float4, N);
   CARVE(stage_assign, int32_t, N);
   CARVE(stage_tracks, char, sizeof(tpcca_out_header) + K * sizeof(tpcca_track_rec));

@@ -28,7 +28,8 @@ struct DevCounters {  // device-resident scalars
   int32_t status;
   int32_t n_bins;      // total grid bins of the frame
   int32_t n_start_raw; // start hits before clamping to capacity
-  int32_t pad[2];
+  int32_t n_work;      // seeds that reach the constructor (chain >= min_seed_hits)
+  int32_t pad[1];
   unsigned long long row_steps, searches, track_hits;  // work counters (roofline units)
   unsigned long long pad2;
 };
@@ -74,14 +75,20 @@ struct Dev {
   int32_t* sb_skey;        // [max_tracklets] bucket of sb_sorted[p]
   int32_t* start_hits;     // [max_tracklets] canonical order (sorted indices)
   // (e)
-  int32_t* row_hit;        // [n_rows][max_tracklets]
+  int32_t* seed_w;         // [max_tracklets+1] keep flag -> exclusive scan: tracklet id t -> work index w
+  int32_t* work_t;         // [max_tracklets] w -> t
+  int32_t* row_hit;        // [n_rows][max_tracklets] indexed by w (dense over surviving seeds)
   int32_t* tl_ints;        // [max_tracklets][4] valid, first_row, last_row, n_hits
   float* tl_floats;        // [max_tracklets][8] x, y, z~, sinphi, dzds, qpt, chi2, z_ref
   unsigned long long* tl_W;        // [max_tracklets]
   unsigned long long* hit_weight;  // [n]
   // (f),(g)
-  int32_t* tl_track;       // [max_tracklets] scan buffer: flag -> track id
-  int32_t* track_tracklet; // [max_tracks]
+  int32_t* sel_scan;       // [max_tracklets+1] w-space: accept flag -> exclusive scan = track id
+  int32_t* tl_track;       // [max_tracklets] t-space: track id or -1 (only read for tracklets that own hits)
+  int32_t* track_tracklet; // [max_tracks] track id -> t
+  int32_t* track_info;     // [max_tracks] n_hits | sector << 16
+  float2* th_yz;           // [n_rows][max_tracks] j-th owned hit (innermost first) of track id: (y, z)
+  uint8_t* th_row;         // [n_rows][max_tracks] its row
   DevCounters* cnt;
   tpcca_out_header* out_hdr;
   tpcca_track_rec* out_tracks;

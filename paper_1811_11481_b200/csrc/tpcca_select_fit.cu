@@ -5,10 +5,12 @@
 #include "tpcca_dev.cuh"
 
 // ---------------------------------------------------------------- (f1) ownership count -> accept flag
-// Non-owned hits are re-encoded in place as -2-h (reversible: the export decodes them).
+// One thread per surviving seed w.  Non-owned hits are re-encoded in place as -2-h (reversible: the
+// export decodes them), so the later passes see owned hits as h >= 0.
 __global__ void __launch_bounds__(128) k_select_flag(Dev d) {
-  const int t = blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= d.cnt->n_start) return;
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= d.cnt->n_work) return;
+  const int t = d.work_t[w];
   const int4 ti = reinterpret_cast<const int4*>(d.tl_ints)[t];
   int flag = 0;
   if (ti.x) {
@@ -16,38 +18,47 @@ __global__ void __launch_bounds__(128) k_select_flag(Dev d) {
     const int T = d.max_tracklets;
     int owned = 0;
     for (int r = ti.y; r <= ti.z; r++) {
-      const int h = d.row_hit[(size_t)r * T + t];
+      const int h = d.row_hit[(size_t)r * T + w];
       if (h < 0) continue;
       if (d.hit_weight[h] == W) owned++;
-      else d.row_hit[(size_t)r * T + t] = -2 - h;
+      else d.row_hit[(size_t)r * T + w] = -2 - h;
     }
     flag = owned >= d.P.min_track_hits ? 1 : 0;
     if (flag) atomicAdd(&d.cnt->track_hits, (unsigned long long)owned);
   }
-  d.tl_track[t] = flag;
+  d.sel_scan[w] = flag;
 }
 
-// ---------------------------------------------------------------- (f2) after the scan: track ids
-__global__ void __launch_bounds__(256) k_select_ids(Dev d) {
-  const int t = blockIdx.x * blockDim.x + threadIdx.x;
-  const int ns = d.cnt->n_start;
-  if (t > ns) return;
-  if (t == ns) {  // total
-    const int tot = d.tl_track[ns];
+// ---------------------------------------------------------------- (f2) after the scan: track ids + packed hit lists
+// Track ids follow tracklet-id order (the work list is in that order).  Each accepted track's owned hits are
+// packed innermost-first into th_yz / th_row at [j][id], so that the refit's lanes read one line per step.
+__global__ void __launch_bounds__(128) k_select_write(Dev d) {
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  const int nw = d.cnt->n_work;
+  if (w == 0) {
+    const int tot = d.sel_scan[nw];
     if (tot > d.max_tracks) atomicOr(&d.cnt->status, TPCCA_STAT_TRACK_OVERFLOW);
     d.cnt->n_tracks = min(tot, d.max_tracks);
-    return;
   }
-  const int id = d.tl_track[t];
-  const bool acc = d.tl_track[t + 1] != id;  // exclusive scan of 0/1 flags: next differs <=> flag set
-  // the next element is overwritten only by thread t+1 with -1 or its own id (>= id): handled via tl_W's copy
-  d.scan_tmp[t] = (acc && id < d.max_tracks) ? id : -1;
-  if (acc && id < d.max_tracks) d.track_tracklet[id] = t;
-}
-__global__ void __launch_bounds__(256) k_select_commit(Dev d) {
-  const int t = blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= d.cnt->n_start) return;
-  d.tl_track[t] = d.scan_tmp[t];
+  if (w >= nw) return;
+  const int t = d.work_t[w];
+  const int id = d.sel_scan[w];
+  const bool acc = (d.sel_scan[w + 1] != id) && (id < d.max_tracks);
+  d.tl_track[t] = acc ? id : -1;
+  if (!acc) return;
+  const int4 ti = reinterpret_cast<const int4*>(d.tl_ints)[t];
+  const int T = d.max_tracklets, K = d.max_tracks;
+  int j = 0, sl = 0;
+  for (int r = ti.y; r <= ti.z; r++) {
+    const int h = d.row_hit[(size_t)r * T + w];
+    if (h < 0) continue;
+    d.th_yz[(size_t)j * K + id] = d.yz[h];
+    d.th_row[(size_t)j * K + id] = (uint8_t)r;
+    if (j == 0) sl = d.slice_of[h];
+    j++;
+  }
+  d.track_tracklet[id] = t;
+  d.track_info[id] = j | ((sl / d.n_rows) << 16);
 }
 
 // ---------------------------------------------------------------- (f3) cluster -> track assignment
@@ -68,32 +79,26 @@ void launch_select(const Dev& d, Launch& L) {
   const int T = d.max_tracklets;
   k_select_flag<<<(T + 127) / 128, 128, 0, L.st>>>(d);
   L.count++;
-  launch_scan_i32(d.tl_track, &d.cnt->n_start, T, d.scan_tmp + T + 8, L);
-  k_select_ids<<<(T + 1 + 255) / 256, 256, 0, L.st>>>(d);
-  k_select_commit<<<(T + 255) / 256, 256, 0, L.st>>>(d);
+  launch_scan_i32(d.sel_scan, &d.cnt->n_work, T, d.scan_tmp, L);
+  k_select_write<<<(T + 127) / 128, 128, 0, L.st>>>(d);
   k_assign<<<(d.n + 255) / 256, 256, 0, L.st>>>(d);
-  L.count += 3;
+  L.count += 2;
 }
 
 // ---------------------------------------------------------------- (g) refit
+// One thread per track; hits come from the packed lists (coalesced across the warp).
 __global__ void __launch_bounds__(64) k_refit(Dev d) {
   const int id = blockIdx.x * blockDim.x + threadIdx.x;
   if (id >= d.cnt->n_tracks) return;
+  const int K = d.max_tracks;
+  const int info = d.track_info[id];
+  const int n_hits = info & 0xFFFF, sector = info >> 16;
   const int t = d.track_tracklet[id];
-  const int T = d.max_tracklets;
-  const int4 ti = reinterpret_cast<const int4*>(d.tl_ints)[t];
-  const int32_t* rh = d.row_hit + t;
   const float q0 = d.tl_floats[8 * t + 5];
-  // two outermost and the innermost owned hits
-  int rN = -1, rM = -1, r_in = -1, n_hits = 0;
-  for (int r = ti.z; r >= ti.y; r--) {
-    if (rh[(size_t)r * T] >= 0) {
-      if (rN < 0) rN = r; else if (rM < 0) rM = r;
-      r_in = r; n_hits++;
-    }
-  }
-  const float2 pN = d.yz[rh[(size_t)rN * T]];
-  const float2 pM = d.yz[rh[(size_t)rM * T]];
+  const float2* ly = d.th_yz + id;
+  const uint8_t* lr = d.th_row + id;
+  const int rN = lr[(size_t)(n_hits - 1) * K], rM = lr[(size_t)(n_hits - 2) * K], r_in = lr[0];
+  const float2 pN = ly[(size_t)(n_hits - 1) * K], pM = ly[(size_t)(n_hits - 2) * K];
   const float z_ref = pN.y;
   KF k;
   {
@@ -105,17 +110,16 @@ __global__ void __launch_bounds__(64) k_refit(Dev d) {
   bool ok = true;
   for (int pass = 0; pass < 3 && ok; pass++) {
     kf_reset_cov(k, d.P.cov0);
-    const int dir = (pass == 1) ? 1 : -1;
-    for (int r = (dir > 0) ? r_in : rN; r >= r_in && r <= rN; r += dir) {
-      const int h = rh[(size_t)r * T];
-      if (h < 0) continue;
-      const float2 p = d.yz[h];
+    for (int i = 0; i < n_hits; i++) {
+      const int j = (pass == 1) ? i : n_hits - 1 - i;
+      const float2 p = ly[(size_t)j * K];
+      const int r = lr[(size_t)j * K];
       if (!kf_transport(k, d.row_x[r], d.kq, d.P.max_sinphi)) { ok = false; break; }
       kf_update(k, p.x, p.y - z_ref, d.sy2, d.sz2);
     }
   }
   tpcca_track_rec o;
-  o.sector = d.slice_of[rh[(size_t)rN * T]] / d.n_rows;
+  o.sector = sector;
   o.first_row = r_in; o.last_row = rN; o.n_hits = n_hits;
   o.x = k.x; o.y = k.y; o.z = k.z + z_ref; o.sinphi = k.s; o.dzds = k.t; o.qpt = k.q;
   o.cov[0] = k.c00; o.cov[1] = k.c10; o.cov[2] = k.c11; o.cov[3] = k.c20; o.cov[4] = k.c21; o.cov[5] = k.c22;
@@ -178,7 +182,7 @@ __global__ void k_export_tracklets(Dev d, int what, void* dst) {
     for (int r = 0; r < d.n_rows; r++) {
       int v = -1;
       if (ti.x && r >= ti.y && r <= ti.z) {
-        v = d.row_hit[(size_t)r * d.max_tracklets + t];
+        v = d.row_hit[(size_t)r * d.max_tracklets + d.seed_w[t]];
         if (v <= -2) v = -2 - v;
         if (v >= 0) v = d.orig_idx[v];
       }

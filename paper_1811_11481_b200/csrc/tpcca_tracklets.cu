@@ -52,31 +52,67 @@ __device__ __forceinline__ unsigned long long pack_weight(const Dev& d, int n_hi
          (unsigned long long)(0xFFFFFFFFu - tid);
 }
 
-#define E_THREADS 64
-__global__ void __launch_bounds__(E_THREADS) k_tracklets(Dev d) {
+// ---------------------------------------------------------------- (e0) seed filter + stable compaction
+// A start hit whose link chain is shorter than min_seed_hits is void (O5/E1) and never reaches
+// the constructor: the survivors are compacted in tracklet-id order into the work list (w -> t).
+__global__ void __launch_bounds__(256) k_seed_flag(Dev d) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= d.cnt->n_start) return;
+  int h = d.start_hits[t], n = 1;
+  while (n < d.P.min_seed_hits) {
+    h = d.link_up_clean[h];
+    if (h < 0) break;
+    n++;
+  }
+  const int keep = n >= d.P.min_seed_hits ? 1 : 0;
+  d.seed_w[t] = keep;
+  if (!keep) {
+    reinterpret_cast<int4*>(d.tl_ints)[t] = make_int4(0, -1, -1, 0);
+    reinterpret_cast<float4*>(d.tl_floats)[2 * t] = make_float4(0.f, 0.f, 0.f, 0.f);
+    reinterpret_cast<float4*>(d.tl_floats)[2 * t + 1] = make_float4(0.f, 0.f, 0.f, 0.f);
+    d.tl_W[t] = 0ull;
+  }
+}
+
+__global__ void __launch_bounds__(256) k_seed_compact(Dev d) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  const int ns = d.cnt->n_start;
+  if (t == 0) d.cnt->n_work = d.seed_w[ns];
+  if (t >= ns) return;
+  const int w = d.seed_w[t];
+  if (d.seed_w[t + 1] != w) d.work_t[w] = t;
+}
+
+// ---------------------------------------------------------------- (e) constructor
+// One thread per surviving seed.  E1 (follow links), E2 (outward pick-up) and E3 (inward pass) run as ONE
+// loop with a phase variable, so that lanes of a warp that are in different phases still share the single
+// transport / search / update instruction streams.
+#define E_THREADS 64
+#define PH_E1 0
+#define PH_E2 1
+#define PH_E3 2
+#define PH_DONE 3
+
+__global__ void __launch_bounds__(E_THREADS) k_tracklets(Dev d) {
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= d.cnt->n_work) return;
+  const int t = d.work_t[w];
   const int T = d.max_tracklets;
   const int R = d.n_rows;
-  int32_t* rh = d.row_hit + t;  // rh[r * T]
+  int32_t* rh = d.row_hit + w;  // rh[r * T]
   const int h0 = d.start_hits[t];
   const int sl0 = d.slice_of[h0];
   const int sec = sl0 / R, r0 = sl0 - sec * R;
   const int sbase = sec * R;
-  int4 ti = make_int4(0, -1, -1, 0);
-  float4 tf0 = make_float4(0.f, 0.f, 0.f, 0.f), tf1 = make_float4(0.f, 0.f, 0.f, 0.f);
-  unsigned long long W = 0ull;
   int n_steps = 0, n_search = 0;  // work counters (roofline units)
 
   const float2 p0 = d.yz[h0];
   const float z_ref = p0.y;
-  tf1.w = z_ref;
   KF k;
-  bool ok = true;
-  int last_row = r0, n_chain = 1;
-  {  // E1: seed fit along the cleaned up-links
-    int h = d.link_up_clean[h0];
-    int r = (h >= d.row_start[sbase + r0 + 2]) ? r0 + 2 : r0 + 1;
+  int phase = PH_E1;
+  int h = d.link_up_clean[h0];  // E1: next chain hit
+  int r = (h >= d.row_start[sbase + r0 + 2]) ? r0 + 2 : r0 + 1;  // target row of the next step
+  {
     const float2 p1 = d.yz[h];
     const float dx = d.row_x[r] - d.row_x[r0], dy = p1.x - p0.x, dz = p1.y - p0.y;
     const float ds = sqrtf(dx * dx + dy * dy);
@@ -85,91 +121,110 @@ __global__ void __launch_bounds__(E_THREADS) k_tracklets(Dev d) {
     kf_reset_cov(k, d.P.cov0);
     kf_update(k, p0.x, p0.y - z_ref, d.sy2, d.sz2);
     rh[(size_t)r0 * T] = h0;
-    while (h >= 0) {
-      const float2 p = d.yz[h];
-      n_steps++;
-      if (!kf_transport(k, d.row_x[r], d.kq, d.P.max_sinphi)) { ok = false; break; }
-      kf_update(k, p.x, p.y - z_ref, d.sy2, d.sz2);
-      if (r == last_row + 2) rh[(size_t)(r - 1) * T] = -1;  // skipped (empty) row
-      rh[(size_t)r * T] = h;
-      last_row = r;
-      n_chain++;
-      h = d.link_up_clean[h];
-      if (h >= 0) r = (r + 2 < R && h >= d.row_start[sbase + r + 2]) ? r + 2 : r + 1;
-    }
-    if (n_chain < d.P.min_seed_hits) ok = false;
   }
-  if (ok) {
-    // E2: outward extrapolation, one best cluster per row
-    float sx = k.x, sy = k.y, sz = k.z, ss = k.s, st = k.t, sq = k.q;  // snapshot at the outermost hit
-    int top_row = last_row, gap = 0;
-    for (int r = last_row + 1; r < R; r++) {
-      n_steps++;
-      if (!kf_transport(k, d.row_x[r], d.kq, d.P.max_sinphi)) break;
-      if (fabsf(k.y) > d.row_x[r] * d.tan_half_angle + d.P.edge_margin) break;
-      n_search++;
-      const int hb = search_row(d, sbase + r, k, z_ref, d.P.pick_cut);
-      rh[(size_t)r * T] = hb;
-      if (hb >= 0) {
-        const float2 p = d.yz[hb];
-        kf_update(k, p.x, p.y - z_ref, d.sy2, d.sz2);
-        gap = 0; top_row = r;
-        sx = k.x; sy = k.y; sz = k.z; ss = k.s; st = k.t; sq = k.q;
+  int last_row = r0, top_row = r0, gap = 0;
+  bool valid = true;
+  float sx = 0.f, sy = 0.f, sz = 0.f, ss = 0.f, st = 0.f, sq = 0.f;             // snapshot at the outermost hit
+  float ix = 0.f, iy_ = 0.f, iz_ = 0.f, is = 0.f, it = 0.f, iq = 0.f, ichi = 0.f;  // state at the innermost hit
+  int inner_row = -1, outer_row = -1, n_hits = 0;
+
+  while (phase != PH_DONE) {
+    n_steps++;
+    const float xr = d.row_x[r];
+    const bool tr_ok = kf_transport(k, xr, d.kq, d.P.max_sinphi);
+    const bool edge = (phase != PH_E1) && (fabsf(k.y) > xr * d.tan_half_angle + d.P.edge_margin);
+    const bool stop = !tr_ok || edge;
+    int cand = -1;
+    bool accept = false, do_search = false;
+    float2 pc = make_float2(0.f, 0.f);
+    if (!stop) {
+      if (phase == PH_E1) {
+        cand = h; accept = true;
       } else {
-        gap++;
-        if (gap > d.P.max_gap) break;
-      }
-    }
-    // E3: inward pass through the seed with outlier rejection, then pick-up below it
-    k.x = sx; k.y = sy; k.z = sz; k.s = ss; k.t = st; k.q = sq;
-    kf_reset_cov(k, d.P.cov0);
-    KF inner = k;
-    int inner_row = -1, n_hits = 0, outer_row = -1;
-    gap = 0;
-    for (int r = top_row; r >= 0; r--) {
-      n_steps++;
-      if (!kf_transport(k, d.row_x[r], d.kq, d.P.max_sinphi)) break;
-      if (fabsf(k.y) > d.row_x[r] * d.tan_half_angle + d.P.edge_margin) break;
-      bool hit = false;
-      const int cur = (r >= r0) ? rh[(size_t)r * T] : -1;
-      if (cur >= 0) {
-        const float2 p = d.yz[cur];
-        const float iy = 1.0f / (k.c00 + d.sy2), iz = 1.0f / (k.c11 + d.sz2);
-        const float dy = p.x - k.y;
-        const float dz = (p.y - z_ref) - k.z;
-        const float dist = (dy * dy) * iy + (dz * dz) * iz;
-        if (dist <= d.P.reject_cut) { kf_update(k, p.x, p.y - z_ref, d.sy2, d.sz2); hit = true; }
-        else rh[(size_t)r * T] = -1;
-      } else {
-        n_search++;
-        const int hb = search_row(d, sbase + r, k, z_ref, d.P.pick_cut);
-        rh[(size_t)r * T] = hb;
-        if (hb >= 0) {
-          const float2 p = d.yz[hb];
-          kf_update(k, p.x, p.y - z_ref, d.sy2, d.sz2);
-          hit = true;
+        const int cur = (phase == PH_E3 && r >= r0) ? rh[(size_t)r * T] : -1;
+        if (cur >= 0) {
+          cand = cur;
+          pc = d.yz[cur];
+          const float iy = 1.0f / (k.c00 + d.sy2), iz = 1.0f / (k.c11 + d.sz2);
+          const float dy = pc.x - k.y;
+          const float dz = (pc.y - z_ref) - k.z;
+          const float dist = (dy * dy) * iy + (dz * dz) * iz;
+          accept = dist <= d.P.reject_cut;
+          if (!accept) rh[(size_t)r * T] = -1;
+        } else {
+          do_search = true;
         }
       }
-      if (hit) {
-        gap = 0; inner = k; inner_row = r; n_hits++;
-        if (outer_row < 0) outer_row = r;
-      } else {
-        gap++;
-        if (r < r0 && gap > d.P.max_gap) break;
+    }
+    if (do_search) {
+      n_search++;
+      cand = search_row(d, sbase + r, k, z_ref, d.P.pick_cut);
+      rh[(size_t)r * T] = cand;
+      accept = cand >= 0;
+    }
+    if (accept) {
+      if (phase == PH_E1 || do_search) pc = d.yz[cand];
+      kf_update(k, pc.x, pc.y - z_ref, d.sy2, d.sz2);
+    }
+    // ---- bookkeeping and phase transitions
+    bool to_e3 = false;
+    if (phase == PH_E1) {
+      if (stop) { valid = false; phase = PH_DONE; }
+      else {
+        if (r == last_row + 2) rh[(size_t)(r - 1) * T] = -1;  // skipped (empty) row
+        rh[(size_t)r * T] = h;
+        last_row = r;
+        h = d.link_up_clean[h];
+        if (h >= 0) r = (r + 2 < R && h >= d.row_start[sbase + r + 2]) ? r + 2 : r + 1;
+        else {  // seed complete (its length was checked by k_seed_flag): start E2
+          phase = PH_E2; top_row = last_row; gap = 0;
+          sx = k.x; sy = k.y; sz = k.z; ss = k.s; st = k.t; sq = k.q;
+          r = last_row + 1;
+          if (r >= R) to_e3 = true;
+        }
+      }
+    } else if (phase == PH_E2) {
+      if (stop) to_e3 = true;
+      else {
+        if (accept) { gap = 0; top_row = r; sx = k.x; sy = k.y; sz = k.z; ss = k.s; st = k.t; sq = k.q; }
+        else { gap++; if (gap > d.P.max_gap) to_e3 = true; }
+        r++;
+        if (r >= R) to_e3 = true;
+      }
+    } else {  // PH_E3
+      if (stop) phase = PH_DONE;
+      else {
+        if (accept) {
+          gap = 0; inner_row = r; n_hits++;
+          if (outer_row < 0) outer_row = r;
+          ix = k.x; iy_ = k.y; iz_ = k.z; is = k.s; it = k.t; iq = k.q; ichi = k.chi2;
+        } else {
+          gap++;
+          if (r < r0 && gap > d.P.max_gap) phase = PH_DONE;
+        }
+        r--;
+        if (r < 0) phase = PH_DONE;
       }
     }
-    // rows below inner_row hold no accepted hit: consumers only read [first_row, last_row]
-    if (inner_row >= 0 && n_hits >= d.P.min_tracklet_hits) {
-      ti = make_int4(1, inner_row, outer_row, n_hits);
-      tf0 = make_float4(inner.x, inner.y, inner.z, inner.s);
-      tf1 = make_float4(inner.t, inner.q, inner.chi2, z_ref);
-      W = pack_weight(d, n_hits, inner.chi2, (uint32_t)t);
-      for (int r = inner_row; r <= outer_row; r++) {
-        const int h = rh[(size_t)r * T];
-        if (h >= 0) atomicMax(&d.hit_weight[h], W);
-      }
-      atomicAdd(&d.cnt->n_valid, 1);
+    if (to_e3) {  // restore the state at the outermost hit, reset the covariance, go inward through the seed
+      k.x = sx; k.y = sy; k.z = sz; k.s = ss; k.t = st; k.q = sq;
+      kf_reset_cov(k, d.P.cov0);
+      gap = 0; r = top_row; phase = PH_E3;
     }
+  }
+  int4 ti = make_int4(0, -1, -1, 0);
+  float4 tf0 = make_float4(0.f, 0.f, 0.f, 0.f), tf1 = make_float4(0.f, 0.f, 0.f, z_ref);
+  unsigned long long W = 0ull;
+  if (valid && inner_row >= 0 && n_hits >= d.P.min_tracklet_hits) {
+    ti = make_int4(1, inner_row, outer_row, n_hits);
+    tf0 = make_float4(ix, iy_, iz_, is);
+    tf1 = make_float4(it, iq, ichi, z_ref);
+    W = pack_weight(d, n_hits, ichi, (uint32_t)t);
+    for (int rr = inner_row; rr <= outer_row; rr++) {
+      const int hh = rh[(size_t)rr * T];
+      if (hh >= 0) atomicMax(&d.hit_weight[hh], W);
+    }
+    atomicAdd(&d.cnt->n_valid, 1);
   }
   {
     const unsigned m = __activemask();
@@ -187,6 +242,11 @@ __global__ void __launch_bounds__(E_THREADS) k_tracklets(Dev d) {
 
 void launch_tracklets(const Dev& d, Launch& L) {
   if (d.n <= 0 || d.max_tracklets <= 0) return;
-  k_tracklets<<<(d.max_tracklets + E_THREADS - 1) / E_THREADS, E_THREADS, 0, L.st>>>(d);
+  const int T = d.max_tracklets;
+  k_seed_flag<<<(T + 255) / 256, 256, 0, L.st>>>(d);
   L.count++;
+  launch_scan_i32(d.seed_w, &d.cnt->n_start, T, d.scan_tmp, L);
+  k_seed_compact<<<(T + 255) / 256, 256, 0, L.st>>>(d);
+  k_tracklets<<<(T + E_THREADS - 1) / E_THREADS, E_THREADS, 0, L.st>>>(d);
+  L.count += 2;
 }
