@@ -129,8 +129,9 @@ def run_gpu(args):
     fr = synth.generate(synth.config(5, seed=5 + 1000 * rank))
     rx = synth.row_x()
     n = fr.n
+    extra = {k: float(v) for k, v in (kv.split("=") for kv in args.params.split(",") if kv)}
     trk = binding.Tracker(rx, n_sectors=36, max_clusters=n, max_tracklets=max(1 << 16, n // 8),
-                          max_tracks=max(1 << 16, n // 24), device=f"cuda:{local}")
+                          max_tracks=max(1 << 16, n // 24), device=f"cuda:{local}", **extra)
     dev_clusters = trk.upload(fr.clusters)
     stream = torch.cuda.current_stream()
 
@@ -236,6 +237,7 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="tpcca", choices=["tpcca", "reference"])
+    ap.add_argument("--params", default="", help="k=v,k=v overrides of tpcca_params (tuning experiments)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "tpcca" else args.warmup
     return run_reference(args) if args.impl == "reference" else run_gpu(args)

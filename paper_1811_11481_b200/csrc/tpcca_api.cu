@@ -114,7 +114,7 @@ void tpcca_default_params(tpcca_params* p) {
   p->cov0[0] = 1.0f; p->cov0[1] = 1.0f; p->cov0[2] = 0.25f; p->cov0[3] = 1.0f; p->cov0[4] = 100.0f;
   p->pick_cut = 16.0f; p->reject_cut = 25.0f; p->max_gap = 5; p->edge_margin = 3.0f; p->max_sinphi = 0.95f;
   p->min_seed_hits = 4; p->min_tracklet_hits = 10; p->min_track_hits = 10; p->qual_scale = 1000.0f;
-  p->grid_bin_y = 2.0f; p->grid_bin_z_min = 2.5f; p->grid_bins_per_cluster = 1.0f;
+  p->grid_bin_y = 4.0f; p->grid_bin_z_min = 2.5f; p->grid_bins_per_cluster = 1.0f;
 }
 
 size_t tpcca_workspace_bytes(const tpcca_geometry* g, const tpcca_params* p) {

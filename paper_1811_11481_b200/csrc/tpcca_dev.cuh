@@ -29,7 +29,7 @@ struct DevCounters {  // device-resident scalars
   int32_t n_bins;      // total grid bins of the frame
   int32_t n_start_raw; // start hits before clamping to capacity
   int32_t n_work;      // seeds that reach the constructor (chain >= min_seed_hits)
-  int32_t pad[1];
+  int32_t work_next;   // queue head of the tracklet constructor
   unsigned long long row_steps, searches, track_hits;  // work counters (roofline units)
   unsigned long long pad2;
 };
@@ -77,7 +77,7 @@ struct Dev {
   // (e)
   int32_t* seed_w;         // [max_tracklets+1] keep flag -> exclusive scan: tracklet id t -> work index w
   int32_t* work_t;         // [max_tracklets] w -> t
-  int32_t* row_hit;        // [n_rows][max_tracklets] indexed by w (dense over surviving seeds)
+  int32_t* row_hit;        // [max_tracklets][n_rows] indexed by w (dense over surviving seeds)
   int32_t* tl_ints;        // [max_tracklets][4] valid, first_row, last_row, n_hits
   float* tl_floats;        // [max_tracklets][8] x, y, z~, sinphi, dzds, qpt, chi2, z_ref
   unsigned long long* tl_W;        // [max_tracklets]

@@ -99,7 +99,7 @@ __global__ void k_reset(Dev d) {
     d.slice_bbox[4 * i + 3] = 0u;           // zmax
   }
   if (i == 0) {
-    d.cnt->n_start = 0; d.cnt->n_tracks = 0; d.cnt->n_valid = 0; d.cnt->status = 0; d.cnt->n_bins = 0; d.cnt->n_start_raw = 0; d.cnt->n_work = 0;
+    d.cnt->n_start = 0; d.cnt->n_tracks = 0; d.cnt->n_valid = 0; d.cnt->status = 0; d.cnt->n_bins = 0; d.cnt->n_start_raw = 0; d.cnt->n_work = 0; d.cnt->work_next = 0;
     d.cnt->row_steps = 0ull; d.cnt->searches = 0ull; d.cnt->track_hits = 0ull;
   }
 }

@@ -15,13 +15,13 @@ __global__ void __launch_bounds__(128) k_select_flag(Dev d) {
   int flag = 0;
   if (ti.x) {
     const unsigned long long W = d.tl_W[t];
-    const int T = d.max_tracklets;
+    int32_t* rh = d.row_hit + (size_t)w * d.n_rows;
     int owned = 0;
     for (int r = ti.y; r <= ti.z; r++) {
-      const int h = d.row_hit[(size_t)r * T + w];
+      const int h = rh[r];
       if (h < 0) continue;
       if (d.hit_weight[h] == W) owned++;
-      else d.row_hit[(size_t)r * T + w] = -2 - h;
+      else rh[r] = -2 - h;
     }
     flag = owned >= d.P.min_track_hits ? 1 : 0;
     if (flag) atomicAdd(&d.cnt->track_hits, (unsigned long long)owned);
@@ -47,10 +47,11 @@ __global__ void __launch_bounds__(128) k_select_write(Dev d) {
   d.tl_track[t] = acc ? id : -1;
   if (!acc) return;
   const int4 ti = reinterpret_cast<const int4*>(d.tl_ints)[t];
-  const int T = d.max_tracklets, K = d.max_tracks;
+  const int K = d.max_tracks;
+  const int32_t* rh = d.row_hit + (size_t)w * d.n_rows;
   int j = 0, sl = 0;
   for (int r = ti.y; r <= ti.z; r++) {
-    const int h = d.row_hit[(size_t)r * T + w];
+    const int h = rh[r];
     if (h < 0) continue;
     d.th_yz[(size_t)j * K + id] = d.yz[h];
     d.th_row[(size_t)j * K + id] = (uint8_t)r;
@@ -182,7 +183,7 @@ __global__ void k_export_tracklets(Dev d, int what, void* dst) {
     for (int r = 0; r < d.n_rows; r++) {
       int v = -1;
       if (ti.x && r >= ti.y && r <= ti.z) {
-        v = d.row_hit[(size_t)r * d.max_tracklets + d.seed_w[t]];
+        v = d.row_hit[(size_t)d.seed_w[t] * d.n_rows + r];
         if (v <= -2) v = -2 - v;
         if (v >= 0) v = d.orig_idx[v];
       }

@@ -84,51 +84,94 @@ __global__ void __launch_bounds__(256) k_seed_compact(Dev d) {
 }
 
 // ---------------------------------------------------------------- (e) constructor
-// One thread per surviving seed.  E1 (follow links), E2 (outward pick-up) and E3 (inward pass) run as ONE
-// loop with a phase variable, so that lanes of a warp that are in different phases still share the single
-// transport / search / update instruction streams.
-#define E_THREADS 64
+// Persistent warps: every lane runs one seed at a time and, when it is done, takes the next one from a
+// global queue (one atomic per warp refill, ballot + popc ranks), so a warp never idles on its longest
+// tracklet.  E1 (follow links), E2 (outward pick-up) and E3 (inward pass) run as ONE loop with a phase
+// variable, so lanes in different phases share the single transport / search / update instruction streams.
+// row_hit is [w][row]: a lane's consecutive rows fall into the same 32-byte sector, which L2 merges.
+#define E_THREADS 128
+#define E_BLOCKS_PER_SM 6
 #define PH_E1 0
 #define PH_E2 1
 #define PH_E3 2
 #define PH_DONE 3
 
-__global__ void __launch_bounds__(E_THREADS) k_tracklets(Dev d) {
-  const int w = blockIdx.x * blockDim.x + threadIdx.x;
-  if (w >= d.cnt->n_work) return;
-  const int t = d.work_t[w];
-  const int T = d.max_tracklets;
+__global__ void __launch_bounds__(E_THREADS, E_BLOCKS_PER_SM) k_tracklets(Dev d) {
   const int R = d.n_rows;
-  int32_t* rh = d.row_hit + w;  // rh[r * T]
-  const int h0 = d.start_hits[t];
-  const int sl0 = d.slice_of[h0];
-  const int sec = sl0 / R, r0 = sl0 - sec * R;
-  const int sbase = sec * R;
-  int n_steps = 0, n_search = 0;  // work counters (roofline units)
-
-  const float2 p0 = d.yz[h0];
-  const float z_ref = p0.y;
+  const int n_work = d.cnt->n_work;
+  const unsigned lane = threadIdx.x & 31;
+  int n_steps = 0, n_search = 0, n_val = 0;  // work counters (roofline units)
+  // per-seed state
+  int t = -1, r0 = 0, sbase = 0, h = -1, r = 0;
+  int32_t* rh = nullptr;
+  float z_ref = 0.f;
   KF k;
-  int phase = PH_E1;
-  int h = d.link_up_clean[h0];  // E1: next chain hit
-  int r = (h >= d.row_start[sbase + r0 + 2]) ? r0 + 2 : r0 + 1;  // target row of the next step
-  {
-    const float2 p1 = d.yz[h];
-    const float dx = d.row_x[r] - d.row_x[r0], dy = p1.x - p0.x, dz = p1.y - p0.y;
-    const float ds = sqrtf(dx * dx + dy * dy);
-    k.x = d.row_x[r0];
-    k.y = p0.x; k.z = 0.0f; k.s = dy / ds; k.t = dz / ds; k.q = 0.0f;
-    kf_reset_cov(k, d.P.cov0);
-    kf_update(k, p0.x, p0.y - z_ref, d.sy2, d.sz2);
-    rh[(size_t)r0 * T] = h0;
-  }
-  int last_row = r0, top_row = r0, gap = 0;
-  bool valid = true;
+  k.x = 0.f; k.y = k.z = k.s = k.t = k.q = 0.f; kf_reset_cov(k, d.P.cov0);
+  int phase = PH_DONE;
+  bool exhausted = false, valid = true;
+  int last_row = 0, top_row = 0, gap = 0;
   float sx = 0.f, sy = 0.f, sz = 0.f, ss = 0.f, st = 0.f, sq = 0.f;             // snapshot at the outermost hit
   float ix = 0.f, iy_ = 0.f, iz_ = 0.f, is = 0.f, it = 0.f, iq = 0.f, ichi = 0.f;  // state at the innermost hit
   int inner_row = -1, outer_row = -1, n_hits = 0;
 
-  while (phase != PH_DONE) {
+  while (true) {
+    const bool need = (phase == PH_DONE) && !exhausted;
+    const unsigned need_mask = __ballot_sync(0xffffffffu, need);
+    if (need_mask) {
+      if (need && t >= 0) {  // retire the finished seed
+        int4 ti = make_int4(0, -1, -1, 0);
+        float4 tf0 = make_float4(0.f, 0.f, 0.f, 0.f), tf1 = make_float4(0.f, 0.f, 0.f, z_ref);
+        unsigned long long W = 0ull;
+        if (valid && inner_row >= 0 && n_hits >= d.P.min_tracklet_hits) {
+          ti = make_int4(1, inner_row, outer_row, n_hits);
+          tf0 = make_float4(ix, iy_, iz_, is);
+          tf1 = make_float4(it, iq, ichi, z_ref);
+          W = pack_weight(d, n_hits, ichi, (uint32_t)t);
+          n_val++;
+        }
+        reinterpret_cast<int4*>(d.tl_ints)[t] = ti;
+        reinterpret_cast<float4*>(d.tl_floats)[2 * t] = tf0;
+        reinterpret_cast<float4*>(d.tl_floats)[2 * t + 1] = tf1;
+        d.tl_W[t] = W;
+        t = -1;
+      }
+      int base = 0;
+      const int leader = __ffs(need_mask) - 1;
+      if ((int)lane == leader) base = atomicAdd(&d.cnt->work_next, __popc(need_mask));
+      base = __shfl_sync(0xffffffffu, base, leader);
+      if (need) {
+        const int w = base + __popc(need_mask & ((1u << lane) - 1u));
+        if (w >= n_work) exhausted = true;
+        else {  // start seed w (E1 initial state: DESIGN.md O5)
+          t = d.work_t[w];
+          rh = d.row_hit + (size_t)w * R;
+          const int h0 = d.start_hits[t];
+          const int sl0 = d.slice_of[h0];
+          const int sec = sl0 / R;
+          r0 = sl0 - sec * R;
+          sbase = sec * R;
+          const float2 p0 = d.yz[h0];
+          z_ref = p0.y;
+          h = d.link_up_clean[h0];
+          r = (h >= d.row_start[sbase + r0 + 2]) ? r0 + 2 : r0 + 1;
+          const float2 p1 = d.yz[h];
+          const float dx = d.row_x[r] - d.row_x[r0], dy = p1.x - p0.x, dz = p1.y - p0.y;
+          const float ds = sqrtf(dx * dx + dy * dy);
+          k.x = d.row_x[r0];
+          k.y = p0.x; k.z = 0.0f; k.s = dy / ds; k.t = dz / ds; k.q = 0.0f;
+          kf_reset_cov(k, d.P.cov0);
+          kf_update(k, p0.x, p0.y - z_ref, d.sy2, d.sz2);
+          rh[r0] = h0;
+          phase = PH_E1; valid = true;
+          last_row = r0; top_row = r0; gap = 0;
+          inner_row = -1; outer_row = -1; n_hits = 0;
+        }
+      }
+      if (__ballot_sync(0xffffffffu, !exhausted) == 0u) break;
+    }
+    if (phase == PH_DONE) continue;  // exhausted lane: idle until the warp is finished
+
+    // ---- one row step
     n_steps++;
     const float xr = d.row_x[r];
     const bool tr_ok = kf_transport(k, xr, d.kq, d.P.max_sinphi);
@@ -141,7 +184,7 @@ __global__ void __launch_bounds__(E_THREADS) k_tracklets(Dev d) {
       if (phase == PH_E1) {
         cand = h; accept = true;
       } else {
-        const int cur = (phase == PH_E3 && r >= r0) ? rh[(size_t)r * T] : -1;
+        const int cur = (phase == PH_E3 && r >= r0) ? rh[r] : -1;
         if (cur >= 0) {
           cand = cur;
           pc = d.yz[cur];
@@ -150,7 +193,7 @@ __global__ void __launch_bounds__(E_THREADS) k_tracklets(Dev d) {
           const float dz = (pc.y - z_ref) - k.z;
           const float dist = (dy * dy) * iy + (dz * dz) * iz;
           accept = dist <= d.P.reject_cut;
-          if (!accept) rh[(size_t)r * T] = -1;
+          if (!accept) rh[r] = -1;
         } else {
           do_search = true;
         }
@@ -159,7 +202,7 @@ __global__ void __launch_bounds__(E_THREADS) k_tracklets(Dev d) {
     if (do_search) {
       n_search++;
       cand = search_row(d, sbase + r, k, z_ref, d.P.pick_cut);
-      rh[(size_t)r * T] = cand;
+      rh[r] = cand;
       accept = cand >= 0;
     }
     if (accept) {
@@ -171,8 +214,8 @@ __global__ void __launch_bounds__(E_THREADS) k_tracklets(Dev d) {
     if (phase == PH_E1) {
       if (stop) { valid = false; phase = PH_DONE; }
       else {
-        if (r == last_row + 2) rh[(size_t)(r - 1) * T] = -1;  // skipped (empty) row
-        rh[(size_t)r * T] = h;
+        if (r == last_row + 2) rh[r - 1] = -1;  // skipped (empty) row
+        rh[r] = h;
         last_row = r;
         h = d.link_up_clean[h];
         if (h >= 0) r = (r + 2 < R && h >= d.row_start[sbase + r + 2]) ? r + 2 : r + 1;
@@ -212,32 +255,28 @@ __global__ void __launch_bounds__(E_THREADS) k_tracklets(Dev d) {
       gap = 0; r = top_row; phase = PH_E3;
     }
   }
-  int4 ti = make_int4(0, -1, -1, 0);
-  float4 tf0 = make_float4(0.f, 0.f, 0.f, 0.f), tf1 = make_float4(0.f, 0.f, 0.f, z_ref);
-  unsigned long long W = 0ull;
-  if (valid && inner_row >= 0 && n_hits >= d.P.min_tracklet_hits) {
-    ti = make_int4(1, inner_row, outer_row, n_hits);
-    tf0 = make_float4(ix, iy_, iz_, is);
-    tf1 = make_float4(it, iq, ichi, z_ref);
-    W = pack_weight(d, n_hits, ichi, (uint32_t)t);
-    for (int rr = inner_row; rr <= outer_row; rr++) {
-      const int hh = rh[(size_t)rr * T];
-      if (hh >= 0) atomicMax(&d.hit_weight[hh], W);
-    }
-    atomicAdd(&d.cnt->n_valid, 1);
+  const int ws = __reduce_add_sync(0xffffffffu, n_steps), wq = __reduce_add_sync(0xffffffffu, n_search),
+            wv = __reduce_add_sync(0xffffffffu, n_val);
+  if (lane == 0 && ws) {
+    atomicAdd(&d.cnt->row_steps, (unsigned long long)ws);
+    atomicAdd(&d.cnt->searches, (unsigned long long)wq);
+    atomicAdd(&d.cnt->n_valid, wv);
   }
-  {
-    const unsigned m = __activemask();
-    const int ws = __reduce_add_sync(m, n_steps), wq = __reduce_add_sync(m, n_search);
-    if ((threadIdx.x & 31) == (__ffs(m) - 1)) {
-      atomicAdd(&d.cnt->row_steps, (unsigned long long)ws);
-      atomicAdd(&d.cnt->searches, (unsigned long long)wq);
-    }
+}
+
+// (e2) every hit of a valid tracklet receives max(weight) (O5 "Result")
+__global__ void __launch_bounds__(128) k_tracklet_weights(Dev d) {
+  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  if (w >= d.cnt->n_work) return;
+  const int t = d.work_t[w];
+  const int4 ti = reinterpret_cast<const int4*>(d.tl_ints)[t];
+  if (!ti.x) return;
+  const unsigned long long W = d.tl_W[t];
+  const int32_t* rh = d.row_hit + (size_t)w * d.n_rows;
+  for (int r = ti.y; r <= ti.z; r++) {
+    const int h = rh[r];
+    if (h >= 0) atomicMax(&d.hit_weight[h], W);
   }
-  reinterpret_cast<int4*>(d.tl_ints)[t] = ti;
-  reinterpret_cast<float4*>(d.tl_floats)[2 * t] = tf0;
-  reinterpret_cast<float4*>(d.tl_floats)[2 * t + 1] = tf1;
-  d.tl_W[t] = W;
 }
 
 void launch_tracklets(const Dev& d, Launch& L) {
@@ -247,6 +286,7 @@ void launch_tracklets(const Dev& d, Launch& L) {
   L.count++;
   launch_scan_i32(d.seed_w, &d.cnt->n_start, T, d.scan_tmp, L);
   k_seed_compact<<<(T + 255) / 256, 256, 0, L.st>>>(d);
-  k_tracklets<<<(T + E_THREADS - 1) / E_THREADS, E_THREADS, 0, L.st>>>(d);
-  L.count += 2;
+  k_tracklets<<<148 * E_BLOCKS_PER_SM, E_THREADS, 0, L.st>>>(d);
+  k_tracklet_weights<<<(T + 127) / 128, 128, 0, L.st>>>(d);
+  L.count += 3;
 }
