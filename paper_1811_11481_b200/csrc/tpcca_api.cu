@@ -71,6 +71,7 @@ static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params
   CARVE(d.seed_w, int32_t, T + 1);
   CARVE(d.work_t, int32_t, T);
   CARVE(d.row_hit, int32_t, T * (size_t)g->n_rows);
+  CARVE(d.tl_state, float, T * 24);
   CARVE(d.tl_ints, int32_t, T * 4);
   CARVE(d.tl_floats, float, T * 8);
   CARVE(d.tl_W, unsigned long long, T);

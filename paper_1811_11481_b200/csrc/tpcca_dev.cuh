@@ -12,7 +12,7 @@
 
 struct GridHdr {  // 32 B per (sector,row) slice
   float ymin, zmin, inv_by, inv_bz;
-  int32_t ny, nz, bin_base, pad;
+  int32_t ny, nz, bin_base, pad;  // pad = clusters in the slice
 };
 
 struct NbrHdr {  // 32 B per slice: the per-row constants of the neighbours finder (O2)
@@ -29,7 +29,7 @@ struct DevCounters {  // device-resident scalars
   int32_t n_bins;      // total grid bins of the frame
   int32_t n_start_raw; // start hits before clamping to capacity
   int32_t n_work;      // seeds that reach the constructor (chain >= min_seed_hits)
-  int32_t work_next;   // queue head of the tracklet constructor
+  int32_t work_next[3];  // queue heads of the three tracklet-constructor kernels
   unsigned long long row_steps, searches, track_hits;  // work counters (roofline units)
   unsigned long long pad2;
 };
@@ -78,6 +78,7 @@ struct Dev {
   int32_t* seed_w;         // [max_tracklets+1] keep flag -> exclusive scan: tracklet id t -> work index w
   int32_t* work_t;         // [max_tracklets] w -> t
   int32_t* row_hit;        // [max_tracklets][n_rows] indexed by w (dense over surviving seeds)
+  float* tl_state;         // [max_tracklets][24] w-space: x, 5 parameters, 15 cov, chi2, row, valid
   int32_t* tl_ints;        // [max_tracklets][4] valid, first_row, last_row, n_hits
   float* tl_floats;        // [max_tracklets][8] x, y, z~, sinphi, dzds, qpt, chi2, z_ref
   unsigned long long* tl_W;        // [max_tracklets]

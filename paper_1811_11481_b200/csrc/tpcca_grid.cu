@@ -99,7 +99,7 @@ __global__ void k_reset(Dev d) {
     d.slice_bbox[4 * i + 3] = 0u;           // zmax
   }
   if (i == 0) {
-    d.cnt->n_start = 0; d.cnt->n_tracks = 0; d.cnt->n_valid = 0; d.cnt->status = 0; d.cnt->n_bins = 0; d.cnt->n_start_raw = 0; d.cnt->n_work = 0; d.cnt->work_next = 0;
+    d.cnt->n_start = 0; d.cnt->n_tracks = 0; d.cnt->n_valid = 0; d.cnt->status = 0; d.cnt->n_bins = 0; d.cnt->n_start_raw = 0; d.cnt->n_work = 0; d.cnt->work_next[0] = 0; d.cnt->work_next[1] = 0; d.cnt->work_next[2] = 0;
     d.cnt->row_steps = 0ull; d.cnt->searches = 0ull; d.cnt->track_hits = 0ull;
   }
 }
@@ -175,7 +175,7 @@ __global__ void __launch_bounds__(1024) k_slice_setup(Dev d) {
         g.ymin = ymin; g.zmin = zmin;
         g.inv_by = ((float)ny / ye) * 0.9999f;
         g.inv_bz = ((float)nz / ze) * 0.9999f;
-        g.ny = ny; g.nz = nz;
+        g.ny = ny; g.nz = nz; g.pad = cnt;
         nb = ny * nz;
       }
     }
@@ -186,7 +186,7 @@ __global__ void __launch_bounds__(1024) k_slice_setup(Dev d) {
       d.row_start[sl] = carry_c + ec;
       g.bin_base = carry_b + eb;
       if (g.bin_base + nb > d.max_bins) {  // cannot happen with the default sizing; degrade to one bin
-        g.ny = g.nz = 1; g.bin_base = min(g.bin_base, d.max_bins - 1);
+        g.ny = g.nz = 1; g.pad = 0; g.bin_base = min(g.bin_base, d.max_bins - 1);
         atomicOr(&d.cnt->status, TPCCA_STAT_BIN_OVERFLOW);
       }
       d.grid[sl] = g;

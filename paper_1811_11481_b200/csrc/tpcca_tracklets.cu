@@ -6,42 +6,6 @@
 // One thread per start hit.  E1 seed fit along the links, E2 outward pick-up, E3 inward pass.
 #include "tpcca_dev.cuh"
 
-// Best pick-up candidate of slice `sl` for the predicted state; sorted index or -1.  (O5 "search")
-__device__ __forceinline__ int search_row(const Dev& d, int sl, const KF& k, float z_ref, float cut) {
-  const int rb = d.row_start[sl], re = d.row_start[sl + 1];
-  if (re <= rb) return -1;
-  const float vy = k.c00 + d.sy2, vz = k.c11 + d.sz2;
-  const float iy = 1.0f / vy, iz = 1.0f / vz;
-  const float wy = sqrtf(cut * vy), wz = sqrtf(cut * vz);
-  const GridHdr g = d.grid[sl];
-  const float zc = z_ref + k.z;  // search centre in frame coordinates (bin lookup only)
-  const float mz = 2e-3f + (fabsf(zc) + fabsf(z_ref) + fabsf(k.z)) * 4e-7f;
-  int y0, y1, z0, z1;
-  bin_range(k.y - wy - 1e-3f, k.y + wy + 1e-3f, g.ymin, g.inv_by, g.ny, y0, y1);
-  bin_range(zc - wz - mz, zc + wz + mz, g.zmin, g.inv_bz, g.nz, z0, z1);
-  int best = -1;
-  float bd = 0.0f, by = 0.0f, bz = 0.0f;
-  if (z0 > z1) return -1;
-  for (int yb = y0; yb <= y1; yb++) {
-    const int cb = d.bin_start[g.bin_base + yb * g.nz + z0];
-    const int ce = d.bin_start[g.bin_base + yb * g.nz + z1 + 1];
-    for (int c = cb; c < ce; c++) {
-      const float2 p = d.yz[c];
-      const float dy = p.x - k.y;
-      const float dz = (p.y - z_ref) - k.z;
-      if (!(fabsf(dy) <= wy) || !(fabsf(dz) <= wz)) continue;
-      const float dist = (dy * dy) * iy + (dz * dz) * iz;
-      if (!(dist <= cut)) continue;
-      bool better;
-      if (best < 0) better = true;
-      else if (dist != bd) better = dist < bd;
-      else better = key_less(p.y, p.x, d.orig_idx[c], bz, by, d.orig_idx[best]);
-      if (better) { best = c; bd = dist; by = p.x; bz = p.y; }
-    }
-  }
-  return best;
-}
-
 __device__ __forceinline__ unsigned long long pack_weight(const Dev& d, int n_hits, float chi2, uint32_t tid) {
   float qf = (d.P.qual_scale * chi2) / (float)(2 * n_hits);
   qf = fminf(65535.0f, qf);
@@ -84,71 +48,133 @@ __global__ void __launch_bounds__(256) k_seed_compact(Dev d) {
 }
 
 // ---------------------------------------------------------------- (e) constructor
-// Persistent warps: every lane runs one seed at a time and, when it is done, takes the next one from a
-// global queue (one atomic per warp refill, ballot + popc ranks), so a warp never idles on its longest
-// tracklet.  E1 (follow links), E2 (outward pick-up) and E3 (inward pass) run as ONE loop with a phase
-// variable, so lanes in different phases share the single transport / search / update instruction streams.
-// row_hit is [w][row]: a lane's consecutive rows fall into the same 32-byte sector, which L2 merges.
+// Three persistent kernels, one per phase of DESIGN.md O5, so that every warp runs ONE uniform step body:
+//   k_tl_e1  seed fit along the links            (transport + update)
+//   k_tl_e2  outward extrapolation and pick-up   (transport + search + update)
+//   k_tl_e3  inward pass through the seed        (transport + [existing hit | search] + update)
+// Every lane runs one seed at a time and, when it is done, takes the next one from a global queue (one atomic
+// per warp refill; ballot + popc give the lanes their ranks), so a warp never idles on its longest seed.
+// The Kalman state travels between the kernels through tl_state[w][24].  row_hit is [w][row]: a lane's
+// consecutive rows share a 32-byte sector, which L2 merges.
 #define E_THREADS 128
-#define E_BLOCKS_PER_SM 6
-#define PH_E1 0
-#define PH_E2 1
-#define PH_E3 2
-#define PH_DONE 3
+#define FULL 0xffffffffu
 
-__global__ void __launch_bounds__(E_THREADS, E_BLOCKS_PER_SM) k_tracklets(Dev d) {
-  const int R = d.n_rows;
-  const int n_work = d.cnt->n_work;
+// warp-collective: lanes with need=true receive consecutive queue positions
+__device__ __forceinline__ int fetch_work(int* counter, bool need, unsigned lane, unsigned need_mask) {
+  int base = 0;
+  const int leader = __ffs(need_mask) - 1;
+  if ((int)lane == leader) base = atomicAdd(counter, __popc(need_mask));
+  base = __shfl_sync(FULL, base, leader);
+  return need ? base + __popc(need_mask & ((1u << lane) - 1u)) : -1;
+}
+
+__device__ __forceinline__ void st_store_kf(float* st, const KF& k) {
+  float4* p = reinterpret_cast<float4*>(st);
+  p[0] = make_float4(k.x, k.y, k.z, k.s);
+  p[1] = make_float4(k.t, k.q, k.c00, k.c10);
+  p[2] = make_float4(k.c11, k.c20, k.c21, k.c22);
+  p[3] = make_float4(k.c30, k.c31, k.c32, k.c33);
+  p[4] = make_float4(k.c40, k.c41, k.c42, k.c43);
+  st[20] = k.c44; st[21] = k.chi2;
+}
+__device__ __forceinline__ void st_load_kf(const float* st, KF& k) {
+  const float4* p = reinterpret_cast<const float4*>(st);
+  const float4 a = p[0], b = p[1], c = p[2], e = p[3], f = p[4];
+  k.x = a.x; k.y = a.y; k.z = a.z; k.s = a.w;
+  k.t = b.x; k.q = b.y; k.c00 = b.z; k.c10 = b.w;
+  k.c11 = c.x; k.c20 = c.y; k.c21 = c.z; k.c22 = c.w;
+  k.c30 = e.x; k.c31 = e.y; k.c32 = e.z; k.c33 = e.w;
+  k.c40 = f.x; k.c41 = f.y; k.c42 = f.z; k.c43 = f.w;
+  k.c44 = st[20]; k.chi2 = st[21];
+}
+
+__device__ __noinline__ bool tie_less(const Dev& d, int c, float2 p, int best) {
+  const float2 q = d.yz[best];
+  return key_less(p.y, p.x, d.orig_idx[c], q.y, q.x, d.orig_idx[best]);
+}
+
+// Candidate choice of one row step (O5 "Search" and the E3 keep/reject test) in ONE code path:
+// cur >= 0  -> the only candidate is the existing hit `cur`, kept iff d <= reject_cut (no window);
+// cur <  0  -> the clusters of slice g inside the window compete, best = min by (d, key), d <= pick_cut.
+// Returns the chosen sorted index or -1; pbest = its (y, z).
+__device__ __forceinline__ int choose_hit(const Dev& d, const GridHdr& g, const KF& k, float z_ref, int cur,
+                                          float2& pbest) {
+  const bool hit = cur >= 0;
+  const float cut = hit ? d.P.reject_cut : d.P.pick_cut;
+  const float vy = k.c00 + d.sy2, vz = k.c11 + d.sz2;
+  const float iy = 1.0f / vy, iz = 1.0f / vz;
+  float wy = sqrtf(cut * vy), wz = sqrtf(cut * vz);
+  int y0 = 0, y1 = 0, z0 = 0, z1 = 0;
+  if (hit) {
+    wy = wz = __int_as_float(0x7f800000);  // +inf: no window on the keep/reject test
+  } else {
+    const float zc = z_ref + k.z;  // search centre in frame coordinates (bin lookup only)
+    const float mz = 2e-3f + (fabsf(zc) + fabsf(z_ref) + fabsf(k.z)) * 4e-7f;
+    bin_range(k.y - wy - 1e-3f, k.y + wy + 1e-3f, g.ymin, g.inv_by, g.ny, y0, y1);
+    bin_range(zc - wz - mz, zc + wz + mz, g.zmin, g.inv_bz, g.nz, z0, z1);
+    if (z0 > z1 || g.pad == 0) { y0 = 1; y1 = 0; }  // NaN / empty window, or empty row
+  }
+  int best = -1;
+  float bd = 0.0f;
+  for (int yb = y0; yb <= y1; yb += 2) {  // two y-bin rows per pass, their candidates in one flat loop
+    int a0, a1, b0 = 0, b1 = 0;
+    if (hit) { a0 = cur; a1 = cur + 1; }
+    else {
+      const int* bs = d.bin_start + g.bin_base + yb * g.nz;
+      a0 = bs[z0]; a1 = bs[z1 + 1];
+      if (yb + 1 <= y1) { b0 = bs[g.nz + z0]; b1 = bs[g.nz + z1 + 1]; }
+    }
+    const int na = a1 - a0, ntot = na + (b1 - b0);
+    for (int i = 0; i < ntot; i++) {
+      const int c = (i < na) ? a0 + i : b0 + (i - na);
+      const float2 p = d.yz[c];
+      const float dy = p.x - k.y;
+      const float dz = (p.y - z_ref) - k.z;
+      if (!(fabsf(dy) <= wy) || !(fabsf(dz) <= wz)) continue;
+      const float dist = (dy * dy) * iy + (dz * dz) * iz;
+      if (!(dist <= cut)) continue;
+      bool better;
+      if (best < 0) better = true;
+      else if (dist != bd) better = dist < bd;
+      else better = tie_less(d, c, p, best);
+      if (better) { best = c; bd = dist; pbest = p; }
+    }
+  }
+  return best;
+}
+
+// ---- E1: seed fit along the cleaned up-links
+__global__ void __launch_bounds__(E_THREADS, 8) k_tl_e1(Dev d) {
+  const int R = d.n_rows, n_work = d.cnt->n_work;
   const unsigned lane = threadIdx.x & 31;
-  int n_steps = 0, n_search = 0, n_val = 0;  // work counters (roofline units)
-  // per-seed state
-  int t = -1, r0 = 0, sbase = 0, h = -1, r = 0;
+  int n_steps = 0;
+  int w = -1, sbase = 0, h = -1, r = 0, last_row = 0;
   int32_t* rh = nullptr;
   float z_ref = 0.f;
   KF k;
-  k.x = 0.f; k.y = k.z = k.s = k.t = k.q = 0.f; kf_reset_cov(k, d.P.cov0);
-  int phase = PH_DONE;
-  bool exhausted = false, valid = true;
-  int last_row = 0, top_row = 0, gap = 0;
-  float sx = 0.f, sy = 0.f, sz = 0.f, ss = 0.f, st = 0.f, sq = 0.f;             // snapshot at the outermost hit
-  float ix = 0.f, iy_ = 0.f, iz_ = 0.f, is = 0.f, it = 0.f, iq = 0.f, ichi = 0.f;  // state at the innermost hit
-  int inner_row = -1, outer_row = -1, n_hits = 0;
-
+  k.x = k.y = k.z = k.s = k.t = k.q = 0.f; kf_reset_cov(k, d.P.cov0);
+  bool busy = false, exhausted = false, valid = true;
   while (true) {
-    const bool need = (phase == PH_DONE) && !exhausted;
-    const unsigned need_mask = __ballot_sync(0xffffffffu, need);
-    if (need_mask) {
-      if (need && t >= 0) {  // retire the finished seed
-        int4 ti = make_int4(0, -1, -1, 0);
-        float4 tf0 = make_float4(0.f, 0.f, 0.f, 0.f), tf1 = make_float4(0.f, 0.f, 0.f, z_ref);
-        unsigned long long W = 0ull;
-        if (valid && inner_row >= 0 && n_hits >= d.P.min_tracklet_hits) {
-          ti = make_int4(1, inner_row, outer_row, n_hits);
-          tf0 = make_float4(ix, iy_, iz_, is);
-          tf1 = make_float4(it, iq, ichi, z_ref);
-          W = pack_weight(d, n_hits, ichi, (uint32_t)t);
-          n_val++;
-        }
-        reinterpret_cast<int4*>(d.tl_ints)[t] = ti;
-        reinterpret_cast<float4*>(d.tl_floats)[2 * t] = tf0;
-        reinterpret_cast<float4*>(d.tl_floats)[2 * t + 1] = tf1;
-        d.tl_W[t] = W;
-        t = -1;
+    const bool need = !busy && !exhausted;
+    const unsigned nm = __ballot_sync(FULL, need);
+    if (nm) {
+      if (need && w >= 0) {  // retire
+        float* st = d.tl_state + (size_t)w * 24;
+        st_store_kf(st, k);
+        reinterpret_cast<int*>(st)[22] = last_row;
+        reinterpret_cast<int*>(st)[23] = valid ? 1 : 0;
+        w = -1;
       }
-      int base = 0;
-      const int leader = __ffs(need_mask) - 1;
-      if ((int)lane == leader) base = atomicAdd(&d.cnt->work_next, __popc(need_mask));
-      base = __shfl_sync(0xffffffffu, base, leader);
+      const int nw = fetch_work(&d.cnt->work_next[0], need, lane, nm);
       if (need) {
-        const int w = base + __popc(need_mask & ((1u << lane) - 1u));
-        if (w >= n_work) exhausted = true;
-        else {  // start seed w (E1 initial state: DESIGN.md O5)
-          t = d.work_t[w];
+        if (nw >= n_work) exhausted = true;
+        else {
+          w = nw;
+          const int t = d.work_t[w];
           rh = d.row_hit + (size_t)w * R;
           const int h0 = d.start_hits[t];
           const int sl0 = d.slice_of[h0];
-          const int sec = sl0 / R;
-          r0 = sl0 - sec * R;
+          const int sec = sl0 / R, r0 = sl0 - sec * R;
           sbase = sec * R;
           const float2 p0 = d.yz[h0];
           z_ref = p0.y;
@@ -162,101 +188,196 @@ __global__ void __launch_bounds__(E_THREADS, E_BLOCKS_PER_SM) k_tracklets(Dev d)
           kf_reset_cov(k, d.P.cov0);
           kf_update(k, p0.x, p0.y - z_ref, d.sy2, d.sz2);
           rh[r0] = h0;
-          phase = PH_E1; valid = true;
-          last_row = r0; top_row = r0; gap = 0;
-          inner_row = -1; outer_row = -1; n_hits = 0;
+          last_row = r0; valid = true; busy = true;
         }
       }
-      if (__ballot_sync(0xffffffffu, !exhausted) == 0u) break;
+      if (__ballot_sync(FULL, !exhausted) == 0u) break;
     }
-    if (phase == PH_DONE) continue;  // exhausted lane: idle until the warp is finished
+    if (!busy) continue;
+    // ---- one chain step (loads first: they do not depend on the filter state)
+    n_steps++;
+    const float2 pc = d.yz[h];
+    const int hn = d.link_up_clean[h];
+    const int rs2 = (r + 2 < R) ? d.row_start[sbase + r + 2] : 0x7fffffff;
+    if (!kf_transport(k, d.row_x[r], d.kq, d.P.max_sinphi)) { valid = false; busy = false; continue; }
+    kf_update(k, pc.x, pc.y - z_ref, d.sy2, d.sz2);
+    if (r == last_row + 2) rh[r - 1] = -1;  // skipped (empty) row
+    rh[r] = h;
+    last_row = r;
+    h = hn;
+    if (h < 0) busy = false;
+    else r = (h >= rs2) ? r + 2 : r + 1;
+  }
+  const int ws = __reduce_add_sync(FULL, n_steps);
+  if (lane == 0 && ws) atomicAdd(&d.cnt->row_steps, (unsigned long long)ws);
+}
 
+// ---- E2: outward extrapolation, one best cluster per row
+__global__ void __launch_bounds__(E_THREADS, 6) k_tl_e2(Dev d) {
+  const int R = d.n_rows, n_work = d.cnt->n_work;
+  const unsigned lane = threadIdx.x & 31;
+  int n_steps = 0;
+  int w = -1, sbase = 0, r = 0, top_row = 0, gap = 0;
+  int32_t* rh = nullptr;
+  float z_ref = 0.f;
+  KF k;
+  k.x = k.y = k.z = k.s = k.t = k.q = 0.f; kf_reset_cov(k, d.P.cov0);
+  float sx = 0.f, sy = 0.f, sz = 0.f, ss = 0.f, st_ = 0.f, sq = 0.f;  // snapshot at the outermost hit
+  bool busy = false, exhausted = false, live = false;
+  while (true) {
+    const bool need = !busy && !exhausted;
+    const unsigned nm = __ballot_sync(FULL, need);
+    if (nm) {
+      if (need && w >= 0) {  // retire: the snapshot replaces the state, top_row replaces last_row
+        if (live) {
+          float* st = d.tl_state + (size_t)w * 24;
+          reinterpret_cast<float4*>(st)[0] = make_float4(sx, sy, sz, ss);
+          st[4] = st_; st[5] = sq;
+          reinterpret_cast<int*>(st)[22] = top_row;
+        }
+        w = -1;
+      }
+      const int nw = fetch_work(&d.cnt->work_next[1], need, lane, nm);
+      if (need) {
+        if (nw >= n_work) exhausted = true;
+        else {
+          w = nw;
+          const float* st = d.tl_state + (size_t)w * 24;
+          live = reinterpret_cast<const int*>(st)[23] != 0;
+          if (live) {
+            st_load_kf(st, k);
+            const int last_row = reinterpret_cast<const int*>(st)[22];
+            const int t = d.work_t[w];
+            const int h0 = d.start_hits[t];
+            sbase = (d.slice_of[h0] / R) * R;
+            z_ref = d.yz[h0].y;
+            rh = d.row_hit + (size_t)w * R;
+            sx = k.x; sy = k.y; sz = k.z; ss = k.s; st_ = k.t; sq = k.q;
+            top_row = last_row; gap = 0; r = last_row + 1;
+            busy = r < R;
+          }
+        }
+      }
+      if (__ballot_sync(FULL, !exhausted) == 0u) break;
+    }
+    if (!busy) continue;
     // ---- one row step
     n_steps++;
+    const GridHdr g = d.grid[sbase + r];
     const float xr = d.row_x[r];
-    const bool tr_ok = kf_transport(k, xr, d.kq, d.P.max_sinphi);
-    const bool edge = (phase != PH_E1) && (fabsf(k.y) > xr * d.tan_half_angle + d.P.edge_margin);
-    const bool stop = !tr_ok || edge;
-    int cand = -1;
-    bool accept = false, do_search = false;
-    float2 pc = make_float2(0.f, 0.f);
-    if (!stop) {
-      if (phase == PH_E1) {
-        cand = h; accept = true;
-      } else {
-        const int cur = (phase == PH_E3 && r >= r0) ? rh[r] : -1;
-        if (cur >= 0) {
-          cand = cur;
-          pc = d.yz[cur];
-          const float iy = 1.0f / (k.c00 + d.sy2), iz = 1.0f / (k.c11 + d.sz2);
-          const float dy = pc.x - k.y;
-          const float dz = (pc.y - z_ref) - k.z;
-          const float dist = (dy * dy) * iy + (dz * dz) * iz;
-          accept = dist <= d.P.reject_cut;
-          if (!accept) rh[r] = -1;
-        } else {
-          do_search = true;
-        }
-      }
+    if (!kf_transport(k, xr, d.kq, d.P.max_sinphi) || fabsf(k.y) > xr * d.tan_half_angle + d.P.edge_margin) {
+      busy = false;
+      continue;
     }
-    if (do_search) {
-      n_search++;
-      cand = search_row(d, sbase + r, k, z_ref, d.P.pick_cut);
-      rh[r] = cand;
-      accept = cand >= 0;
+    float2 pb = make_float2(0.f, 0.f);
+    const int cand = choose_hit(d, g, k, z_ref, -1, pb);
+    rh[r] = cand;
+    if (cand >= 0) {
+      kf_update(k, pb.x, pb.y - z_ref, d.sy2, d.sz2);
+      gap = 0; top_row = r;
+      sx = k.x; sy = k.y; sz = k.z; ss = k.s; st_ = k.t; sq = k.q;
+    } else {
+      gap++;
+      if (gap > d.P.max_gap) busy = false;
     }
-    if (accept) {
-      if (phase == PH_E1 || do_search) pc = d.yz[cand];
-      kf_update(k, pc.x, pc.y - z_ref, d.sy2, d.sz2);
-    }
-    // ---- bookkeeping and phase transitions
-    bool to_e3 = false;
-    if (phase == PH_E1) {
-      if (stop) { valid = false; phase = PH_DONE; }
-      else {
-        if (r == last_row + 2) rh[r - 1] = -1;  // skipped (empty) row
-        rh[r] = h;
-        last_row = r;
-        h = d.link_up_clean[h];
-        if (h >= 0) r = (r + 2 < R && h >= d.row_start[sbase + r + 2]) ? r + 2 : r + 1;
-        else {  // seed complete (its length was checked by k_seed_flag): start E2
-          phase = PH_E2; top_row = last_row; gap = 0;
-          sx = k.x; sy = k.y; sz = k.z; ss = k.s; st = k.t; sq = k.q;
-          r = last_row + 1;
-          if (r >= R) to_e3 = true;
-        }
-      }
-    } else if (phase == PH_E2) {
-      if (stop) to_e3 = true;
-      else {
-        if (accept) { gap = 0; top_row = r; sx = k.x; sy = k.y; sz = k.z; ss = k.s; st = k.t; sq = k.q; }
-        else { gap++; if (gap > d.P.max_gap) to_e3 = true; }
-        r++;
-        if (r >= R) to_e3 = true;
-      }
-    } else {  // PH_E3
-      if (stop) phase = PH_DONE;
-      else {
-        if (accept) {
-          gap = 0; inner_row = r; n_hits++;
-          if (outer_row < 0) outer_row = r;
-          ix = k.x; iy_ = k.y; iz_ = k.z; is = k.s; it = k.t; iq = k.q; ichi = k.chi2;
-        } else {
-          gap++;
-          if (r < r0 && gap > d.P.max_gap) phase = PH_DONE;
-        }
-        r--;
-        if (r < 0) phase = PH_DONE;
-      }
-    }
-    if (to_e3) {  // restore the state at the outermost hit, reset the covariance, go inward through the seed
-      k.x = sx; k.y = sy; k.z = sz; k.s = ss; k.t = st; k.q = sq;
-      kf_reset_cov(k, d.P.cov0);
-      gap = 0; r = top_row; phase = PH_E3;
-    }
+    r++;
+    if (r >= R) busy = false;
   }
-  const int ws = __reduce_add_sync(0xffffffffu, n_steps), wq = __reduce_add_sync(0xffffffffu, n_search),
-            wv = __reduce_add_sync(0xffffffffu, n_val);
+  const int ws = __reduce_add_sync(FULL, n_steps);
+  if (lane == 0 && ws) {
+    atomicAdd(&d.cnt->row_steps, (unsigned long long)ws);
+    atomicAdd(&d.cnt->searches, (unsigned long long)ws);
+  }
+}
+
+// ---- E3: inward pass through the seed with outlier rejection, then pick-up below it
+__global__ void __launch_bounds__(E_THREADS, 6) k_tl_e3(Dev d) {
+  const int R = d.n_rows, n_work = d.cnt->n_work;
+  const unsigned lane = threadIdx.x & 31;
+  int n_steps = 0, n_search = 0, n_val = 0;
+  int w = -1, t = -1, sbase = 0, r0 = 0, r = 0, gap = 0;
+  int32_t* rh = nullptr;
+  float z_ref = 0.f;
+  KF k;
+  k.x = k.y = k.z = k.s = k.t = k.q = 0.f; kf_reset_cov(k, d.P.cov0);
+  float ix = 0.f, iy_ = 0.f, iz_ = 0.f, is = 0.f, it = 0.f, iq = 0.f, ichi = 0.f;  // state at the innermost hit
+  int inner_row = -1, outer_row = -1, n_hits = 0;
+  bool busy = false, exhausted = false, live = false;
+  while (true) {
+    const bool need = !busy && !exhausted;
+    const unsigned nm = __ballot_sync(FULL, need);
+    if (nm) {
+      if (need && w >= 0) {  // retire: tracklet record (void unless enough hits)
+        int4 ti = make_int4(0, -1, -1, 0);
+        float4 tf0 = make_float4(0.f, 0.f, 0.f, 0.f), tf1 = make_float4(0.f, 0.f, 0.f, z_ref);
+        unsigned long long W = 0ull;
+        if (live && inner_row >= 0 && n_hits >= d.P.min_tracklet_hits) {
+          ti = make_int4(1, inner_row, outer_row, n_hits);
+          tf0 = make_float4(ix, iy_, iz_, is);
+          tf1 = make_float4(it, iq, ichi, z_ref);
+          W = pack_weight(d, n_hits, ichi, (uint32_t)t);
+          n_val++;
+        }
+        reinterpret_cast<int4*>(d.tl_ints)[t] = ti;
+        reinterpret_cast<float4*>(d.tl_floats)[2 * t] = tf0;
+        reinterpret_cast<float4*>(d.tl_floats)[2 * t + 1] = tf1;
+        d.tl_W[t] = W;
+        w = -1;
+      }
+      const int nw = fetch_work(&d.cnt->work_next[2], need, lane, nm);
+      if (need) {
+        if (nw >= n_work) exhausted = true;
+        else {
+          w = nw;
+          t = d.work_t[w];
+          const float* st = d.tl_state + (size_t)w * 24;
+          live = reinterpret_cast<const int*>(st)[23] != 0;
+          const int h0 = d.start_hits[t];
+          const int sl0 = d.slice_of[h0];
+          const int sec = sl0 / R;
+          r0 = sl0 - sec * R; sbase = sec * R;
+          z_ref = d.yz[h0].y;
+          inner_row = -1; outer_row = -1; n_hits = 0; gap = 0;
+          if (live) {
+            const float4 a = reinterpret_cast<const float4*>(st)[0];
+            k.x = a.x; k.y = a.y; k.z = a.z; k.s = a.w; k.t = st[4]; k.q = st[5];
+            kf_reset_cov(k, d.P.cov0);
+            r = reinterpret_cast<const int*>(st)[22];
+            rh = d.row_hit + (size_t)w * R;
+            busy = true;
+          }
+        }
+      }
+      if (__ballot_sync(FULL, !exhausted) == 0u) break;
+    }
+    if (!busy) continue;
+    // ---- one row step
+    n_steps++;
+    const int cur = (r >= r0) ? rh[r] : -1;
+    const GridHdr g = d.grid[sbase + r];
+    const float xr = d.row_x[r];
+    if (!kf_transport(k, xr, d.kq, d.P.max_sinphi) || fabsf(k.y) > xr * d.tan_half_angle + d.P.edge_margin) {
+      busy = false;
+      continue;
+    }
+    if (cur < 0) n_search++;
+    float2 pb = make_float2(0.f, 0.f);
+    const int cand = choose_hit(d, g, k, z_ref, cur, pb);
+    if (cand != cur || r < r0) rh[r] = cand;  // rejected seed hit -> -1, or the search result (rows below the seed are unwritten)
+    if (cand >= 0) {
+      kf_update(k, pb.x, pb.y - z_ref, d.sy2, d.sz2);
+      gap = 0; inner_row = r; n_hits++;
+      if (outer_row < 0) outer_row = r;
+      ix = k.x; iy_ = k.y; iz_ = k.z; is = k.s; it = k.t; iq = k.q; ichi = k.chi2;
+    } else {
+      gap++;
+      if (r < r0 && gap > d.P.max_gap) busy = false;
+    }
+    r--;
+    if (r < 0) busy = false;
+  }
+  const int ws = __reduce_add_sync(FULL, n_steps), wq = __reduce_add_sync(FULL, n_search),
+            wv = __reduce_add_sync(FULL, n_val);
   if (lane == 0 && ws) {
     atomicAdd(&d.cnt->row_steps, (unsigned long long)ws);
     atomicAdd(&d.cnt->searches, (unsigned long long)wq);
@@ -264,7 +385,7 @@ __global__ void __launch_bounds__(E_THREADS, E_BLOCKS_PER_SM) k_tracklets(Dev d)
   }
 }
 
-// (e2) every hit of a valid tracklet receives max(weight) (O5 "Result")
+// (e4) every hit of a valid tracklet receives max(weight) (O5 "Result")
 __global__ void __launch_bounds__(128) k_tracklet_weights(Dev d) {
   const int w = blockIdx.x * blockDim.x + threadIdx.x;
   if (w >= d.cnt->n_work) return;
@@ -286,7 +407,9 @@ void launch_tracklets(const Dev& d, Launch& L) {
   L.count++;
   launch_scan_i32(d.seed_w, &d.cnt->n_start, T, d.scan_tmp, L);
   k_seed_compact<<<(T + 255) / 256, 256, 0, L.st>>>(d);
-  k_tracklets<<<148 * E_BLOCKS_PER_SM, E_THREADS, 0, L.st>>>(d);
+  k_tl_e1<<<148 * 8, E_THREADS, 0, L.st>>>(d);
+  k_tl_e2<<<148 * 6, E_THREADS, 0, L.st>>>(d);
+  k_tl_e3<<<148 * 6, E_THREADS, 0, L.st>>>(d);
   k_tracklet_weights<<<(T + 127) / 128, 128, 0, L.st>>>(d);
-  L.count += 3;
+  L.count += 5;
 }
