@@ -69,6 +69,7 @@ static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params
   CARVE(d.sb_skey, int32_t, T);
   CARVE(d.start_hits, int32_t, T);
   CARVE(d.seed_w, int32_t, T + 1);
+  CARVE(d.ord, int32_t, 9 * 256);
   CARVE(d.work_t, int32_t, T);
   CARVE(d.row_hit, int32_t, T * (size_t)g->n_rows);
   CARVE(d.tl_state, float, T * 24);

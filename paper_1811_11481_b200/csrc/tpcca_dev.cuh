@@ -75,7 +75,8 @@ struct Dev {
   int32_t* sb_skey;        // [max_tracklets] bucket of sb_sorted[p]
   int32_t* start_hits;     // [max_tracklets] canonical order (sorted indices)
   // (e)
-  int32_t* seed_w;         // [max_tracklets+1] keep flag -> exclusive scan: tracklet id t -> work index w
+  int32_t* seed_w;         // [max_tracklets+1] tracklet id t -> work index w, -1 for void seeds
+  int32_t* ord;            // [3 orders][count | base | fill][256] bucket-order scratch (zeroed per call)
   int32_t* work_t;         // [max_tracklets] w -> t
   int32_t* row_hit;        // [max_tracklets][n_rows] indexed by w (dense over surviving seeds)
   float* tl_state;         // [max_tracklets][24] w-space: x, 5 parameters, 15 cov, chi2, row, valid
@@ -84,7 +85,7 @@ struct Dev {
   unsigned long long* tl_W;        // [max_tracklets]
   unsigned long long* hit_weight;  // [n]
   // (f),(g)
-  int32_t* sel_scan;       // [max_tracklets+1] w-space: accept flag -> exclusive scan = track id
+  int32_t* sel_scan;       // [max_tracklets+1] t-space: accept flag -> exclusive scan = track id
   int32_t* tl_track;       // [max_tracklets] t-space: track id or -1 (only read for tracklets that own hits)
   int32_t* track_tracklet; // [max_tracks] track id -> t
   int32_t* track_info;     // [max_tracks] n_hits | sector << 16

@@ -26,7 +26,7 @@ __global__ void __launch_bounds__(128) k_select_flag(Dev d) {
     flag = owned >= d.P.min_track_hits ? 1 : 0;
     if (flag) atomicAdd(&d.cnt->track_hits, (unsigned long long)owned);
   }
-  d.sel_scan[w] = flag;
+  if (flag) d.sel_scan[t] = 1;
 }
 
 // ---------------------------------------------------------------- (f2) after the scan: track ids + packed hit lists
@@ -36,14 +36,14 @@ __global__ void __launch_bounds__(128) k_select_write(Dev d) {
   const int w = blockIdx.x * blockDim.x + threadIdx.x;
   const int nw = d.cnt->n_work;
   if (w == 0) {
-    const int tot = d.sel_scan[nw];
+    const int tot = d.sel_scan[d.cnt->n_start];
     if (tot > d.max_tracks) atomicOr(&d.cnt->status, TPCCA_STAT_TRACK_OVERFLOW);
     d.cnt->n_tracks = min(tot, d.max_tracks);
   }
   if (w >= nw) return;
   const int t = d.work_t[w];
-  const int id = d.sel_scan[w];
-  const bool acc = (d.sel_scan[w + 1] != id) && (id < d.max_tracks);
+  const int id = d.sel_scan[t];
+  const bool acc = (d.sel_scan[t + 1] != id) && (id < d.max_tracks);
   d.tl_track[t] = acc ? id : -1;
   if (!acc) return;
   const int4 ti = reinterpret_cast<const int4*>(d.tl_ints)[t];
@@ -80,7 +80,7 @@ void launch_select(const Dev& d, Launch& L) {
   const int T = d.max_tracklets;
   k_select_flag<<<(T + 127) / 128, 128, 0, L.st>>>(d);
   L.count++;
-  launch_scan_i32(d.sel_scan, &d.cnt->n_work, T, d.scan_tmp, L);
+  launch_scan_i32(d.sel_scan, &d.cnt->n_start, T, d.scan_tmp, L);
   k_select_write<<<(T + 127) / 128, 128, 0, L.st>>>(d);
   k_assign<<<(d.n + 255) / 256, 256, 0, L.st>>>(d);
   L.count += 2;

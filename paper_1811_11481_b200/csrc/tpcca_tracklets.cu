@@ -18,7 +18,8 @@ __device__ __forceinline__ unsigned long long pack_weight(const Dev& d, int n_hi
 
 // ---------------------------------------------------------------- (e0) seed filter + stable compaction
 // A start hit whose link chain is shorter than min_seed_hits is void (O5/E1) and never reaches
-// the constructor: the survivors are compacted in tracklet-id order into the work list (w -> t).
+// the constructor: the survivors are compacted in tracklet-id order into the work list (w -> t), which keeps
+// seeds of the same sector and row next to each other (shared grid headers and bins in L1/L2).
 __global__ void __launch_bounds__(256) k_seed_flag(Dev d) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= d.cnt->n_start) return;
@@ -30,6 +31,7 @@ __global__ void __launch_bounds__(256) k_seed_flag(Dev d) {
   }
   const int keep = n >= d.P.min_seed_hits ? 1 : 0;
   d.seed_w[t] = keep;
+  d.sel_scan[t] = 0;
   if (!keep) {
     reinterpret_cast<int4*>(d.tl_ints)[t] = make_int4(0, -1, -1, 0);
     reinterpret_cast<float4*>(d.tl_floats)[2 * t] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -47,6 +49,17 @@ __global__ void __launch_bounds__(256) k_seed_compact(Dev d) {
   if (d.seed_w[t + 1] != w) d.work_t[w] = t;
 }
 
+#define ORD_KEYS 256
+// exclusive scan of the 256 bucket counts of order `m`; total -> *total_out
+__global__ void __launch_bounds__(ORD_KEYS) k_ord_offsets(Dev d, int m, int32_t* total_out) {
+  __shared__ int sm[32];
+  int* cnt = d.ord + (3 * m + 0) * ORD_KEYS;
+  int tot;
+  const int e = block_scan_excl(cnt[threadIdx.x], &tot, sm);
+  d.ord[(3 * m + 1) * ORD_KEYS + threadIdx.x] = e;
+  if (threadIdx.x == 0 && total_out) *total_out = tot;
+}
+
 // ---------------------------------------------------------------- (e) constructor
 // Three persistent kernels, one per phase of DESIGN.md O5, so that every warp runs ONE uniform step body:
 //   k_tl_e1  seed fit along the links            (transport + update)
@@ -58,6 +71,7 @@ __global__ void __launch_bounds__(256) k_seed_compact(Dev d) {
 // consecutive rows share a 32-byte sector, which L2 merges.
 #define E_THREADS 128
 #define FULL 0xffffffffu
+#define REFILL_MIN 8  // refill a warp when this many lanes are idle (amortises the divergent start-up code)
 
 // warp-collective: lanes with need=true receive consecutive queue positions
 __device__ __forceinline__ int fetch_work(int* counter, bool need, unsigned lane, unsigned need_mask) {
@@ -157,7 +171,7 @@ __global__ void __launch_bounds__(E_THREADS, 8) k_tl_e1(Dev d) {
   while (true) {
     const bool need = !busy && !exhausted;
     const unsigned nm = __ballot_sync(FULL, need);
-    if (nm) {
+    if (nm && (__popc(nm) >= REFILL_MIN || __ballot_sync(FULL, busy) == 0u)) {
       if (need && w >= 0) {  // retire
         float* st = d.tl_state + (size_t)w * 24;
         st_store_kf(st, k);
@@ -227,7 +241,7 @@ __global__ void __launch_bounds__(E_THREADS, 6) k_tl_e2(Dev d) {
   while (true) {
     const bool need = !busy && !exhausted;
     const unsigned nm = __ballot_sync(FULL, need);
-    if (nm) {
+    if (nm && (__popc(nm) >= REFILL_MIN || __ballot_sync(FULL, busy) == 0u)) {
       if (need && w >= 0) {  // retire: the snapshot replaces the state, top_row replaces last_row
         if (live) {
           float* st = d.tl_state + (size_t)w * 24;
@@ -306,7 +320,7 @@ __global__ void __launch_bounds__(E_THREADS, 6) k_tl_e3(Dev d) {
   while (true) {
     const bool need = !busy && !exhausted;
     const unsigned nm = __ballot_sync(FULL, need);
-    if (nm) {
+    if (nm && (__popc(nm) >= REFILL_MIN || __ballot_sync(FULL, busy) == 0u)) {
       if (need && w >= 0) {  // retire: tracklet record (void unless enough hits)
         int4 ti = make_int4(0, -1, -1, 0);
         float4 tf0 = make_float4(0.f, 0.f, 0.f, 0.f), tf1 = make_float4(0.f, 0.f, 0.f, z_ref);
