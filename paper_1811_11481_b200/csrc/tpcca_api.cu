@@ -69,7 +69,7 @@ static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params
   CARVE(d.sb_skey, int32_t, T);
   CARVE(d.start_hits, int32_t, T);
   CARVE(d.seed_w, int32_t, T + 1);
-  CARVE(d.ord, int32_t, 9 * 256);
+  CARVE(d.ord, int32_t, 1024);
   CARVE(d.work_t, int32_t, T);
   CARVE(d.row_hit, int32_t, T * (size_t)g->n_rows);
   CARVE(d.tl_state, float, T * 24);
@@ -79,9 +79,11 @@ static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params
   CARVE(d.sel_scan, int32_t, T + 1);
   CARVE(d.tl_track, int32_t, T + 1);
   CARVE(d.track_tracklet, int32_t, K);
-  CARVE(d.track_info, int32_t, K);
-  CARVE(d.th_yz, float2, K * (size_t)g->n_rows);
-  CARVE(d.th_row, uint8_t, K * (size_t)g->n_rows);
+  CARVE(d.track_w, int32_t, K);
+  CARVE(d.track_order, int32_t, K);
+  CARVE(d.w_list, int2, T);
+  CARVE(d.th_yz, float2, N);
+  CARVE(d.th_row, uint8_t, N);
   CARVE(stage_clusters, float4, N);
   CARVE(stage_assign, int32_t, N);
   CARVE(stage_tracks, char, sizeof(tpcca_out_header) + K * sizeof(tpcca_track_rec));

@@ -76,7 +76,7 @@ struct Dev {
   int32_t* start_hits;     // [max_tracklets] canonical order (sorted indices)
   // (e)
   int32_t* seed_w;         // [max_tracklets+1] tracklet id t -> work index w, -1 for void seeds
-  int32_t* ord;            // [3 orders][count | base | fill][256] bucket-order scratch (zeroed per call)
+  int32_t* ord;            // [1024] track-length histogram [0,512) and bucket cursors [512,1024) (zeroed per call)
   int32_t* work_t;         // [max_tracklets] w -> t
   int32_t* row_hit;        // [max_tracklets][n_rows] indexed by w (dense over surviving seeds)
   float* tl_state;         // [max_tracklets][24] w-space: x, 5 parameters, 15 cov, chi2, row, valid
@@ -88,9 +88,11 @@ struct Dev {
   int32_t* sel_scan;       // [max_tracklets+1] t-space: accept flag -> exclusive scan = track id
   int32_t* tl_track;       // [max_tracklets] t-space: track id or -1 (only read for tracklets that own hits)
   int32_t* track_tracklet; // [max_tracks] track id -> t
-  int32_t* track_info;     // [max_tracks] n_hits | sector << 16
-  float2* th_yz;           // [n_rows][max_tracks] j-th owned hit (innermost first) of track id: (y, z)
-  uint8_t* th_row;         // [n_rows][max_tracks] its row
+  int32_t* track_w;        // [max_tracks] track id -> w
+  int32_t* track_order;    // [max_tracks] refit order: track ids by decreasing hit count
+  int2* w_list;            // [max_tracklets] w-space, accepted tracklets: (offset, count) of the owned-hit list
+  float2* th_yz;           // [n] owned-hit lists (innermost first): (y, z)
+  uint8_t* th_row;         // [n] their rows
   DevCounters* cnt;
   tpcca_out_header* out_hdr;
   tpcca_track_rec* out_tracks;

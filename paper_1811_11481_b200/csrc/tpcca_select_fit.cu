@@ -4,35 +4,60 @@
 // (g) PAPER.md:71 "The final Kalman refit is iterated three times: inward, outward, and inward" (O7).
 #include "tpcca_dev.cuh"
 
-// ---------------------------------------------------------------- (f1) ownership count -> accept flag
-// One thread per surviving seed w.  Non-owned hits are re-encoded in place as -2-h (reversible: the
-// export decodes them), so the later passes see owned hits as h >= 0.
-__global__ void __launch_bounds__(128) k_select_flag(Dev d) {
-  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+// ---------------------------------------------------------------- (f1) ownership -> accept flag + packed hit list
+// One warp per surviving seed w: lanes take consecutive rows (coalesced row_hit reads, 32 independent weight
+// gathers).  An accepted tracklet's owned hits are packed innermost-first into th_yz / th_row at a slot range
+// taken from a bump allocator (every hit has one owner, so all lists together hold at most n entries).
+#define SEL_THREADS 128
+#define SEL_CHUNKS (TPCCA_MAX_ROWS / 32)
+__global__ void __launch_bounds__(SEL_THREADS) k_select_own(Dev d) {
+  const int w = (blockIdx.x * SEL_THREADS + threadIdx.x) >> 5;
+  const unsigned lane = threadIdx.x & 31;
   if (w >= d.cnt->n_work) return;
   const int t = d.work_t[w];
   const int4 ti = reinterpret_cast<const int4*>(d.tl_ints)[t];
-  int flag = 0;
-  if (ti.x) {
-    const unsigned long long W = d.tl_W[t];
-    int32_t* rh = d.row_hit + (size_t)w * d.n_rows;
-    int owned = 0;
-    for (int r = ti.y; r <= ti.z; r++) {
-      const int h = rh[r];
-      if (h < 0) continue;
-      if (d.hit_weight[h] == W) owned++;
-      else rh[r] = -2 - h;
-    }
-    flag = owned >= d.P.min_track_hits ? 1 : 0;
-    if (flag) atomicAdd(&d.cnt->track_hits, (unsigned long long)owned);
+  if (!ti.x) return;
+  const unsigned long long W = d.tl_W[t];
+  const int32_t* rh = d.row_hit + (size_t)w * d.n_rows;
+  int hh[SEL_CHUNKS];
+  unsigned mm[SEL_CHUNKS];
+  int owned = 0;
+#pragma unroll
+  for (int c = 0; c < SEL_CHUNKS; c++) {
+    const int r = ti.y + 32 * c + (int)lane;
+    int h = -1;
+    if (r <= ti.z) h = rh[r];
+    const bool own = (h >= 0) && (d.hit_weight[h] == W);
+    hh[c] = own ? h : -1;
+    mm[c] = __ballot_sync(0xffffffffu, own);
+    owned += __popc(mm[c]);
   }
-  if (flag) d.sel_scan[t] = 1;
+  if (owned < d.P.min_track_hits) return;
+  int off = 0;
+  if (lane == 0) off = (int)atomicAdd(&d.cnt->track_hits, (unsigned long long)owned);
+  off = __shfl_sync(0xffffffffu, off, 0);
+  int base = off;
+#pragma unroll
+  for (int c = 0; c < SEL_CHUNKS; c++) {
+    if (hh[c] >= 0) {
+      const int j = base + __popc(mm[c] & ((1u << lane) - 1u));
+      d.th_yz[j] = d.yz[hh[c]];
+      d.th_row[j] = (uint8_t)(ti.y + 32 * c + (int)lane);
+    }
+    base += __popc(mm[c]);
+  }
+  if (lane == 0) {
+    d.sel_scan[t] = 1;
+    d.w_list[w] = make_int2(off, owned);
+  }
 }
 
-// ---------------------------------------------------------------- (f2) after the scan: track ids + packed hit lists
-// Track ids follow tracklet-id order (the work list is in that order).  Each accepted track's owned hits are
-// packed innermost-first into th_yz / th_row at [j][id], so that the refit's lanes read one line per step.
-__global__ void __launch_bounds__(128) k_select_write(Dev d) {
+// ---------------------------------------------------------------- (f2) after the scan: track ids, length histogram
+// Track ids follow tracklet-id order (the work list is in that order).
+__global__ void __launch_bounds__(256) k_select_ids(Dev d) {
+  __shared__ int s_hist[TPCCA_MAX_ROWS + 1];
+  for (int i = threadIdx.x; i <= TPCCA_MAX_ROWS; i += blockDim.x) s_hist[i] = 0;
+  __syncthreads();
   const int w = blockIdx.x * blockDim.x + threadIdx.x;
   const int nw = d.cnt->n_work;
   if (w == 0) {
@@ -40,26 +65,38 @@ __global__ void __launch_bounds__(128) k_select_write(Dev d) {
     if (tot > d.max_tracks) atomicOr(&d.cnt->status, TPCCA_STAT_TRACK_OVERFLOW);
     d.cnt->n_tracks = min(tot, d.max_tracks);
   }
-  if (w >= nw) return;
-  const int t = d.work_t[w];
-  const int id = d.sel_scan[t];
-  const bool acc = (d.sel_scan[t + 1] != id) && (id < d.max_tracks);
-  d.tl_track[t] = acc ? id : -1;
-  if (!acc) return;
-  const int4 ti = reinterpret_cast<const int4*>(d.tl_ints)[t];
-  const int K = d.max_tracks;
-  const int32_t* rh = d.row_hit + (size_t)w * d.n_rows;
-  int j = 0, sl = 0;
-  for (int r = ti.y; r <= ti.z; r++) {
-    const int h = rh[r];
-    if (h < 0) continue;
-    d.th_yz[(size_t)j * K + id] = d.yz[h];
-    d.th_row[(size_t)j * K + id] = (uint8_t)r;
-    if (j == 0) sl = d.slice_of[h];
-    j++;
+  if (w < nw) {
+    const int t = d.work_t[w];
+    const int id = d.sel_scan[t];
+    const bool acc = (d.sel_scan[t + 1] != id) && (id < d.max_tracks);
+    d.tl_track[t] = acc ? id : -1;
+    if (acc) {
+      d.track_w[id] = w;
+      d.track_tracklet[id] = t;
+      atomicAdd(&s_hist[d.w_list[w].y], 1);
+    }
   }
-  d.track_tracklet[id] = t;
-  d.track_info[id] = j | ((sl / d.n_rows) << 16);
+  __syncthreads();
+  for (int i = threadIdx.x; i <= TPCCA_MAX_ROWS; i += blockDim.x)
+    if (s_hist[i]) atomicAdd(&d.ord[i], s_hist[i]);
+}
+
+// (f2') refit order: tracks sorted by decreasing hit count (counting sort), so that the lanes of a refit warp run
+// the same number of steps and the longest tracks start first.  The order inside a bucket is arbitrary: every track
+// writes its own record, no result depends on it.
+__global__ void __launch_bounds__(512) k_len_offsets(Dev d) {
+  __shared__ int sm[32];
+  const int i = threadIdx.x;  // bucket i holds length TPCCA_MAX_ROWS - i
+  const int v = (i <= TPCCA_MAX_ROWS) ? d.ord[TPCCA_MAX_ROWS - i] : 0;
+  int tot;
+  const int e = block_scan_excl(v, &tot, sm);
+  if (i <= TPCCA_MAX_ROWS) d.ord[512 + TPCCA_MAX_ROWS - i] = e;
+}
+__global__ void __launch_bounds__(256) k_len_scatter(Dev d) {
+  const int id = blockIdx.x * blockDim.x + threadIdx.x;
+  if (id >= d.cnt->n_tracks) return;
+  const int n = d.w_list[d.track_w[id]].y;
+  d.track_order[atomicAdd(&d.ord[512 + n], 1)] = id;
 }
 
 // ---------------------------------------------------------------- (f3) cluster -> track assignment
@@ -78,28 +115,35 @@ __global__ void __launch_bounds__(256) k_assign(Dev d) {
 void launch_select(const Dev& d, Launch& L) {
   if (d.n <= 0 || d.max_tracklets <= 0) return;
   const int T = d.max_tracklets;
-  k_select_flag<<<(T + 127) / 128, 128, 0, L.st>>>(d);
+  k_select_own<<<(int)(((size_t)T * 32 + SEL_THREADS - 1) / SEL_THREADS), SEL_THREADS, 0, L.st>>>(d);
   L.count++;
   launch_scan_i32(d.sel_scan, &d.cnt->n_start, T, d.scan_tmp, L);
-  k_select_write<<<(T + 127) / 128, 128, 0, L.st>>>(d);
+  k_select_ids<<<(T + 255) / 256, 256, 0, L.st>>>(d);
+  k_len_offsets<<<1, 512, 0, L.st>>>(d);
   k_assign<<<(d.n + 255) / 256, 256, 0, L.st>>>(d);
-  L.count += 2;
+  L.count += 3;
+  if (d.max_tracks > 0) {
+    k_len_scatter<<<(d.max_tracks + 255) / 256, 256, 0, L.st>>>(d);
+    L.count++;
+  }
 }
 
 // ---------------------------------------------------------------- (g) refit
-// One thread per track; hits come from the packed lists (coalesced across the warp).
+// One thread per track, tracks taken in decreasing-length order; a track's hits are one contiguous list.
 __global__ void __launch_bounds__(64) k_refit(Dev d) {
-  const int id = blockIdx.x * blockDim.x + threadIdx.x;
-  if (id >= d.cnt->n_tracks) return;
-  const int K = d.max_tracks;
-  const int info = d.track_info[id];
-  const int n_hits = info & 0xFFFF, sector = info >> 16;
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= d.cnt->n_tracks) return;
+  const int id = d.track_order[p];
+  const int w = d.track_w[id];
+  const int2 wl = d.w_list[w];
+  const int n_hits = wl.y;
   const int t = d.track_tracklet[id];
+  const int sector = d.slice_of[d.start_hits[t]] / d.n_rows;
   const float q0 = d.tl_floats[8 * t + 5];
-  const float2* ly = d.th_yz + id;
-  const uint8_t* lr = d.th_row + id;
-  const int rN = lr[(size_t)(n_hits - 1) * K], rM = lr[(size_t)(n_hits - 2) * K], r_in = lr[0];
-  const float2 pN = ly[(size_t)(n_hits - 1) * K], pM = ly[(size_t)(n_hits - 2) * K];
+  const float2* ly = d.th_yz + wl.x;
+  const uint8_t* lr = d.th_row + wl.x;
+  const int rN = lr[n_hits - 1], rM = lr[n_hits - 2], r_in = lr[0];
+  const float2 pN = ly[n_hits - 1], pM = ly[n_hits - 2];
   const float z_ref = pN.y;
   KF k;
   {
@@ -113,10 +157,10 @@ __global__ void __launch_bounds__(64) k_refit(Dev d) {
     kf_reset_cov(k, d.P.cov0);
     for (int i = 0; i < n_hits; i++) {
       const int j = (pass == 1) ? i : n_hits - 1 - i;
-      const float2 p = ly[(size_t)j * K];
-      const int r = lr[(size_t)j * K];
+      const float2 pj = ly[j];
+      const int r = lr[j];
       if (!kf_transport(k, d.row_x[r], d.kq, d.P.max_sinphi)) { ok = false; break; }
-      kf_update(k, p.x, p.y - z_ref, d.sy2, d.sz2);
+      kf_update(k, pj.x, pj.y - z_ref, d.sy2, d.sz2);
     }
   }
   tpcca_track_rec o;
@@ -184,7 +228,6 @@ __global__ void k_export_tracklets(Dev d, int what, void* dst) {
       int v = -1;
       if (ti.x && r >= ti.y && r <= ti.z) {
         v = d.row_hit[(size_t)d.seed_w[t] * d.n_rows + r];
-        if (v <= -2) v = -2 - v;
         if (v >= 0) v = d.orig_idx[v];
       }
       o[r] = v;

@@ -49,17 +49,6 @@ __global__ void __launch_bounds__(256) k_seed_compact(Dev d) {
   if (d.seed_w[t + 1] != w) d.work_t[w] = t;
 }
 
-#define ORD_KEYS 256
-// exclusive scan of the 256 bucket counts of order `m`; total -> *total_out
-__global__ void __launch_bounds__(ORD_KEYS) k_ord_offsets(Dev d, int m, int32_t* total_out) {
-  __shared__ int sm[32];
-  int* cnt = d.ord + (3 * m + 0) * ORD_KEYS;
-  int tot;
-  const int e = block_scan_excl(cnt[threadIdx.x], &tot, sm);
-  d.ord[(3 * m + 1) * ORD_KEYS + threadIdx.x] = e;
-  if (threadIdx.x == 0 && total_out) *total_out = tot;
-}
-
 // ---------------------------------------------------------------- (e) constructor
 // Three persistent kernels, one per phase of DESIGN.md O5, so that every warp runs ONE uniform step body:
 //   k_tl_e1  seed fit along the links            (transport + update)
@@ -399,16 +388,18 @@ __global__ void __launch_bounds__(E_THREADS, 6) k_tl_e3(Dev d) {
   }
 }
 
-// (e4) every hit of a valid tracklet receives max(weight) (O5 "Result")
+// (e4) every hit of a valid tracklet receives max(weight) (O5 "Result").  One warp per seed: lanes take
+// consecutive rows, so the row_hit reads are coalesced and 32 atomics are in flight per warp.
 __global__ void __launch_bounds__(128) k_tracklet_weights(Dev d) {
-  const int w = blockIdx.x * blockDim.x + threadIdx.x;
+  const int w = (blockIdx.x * 128 + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
   if (w >= d.cnt->n_work) return;
   const int t = d.work_t[w];
   const int4 ti = reinterpret_cast<const int4*>(d.tl_ints)[t];
   if (!ti.x) return;
   const unsigned long long W = d.tl_W[t];
   const int32_t* rh = d.row_hit + (size_t)w * d.n_rows;
-  for (int r = ti.y; r <= ti.z; r++) {
+  for (int r = ti.y + lane; r <= ti.z; r += 32) {
     const int h = rh[r];
     if (h >= 0) atomicMax(&d.hit_weight[h], W);
   }
@@ -424,6 +415,6 @@ void launch_tracklets(const Dev& d, Launch& L) {
   k_tl_e1<<<148 * 8, E_THREADS, 0, L.st>>>(d);
   k_tl_e2<<<148 * 6, E_THREADS, 0, L.st>>>(d);
   k_tl_e3<<<148 * 6, E_THREADS, 0, L.st>>>(d);
-  k_tracklet_weights<<<(T + 127) / 128, 128, 0, L.st>>>(d);
+  k_tracklet_weights<<<(int)(((size_t)T * 32 + 127) / 128), 128, 0, L.st>>>(d);
   L.count += 5;
 }
