@@ -11,44 +11,45 @@
 #define SEL_THREADS 128
 #define SEL_CHUNKS (TPCCA_MAX_ROWS / 32)
 __global__ void __launch_bounds__(SEL_THREADS) k_select_own(Dev d) {
-  const int w = (blockIdx.x * SEL_THREADS + threadIdx.x) >> 5;
   const unsigned lane = threadIdx.x & 31;
-  if (w >= d.cnt->n_work) return;
-  const int t = d.work_t[w];
-  const int4 ti = reinterpret_cast<const int4*>(d.tl_ints)[t];
-  if (!ti.x) return;
-  const unsigned long long W = d.tl_W[t];
-  const int32_t* rh = d.row_hit + (size_t)w * d.n_rows;
-  int hh[SEL_CHUNKS];
-  unsigned mm[SEL_CHUNKS];
-  int owned = 0;
+  const int n_work = d.cnt->n_work, n_warps = (gridDim.x * SEL_THREADS) >> 5;
+  for (int w = (blockIdx.x * SEL_THREADS + threadIdx.x) >> 5; w < n_work; w += n_warps) {
+    const int t = d.work_t[w];
+    const int4 ti = reinterpret_cast<const int4*>(d.tl_ints)[t];
+    if (!ti.x) continue;
+    const unsigned long long W = d.tl_W[t];
+    const int32_t* rh = d.row_hit + (size_t)w * d.n_rows;
+    int hh[SEL_CHUNKS];
+    unsigned mm[SEL_CHUNKS];
+    int owned = 0;
 #pragma unroll
-  for (int c = 0; c < SEL_CHUNKS; c++) {
-    const int r = ti.y + 32 * c + (int)lane;
-    int h = -1;
-    if (r <= ti.z) h = rh[r];
-    const bool own = (h >= 0) && (d.hit_weight[h] == W);
-    hh[c] = own ? h : -1;
-    mm[c] = __ballot_sync(0xffffffffu, own);
-    owned += __popc(mm[c]);
-  }
-  if (owned < d.P.min_track_hits) return;
-  int off = 0;
-  if (lane == 0) off = (int)atomicAdd(&d.cnt->track_hits, (unsigned long long)owned);
-  off = __shfl_sync(0xffffffffu, off, 0);
-  int base = off;
-#pragma unroll
-  for (int c = 0; c < SEL_CHUNKS; c++) {
-    if (hh[c] >= 0) {
-      const int j = base + __popc(mm[c] & ((1u << lane) - 1u));
-      d.th_yz[j] = d.yz[hh[c]];
-      d.th_row[j] = (uint8_t)(ti.y + 32 * c + (int)lane);
+    for (int c = 0; c < SEL_CHUNKS; c++) {
+      const int r = ti.y + 32 * c + (int)lane;
+      int h = -1;
+      if (r <= ti.z) h = rh[r];
+      const bool own = (h >= 0) && (d.hit_weight[h] == W);
+      hh[c] = own ? h : -1;
+      mm[c] = __ballot_sync(0xffffffffu, own);
+      owned += __popc(mm[c]);
     }
-    base += __popc(mm[c]);
-  }
-  if (lane == 0) {
-    d.sel_scan[t] = 1;
-    d.w_list[w] = make_int2(off, owned);
+    if (owned < d.P.min_track_hits) continue;
+    int off = 0;
+    if (lane == 0) off = (int)atomicAdd(&d.cnt->track_hits, (unsigned long long)owned);
+    off = __shfl_sync(0xffffffffu, off, 0);
+    int base = off;
+#pragma unroll
+    for (int c = 0; c < SEL_CHUNKS; c++) {
+      if (hh[c] >= 0) {
+        const int j = base + __popc(mm[c] & ((1u << lane) - 1u));
+        d.th_yz[j] = d.yz[hh[c]];
+        d.th_row[j] = (uint8_t)(ti.y + 32 * c + (int)lane);
+      }
+      base += __popc(mm[c]);
+    }
+    if (lane == 0) {
+      d.sel_scan[t] = 1;
+      d.w_list[w] = make_int2(off, owned);
+    }
   }
 }
 
@@ -115,7 +116,7 @@ __global__ void __launch_bounds__(256) k_assign(Dev d) {
 void launch_select(const Dev& d, Launch& L) {
   if (d.n <= 0 || d.max_tracklets <= 0) return;
   const int T = d.max_tracklets;
-  k_select_own<<<(int)(((size_t)T * 32 + SEL_THREADS - 1) / SEL_THREADS), SEL_THREADS, 0, L.st>>>(d);
+  k_select_own<<<148 * 16, SEL_THREADS, 0, L.st>>>(d);
   L.count++;
   launch_scan_i32(d.sel_scan, &d.cnt->n_start, T, d.scan_tmp, L);
   k_select_ids<<<(T + 255) / 256, 256, 0, L.st>>>(d);

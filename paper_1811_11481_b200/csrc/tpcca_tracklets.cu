@@ -60,7 +60,10 @@ __global__ void __launch_bounds__(256) k_seed_compact(Dev d) {
 // consecutive rows share a 32-byte sector, which L2 merges.
 #define E_THREADS 128
 #define FULL 0xffffffffu
-#define REFILL_MIN 8  // refill a warp when this many lanes are idle (amortises the divergent start-up code)
+#ifndef E_REFILL_MIN
+#define E_REFILL_MIN 8  // refill a warp when this many lanes are idle (amortises the divergent start-up code)
+#endif
+#define REFILL_MIN E_REFILL_MIN
 
 // warp-collective: lanes with need=true receive consecutive queue positions
 __device__ __forceinline__ int fetch_work(int* counter, bool need, unsigned lane, unsigned need_mask) {
@@ -391,17 +394,18 @@ __global__ void __launch_bounds__(E_THREADS, 6) k_tl_e3(Dev d) {
 // (e4) every hit of a valid tracklet receives max(weight) (O5 "Result").  One warp per seed: lanes take
 // consecutive rows, so the row_hit reads are coalesced and 32 atomics are in flight per warp.
 __global__ void __launch_bounds__(128) k_tracklet_weights(Dev d) {
-  const int w = (blockIdx.x * 128 + threadIdx.x) >> 5;
   const int lane = threadIdx.x & 31;
-  if (w >= d.cnt->n_work) return;
-  const int t = d.work_t[w];
-  const int4 ti = reinterpret_cast<const int4*>(d.tl_ints)[t];
-  if (!ti.x) return;
-  const unsigned long long W = d.tl_W[t];
-  const int32_t* rh = d.row_hit + (size_t)w * d.n_rows;
-  for (int r = ti.y + lane; r <= ti.z; r += 32) {
-    const int h = rh[r];
-    if (h >= 0) atomicMax(&d.hit_weight[h], W);
+  const int n_work = d.cnt->n_work, n_warps = (gridDim.x * 128) >> 5;
+  for (int w = (blockIdx.x * 128 + threadIdx.x) >> 5; w < n_work; w += n_warps) {
+    const int t = d.work_t[w];
+    const int4 ti = reinterpret_cast<const int4*>(d.tl_ints)[t];
+    if (!ti.x) continue;
+    const unsigned long long W = d.tl_W[t];
+    const int32_t* rh = d.row_hit + (size_t)w * d.n_rows;
+    for (int r = ti.y + lane; r <= ti.z; r += 32) {
+      const int h = rh[r];
+      if (h >= 0) atomicMax(&d.hit_weight[h], W);
+    }
   }
 }
 
@@ -415,6 +419,6 @@ void launch_tracklets(const Dev& d, Launch& L) {
   k_tl_e1<<<148 * 8, E_THREADS, 0, L.st>>>(d);
   k_tl_e2<<<148 * 6, E_THREADS, 0, L.st>>>(d);
   k_tl_e3<<<148 * 6, E_THREADS, 0, L.st>>>(d);
-  k_tracklet_weights<<<(int)(((size_t)T * 32 + 127) / 128), 128, 0, L.st>>>(d);
+  k_tracklet_weights<<<148 * 16, 128, 0, L.st>>>(d);
   L.count += 5;
 }
