@@ -30,6 +30,17 @@ BYTES_PER_CLUSTER_NEIGHBOURS = 24.0      # 8 own yz + 8 links out + ~8 bin_start
 BYTES_PER_ROW_STEP_TRACKLETS = 22.0      # 8 bin range + ~1.2*8 candidates + 4 row_hit
 BYTES_PER_TRACKLET = 112.0               # record
 BYTES_PER_TRACKLET_HIT = 8.0             # weight atomic
+FP32_OPS_PER_ROW_STEP = 270.0            # transport 48 + covariance 102 + update 102 + search ~18
+
+
+def ncu_traffic(stage: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the stage's kernels, from the committed ncu
+    --set full summary of this round (profiles/traffic.json.txt), or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.json.txt")
+    try:
+        return float(json.load(open(p))[stage])
+    except Exception:
+        return None
 
 
 def peaks():
@@ -43,30 +54,59 @@ def peaks():
 
 
 class ClockSampler:
-    """Samples nvidia-smi clocks and throttle reasons during the timed region."""
+    """Samples SM clocks and throttle reasons during the timed region (NVML; nvidia-smi as a fallback)."""
+
+    NAMES = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
 
     def __init__(self, gpu_index: int):
         self.idx, self.samples, self.reasons, self.max_mhz = gpu_index, [], set(), None
         self._stop = threading.Event()
         self._t = threading.Thread(target=self._run, daemon=True)
+        self._nvml = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+            phys = int(vis.split(",")[gpu_index]) if vis and vis.split(",")[gpu_index].isdigit() else gpu_index
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+            self._nvml = pynvml
+        except Exception:
+            self._nvml = None
 
-    def _run(self):
+    def _sample_nvml(self):
+        n = self._nvml
+        self.samples.append(float(n.nvmlDeviceGetClockInfo(self._h, n.NVML_CLOCK_SM)))
+        r = n.nvmlDeviceGetCurrentClocksEventReasons(self._h)
+        for name, bit in (("hw_slowdown", n.nvmlClocksEventReasonHwSlowdown),
+                          ("hw_thermal_slowdown", n.nvmlClocksEventReasonHwThermalSlowdown),
+                          ("sw_thermal_slowdown", n.nvmlClocksEventReasonSwThermalSlowdown),
+                          ("sw_power_cap", n.nvmlClocksEventReasonSwPowerCap)):
+            if r & bit:
+                self.reasons.add(name)
+
+    def _sample_smi(self):
         q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
-        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        out = subprocess.run(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-i", str(self.idx)],
+                             capture_output=True, text=True, timeout=5).stdout.strip()
+        f = [x.strip() for x in out.split(",")]
+        self.samples.append(float(f[0]))
+        self.max_mhz = float(f[1])
+        for n, v in zip(self.NAMES, f[2:6]):
+            if v.lower().startswith("active"):
+                self.reasons.add(n)
+
+    def _run(self):
         while not self._stop.is_set():
             try:
-                out = subprocess.run(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-i",
-                                      str(self.idx)], capture_output=True, text=True, timeout=5).stdout.strip()
-                f = [x.strip() for x in out.split(",")]
-                self.samples.append(float(f[0]))
-                self.max_mhz = float(f[1])
-                for n, v in zip(names, f[2:6]):
-                    if v.lower().startswith("active"):
-                        self.reasons.add(n)
+                if self._nvml is not None:
+                    self._sample_nvml()
+                else:
+                    self._sample_smi()
             except Exception:
                 pass
-            self._stop.wait(0.1)
+            self._stop.wait(0.004 if self._nvml is not None else 0.1)
 
     def start(self):
         self._t.start()
@@ -75,14 +115,16 @@ class ClockSampler:
         self._stop.set()
         self._t.join(timeout=10)
         return {"sm_mhz": float(np.median(self.samples)) if self.samples else None, "sm_max_mhz": self.max_mhz,
-                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+                "reasons": sorted(self.reasons), "samples": len(self.samples),
+                "source": "nvml" if self._nvml is not None else "nvidia-smi"}
 
 
-def oracle_timed(scale: float, seed: int, steps: int, warmup: int):
-    """The CPU oracle as it stands on a bounded sample of the workload (config 5 at `scale` collisions)."""
+def oracle_timed(scale: float, seed: int, steps: int, warmup: int, fr=None):
+    """The CPU oracle as it stands on `fr`, or on a bounded sample of the workload (config 5 at `scale` collisions)."""
     import oracle
     from paper_1811_11481_b200 import synth
-    fr = synth.generate(synth.config(5, scale=scale, seed=seed))
+    if fr is None:
+        fr = synth.generate(synth.config(5, scale=scale, seed=seed))
     rx = synth.row_x()
     times = []
     for i in range(warmup + steps):
@@ -98,7 +140,7 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    scale = 0.1
+    scale = 0.2
     v, t, n = oracle_timed(scale, 5, args.steps, args.warmup)
     sample = f"config 5 at {int(round(50 * scale))} collisions in {1000 * scale:.0f} us (same occupancy), {n} clusters/step"
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
@@ -207,15 +249,24 @@ def run_gpu(args):
     per_stage = {k: {"ms": stage[k], "alg_GBps": alg[k] / (stage[k] * 1e-3) / 1e9 if stage[k] > 0 else None,
                      "frac": alg[k] / (stage[k] * 1e-3) / 1e9 / peak if stage[k] > 0 else None} for k in stage}
     ach = alg[dom] / (stage[dom] * 1e-3) / 1e9
+    # the Kalman stages are fp32-issue bound: useful fp32 operations of the section-3
+    # arithmetic per row step against 148 SM x 128 lanes x SM clock (no FMA: one operation per lane and clock)
+    sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
+    alu_peak = 148 * 128 * sm_mhz * 1e6 / 1e9
+    alu_ops = FP32_OPS_PER_ROW_STEP * (stats["row_steps"] + 3 * stats["track_hits"])
+    alu_ms = stage["tracklets"] + stage["refit"]
+    alu = {"achieved": alu_ops / (alu_ms * 1e-3) / 1e9, "peak": alu_peak, "unit": "Gop/s",
+           "frac": alu_ops / (alu_ms * 1e-3) / 1e9 / alu_peak, "kernels": "tracklets+refit",
+           "ops_per_row_step": FP32_OPS_PER_ROW_STEP}
     roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": None, "peak_source": peak_src, "algorithmic_bytes": alg[dom], "kernel_ms": stage[dom],
-                "stages": per_stage}
-    # ---- CPU baseline: the oracle on a bounded sample of the same workload
-    cb_scale = 0.1
-    cv, ct, cn = oracle_timed(cb_scale, 5, 1, 0)
-    cpu_baseline = {"value": cv, "unit": UNIT, "cores": 1, "kind": "oracle",
-                    "sample": f"config 5 at {int(round(50 * cb_scale))} collisions in {1000 * cb_scale:.0f} us "
-                              f"(same occupancy), {cn} clusters, {ct:.1f} s"}
+                "traffic": ncu_traffic(dom), "peak_source": peak_src, "algorithmic_bytes": alg[dom],
+                "kernel_ms": stage[dom], "stages": per_stage, "alu": alu}
+    # ---- CPU baseline: the oracle as it stands, one pass over the same frame (rank 0, N = 1 only)
+    cpu_baseline = None
+    if world == 1:
+        cv, ct, cn = oracle_timed(1.0, 5, 1, 0, fr=fr)
+        cpu_baseline = {"value": cv, "unit": UNIT, "cores": 1, "kind": "oracle",
+                        "sample": f"one pass over the same config-5 frame, {cn} clusters, {ct:.1f} s"}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
@@ -234,7 +285,7 @@ def run_gpu(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="tpcca", choices=["tpcca", "reference"])
     ap.add_argument("--params", default="", help="k=v,k=v overrides of tpcca_params (tuning experiments)")

@@ -385,3 +385,20 @@ def test_edge_cases(row_x):
     y, z, s = helix_points(row_x[rows].astype(np.float64), 85.0, 0.0, 10.0, 0.05, 0.4, 1.0, 0.5)
     r = oracle.track(_mk(rows, y, z, row_x), np.array([0, len(rows)], np.int32), row_x)
     assert (r.link_up_raw == -1).all() and len(r.tracks) == 0
+
+
+def test_golden_oracle_regression():
+    """The oracle still reproduces tests/golden/oracle_regression.json (written by make_golden.py from the
+    oracle alone): guards the oracle's arithmetic against unintended change."""
+    import importlib.util
+    import json
+    import os
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(here, "make_golden.py"))
+    mg = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mg)
+    stored = json.load(open(os.path.join(here, "oracle_regression.json")))
+    assert len(stored) == len(mg.CASES)
+    for exp in stored:
+        got = mg.digest(exp["case"])
+        assert got == exp, (got, exp)
