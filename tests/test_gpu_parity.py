@@ -22,6 +22,18 @@ def test_parity_config5_reduced(row_x):
     compare(fr, row_x)
 
 
+@pytest.mark.parametrize("cfg", [4, 5])
+def test_parity_full_size_bench_configuration(row_x, cfg):
+    """BASELINE.json's full sizes (config 4: 6.5 M, config 5: 15.2 M clusters) in the launch configuration bench.py
+    times (same capacities): every link, start hit, tracklet table, assignment and track record against the oracle."""
+    fr = synth.generate(synth.config(cfg, seed=cfg))
+    t = B.Tracker(row_x, n_sectors=36, max_clusters=fr.n, max_tracklets=max(1 << 16, fr.n // 8),
+                  max_tracks=max(1 << 16, fr.n // 24))
+    t, orc, exact = compare(fr, row_x, tracker=t)
+    assert len(orc.tracks) > 50000
+    assert exact
+
+
 def test_grid_policy_does_not_change_results(row_x):
     fr = synth.generate(synth.config(2, scale=0.1, seed=21))
     base = run_gpu(fr, row_x)
