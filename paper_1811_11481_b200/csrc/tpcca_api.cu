@@ -69,7 +69,9 @@ static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params
   CARVE(d.sb_skey, int32_t, T);
   CARVE(d.start_hits, int32_t, T);
   CARVE(d.seed_w, int32_t, T + 1);
-  CARVE(d.ord, int32_t, 1024);
+  CARVE(d.ord, int32_t, 3 * 1024);
+  CARVE(d.e_key, int32_t, 2 * T);
+  CARVE(d.e_order, int32_t, 2 * T);
   CARVE(d.work_t, int32_t, T);
   CARVE(d.row_hit, int32_t, T * (size_t)g->n_rows);
   CARVE(d.tl_state, float, T * 24);
@@ -81,6 +83,7 @@ static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params
   CARVE(d.track_tracklet, int32_t, K);
   CARVE(d.track_w, int32_t, K);
   CARVE(d.track_order, int32_t, K);
+  CARVE(d.track_len, int32_t, K);
   CARVE(d.w_list, int2, T);
   CARVE(d.th_yz, float2, N);
   CARVE(d.th_row, uint8_t, N);

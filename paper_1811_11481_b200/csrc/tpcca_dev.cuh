@@ -76,7 +76,9 @@ struct Dev {
   int32_t* start_hits;     // [max_tracklets] canonical order (sorted indices)
   // (e)
   int32_t* seed_w;         // [max_tracklets+1] tracklet id t -> work index w, -1 for void seeds
-  int32_t* ord;            // [1024] track-length histogram [0,512) and bucket cursors [512,1024) (zeroed per call)
+  int32_t* ord;            // [3][1024] counting-sort scratch per order (0 refit, 1 E2, 2 E3): histogram [0,512), cursors [512,1024); zeroed per call
+  int32_t* e_key;          // [2][max_tracklets] w-space sort keys (expected row steps) of the E2 / E3 work orders
+  int32_t* e_order;        // [2][max_tracklets] E2 / E3 work orders: w by decreasing key
   int32_t* work_t;         // [max_tracklets] w -> t
   int32_t* row_hit;        // [max_tracklets][n_rows] indexed by w (dense over surviving seeds)
   float* tl_state;         // [max_tracklets][24] w-space: x, 5 parameters, 15 cov, chi2, row, valid
@@ -90,6 +92,7 @@ struct Dev {
   int32_t* track_tracklet; // [max_tracks] track id -> t
   int32_t* track_w;        // [max_tracks] track id -> w
   int32_t* track_order;    // [max_tracks] refit order: track ids by decreasing hit count
+  int32_t* track_len;      // [max_tracks] hit count of track id (sort key of the refit order)
   int2* w_list;            // [max_tracklets] w-space, accepted tracklets: (offset, count) of the owned-hit list
   float2* th_yz;           // [n] owned-hit lists (innermost first): (y, z)
   uint8_t* th_row;         // [n] their rows
@@ -287,3 +290,7 @@ void launch_refit(const Dev& d, Launch& L);
 void launch_export(const Dev& d, int what, void* dst, Launch& L);
 // exclusive scan of data[0..n) in place, n read from *n_dev (<= n_max); data[n] receives the total
 void launch_scan_i32(int32_t* data, const int32_t* n_dev, int32_t n_max, int32_t* tmp, Launch& L);
+// out[0..n) = indices 0..n-1 ordered by decreasing key[i] (keys in [0,256]; order inside a key is arbitrary);
+// n read from *n_dev (<= n_max); slot selects the scratch block of Dev::ord
+void launch_order_desc(const Dev& d, int slot, const int32_t* key, const int32_t* n_dev, int32_t n_max, int32_t* out,
+                       Launch& L);

@@ -85,6 +85,64 @@ void launch_scan_i32(int32_t* data, const int32_t* n_dev, int32_t n_max, int32_t
   L.count += 4;
 }
 
+// ---------------------------------------------------------------- counting sort by decreasing key (work orders)
+// Longest-first work orders for the persistent Kalman kernels and the refit: lanes of a warp then run about the
+// same number of row steps and the short items fill the tail.  ord = [hist 0..511 | cursors 512..1023], zeroed.
+#define ORD_THREADS 1024
+#define ORD_KEYS 257
+__global__ void __launch_bounds__(ORD_THREADS) k_order_hist(int32_t* __restrict__ ord, const int32_t* __restrict__ key,
+                                                            const int32_t* __restrict__ n_dev, int32_t n_max) {
+  __shared__ int s_hist[ORD_KEYS];
+  const int n = min(*n_dev, n_max);
+  if (blockIdx.x * ORD_THREADS >= n) return;
+  for (int i = threadIdx.x; i < ORD_KEYS; i += ORD_THREADS) s_hist[i] = 0;
+  __syncthreads();
+  const int i = blockIdx.x * ORD_THREADS + threadIdx.x;
+  if (i < n) atomicAdd(&s_hist[min(max(key[i], 0), ORD_KEYS - 1)], 1);
+  __syncthreads();
+  for (int k = threadIdx.x; k < ORD_KEYS; k += ORD_THREADS)
+    if (s_hist[k]) atomicAdd(&ord[k], s_hist[k]);
+}
+__global__ void __launch_bounds__(512) k_order_offsets(int32_t* __restrict__ ord) {
+  __shared__ int sm[32];
+  const int i = threadIdx.x;  // position i holds key ORD_KEYS-1-i
+  const int v = (i < ORD_KEYS) ? ord[ORD_KEYS - 1 - i] : 0;
+  int tot;
+  const int e = block_scan_excl(v, &tot, sm);
+  if (i < ORD_KEYS) ord[512 + ORD_KEYS - 1 - i] = e;
+}
+__global__ void __launch_bounds__(ORD_THREADS) k_order_scatter(int32_t* __restrict__ ord, const int32_t* __restrict__ key,
+                                                               const int32_t* __restrict__ n_dev, int32_t n_max,
+                                                               int32_t* __restrict__ out) {
+  __shared__ int s_cnt[ORD_KEYS], s_base[ORD_KEYS];
+  const int n = min(*n_dev, n_max);
+  if (blockIdx.x * ORD_THREADS >= n) return;
+  for (int i = threadIdx.x; i < ORD_KEYS; i += ORD_THREADS) s_cnt[i] = 0;
+  __syncthreads();
+  const int i = blockIdx.x * ORD_THREADS + threadIdx.x;
+  int k = 0, rank = 0;
+  if (i < n) {
+    k = min(max(key[i], 0), ORD_KEYS - 1);
+    rank = atomicAdd(&s_cnt[k], 1);
+  }
+  __syncthreads();
+  for (int q = threadIdx.x; q < ORD_KEYS; q += ORD_THREADS)
+    if (s_cnt[q]) s_base[q] = atomicAdd(&ord[512 + q], s_cnt[q]);
+  __syncthreads();
+  if (i < n) out[s_base[k] + rank] = i;
+}
+
+void launch_order_desc(const Dev& d, int slot, const int32_t* key, const int32_t* n_dev, int32_t n_max, int32_t* out,
+                       Launch& L) {
+  if (n_max <= 0) return;
+  int32_t* ord = d.ord + 1024 * slot;
+  const int nb = (n_max + ORD_THREADS - 1) / ORD_THREADS;
+  k_order_hist<<<nb, ORD_THREADS, 0, L.st>>>(ord, key, n_dev, n_max);
+  k_order_offsets<<<1, 512, 0, L.st>>>(ord);
+  k_order_scatter<<<nb, ORD_THREADS, 0, L.st>>>(ord, key, n_dev, n_max, out);
+  L.count += 3;
+}
+
 // ---------------------------------------------------------------- (a0) reset per-call state
 __global__ void k_reset(Dev d) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -98,7 +156,7 @@ __global__ void k_reset(Dev d) {
     d.slice_bbox[4 * i + 2] = 0xFFFFFFFFu;  // zmin
     d.slice_bbox[4 * i + 3] = 0u;           // zmax
   }
-  if (i < 1024) d.ord[i] = 0;
+  if (i < 3 * 1024) d.ord[i] = 0;
   if (i == 0) {
     d.cnt->n_start = 0; d.cnt->n_tracks = 0; d.cnt->n_valid = 0; d.cnt->status = 0; d.cnt->n_bins = 0; d.cnt->n_start_raw = 0; d.cnt->n_work = 0; d.cnt->work_next[0] = 0; d.cnt->work_next[1] = 0; d.cnt->work_next[2] = 0;
     d.cnt->row_steps = 0ull; d.cnt->searches = 0ull; d.cnt->track_hits = 0ull;
@@ -261,7 +319,7 @@ __global__ void __launch_bounds__(256) k_scatter(Dev d, SecOff so) {
 }
 
 void launch_grid(const Dev& d, const SecOff& so, Launch& L) {
-  k_reset<<<(max(d.n_slices, 1024) + 256) / 256, 256, 0, L.st>>>(d);
+  k_reset<<<(max(d.n_slices, 3 * 1024) + 256) / 256, 256, 0, L.st>>>(d);
   L.count++;
   if (d.n > 0) {
     k_slice_count<<<(d.n + A1_THREADS * A1_ITEMS - 1) / (A1_THREADS * A1_ITEMS), A1_THREADS, 0, L.st>>>(d, so);

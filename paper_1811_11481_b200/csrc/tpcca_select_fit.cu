@@ -56,9 +56,6 @@ __global__ void __launch_bounds__(SEL_THREADS) k_select_own(Dev d) {
 // ---------------------------------------------------------------- (f2) after the scan: track ids, length histogram
 // Track ids follow tracklet-id order (the work list is in that order).
 __global__ void __launch_bounds__(256) k_select_ids(Dev d) {
-  __shared__ int s_hist[TPCCA_MAX_ROWS + 1];
-  for (int i = threadIdx.x; i <= TPCCA_MAX_ROWS; i += blockDim.x) s_hist[i] = 0;
-  __syncthreads();
   const int w = blockIdx.x * blockDim.x + threadIdx.x;
   const int nw = d.cnt->n_work;
   if (w == 0) {
@@ -66,38 +63,16 @@ __global__ void __launch_bounds__(256) k_select_ids(Dev d) {
     if (tot > d.max_tracks) atomicOr(&d.cnt->status, TPCCA_STAT_TRACK_OVERFLOW);
     d.cnt->n_tracks = min(tot, d.max_tracks);
   }
-  if (w < nw) {
-    const int t = d.work_t[w];
-    const int id = d.sel_scan[t];
-    const bool acc = (d.sel_scan[t + 1] != id) && (id < d.max_tracks);
-    d.tl_track[t] = acc ? id : -1;
-    if (acc) {
-      d.track_w[id] = w;
-      d.track_tracklet[id] = t;
-      atomicAdd(&s_hist[d.w_list[w].y], 1);
-    }
+  if (w >= nw) return;
+  const int t = d.work_t[w];
+  const int id = d.sel_scan[t];
+  const bool acc = (d.sel_scan[t + 1] != id) && (id < d.max_tracks);
+  d.tl_track[t] = acc ? id : -1;
+  if (acc) {
+    d.track_w[id] = w;
+    d.track_tracklet[id] = t;
+    d.track_len[id] = d.w_list[w].y;
   }
-  __syncthreads();
-  for (int i = threadIdx.x; i <= TPCCA_MAX_ROWS; i += blockDim.x)
-    if (s_hist[i]) atomicAdd(&d.ord[i], s_hist[i]);
-}
-
-// (f2') refit order: tracks sorted by decreasing hit count (counting sort), so that the lanes of a refit warp run
-// the same number of steps and the longest tracks start first.  The order inside a bucket is arbitrary: every track
-// writes its own record, no result depends on it.
-__global__ void __launch_bounds__(512) k_len_offsets(Dev d) {
-  __shared__ int sm[32];
-  const int i = threadIdx.x;  // bucket i holds length TPCCA_MAX_ROWS - i
-  const int v = (i <= TPCCA_MAX_ROWS) ? d.ord[TPCCA_MAX_ROWS - i] : 0;
-  int tot;
-  const int e = block_scan_excl(v, &tot, sm);
-  if (i <= TPCCA_MAX_ROWS) d.ord[512 + TPCCA_MAX_ROWS - i] = e;
-}
-__global__ void __launch_bounds__(256) k_len_scatter(Dev d) {
-  const int id = blockIdx.x * blockDim.x + threadIdx.x;
-  if (id >= d.cnt->n_tracks) return;
-  const int n = d.w_list[d.track_w[id]].y;
-  d.track_order[atomicAdd(&d.ord[512 + n], 1)] = id;
 }
 
 // ---------------------------------------------------------------- (f3) cluster -> track assignment
@@ -120,13 +95,10 @@ void launch_select(const Dev& d, Launch& L) {
   L.count++;
   launch_scan_i32(d.sel_scan, &d.cnt->n_start, T, d.scan_tmp, L);
   k_select_ids<<<(T + 255) / 256, 256, 0, L.st>>>(d);
-  k_len_offsets<<<1, 512, 0, L.st>>>(d);
   k_assign<<<(d.n + 255) / 256, 256, 0, L.st>>>(d);
-  L.count += 3;
-  if (d.max_tracks > 0) {
-    k_len_scatter<<<(d.max_tracks + 255) / 256, 256, 0, L.st>>>(d);
-    L.count++;
-  }
+  L.count += 2;
+  // refit order: tracks by decreasing hit count, so that the lanes of a refit warp run the same number of steps
+  launch_order_desc(d, 0, d.track_len, &d.cnt->n_tracks, d.max_tracks, d.track_order, L);
 }
 
 // ---------------------------------------------------------------- (g) refit

@@ -169,6 +169,7 @@ __global__ void __launch_bounds__(E_THREADS, 8) k_tl_e1(Dev d) {
         st_store_kf(st, k);
         reinterpret_cast<int*>(st)[22] = last_row;
         reinterpret_cast<int*>(st)[23] = valid ? 1 : 0;
+        d.e_key[w] = valid ? R - 1 - last_row : 0;  // E2 work order: rows left above the chain
         w = -1;
       }
       const int nw = fetch_work(&d.cnt->work_next[0], need, lane, nm);
@@ -241,13 +242,14 @@ __global__ void __launch_bounds__(E_THREADS, 6) k_tl_e2(Dev d) {
           st[4] = st_; st[5] = sq;
           reinterpret_cast<int*>(st)[22] = top_row;
         }
+        d.e_key[d.max_tracklets + w] = live ? top_row + 1 : 0;  // E3 work order: rows from the outermost hit down
         w = -1;
       }
       const int nw = fetch_work(&d.cnt->work_next[1], need, lane, nm);
       if (need) {
         if (nw >= n_work) exhausted = true;
         else {
-          w = nw;
+          w = d.e_order[nw];
           const float* st = d.tl_state + (size_t)w * 24;
           live = reinterpret_cast<const int*>(st)[23] != 0;
           if (live) {
@@ -334,7 +336,7 @@ __global__ void __launch_bounds__(E_THREADS, 6) k_tl_e3(Dev d) {
       if (need) {
         if (nw >= n_work) exhausted = true;
         else {
-          w = nw;
+          w = d.e_order[d.max_tracklets + nw];
           t = d.work_t[w];
           const float* st = d.tl_state + (size_t)w * 24;
           live = reinterpret_cast<const int*>(st)[23] != 0;
@@ -417,7 +419,9 @@ void launch_tracklets(const Dev& d, Launch& L) {
   launch_scan_i32(d.seed_w, &d.cnt->n_start, T, d.scan_tmp, L);
   k_seed_compact<<<(T + 255) / 256, 256, 0, L.st>>>(d);
   k_tl_e1<<<148 * 8, E_THREADS, 0, L.st>>>(d);
+  launch_order_desc(d, 1, d.e_key, &d.cnt->n_work, T, d.e_order, L);
   k_tl_e2<<<148 * 6, E_THREADS, 0, L.st>>>(d);
+  launch_order_desc(d, 2, d.e_key + T, &d.cnt->n_work, T, d.e_order + T, L);
   k_tl_e3<<<148 * 6, E_THREADS, 0, L.st>>>(d);
   k_tracklet_weights<<<148 * 16, 128, 0, L.st>>>(d);
   L.count += 5;
