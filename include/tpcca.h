@@ -65,7 +65,7 @@ typedef struct {
   int32_t min_seed_hits, min_tracklet_hits, min_track_hits;
   float qual_scale;
   float grid_bin_y, grid_bin_z_min;         /* cm */
-  float grid_bins_per_cluster;              /* target bins per cluster in a row slice, <= 2 */
+  float grid_bins_per_cluster;              /* target bins per cluster in a row slice, <= 4 */
   int64_t max_clusters;                     /* capacity per call */
   int32_t max_tracklets, max_tracks;
   void* workspace;                          /* device, >= tpcca_workspace_bytes(), 256-byte aligned; caller-owned */

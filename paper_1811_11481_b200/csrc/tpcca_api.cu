@@ -35,7 +35,7 @@ static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params
   size_t off = 0;
   const size_t N = (size_t)p->max_clusters, T = (size_t)p->max_tracklets, K = (size_t)p->max_tracks;
   const size_t SL = (size_t)g->n_sectors * g->n_rows;
-  const size_t NB = 2 * N + 128 * SL + 1;
+  const size_t NB = 4 * N + 128 * SL + 1;
   const size_t NSCAN = T + 8 + NB / 2048 + T / 2048 + 64;
 #define CARVE(field, type, count)                                  \
   do {                                                             \
@@ -105,7 +105,7 @@ static bool check_geo_params(const tpcca_geometry* g, const tpcca_params* p) {
   }
   if (p->min_track_hits < 2 || p->min_tracklet_hits < 2 || p->min_seed_hits < 2) { set_err("min_*_hits must be >= 2"); return false; }
   if (!(p->sigma_y > 0) || !(p->sigma_z > 0)) { set_err("sigma_y/sigma_z must be > 0"); return false; }
-  if (!(p->grid_bin_y > 0) || !(p->grid_bin_z_min > 0) || !(p->grid_bins_per_cluster > 0) || p->grid_bins_per_cluster > 2.0f) {
+  if (!(p->grid_bin_y > 0) || !(p->grid_bin_z_min > 0) || !(p->grid_bins_per_cluster > 0) || p->grid_bins_per_cluster > 4.0f) {
     set_err("grid_* parameters out of range"); return false;
   }
   return true;
@@ -121,7 +121,7 @@ void tpcca_default_params(tpcca_params* p) {
   p->cov0[0] = 1.0f; p->cov0[1] = 1.0f; p->cov0[2] = 0.25f; p->cov0[3] = 1.0f; p->cov0[4] = 100.0f;
   p->pick_cut = 16.0f; p->reject_cut = 25.0f; p->max_gap = 5; p->edge_margin = 3.0f; p->max_sinphi = 0.95f;
   p->min_seed_hits = 4; p->min_tracklet_hits = 10; p->min_track_hits = 10; p->qual_scale = 1000.0f;
-  p->grid_bin_y = 4.0f; p->grid_bin_z_min = 2.5f; p->grid_bins_per_cluster = 1.0f;
+  p->grid_bin_y = 6.0f; p->grid_bin_z_min = 2.5f; p->grid_bins_per_cluster = 2.0f;
 }
 
 size_t tpcca_workspace_bytes(const tpcca_geometry* g, const tpcca_params* p) {

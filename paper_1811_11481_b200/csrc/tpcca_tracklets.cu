@@ -99,51 +99,54 @@ __device__ __noinline__ bool tie_less(const Dev& d, int c, float2 p, int best) {
   return key_less(p.y, p.x, d.orig_idx[c], q.y, q.x, d.orig_idx[best]);
 }
 
-// Candidate choice of one row step (O5 "Search" and the E3 keep/reject test) in ONE code path:
-// cur >= 0  -> the only candidate is the existing hit `cur`, kept iff d <= reject_cut (no window);
-// cur <  0  -> the clusters of slice g inside the window compete, best = min by (d, key), d <= pick_cut.
-// Returns the chosen sorted index or -1; pbest = its (y, z).
-__device__ __forceinline__ int choose_hit(const Dev& d, const GridHdr& g, const KF& k, float z_ref, int cur,
-                                          float2& pbest) {
-  const bool hit = cur >= 0;
-  const float cut = hit ? d.P.reject_cut : d.P.pick_cut;
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+
+// Pick-up search of one row step (O5 "Search"): the clusters of slice g inside the window compete,
+// best = min by (d, key) among d <= pick_cut.  Returns the chosen sorted index or -1; pbest = its (y, z).
+// The candidates of up to two y-bin rows form one flat index space that is walked four at a time: the four loads
+// are independent and every lane runs the same four evaluations, so a warp whose lanes hold 0..4 candidates
+// (the usual case) makes one converged pass.
+#define SEARCH_UNROLL 4
+__device__ __forceinline__ int search_row(const Dev& d, const GridHdr& g, const KF& k, float z_ref, float2& pbest) {
+  const float cut = d.P.pick_cut;
   const float vy = k.c00 + d.sy2, vz = k.c11 + d.sz2;
   const float iy = 1.0f / vy, iz = 1.0f / vz;
-  float wy = sqrtf(cut * vy), wz = sqrtf(cut * vz);
-  int y0 = 0, y1 = 0, z0 = 0, z1 = 0;
-  if (hit) {
-    wy = wz = __int_as_float(0x7f800000);  // +inf: no window on the keep/reject test
-  } else {
-    const float zc = z_ref + k.z;  // search centre in frame coordinates (bin lookup only)
-    const float mz = 2e-3f + (fabsf(zc) + fabsf(z_ref) + fabsf(k.z)) * 4e-7f;
-    bin_range(k.y - wy - 1e-3f, k.y + wy + 1e-3f, g.ymin, g.inv_by, g.ny, y0, y1);
-    bin_range(zc - wz - mz, zc + wz + mz, g.zmin, g.inv_bz, g.nz, z0, z1);
-    if (z0 > z1 || g.pad == 0) { y0 = 1; y1 = 0; }  // NaN / empty window, or empty row
-  }
+  const float wy = sqrtf(cut * vy), wz = sqrtf(cut * vz);
+  int y0, y1, z0, z1;
+  const float zc = z_ref + k.z;  // search centre in frame coordinates (bin lookup only)
+  const float mz = 2e-3f + (fabsf(zc) + fabsf(z_ref) + fabsf(k.z)) * 4e-7f;
+  bin_range(k.y - wy - 1e-3f, k.y + wy + 1e-3f, g.ymin, g.inv_by, g.ny, y0, y1);
+  bin_range(zc - wz - mz, zc + wz + mz, g.zmin, g.inv_bz, g.nz, z0, z1);
+  if (z0 > z1 || g.pad == 0) { y0 = 1; y1 = 0; }  // NaN / empty window, or empty row
   int best = -1;
   float bd = 0.0f;
-  for (int yb = y0; yb <= y1; yb += 2) {  // two y-bin rows per pass, their candidates in one flat loop
-    int a0, a1, b0 = 0, b1 = 0;
-    if (hit) { a0 = cur; a1 = cur + 1; }
-    else {
-      const int* bs = d.bin_start + g.bin_base + yb * g.nz;
-      a0 = bs[z0]; a1 = bs[z1 + 1];
-      if (yb + 1 <= y1) { b0 = bs[g.nz + z0]; b1 = bs[g.nz + z1 + 1]; }
-    }
+  for (int yb = y0; yb <= y1; yb += 2) {
+    const int* bs = d.bin_start + g.bin_base + yb * g.nz;
+    const bool two = yb + 1 <= y1;
+    const int a0 = bs[z0], a1 = bs[z1 + 1];
+    int b0 = 0, b1 = 0;
+    if (two) { b0 = bs[g.nz + z0]; b1 = bs[g.nz + z1 + 1]; }
     const int na = a1 - a0, ntot = na + (b1 - b0);
-    for (int i = 0; i < ntot; i++) {
-      const int c = (i < na) ? a0 + i : b0 + (i - na);
-      const float2 p = d.yz[c];
-      const float dy = p.x - k.y;
-      const float dz = (p.y - z_ref) - k.z;
-      if (!(fabsf(dy) <= wy) || !(fabsf(dz) <= wz)) continue;
-      const float dist = (dy * dy) * iy + (dz * dz) * iz;
-      if (!(dist <= cut)) continue;
-      bool better;
-      if (best < 0) better = true;
-      else if (dist != bd) better = dist < bd;
-      else better = tie_less(d, c, p, best);
-      if (better) { best = c; bd = dist; pbest = p; }
+    for (int i = 0; i < ntot; i += SEARCH_UNROLL) {
+      float2 p[SEARCH_UNROLL];
+      int c[SEARCH_UNROLL];
+#pragma unroll
+      for (int j = 0; j < SEARCH_UNROLL; j++) {
+        const int ii = min(i + j, ntot - 1);  // clamped: a repeated candidate cannot change the minimum
+        c[j] = (ii < na) ? a0 + ii : b0 + (ii - na);
+        p[j] = d.yz[c[j]];
+      }
+#pragma unroll
+      for (int j = 0; j < SEARCH_UNROLL; j++) {
+        const float dy = p[j].x - k.y;
+        const float dz = (p[j].y - z_ref) - k.z;
+        const float dist = (dy * dy) * iy + (dz * dz) * iz;
+        if ((fabsf(dy) <= wy) && (fabsf(dz) <= wz) && (dist <= cut) && c[j] != best) {
+          bool better = (best < 0) || (dist < bd);
+          if (!better && dist == bd) better = tie_less(d, c[j], p[j], best);
+          if (better) { best = c[j]; bd = dist; pbest = p[j]; }
+        }
+      }
     }
   }
   return best;
@@ -272,13 +275,14 @@ __global__ void __launch_bounds__(E_THREADS, 6) k_tl_e2(Dev d) {
     // ---- one row step
     n_steps++;
     const GridHdr g = d.grid[sbase + r];
+    if (r + 1 < R) prefetch_l1(&d.grid[sbase + r + 1]);
     const float xr = d.row_x[r];
     if (!kf_transport(k, xr, d.kq, d.P.max_sinphi) || fabsf(k.y) > xr * d.tan_half_angle + d.P.edge_margin) {
       busy = false;
       continue;
     }
     float2 pb = make_float2(0.f, 0.f);
-    const int cand = choose_hit(d, g, k, z_ref, -1, pb);
+    const int cand = search_row(d, g, k, z_ref, pb);
     rh[r] = cand;
     if (cand >= 0) {
       kf_update(k, pb.x, pb.y - z_ref, d.sy2, d.sz2);
@@ -359,18 +363,29 @@ __global__ void __launch_bounds__(E_THREADS, 6) k_tl_e3(Dev d) {
       if (__ballot_sync(FULL, !exhausted) == 0u) break;
     }
     if (!busy) continue;
-    // ---- one row step
+    // ---- one row step.  Loads that do not depend on the filter state go first; the next row's are prefetched.
     n_steps++;
     const int cur = (r >= r0) ? rh[r] : -1;
-    const GridHdr g = d.grid[sbase + r];
+    float2 pb = make_float2(0.f, 0.f);
+    if (cur >= 0) pb = d.yz[cur];
+    if (r > 0) prefetch_l1(&d.grid[sbase + r - 1]);
     const float xr = d.row_x[r];
     if (!kf_transport(k, xr, d.kq, d.P.max_sinphi) || fabsf(k.y) > xr * d.tan_half_angle + d.P.edge_margin) {
       busy = false;
       continue;
     }
-    if (cur < 0) n_search++;
-    float2 pb = make_float2(0.f, 0.f);
-    const int cand = choose_hit(d, g, k, z_ref, cur, pb);
+    int cand;
+    if (cur >= 0) {  // existing hit: kept iff d <= reject_cut (no window), O5/E3
+      const float iy = 1.0f / (k.c00 + d.sy2), iz = 1.0f / (k.c11 + d.sz2);
+      const float dy = pb.x - k.y;
+      const float dz = (pb.y - z_ref) - k.z;
+      const float dist = (dy * dy) * iy + (dz * dz) * iz;
+      cand = (dist <= d.P.reject_cut) ? cur : -1;
+    } else {
+      n_search++;
+      const GridHdr g = d.grid[sbase + r];
+      cand = search_row(d, g, k, z_ref, pb);
+    }
     if (cand != cur || r < r0) rh[r] = cand;  // rejected seed hit -> -1, or the search result (rows below the seed are unwritten)
     if (cand >= 0) {
       kf_update(k, pb.x, pb.y - z_ref, d.sy2, d.sz2);
