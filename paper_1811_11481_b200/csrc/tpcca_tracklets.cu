@@ -106,7 +106,9 @@ __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefe
 // The candidates of up to two y-bin rows form one flat index space that is walked four at a time: the four loads
 // are independent and every lane runs the same four evaluations, so a warp whose lanes hold 0..4 candidates
 // (the usual case) makes one converged pass.
-#define SEARCH_UNROLL 4
+#ifndef SEARCH_UNROLL
+#define SEARCH_UNROLL 3
+#endif
 __device__ __forceinline__ int search_row(const Dev& d, const GridHdr& g, const KF& k, float z_ref, float2& pbest) {
   const float cut = d.P.pick_cut;
   const float vy = k.c00 + d.sy2, vz = k.c11 + d.sz2;
