@@ -6,37 +6,113 @@
 
 // ---------------------------------------------------------------- (b)
 // One thread per sorted cluster; consecutive threads are neighbours in (row, y-bin, z-bin), so a warp's
-// candidate ranges coincide and its loop trip counts are nearly uniform.  Two phases keep the lanes
-// converged: first the down-row candidates that pass the window are collected in registers (up to
-// ND_MAX), then every up-row candidate that passes is paired with them.  More than ND_MAX down
-// candidates (dense noise) fall back to the plain nested loops -- same result either way.
-#define ND_MAX 4
+// candidate ranges overlap (L1 hits) and its loop trip counts are close.  Three phases keep the lanes together:
+// the window candidates of the down row and of the up row are collected into per-thread shared-memory lists
+// (NB_CAP entries each; the bins of up to two y-bin rows form one flat index space walked NB_UNROLL at a time
+// with independent loads), then the (up, down) pairs are evaluated from shared memory.  A list that overflows
+// (dense noise) falls back to the plain nested loops -- same result either way.
+#define NB_THREADS 128
+#define NB_CAP 8
+#ifndef NB_UNROLL
+#define NB_UNROLL 2
+#endif
 
 struct Best {
   int bu, bd;
   float bc;
 };
 
+// (plain pointers, not Dev&: a reference to the kernel parameter block would force a local-memory copy of it)
+__device__ __noinline__ bool pair_tie_better(const float2* yz, const int32_t* orig_idx, int bu, int bd, int u, float yu,
+                                             float zu, int dd, float yd, float zd) {
+  if (u != bu) {
+    const float2 q = yz[bu];
+    return key_less(zu, yu, orig_idx[u], q.y, q.x, orig_idx[bu]);
+  }
+  const float2 q = yz[bd];
+  return key_less(zd, yd, orig_idx[dd], q.y, q.x, orig_idx[bd]);
+}
+
 __device__ __forceinline__ void consider(const Dev& d, Best& b, float cost, int u, float yu, float zu, int dd, float yd,
                                          float zd) {
   if (!(cost <= d.P.triplet_cut)) return;
-  bool better;
-  if (b.bu < 0) better = true;
-  else if (cost != b.bc) better = cost < b.bc;
-  else {  // exact tie: value-based key order (rare; keys reloaded)
-    if (u != b.bu) {
-      const float2 q = d.yz[b.bu];
-      better = key_less(zu, yu, d.orig_idx[u], q.y, q.x, d.orig_idx[b.bu]);
-    } else {
-      const float2 q = d.yz[b.bd];
-      better = key_less(zd, yd, d.orig_idx[dd], q.y, q.x, d.orig_idx[b.bd]);
-    }
-  }
+  bool better = (b.bu < 0) || (cost < b.bc);
+  if (!better && cost == b.bc) better = pair_tie_better(d.yz, d.orig_idx, b.bu, b.bd, u, yu, zu, dd, yd, zd);  // exact tie: key order (rare)
   if (better) { b.bu = u; b.bd = dd; b.bc = cost; }
 }
 
-__global__ void __launch_bounds__(128) k_neighbours(Dev d) {
-  const int h = blockIdx.x * blockDim.x + threadIdx.x;
+// Window candidates of one neighbour row: appended to the calling thread's shared-memory list; returns their number
+// (entries beyond NB_CAP are counted, not stored).
+__device__ __forceinline__ int collect(const Dev& d, const GridHdr& g, float y0, float z0, float wy, float wz, float mz,
+                                       float2* __restrict__ lp, int* __restrict__ li) {
+  int by0, by1, bz0, bz1;
+  bin_range(y0 - wy - 1e-3f, y0 + wy + 1e-3f, g.ymin, g.inv_by, g.ny, by0, by1);
+  bin_range(z0 - wz - mz, z0 + wz + mz, g.zmin, g.inv_bz, g.nz, bz0, bz1);
+  if (bz0 > bz1) return 0;
+  int n = 0;
+  for (int by = by0; by <= by1; by += 2) {
+    const int* bs = d.bin_start + g.bin_base + by * g.nz;
+    const int a0 = bs[bz0], a1 = bs[bz1 + 1];
+    int b0 = 0, b1 = 0;
+    if (by + 1 <= by1) { b0 = bs[g.nz + bz0]; b1 = bs[g.nz + bz1 + 1]; }
+    const int na = a1 - a0, ntot = na + (b1 - b0);
+    for (int i = 0; i < ntot; i += NB_UNROLL) {
+      float2 p[NB_UNROLL];
+      int c[NB_UNROLL];
+#pragma unroll
+      for (int j = 0; j < NB_UNROLL; j++) {
+        const int ii = min(i + j, ntot - 1);
+        c[j] = (ii < na) ? a0 + ii : b0 + (ii - na);
+        p[j] = d.yz[c[j]];
+      }
+#pragma unroll
+      for (int j = 0; j < NB_UNROLL; j++) {
+        if ((i + j < ntot) && (fabsf(p[j].x - y0) <= wy) && (fabsf(p[j].y - z0) <= wz)) {
+          if (n < NB_CAP) { lp[n * NB_THREADS] = p[j]; li[n * NB_THREADS] = c[j]; }
+          n++;
+        }
+      }
+    }
+  }
+  return n;
+}
+
+// Fallback for overflowing lists: plain nested loops over both windows (O2 as written).
+__device__ __forceinline__ void nested_pairs(const Dev& d, const NbrHdr& nb, const GridHdr& gu, const GridHdr& gd, float y0,
+                                          float z0, float mz, Best& best) {
+  int uy0, uy1, uz0, uz1, dy0, dy1, dz0, dz1;
+  bin_range(y0 - nb.wyu - 1e-3f, y0 + nb.wyu + 1e-3f, gu.ymin, gu.inv_by, gu.ny, uy0, uy1);
+  bin_range(z0 - nb.wzu - mz, z0 + nb.wzu + mz, gu.zmin, gu.inv_bz, gu.nz, uz0, uz1);
+  bin_range(y0 - nb.wyd - 1e-3f, y0 + nb.wyd + 1e-3f, gd.ymin, gd.inv_by, gd.ny, dy0, dy1);
+  bin_range(z0 - nb.wzd - mz, z0 + nb.wzd + mz, gd.zmin, gd.inv_bz, gd.nz, dz0, dz1);
+  if (uz0 > uz1 || dz0 > dz1) return;
+  const float t = nb.t;
+  for (int by = uy0; by <= uy1; by++) {
+    const int* bs = d.bin_start + gu.bin_base + by * gu.nz;
+    const int ub = bs[uz0], ue = bs[uz1 + 1];
+    for (int u = ub; u < ue; u++) {
+      const float2 pu = d.yz[u];
+      if (!(fabsf(pu.x - y0) <= nb.wyu) || !(fabsf(pu.y - z0) <= nb.wzu)) continue;
+      for (int by2 = dy0; by2 <= dy1; by2++) {
+        const int* bs2 = d.bin_start + gd.bin_base + by2 * gd.nz;
+        const int db = bs2[dz0], de = bs2[dz1 + 1];
+        for (int dd = db; dd < de; dd++) {
+          const float2 pd = d.yz[dd];
+          if (!(fabsf(pd.x - y0) <= nb.wyd) || !(fabsf(pd.y - z0) <= nb.wzd)) continue;
+          const float ey = y0 - (pd.x + t * (pu.x - pd.x));
+          const float ez = z0 - (pd.y + t * (pu.y - pd.y));
+          const float cost = (ey * ey) * d.inv_sy2 + (ez * ez) * d.inv_sz2;
+          consider(d, best, cost, u, pu.x, pu.y, dd, pd.x, pd.y);
+        }
+      }
+    }
+  }
+}
+
+__global__ void __launch_bounds__(NB_THREADS) k_neighbours(Dev d) {
+  __shared__ float2 s_p[2][NB_CAP][NB_THREADS];
+  __shared__ int s_i[2][NB_CAP][NB_THREADS];
+  const int h = blockIdx.x * NB_THREADS + threadIdx.x;
   if (h >= d.n) return;
   const int sl = d.slice_of[h];
   const NbrHdr nb = d.nbr[sl];
@@ -45,66 +121,31 @@ __global__ void __launch_bounds__(128) k_neighbours(Dev d) {
   if (nb.su >= 0) {
     const float2 p0 = d.yz[h];
     const float y0 = p0.x, z0 = p0.y;
-    const float t = nb.t;
     const float mz = 1e-3f + fabsf(z0) * 4e-7f;
-    const GridHdr gu = d.grid[nb.su];
     const GridHdr gd = d.grid[nb.sd];
-    int uy0, uy1, uz0, uz1, dy0, dy1, dz0, dz1;
-    bin_range(y0 - nb.wyu - 1e-3f, y0 + nb.wyu + 1e-3f, gu.ymin, gu.inv_by, gu.ny, uy0, uy1);
-    bin_range(z0 - nb.wzu - mz, z0 + nb.wzu + mz, gu.zmin, gu.inv_bz, gu.nz, uz0, uz1);
-    bin_range(y0 - nb.wyd - 1e-3f, y0 + nb.wyd + 1e-3f, gd.ymin, gd.inv_by, gd.ny, dy0, dy1);
-    bin_range(z0 - nb.wzd - mz, z0 + nb.wzd + mz, gd.zmin, gd.inv_bz, gd.nz, dz0, dz1);
-    if (uz0 <= uz1 && dz0 <= dz1) {
-      // phase 1: down-row candidates inside the window
-      float cy[ND_MAX], cz[ND_MAX];
-      int ci[ND_MAX];
-      int nd = 0;
-      for (int by = dy0; by <= dy1; by++) {
-        const int* bs = d.bin_start + gd.bin_base + by * gd.nz;
-        const int cb = bs[dz0], ce = bs[dz1 + 1];
-        for (int c = cb; c < ce; c++) {
-          const float2 p = d.yz[c];
-          if (!(fabsf(p.x - y0) <= nb.wyd) || !(fabsf(p.y - z0) <= nb.wzd)) continue;
-#pragma unroll
-          for (int j = 0; j < ND_MAX; j++)
-            if (j == nd) { cy[j] = p.x; cz[j] = p.y; ci[j] = c; }
-          nd++;
-        }
-      }
-      if (nd > 0) {
-        // phase 2: up-row candidates, paired with the collected down candidates
-        for (int by = uy0; by <= uy1; by++) {
-          const int* bs = d.bin_start + gu.bin_base + by * gu.nz;
-          const int ub = bs[uz0], ue = bs[uz1 + 1];
-          for (int u = ub; u < ue; u++) {
-            const float2 pu = d.yz[u];
-            if (!(fabsf(pu.x - y0) <= nb.wyu) || !(fabsf(pu.y - z0) <= nb.wzu)) continue;
-            if (nd <= ND_MAX) {
-#pragma unroll
-              for (int j = 0; j < ND_MAX; j++) {
-                if (j < nd) {
-                  const float ey = y0 - (cy[j] + t * (pu.x - cy[j]));
-                  const float ez = z0 - (cz[j] + t * (pu.y - cz[j]));
-                  const float cost = (ey * ey) * d.inv_sy2 + (ez * ez) * d.inv_sz2;
-                  consider(d, best, cost, u, pu.x, pu.y, ci[j], cy[j], cz[j]);
-                }
-              }
-            } else {  // overflow: plain nested loop over the down row
-              for (int by2 = dy0; by2 <= dy1; by2++) {
-                const int* bs2 = d.bin_start + gd.bin_base + by2 * gd.nz;
-                const int db = bs2[dz0], de = bs2[dz1 + 1];
-                for (int dd = db; dd < de; dd++) {
-                  const float2 pd = d.yz[dd];
-                  if (!(fabsf(pd.x - y0) <= nb.wyd) || !(fabsf(pd.y - z0) <= nb.wzd)) continue;
-                  const float ey = y0 - (pd.x + t * (pu.x - pd.x));
-                  const float ez = z0 - (pd.y + t * (pu.y - pd.y));
-                  const float cost = (ey * ey) * d.inv_sy2 + (ez * ez) * d.inv_sz2;
-                  consider(d, best, cost, u, pu.x, pu.y, dd, pd.x, pd.y);
-                }
-              }
-            }
+    float2* lpd = &s_p[0][0][threadIdx.x];
+    int* lid = &s_i[0][0][threadIdx.x];
+    const int nd = collect(d, gd, y0, z0, nb.wyd, nb.wzd, mz, lpd, lid);
+    if (nd > 0) {
+      const GridHdr gu = d.grid[nb.su];
+      float2* lpu = &s_p[1][0][threadIdx.x];
+      int* liu = &s_i[1][0][threadIdx.x];
+      const int nu = collect(d, gu, y0, z0, nb.wyu, nb.wzu, mz, lpu, liu);
+      if (nd <= NB_CAP && nu <= NB_CAP) {
+        const float t = nb.t;
+        for (int ju = 0; ju < nu; ju++) {
+          const float2 pu = lpu[ju * NB_THREADS];
+          const int u = liu[ju * NB_THREADS];
+          for (int jd = 0; jd < nd; jd++) {
+            const float2 pd = lpd[jd * NB_THREADS];
+            const float ey = y0 - (pd.x + t * (pu.x - pd.x));
+            const float ez = z0 - (pd.y + t * (pu.y - pd.y));
+            const float cost = (ey * ey) * d.inv_sy2 + (ez * ez) * d.inv_sz2;
+            consider(d, best, cost, u, pu.x, pu.y, lid[jd * NB_THREADS], pd.x, pd.y);
           }
         }
+      } else if (nu > 0) {
+        nested_pairs(d, nb, gu, gd, y0, z0, mz, best);
       }
     }
   }
@@ -114,7 +155,7 @@ __global__ void __launch_bounds__(128) k_neighbours(Dev d) {
 
 void launch_neighbours(const Dev& d, Launch& L) {
   if (d.n <= 0) return;
-  k_neighbours<<<(d.n + 127) / 128, 128, 0, L.st>>>(d);
+  k_neighbours<<<(d.n + NB_THREADS - 1) / NB_THREADS, NB_THREADS, 0, L.st>>>(d);
   L.count++;
 }
 
