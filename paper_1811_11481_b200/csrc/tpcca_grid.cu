@@ -283,6 +283,10 @@ __global__ void __launch_bounds__(1024) k_slice_setup(Dev d) {
 __global__ void k_zero_bins(Dev d) {
   const int n = d.cnt->n_bins;
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i <= n; i += gridDim.x * blockDim.x) d.bin_start[i] = 0;
+  // hit weights of the selector: cleared here with coalesced stores rather than in the scatter
+  ulonglong2* hw = reinterpret_cast<ulonglong2*>(d.hit_weight);
+  const int n2 = (d.n + 1) >> 1;  // the array is 256-byte aligned and padded
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n2; i += gridDim.x * blockDim.x) hw[i] = make_ulonglong2(0ull, 0ull);
 }
 
 // ---------------------------------------------------------------- (a3) bin histogram (rank = arrival order)
@@ -315,7 +319,6 @@ __global__ void __launch_bounds__(256) k_scatter(Dev d, SecOff so) {
   d.yz[pos] = make_float2(c.y, c.z);
   d.orig_idx[pos] = i;
   d.slice_of[pos] = (uint16_t)sl;
-  d.hit_weight[pos] = 0ull;
 }
 
 void launch_grid(const Dev& d, const SecOff& so, Launch& L) {
