@@ -315,10 +315,15 @@ __global__ void __launch_bounds__(256) k_scatter(Dev d, SecOff so) {
   if (gb < 0) { d.out_assign[i] = -1; return; }
   const float4 c = __ldg(&d.clusters[i]);
   const int pos = d.bin_start[gb] + d.cluster_rank[i];
-  const int sl = sector_of(so, d.n_sectors, i) * d.n_rows + __float_as_int(c.w);
   d.yz[pos] = make_float2(c.y, c.z);
   d.orig_idx[pos] = i;
-  d.slice_of[pos] = (uint16_t)sl;
+}
+
+// slice id of every sorted position: one block per slice, coalesced stores (instead of a 2-byte scatter)
+__global__ void __launch_bounds__(128) k_fill_slice_of(Dev d) {
+  const int sl = blockIdx.x;
+  const int b = d.row_start[sl], e = d.row_start[sl + 1];
+  for (int i = b + threadIdx.x; i < e; i += blockDim.x) d.slice_of[i] = (uint16_t)sl;
 }
 
 void launch_grid(const Dev& d, const SecOff& so, Launch& L) {
@@ -336,6 +341,7 @@ void launch_grid(const Dev& d, const SecOff& so, Launch& L) {
     L.count++;
     launch_scan_i32(d.bin_start, &d.cnt->n_bins, d.max_bins, d.scan_tmp, L);
     k_scatter<<<(d.n + 255) / 256, 256, 0, L.st>>>(d, so);
-    L.count++;
+    k_fill_slice_of<<<d.n_slices, 128, 0, L.st>>>(d);
+    L.count += 2;
   }
 }

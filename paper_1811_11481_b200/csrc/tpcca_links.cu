@@ -113,7 +113,7 @@ __global__ void __launch_bounds__(NB_THREADS) k_neighbours(Dev d) {
   __shared__ float2 s_p[2][NB_CAP][NB_THREADS];
   __shared__ int s_i[2][NB_CAP][NB_THREADS];
   const int h = blockIdx.x * NB_THREADS + threadIdx.x;
-  if (h >= d.n) return;
+  if (h >= d.row_start[d.n_slices]) return;
   const int sl = d.slice_of[h];
   const NbrHdr nb = d.nbr[sl];
   Best best;
@@ -167,7 +167,7 @@ __global__ void __launch_bounds__(256) k_clean(Dev d) {
   __shared__ int s_base;
   const int h = blockIdx.x * blockDim.x + threadIdx.x;
   bool start = false;
-  if (h < d.n) {
+  if (h < d.row_start[d.n_slices]) {
     int u = d.link_up[h], dn = d.link_down[h];
     if (u >= 0 && d.link_down[u] != h) u = -1;
     if (dn >= 0 && d.link_up[dn] != h) dn = -1;

@@ -78,7 +78,7 @@ __global__ void __launch_bounds__(256) k_select_ids(Dev d) {
 // ---------------------------------------------------------------- (f3) cluster -> track assignment
 __global__ void __launch_bounds__(256) k_assign(Dev d) {
   const int h = blockIdx.x * blockDim.x + threadIdx.x;
-  if (h >= d.n) return;
+  if (h >= d.row_start[d.n_slices]) return;
   const unsigned long long w = d.hit_weight[h];
   int tr = -1;
   if (w) {
@@ -171,7 +171,7 @@ void launch_refit(const Dev& d, Launch& L) {
 // ---------------------------------------------------------------- exports (input-index space)
 __global__ void k_export_links(Dev d, int what, int32_t* dst) {
   const int h = blockIdx.x * blockDim.x + threadIdx.x;
-  if (h >= d.n) return;
+  if (h >= d.row_start[d.n_slices]) return;
   int v;
   if (what == TPCCA_LINK_UP_RAW) v = d.link_up[h];
   else if (what == TPCCA_LINK_DOWN_RAW) v = d.link_down[h];
