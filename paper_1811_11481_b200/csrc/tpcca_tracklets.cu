@@ -225,7 +225,10 @@ __global__ void __launch_bounds__(E_THREADS, 8) k_tl_e1(Dev d) {
 }
 
 // ---- E2: outward extrapolation, one best cluster per row
-__global__ void __launch_bounds__(E_THREADS, 6) k_tl_e2(Dev d) {
+#ifndef E2_BLOCKS
+#define E2_BLOCKS 6
+#endif
+__global__ void __launch_bounds__(E_THREADS, E2_BLOCKS) k_tl_e2(Dev d) {
   const int R = d.n_rows, n_work = d.cnt->n_work;
   const unsigned lane = threadIdx.x & 31;
   int n_steps = 0;
@@ -305,7 +308,10 @@ __global__ void __launch_bounds__(E_THREADS, 6) k_tl_e2(Dev d) {
 }
 
 // ---- E3: inward pass through the seed with outlier rejection, then pick-up below it
-__global__ void __launch_bounds__(E_THREADS, 6) k_tl_e3(Dev d) {
+#ifndef E3_BLOCKS
+#define E3_BLOCKS 6
+#endif
+__global__ void __launch_bounds__(E_THREADS, E3_BLOCKS) k_tl_e3(Dev d) {
   const int R = d.n_rows, n_work = d.cnt->n_work;
   const unsigned lane = threadIdx.x & 31;
   int n_steps = 0, n_search = 0, n_val = 0;
@@ -437,9 +443,9 @@ void launch_tracklets(const Dev& d, Launch& L) {
   k_seed_compact<<<(T + 255) / 256, 256, 0, L.st>>>(d);
   k_tl_e1<<<148 * 8, E_THREADS, 0, L.st>>>(d);
   launch_order_desc(d, 1, d.e_key, &d.cnt->n_work, T, d.e_order, L);
-  k_tl_e2<<<148 * 6, E_THREADS, 0, L.st>>>(d);
+  k_tl_e2<<<148 * E2_BLOCKS, E_THREADS, 0, L.st>>>(d);
   launch_order_desc(d, 2, d.e_key + T, &d.cnt->n_work, T, d.e_order + T, L);
-  k_tl_e3<<<148 * 6, E_THREADS, 0, L.st>>>(d);
+  k_tl_e3<<<148 * E3_BLOCKS, E_THREADS, 0, L.st>>>(d);
   k_tracklet_weights<<<148 * 16, 128, 0, L.st>>>(d);
   L.count += 5;
 }
