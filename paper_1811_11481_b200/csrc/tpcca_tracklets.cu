@@ -155,7 +155,13 @@ __device__ __forceinline__ int search_row(const Dev& d, const GridHdr& g, const 
 }
 
 // ---- E1: seed fit along the cleaned up-links
-__global__ void __launch_bounds__(E_THREADS, 8) k_tl_e1(Dev d) {
+#ifndef E1_BLOCKS
+#define E1_BLOCKS 4  // CTAs per SM in the grid: fewer lanes = more seeds per lane = better balance
+#endif
+#ifndef E1_BOUNDS
+#define E1_BOUNDS 8
+#endif
+__global__ void __launch_bounds__(E_THREADS, E1_BOUNDS) k_tl_e1(Dev d) {
   const int R = d.n_rows, n_work = d.cnt->n_work;
   const unsigned lane = threadIdx.x & 31;
   int n_steps = 0;
@@ -434,6 +440,12 @@ __global__ void __launch_bounds__(128) k_tracklet_weights(Dev d) {
   }
 }
 
+#ifndef E2_GRID
+#define E2_GRID E2_BLOCKS
+#endif
+#ifndef E3_GRID
+#define E3_GRID E3_BLOCKS
+#endif
 void launch_tracklets(const Dev& d, Launch& L) {
   if (d.n <= 0 || d.max_tracklets <= 0) return;
   const int T = d.max_tracklets;
@@ -441,11 +453,11 @@ void launch_tracklets(const Dev& d, Launch& L) {
   L.count++;
   launch_scan_i32(d.seed_w, &d.cnt->n_start, T, d.scan_tmp, L);
   k_seed_compact<<<(T + 255) / 256, 256, 0, L.st>>>(d);
-  k_tl_e1<<<148 * 8, E_THREADS, 0, L.st>>>(d);
+  k_tl_e1<<<148 * E1_BLOCKS, E_THREADS, 0, L.st>>>(d);
   launch_order_desc(d, 1, d.e_key, &d.cnt->n_work, T, d.e_order, L);
-  k_tl_e2<<<148 * E2_BLOCKS, E_THREADS, 0, L.st>>>(d);
+  k_tl_e2<<<148 * E2_GRID, E_THREADS, 0, L.st>>>(d);
   launch_order_desc(d, 2, d.e_key + T, &d.cnt->n_work, T, d.e_order + T, L);
-  k_tl_e3<<<148 * E3_BLOCKS, E_THREADS, 0, L.st>>>(d);
+  k_tl_e3<<<148 * E3_GRID, E_THREADS, 0, L.st>>>(d);
   k_tracklet_weights<<<148 * 16, 128, 0, L.st>>>(d);
   L.count += 5;
 }
