@@ -69,12 +69,12 @@ static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params
   CARVE(d.sb_skey, int32_t, T);
   CARVE(d.start_hits, int32_t, T);
   CARVE(d.seed_w, int32_t, T + 1);
-  CARVE(d.ord, int32_t, 3 * 1024);
-  CARVE(d.e_key, int32_t, 2 * T);
-  CARVE(d.e_order, int32_t, 2 * T);
+  CARVE(d.ord, int32_t, 4 * 1024);
+  CARVE(d.e_key, int32_t, 3 * T);
+  CARVE(d.e_order, int32_t, 3 * T);
   CARVE(d.work_t, int32_t, T);
   CARVE(d.row_hit, int32_t, T * (size_t)g->n_rows);
-  CARVE(d.tl_state, float, T * 24);
+  CARVE(d.tl_state, float, T * 40);
   CARVE(d.tl_ints, int32_t, T * 4);
   CARVE(d.tl_floats, float, T * 8);
   CARVE(d.tl_W, unsigned long long, T);

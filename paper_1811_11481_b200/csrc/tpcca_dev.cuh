@@ -29,7 +29,7 @@ struct DevCounters {  // device-resident scalars
   int32_t n_bins;      // total grid bins of the frame
   int32_t n_start_raw; // start hits before clamping to capacity
   int32_t n_work;      // seeds that reach the constructor (chain >= min_seed_hits)
-  int32_t work_next[3];  // queue heads of the three tracklet-constructor kernels
+  int32_t work_next[4];  // queue heads of the four tracklet-constructor kernels
   unsigned long long row_steps, searches, track_hits;  // work counters (roofline units)
   unsigned long long pad2;
 };
@@ -76,12 +76,12 @@ struct Dev {
   int32_t* start_hits;     // [max_tracklets] canonical order (sorted indices)
   // (e)
   int32_t* seed_w;         // [max_tracklets+1] tracklet id t -> work index w, -1 for void seeds
-  int32_t* ord;            // [3][1024] counting-sort scratch per order (0 refit, 1 E2, 2 E3): histogram [0,512), cursors [512,1024); zeroed per call
-  int32_t* e_key;          // [2][max_tracklets] w-space sort keys (expected row steps) of the E2 / E3 work orders
-  int32_t* e_order;        // [2][max_tracklets] E2 / E3 work orders: w by decreasing key
+  int32_t* ord;            // [4][1024] counting-sort scratch per order (0 refit, 1 E2, 2 E3a, 3 E3b): histogram [0,512), cursors [512,1024); zeroed per call
+  int32_t* e_key;          // [3][max_tracklets] w-space sort keys (expected row steps) of the E2 / E3a / E3b work orders
+  int32_t* e_order;        // [3][max_tracklets] E2 / E3a / E3b work orders: w by decreasing key
   int32_t* work_t;         // [max_tracklets] w -> t
   int32_t* row_hit;        // [max_tracklets][n_rows] indexed by w (dense over surviving seeds)
-  float* tl_state;         // [max_tracklets][24] w-space: x, 5 parameters, 15 cov, chi2, row, valid
+  float* tl_state;         // [max_tracklets][40] w-space: x, 5 parameters, 15 cov, chi2, row, status, ... (layout: k_tl_e3a)
   int32_t* tl_ints;        // [max_tracklets][4] valid, first_row, last_row, n_hits
   float* tl_floats;        // [max_tracklets][8] x, y, z~, sinphi, dzds, qpt, chi2, z_ref
   unsigned long long* tl_W;        // [max_tracklets]

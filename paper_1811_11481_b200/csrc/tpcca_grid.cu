@@ -156,9 +156,9 @@ __global__ void k_reset(Dev d) {
     d.slice_bbox[4 * i + 2] = 0xFFFFFFFFu;  // zmin
     d.slice_bbox[4 * i + 3] = 0u;           // zmax
   }
-  if (i < 3 * 1024) d.ord[i] = 0;
+  if (i < 4 * 1024) d.ord[i] = 0;
   if (i == 0) {
-    d.cnt->n_start = 0; d.cnt->n_tracks = 0; d.cnt->n_valid = 0; d.cnt->status = 0; d.cnt->n_bins = 0; d.cnt->n_start_raw = 0; d.cnt->n_work = 0; d.cnt->work_next[0] = 0; d.cnt->work_next[1] = 0; d.cnt->work_next[2] = 0;
+    d.cnt->n_start = 0; d.cnt->n_tracks = 0; d.cnt->n_valid = 0; d.cnt->status = 0; d.cnt->n_bins = 0; d.cnt->n_start_raw = 0; d.cnt->n_work = 0; d.cnt->work_next[0] = 0; d.cnt->work_next[1] = 0; d.cnt->work_next[2] = 0; d.cnt->work_next[3] = 0;
     d.cnt->row_steps = 0ull; d.cnt->searches = 0ull; d.cnt->track_hits = 0ull;
   }
 }
@@ -327,7 +327,7 @@ __global__ void __launch_bounds__(128) k_fill_slice_of(Dev d) {
 }
 
 void launch_grid(const Dev& d, const SecOff& so, Launch& L) {
-  k_reset<<<(max(d.n_slices, 3 * 1024) + 256) / 256, 256, 0, L.st>>>(d);
+  k_reset<<<(max(d.n_slices, 4 * 1024) + 256) / 256, 256, 0, L.st>>>(d);
   L.count++;
   if (d.n > 0) {
     k_slice_count<<<(d.n + A1_THREADS * A1_ITEMS - 1) / (A1_THREADS * A1_ITEMS), A1_THREADS, 0, L.st>>>(d, so);

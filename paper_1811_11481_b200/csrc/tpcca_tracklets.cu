@@ -53,12 +53,14 @@ __global__ void __launch_bounds__(256) k_seed_compact(Dev d) {
 // Three persistent kernels, one per phase of DESIGN.md O5, so that every warp runs ONE uniform step body:
 //   k_tl_e1  seed fit along the links            (transport + update)
 //   k_tl_e2  outward extrapolation and pick-up   (transport + search + update)
-//   k_tl_e3  inward pass through the seed        (transport + [existing hit | search] + update)
+//   k_tl_e3a inward pass through the seed        (transport + keep/reject of the existing hit + update)
+//   k_tl_e3b pick-up below the seed               (transport + search + update)
 // Every lane runs one seed at a time and, when it is done, takes the next one from a global queue (one atomic
 // per warp refill; ballot + popc give the lanes their ranks), so a warp never idles on its longest seed.
 // The Kalman state travels between the kernels through tl_state[w][24].  row_hit is [w][row]: a lane's
 // consecutive rows share a 32-byte sector, which L2 merges.
 #define E_THREADS 128
+#define E_STATE 40  // floats per seed in tl_state (layout: see k_tl_e3a)
 #define FULL 0xffffffffu
 #ifndef E_REFILL_MIN
 #define E_REFILL_MIN 8  // refill a warp when this many lanes are idle (amortises the divergent start-up code)
@@ -176,7 +178,7 @@ __global__ void __launch_bounds__(E_THREADS, E1_BOUNDS) k_tl_e1(Dev d) {
     const unsigned nm = __ballot_sync(FULL, need);
     if (nm && (__popc(nm) >= REFILL_MIN || __ballot_sync(FULL, busy) == 0u)) {
       if (need && w >= 0) {  // retire
-        float* st = d.tl_state + (size_t)w * 24;
+        float* st = d.tl_state + (size_t)w * E_STATE;
         st_store_kf(st, k);
         reinterpret_cast<int*>(st)[22] = last_row;
         reinterpret_cast<int*>(st)[23] = valid ? 1 : 0;
@@ -238,7 +240,7 @@ __global__ void __launch_bounds__(E_THREADS, E2_BLOCKS) k_tl_e2(Dev d) {
   const int R = d.n_rows, n_work = d.cnt->n_work;
   const unsigned lane = threadIdx.x & 31;
   int n_steps = 0;
-  int w = -1, sbase = 0, r = 0, top_row = 0, gap = 0;
+  int w = -1, sbase = 0, r = 0, r0 = 0, top_row = 0, gap = 0;
   int32_t* rh = nullptr;
   float z_ref = 0.f;
   KF k;
@@ -251,12 +253,12 @@ __global__ void __launch_bounds__(E_THREADS, E2_BLOCKS) k_tl_e2(Dev d) {
     if (nm && (__popc(nm) >= REFILL_MIN || __ballot_sync(FULL, busy) == 0u)) {
       if (need && w >= 0) {  // retire: the snapshot replaces the state, top_row replaces last_row
         if (live) {
-          float* st = d.tl_state + (size_t)w * 24;
+          float* st = d.tl_state + (size_t)w * E_STATE;
           reinterpret_cast<float4*>(st)[0] = make_float4(sx, sy, sz, ss);
           st[4] = st_; st[5] = sq;
           reinterpret_cast<int*>(st)[22] = top_row;
         }
-        d.e_key[d.max_tracklets + w] = live ? top_row + 1 : 0;  // E3 work order: rows from the outermost hit down
+        d.e_key[d.max_tracklets + w] = live ? top_row - r0 + 1 : 0;  // E3a work order: rows from the outermost hit down to r0
         w = -1;
       }
       const int nw = fetch_work(&d.cnt->work_next[1], need, lane, nm);
@@ -264,14 +266,16 @@ __global__ void __launch_bounds__(E_THREADS, E2_BLOCKS) k_tl_e2(Dev d) {
         if (nw >= n_work) exhausted = true;
         else {
           w = d.e_order[nw];
-          const float* st = d.tl_state + (size_t)w * 24;
+          const float* st = d.tl_state + (size_t)w * E_STATE;
           live = reinterpret_cast<const int*>(st)[23] != 0;
           if (live) {
             st_load_kf(st, k);
             const int last_row = reinterpret_cast<const int*>(st)[22];
             const int t = d.work_t[w];
             const int h0 = d.start_hits[t];
-            sbase = (d.slice_of[h0] / R) * R;
+            const int sl0 = d.slice_of[h0];
+            sbase = (sl0 / R) * R;
+            r0 = sl0 - sbase;
             z_ref = d.yz[h0].y;
             rh = d.row_hit + (size_t)w * R;
             sx = k.x; sy = k.y; sz = k.z; ss = k.s; st_ = k.t; sq = k.q;
@@ -313,41 +317,51 @@ __global__ void __launch_bounds__(E_THREADS, E2_BLOCKS) k_tl_e2(Dev d) {
   }
 }
 
-// ---- E3: inward pass through the seed with outlier rejection, then pick-up below it
+// ---- E3: inward pass through the seed with outlier rejection, then pick-up below it.
+// Two kernels so that a warp's lanes run the same kind of step:
+//   k_tl_e3a  rows from the outermost hit down to the start row r0: the row already holds a hit (keep/reject test,
+//             no search) except for the rare gap rows;
+//   k_tl_e3b  rows below r0: every step is a pick-up search; stops after max_gap consecutive misses.
+// The state crosses the boundary through tl_state[w][E_STATE] (layout below).
+//   [0..21] Kalman state (st_store_kf)   [22] next row   [23] status: 0 void, 1 continue, 2 stopped (finalise only)
+//   [24..30] state at the innermost accepted hit (x, y, z~, sinphi, dzds, qpt, chi2)
+//   [31] inner_row  [32] outer_row  [33] n_hits  [34] gap
 #ifndef E3_BLOCKS
 #define E3_BLOCKS 6
 #endif
-__global__ void __launch_bounds__(E_THREADS, E3_BLOCKS) k_tl_e3(Dev d) {
+#ifndef E3B_BLOCKS
+#define E3B_BLOCKS 6
+#endif
+
+__global__ void __launch_bounds__(E_THREADS, E3_BLOCKS) k_tl_e3a(Dev d) {
   const int R = d.n_rows, n_work = d.cnt->n_work;
   const unsigned lane = threadIdx.x & 31;
-  int n_steps = 0, n_search = 0, n_val = 0;
-  int w = -1, t = -1, sbase = 0, r0 = 0, r = 0, gap = 0;
+  int n_steps = 0, n_search = 0;
+  int w = -1, sbase = 0, r0 = 0, r = 0, gap = 0;
   int32_t* rh = nullptr;
   float z_ref = 0.f;
   KF k;
   k.x = k.y = k.z = k.s = k.t = k.q = 0.f; kf_reset_cov(k, d.P.cov0);
   float ix = 0.f, iy_ = 0.f, iz_ = 0.f, is = 0.f, it = 0.f, iq = 0.f, ichi = 0.f;  // state at the innermost hit
   int inner_row = -1, outer_row = -1, n_hits = 0;
-  bool busy = false, exhausted = false, live = false;
+  bool busy = false, exhausted = false, live = false, stopped = false;
   while (true) {
     const bool need = !busy && !exhausted;
     const unsigned nm = __ballot_sync(FULL, need);
     if (nm && (__popc(nm) >= REFILL_MIN || __ballot_sync(FULL, busy) == 0u)) {
-      if (need && w >= 0) {  // retire: tracklet record (void unless enough hits)
-        int4 ti = make_int4(0, -1, -1, 0);
-        float4 tf0 = make_float4(0.f, 0.f, 0.f, 0.f), tf1 = make_float4(0.f, 0.f, 0.f, z_ref);
-        unsigned long long W = 0ull;
-        if (live && inner_row >= 0 && n_hits >= d.P.min_tracklet_hits) {
-          ti = make_int4(1, inner_row, outer_row, n_hits);
-          tf0 = make_float4(ix, iy_, iz_, is);
-          tf1 = make_float4(it, iq, ichi, z_ref);
-          W = pack_weight(d, n_hits, ichi, (uint32_t)t);
-          n_val++;
+      if (need && w >= 0) {  // retire: hand the state to k_tl_e3b
+        float* st = d.tl_state + (size_t)w * E_STATE;
+        int* si = reinterpret_cast<int*>(st);
+        const bool cont = live && !stopped && r >= 0;
+        if (live) {
+          st_store_kf(st, k);
+          si[22] = r;
+          reinterpret_cast<float4*>(st)[6] = make_float4(ix, iy_, iz_, is);
+          st[28] = it; st[29] = iq; st[30] = ichi;
+          si[31] = inner_row; si[32] = outer_row; si[33] = n_hits; si[34] = gap;
         }
-        reinterpret_cast<int4*>(d.tl_ints)[t] = ti;
-        reinterpret_cast<float4*>(d.tl_floats)[2 * t] = tf0;
-        reinterpret_cast<float4*>(d.tl_floats)[2 * t + 1] = tf1;
-        d.tl_W[t] = W;
+        si[23] = live ? (cont ? 1 : 2) : 0;
+        d.e_key[2 * d.max_tracklets + w] = cont ? r + 1 : 0;  // E3b work order: rows left below the start row
         w = -1;
       }
       const int nw = fetch_work(&d.cnt->work_next[2], need, lane, nm);
@@ -355,16 +369,17 @@ __global__ void __launch_bounds__(E_THREADS, E3_BLOCKS) k_tl_e3(Dev d) {
         if (nw >= n_work) exhausted = true;
         else {
           w = d.e_order[d.max_tracklets + nw];
-          t = d.work_t[w];
-          const float* st = d.tl_state + (size_t)w * 24;
+          const int t = d.work_t[w];
+          const float* st = d.tl_state + (size_t)w * E_STATE;
           live = reinterpret_cast<const int*>(st)[23] != 0;
-          const int h0 = d.start_hits[t];
-          const int sl0 = d.slice_of[h0];
-          const int sec = sl0 / R;
-          r0 = sl0 - sec * R; sbase = sec * R;
-          z_ref = d.yz[h0].y;
+          stopped = false;
           inner_row = -1; outer_row = -1; n_hits = 0; gap = 0;
           if (live) {
+            const int h0 = d.start_hits[t];
+            const int sl0 = d.slice_of[h0];
+            const int sec = sl0 / R;
+            r0 = sl0 - sec * R; sbase = sec * R;
+            z_ref = d.yz[h0].y;
             const float4 a = reinterpret_cast<const float4*>(st)[0];
             k.x = a.x; k.y = a.y; k.z = a.z; k.s = a.w; k.t = st[4]; k.q = st[5];
             kf_reset_cov(k, d.P.cov0);
@@ -377,15 +392,14 @@ __global__ void __launch_bounds__(E_THREADS, E3_BLOCKS) k_tl_e3(Dev d) {
       if (__ballot_sync(FULL, !exhausted) == 0u) break;
     }
     if (!busy) continue;
-    // ---- one row step.  Loads that do not depend on the filter state go first; the next row's are prefetched.
+    // ---- one row step (r >= r0).  Loads that do not depend on the filter state go first.
     n_steps++;
-    const int cur = (r >= r0) ? rh[r] : -1;
+    const int cur = rh[r];
     float2 pb = make_float2(0.f, 0.f);
     if (cur >= 0) pb = d.yz[cur];
-    if (r > 0) prefetch_l1(&d.grid[sbase + r - 1]);
     const float xr = d.row_x[r];
     if (!kf_transport(k, xr, d.kq, d.P.max_sinphi) || fabsf(k.y) > xr * d.tan_half_angle + d.P.edge_margin) {
-      busy = false;
+      busy = false; stopped = true;
       continue;
     }
     int cand;
@@ -395,12 +409,104 @@ __global__ void __launch_bounds__(E_THREADS, E3_BLOCKS) k_tl_e3(Dev d) {
       const float dz = (pb.y - z_ref) - k.z;
       const float dist = (dy * dy) * iy + (dz * dz) * iz;
       cand = (dist <= d.P.reject_cut) ? cur : -1;
-    } else {
+    } else {  // gap row inside the range (rare): pick-up search
       n_search++;
       const GridHdr g = d.grid[sbase + r];
       cand = search_row(d, g, k, z_ref, pb);
     }
-    if (cand != cur || r < r0) rh[r] = cand;  // rejected seed hit -> -1, or the search result (rows below the seed are unwritten)
+    if (cand != cur) rh[r] = cand;  // rejected hit -> -1, or the search result
+    if (cand >= 0) {
+      kf_update(k, pb.x, pb.y - z_ref, d.sy2, d.sz2);
+      gap = 0; inner_row = r; n_hits++;
+      if (outer_row < 0) outer_row = r;
+      ix = k.x; iy_ = k.y; iz_ = k.z; is = k.s; it = k.t; iq = k.q; ichi = k.chi2;
+    } else {
+      gap++;  // the gap stop is armed only below r0 (E3 gap rule)
+    }
+    r--;
+    if (r < r0) busy = false;
+  }
+  const int ws = __reduce_add_sync(FULL, n_steps), wq = __reduce_add_sync(FULL, n_search);
+  if (lane == 0 && ws) {
+    atomicAdd(&d.cnt->row_steps, (unsigned long long)ws);
+    atomicAdd(&d.cnt->searches, (unsigned long long)wq);
+  }
+}
+
+__global__ void __launch_bounds__(E_THREADS, E3B_BLOCKS) k_tl_e3b(Dev d) {
+  const int R = d.n_rows, n_work = d.cnt->n_work;
+  const unsigned lane = threadIdx.x & 31;
+  int n_steps = 0, n_val = 0;
+  int w = -1, t = -1, sbase = 0, r = 0, gap = 0, status = 0;
+  int32_t* rh = nullptr;
+  float z_ref = 0.f;
+  KF k;
+  k.x = k.y = k.z = k.s = k.t = k.q = 0.f; kf_reset_cov(k, d.P.cov0);
+  float ix = 0.f, iy_ = 0.f, iz_ = 0.f, is = 0.f, it = 0.f, iq = 0.f, ichi = 0.f;  // state at the innermost hit
+  int inner_row = -1, outer_row = -1, n_hits = 0;
+  bool busy = false, exhausted = false;
+  while (true) {
+    const bool need = !busy && !exhausted;
+    const unsigned nm = __ballot_sync(FULL, need);
+    if (nm && (__popc(nm) >= REFILL_MIN || __ballot_sync(FULL, busy) == 0u)) {
+      if (need && w >= 0) {  // retire: tracklet record (void unless enough hits)
+        int4 ti = make_int4(0, -1, -1, 0);
+        float4 tf0 = make_float4(0.f, 0.f, 0.f, 0.f), tf1 = make_float4(0.f, 0.f, 0.f, z_ref);
+        unsigned long long W = 0ull;
+        if (status != 0 && inner_row >= 0 && n_hits >= d.P.min_tracklet_hits) {
+          ti = make_int4(1, inner_row, outer_row, n_hits);
+          tf0 = make_float4(ix, iy_, iz_, is);
+          tf1 = make_float4(it, iq, ichi, z_ref);
+          W = pack_weight(d, n_hits, ichi, (uint32_t)t);
+          n_val++;
+        }
+        reinterpret_cast<int4*>(d.tl_ints)[t] = ti;
+        reinterpret_cast<float4*>(d.tl_floats)[2 * t] = tf0;
+        reinterpret_cast<float4*>(d.tl_floats)[2 * t + 1] = tf1;
+        d.tl_W[t] = W;
+        w = -1;
+      }
+      const int nw = fetch_work(&d.cnt->work_next[3], need, lane, nm);
+      if (need) {
+        if (nw >= n_work) exhausted = true;
+        else {
+          w = d.e_order[2 * d.max_tracklets + nw];
+          t = d.work_t[w];
+          const float* st = d.tl_state + (size_t)w * E_STATE;
+          const int* si = reinterpret_cast<const int*>(st);
+          status = si[23];
+          const int h0 = d.start_hits[t];
+          z_ref = d.yz[h0].y;
+          inner_row = -1; outer_row = -1; n_hits = 0;
+          if (status != 0) {
+            const float4 sn = reinterpret_cast<const float4*>(st)[6];
+            ix = sn.x; iy_ = sn.y; iz_ = sn.z; is = sn.w; it = st[28]; iq = st[29]; ichi = st[30];
+            inner_row = si[31]; outer_row = si[32]; n_hits = si[33];
+          }
+          if (status == 1) {
+            st_load_kf(st, k);
+            r = si[22]; gap = si[34];
+            sbase = (d.slice_of[h0] / R) * R;
+            rh = d.row_hit + (size_t)w * R;
+            busy = true;
+          }
+        }
+      }
+      if (__ballot_sync(FULL, !exhausted) == 0u) break;
+    }
+    if (!busy) continue;
+    // ---- one row step below the start row: transport, pick-up search, update
+    n_steps++;
+    const GridHdr g = d.grid[sbase + r];
+    if (r > 0) prefetch_l1(&d.grid[sbase + r - 1]);
+    const float xr = d.row_x[r];
+    if (!kf_transport(k, xr, d.kq, d.P.max_sinphi) || fabsf(k.y) > xr * d.tan_half_angle + d.P.edge_margin) {
+      busy = false;
+      continue;
+    }
+    float2 pb = make_float2(0.f, 0.f);
+    const int cand = search_row(d, g, k, z_ref, pb);
+    rh[r] = cand;
     if (cand >= 0) {
       kf_update(k, pb.x, pb.y - z_ref, d.sy2, d.sz2);
       gap = 0; inner_row = r; n_hits++;
@@ -408,16 +514,15 @@ __global__ void __launch_bounds__(E_THREADS, E3_BLOCKS) k_tl_e3(Dev d) {
       ix = k.x; iy_ = k.y; iz_ = k.z; is = k.s; it = k.t; iq = k.q; ichi = k.chi2;
     } else {
       gap++;
-      if (r < r0 && gap > d.P.max_gap) busy = false;
+      if (gap > d.P.max_gap) busy = false;
     }
     r--;
     if (r < 0) busy = false;
   }
-  const int ws = __reduce_add_sync(FULL, n_steps), wq = __reduce_add_sync(FULL, n_search),
-            wv = __reduce_add_sync(FULL, n_val);
-  if (lane == 0 && ws) {
+  const int ws = __reduce_add_sync(FULL, n_steps), wv = __reduce_add_sync(FULL, n_val);
+  if (lane == 0 && (ws || wv)) {
     atomicAdd(&d.cnt->row_steps, (unsigned long long)ws);
-    atomicAdd(&d.cnt->searches, (unsigned long long)wq);
+    atomicAdd(&d.cnt->searches, (unsigned long long)ws);
     atomicAdd(&d.cnt->n_valid, wv);
   }
 }
@@ -457,7 +562,9 @@ void launch_tracklets(const Dev& d, Launch& L) {
   launch_order_desc(d, 1, d.e_key, &d.cnt->n_work, T, d.e_order, L);
   k_tl_e2<<<148 * E2_GRID, E_THREADS, 0, L.st>>>(d);
   launch_order_desc(d, 2, d.e_key + T, &d.cnt->n_work, T, d.e_order + T, L);
-  k_tl_e3<<<148 * E3_GRID, E_THREADS, 0, L.st>>>(d);
+  k_tl_e3a<<<148 * E3_GRID, E_THREADS, 0, L.st>>>(d);
+  launch_order_desc(d, 3, d.e_key + 2 * (size_t)T, &d.cnt->n_work, T, d.e_order + 2 * (size_t)T, L);
+  k_tl_e3b<<<148 * E3B_BLOCKS, E_THREADS, 0, L.st>>>(d);
   k_tracklet_weights<<<148 * 16, 128, 0, L.st>>>(d);
-  L.count += 5;
+  L.count += 6;
 }
