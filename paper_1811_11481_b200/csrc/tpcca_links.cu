@@ -133,15 +133,22 @@ __global__ void __launch_bounds__(NB_THREADS) k_neighbours(Dev d) {
       const int nu = collect(d, gu, y0, z0, nb.wyu, nb.wzu, mz, lpu, liu);
       if (nd <= NB_CAP && nu <= NB_CAP) {
         const float t = nb.t;
-        for (int ju = 0; ju < nu; ju++) {
-          const float2 pu = lpu[ju * NB_THREADS];
-          const int u = liu[ju * NB_THREADS];
-          for (int jd = 0; jd < nd; jd++) {
-            const float2 pd = lpd[jd * NB_THREADS];
-            const float ey = y0 - (pd.x + t * (pu.x - pd.x));
-            const float ez = z0 - (pd.y + t * (pu.y - pd.y));
-            const float cost = (ey * ey) * d.inv_sy2 + (ez * ez) * d.inv_sz2;
-            consider(d, best, cost, u, pu.x, pu.y, lid[jd * NB_THREADS], pd.x, pd.y);
+        // one flat loop over the nu x nd pairs: lanes with different list shapes stay together
+        const int np = nu * nd;
+        int ju = 0, jd = 0;
+        float2 pu = lpu[0];
+        int u = liu[0];
+        for (int q = 0; q < np; q++) {
+          const float2 pd = lpd[jd * NB_THREADS];
+          const float ey = y0 - (pd.x + t * (pu.x - pd.x));
+          const float ez = z0 - (pd.y + t * (pu.y - pd.y));
+          const float cost = (ey * ey) * d.inv_sy2 + (ez * ez) * d.inv_sz2;
+          consider(d, best, cost, u, pu.x, pu.y, lid[jd * NB_THREADS], pd.x, pd.y);
+          if (++jd == nd) {
+            jd = 0;
+            ju = min(ju + 1, NB_CAP - 1);
+            pu = lpu[ju * NB_THREADS];
+            u = liu[ju * NB_THREADS];
           }
         }
       } else if (nu > 0) {
