@@ -115,3 +115,51 @@ def test_permutation_invariance_gpu(row_x):
     b = run_gpu(fp, row_x)
     assert np.array_equal(b.assignment(), a.assignment()[p])
     assert b.tracks().tobytes() == a.tracks().tobytes()
+
+
+def test_parity_non_default_parameters(row_x):
+    """Every physics parameter of DESIGN.md Table A reaches the kernels: tighter cuts, shorter gap, longer seeds."""
+    fr = synth.generate(synth.config(2, scale=0.15, seed=41))
+    params = dict(triplet_cut=9.0, nbr_dydx=1.0, nbr_margin_z=0.5, pick_cut=9.0, reject_cut=12.0, max_gap=2,
+                  min_seed_hits=5, min_tracklet_hits=14, min_track_hits=12, edge_margin=1.0, max_sinphi=0.8,
+                  qual_scale=500.0, cov0=(2.0, 2.0, 0.1, 0.5, 50.0), sigma_y=0.12, sigma_z=0.13)
+    t, orc, exact = compare(fr, row_x, params=params)
+    assert len(orc.tracks) > 100 and exact
+
+
+def test_parity_dense_noise_overflows_candidate_lists(row_x):
+    """Noise far above the track density: the neighbour windows hold more candidates than the shared-memory lists
+    (NB_CAP), so the nested-loop fallback of k_neighbours and multi-pass pick-up searches are exercised."""
+    cfg = synth.config(1, scale=0.5, seed=43)
+    cfg["noise_frac"] = 40.0
+    fr = synth.generate(cfg)
+    t, orc, exact = compare(fr, row_x)
+    assert fr.n > 300000 and exact
+
+
+def test_parity_duplicate_clusters_tie_breaks(row_x):
+    """Bit-identical duplicate clusters give exact ties in cost and distance: the (ord z, ord y, input index) order
+    of DESIGN.md A4 decides, identically on both sides."""
+    fr = synth.generate(synth.config(2, scale=0.05, seed=44))
+    cl, so = [], [0]
+    for s in range(36):
+        c = fr.clusters[fr.sector_offsets[s]:fr.sector_offsets[s + 1]]
+        cl.append(np.concatenate([c, c[::3]]))  # every third cluster twice
+        so.append(so[-1] + len(cl[-1]))
+    cl = np.concatenate(cl)
+    f2 = synth.Frame(cl, np.asarray(so, np.int32), np.full(len(cl), -1, np.int32), fr.track_par, 36, "dup")
+    compare(f2, row_x)
+
+
+def test_parity_smaller_geometry(row_x):
+    """n_rows = 100 and n_sectors = 8: nothing in the kernels is tied to 152 x 36."""
+    fr = synth.generate(synth.config(2, scale=0.2, seed=45))
+    cl, so = [], [0]
+    for s in range(8):
+        c = fr.clusters[fr.sector_offsets[s]:fr.sector_offsets[s + 1]]
+        cl.append(c[c["row"] < 100])
+        so.append(so[-1] + len(cl[-1]))
+    cl = np.concatenate(cl)
+    f2 = synth.Frame(cl, np.asarray(so, np.int32), np.full(len(cl), -1, np.int32), fr.track_par, 8, "small")
+    t, orc, exact = compare(f2, row_x[:100])
+    assert len(orc.tracks) > 20 and exact
