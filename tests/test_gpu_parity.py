@@ -163,3 +163,38 @@ def test_parity_smaller_geometry(row_x):
     f2 = synth.Frame(cl, np.asarray(so, np.int32), np.full(len(cl), -1, np.int32), fr.track_par, 8, "small")
     t, orc, exact = compare(f2, row_x[:100])
     assert len(orc.tracks) > 20 and exact
+
+
+def test_concurrent_handles_on_two_streams(row_x):
+    """Two trackers driven from two host threads on two streams (frames in flight) give the results of
+    the serial call: handles share no state."""
+    import threading
+
+    import torch
+    frs = [synth.generate(synth.config(2, scale=0.2, seed=51)), synth.generate(synth.config(3, scale=0.2, seed=52))]
+    ref = []
+    for fr in frs:
+        t = run_gpu(fr, row_x)
+        ref.append((t.assignment(), t.tracks().tobytes()))
+    out = [None, None]
+
+    def work(i):
+        torch.cuda.set_device(0)
+        fr = frs[i]
+        t = B.Tracker(row_x, max_clusters=fr.n, max_tracklets=max(1024, fr.n // 4))
+        hc = torch.from_numpy(fr.clusters.view(np.uint8).reshape(-1).copy()).pin_memory()
+        ot = torch.empty(16 + 128 * t.max_tracks, dtype=torch.uint8).pin_memory()
+        oa = torch.empty(fr.n, dtype=torch.int32).pin_memory()
+        with torch.cuda.stream(torch.cuda.Stream()):
+            for _ in range(4):
+                t.track_host(hc, fr.n, fr.sector_offsets, ot, oa)
+        nt = int(ot[:16].numpy().view(B.HEADER_DTYPE)["n_tracks"][0])
+        out[i] = (oa.numpy().copy(), ot[16:16 + 128 * nt].numpy().tobytes())
+
+    ths = [threading.Thread(target=work, args=(i,)) for i in range(2)]
+    for th in ths:
+        th.start()
+    for th in ths:
+        th.join()
+    for i in range(2):
+        assert np.array_equal(out[i][0], ref[i][0]) and out[i][1] == ref[i][1]
