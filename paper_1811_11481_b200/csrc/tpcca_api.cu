@@ -2,6 +2,7 @@
 // enqueue of steps (a)-(g).  No kernel of the hot path lives here.
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <new>
@@ -35,7 +36,7 @@ static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params
   size_t off = 0;
   const size_t N = (size_t)p->max_clusters, T = (size_t)p->max_tracklets, K = (size_t)p->max_tracks;
   const size_t SL = (size_t)g->n_sectors * g->n_rows;
-  const size_t NB = 4 * N + 128 * SL + 1;
+  const size_t NB = 4 * N + 130 * SL + 2;
   const size_t NSCAN = T + 8 + NB / 2048 + T / 2048 + 64;
 #define CARVE(field, type, count)                                  \
   do {                                                             \
@@ -51,7 +52,9 @@ static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params
   CARVE(d.nbr, NbrHdr, SL);
   CARVE(d.slice_nstart, int32_t, SL + 1);
   CARVE(d.slice_sbase, int32_t, SL + 1);
-  CARVE(d.cluster_bin, int32_t, N);
+  CARVE(d.slice_fill, int32_t, SL + 1);
+  CARVE(d.bin_base, int32_t, SL + 1);
+  CARVE(d.srec, float4, N);
   CARVE(d.cluster_rank, int32_t, N);
   CARVE(d.bin_start, int32_t, NB + 1);
   CARVE(d.scan_tmp, int32_t, NSCAN);
@@ -192,18 +195,32 @@ static int track_impl(tpcca_handle* h, const tpcca_cluster* clusters, int64_t n,
   h->last_n = n;
   const bool prof = h->profiling;
   cudaEvent_t* ev = h->ev[h->prof_calls % PROF_RING];
+  // TPCCA_DEBUG_SYNC=1: synchronise after every stage and name the stage that faulted (debugging aid)
+  static const bool dbg = getenv("TPCCA_DEBUG_SYNC") != nullptr;
+#define DBG_STAGE(name)                                                                          \
+  if (dbg) {                                                                                     \
+    const cudaError_t de = cudaStreamSynchronize(st);                                            \
+    if (de != cudaSuccess) { set_err("stage %s failed: %lld", name, (long long)de); fprintf(stderr, "tpcca: stage %s: %s\n", name, cudaGetErrorString(de)); return TPCCA_ERR_CUDA; } \
+  }
   if (prof) cudaEventRecord(ev[0], st);
   launch_grid(d, so, L);
+  DBG_STAGE("grid");
   if (prof) cudaEventRecord(ev[1], st);
   launch_neighbours(d, L);
+  DBG_STAGE("neighbours");
   if (prof) cudaEventRecord(ev[2], st);
   launch_clean_start(d, L);
+  DBG_STAGE("clean_start");
   if (prof) cudaEventRecord(ev[3], st);
   launch_tracklets(d, L);
+  DBG_STAGE("tracklets");
   if (prof) cudaEventRecord(ev[4], st);
   launch_select(d, L);
+  DBG_STAGE("select");
   if (prof) cudaEventRecord(ev[5], st);
   launch_refit(d, L);
+  DBG_STAGE("refit");
+#undef DBG_STAGE
   if (prof) cudaEventRecord(ev[6], st);
   if (prof) h->prof_calls++;
   h->have_times = prof && h->prof_calls > 0;

@@ -54,9 +54,11 @@ struct Dev {
   uint32_t* slice_bbox;    // [n_slices*4] ordered-uint ymin, ymax, zmin, zmax
   GridHdr* grid;           // [n_slices]
   NbrHdr* nbr;             // [n_slices]
-  int32_t* cluster_bin;    // [n] global bin id (input order)
-  int32_t* cluster_rank;   // [n] arrival rank inside the bin
-  int32_t* bin_start;      // [max_bins+1] counts, then exclusive scan
+  int32_t* slice_fill;     // [n_slices+1] fill cursors of the slice scatter
+  int32_t* bin_base;       // [n_slices+1] first bin of a slice (upper-bound layout from the slice counts)
+  float4* srec;            // [n] clusters in slice order: (y, z, input index, -)
+  int32_t* cluster_rank;   // [n] scratch (start-hit bucket keys, see sb_key)
+  int32_t* bin_start;      // [max_bins+1] per slice at bin_base: start of every bin, then the slice end
   int32_t* scan_tmp;       // partial sums
   float2* yz;              // [n] sorted (sector,row,bin)
   int32_t* orig_idx;       // [n] sorted -> input index

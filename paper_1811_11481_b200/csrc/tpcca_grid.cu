@@ -1,6 +1,6 @@
 // tpcca_grid.cu -- step (a): cluster grid builder (north_star (a); PAPER.md:49 sectors, :41 pad rows).
 // Counting sort of the frame's clusters by (sector, row) slice and, inside a slice, by a 2-D (y,z) bin
-// grid: histogram -> exclusive scan -> scatter.  The grid is an acceleration structure only (DESIGN.md
+// grid: histogram -> exclusive scan -> scatter, in two levels (slices, then bins inside a slice).  The grid is an acceleration structure only (DESIGN.md
 // O1/A3): no tracking result depends on bin sizes or on the order of clusters inside a bin.
 #include "tpcca_dev.cuh"
 
@@ -144,111 +144,81 @@ void launch_order_desc(const Dev& d, int slot, const int32_t* key, const int32_t
 }
 
 // ---------------------------------------------------------------- (a0) reset per-call state
+#define ORD_SLOTS 4  // counting-sort scratch blocks of Dev::ord (refit, E2, E3a, E3b)
 __global__ void k_reset(Dev d) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i <= d.n_slices) {
+  const int stride = gridDim.x * blockDim.x;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i <= d.n_slices; i += stride) {
     d.slice_count[i] = 0;
     d.slice_nstart[i] = 0;
+    if (i < d.n_slices) {
+      d.slice_bbox[4 * i + 0] = 0xFFFFFFFFu;  // ymin
+      d.slice_bbox[4 * i + 1] = 0u;           // ymax
+      d.slice_bbox[4 * i + 2] = 0xFFFFFFFFu;  // zmin
+      d.slice_bbox[4 * i + 3] = 0u;           // zmax
+    }
   }
-  if (i < d.n_slices) {
-    d.slice_bbox[4 * i + 0] = 0xFFFFFFFFu;  // ymin
-    d.slice_bbox[4 * i + 1] = 0u;           // ymax
-    d.slice_bbox[4 * i + 2] = 0xFFFFFFFFu;  // zmin
-    d.slice_bbox[4 * i + 3] = 0u;           // zmax
-  }
-  if (i < 4 * 1024) d.ord[i] = 0;
-  if (i == 0) {
-    d.cnt->n_start = 0; d.cnt->n_tracks = 0; d.cnt->n_valid = 0; d.cnt->status = 0; d.cnt->n_bins = 0; d.cnt->n_start_raw = 0; d.cnt->n_work = 0; d.cnt->work_next[0] = 0; d.cnt->work_next[1] = 0; d.cnt->work_next[2] = 0; d.cnt->work_next[3] = 0;
+  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < ORD_SLOTS * 1024; i += stride) d.ord[i] = 0;
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    d.cnt->n_start = 0; d.cnt->n_tracks = 0; d.cnt->n_valid = 0; d.cnt->status = 0; d.cnt->n_bins = 0;
+    d.cnt->n_start_raw = 0; d.cnt->n_work = 0;
+    for (int q = 0; q < 4; q++) d.cnt->work_next[q] = 0;
     d.cnt->row_steps = 0ull; d.cnt->searches = 0ull; d.cnt->track_hits = 0ull;
   }
 }
 
-// ---------------------------------------------------------------- (a1) slice histogram + bounding boxes
+// ---------------------------------------------------------------- (a) grid builder, two levels
+// Level 1 moves the clusters into (sector, row) slice order as 16-byte records: a slice histogram, one small scan,
+// then a scatter in which every block reserves its rows' ranges once (block-local ranks in shared memory), so that a
+// block's clusters of one row land next to each other.  Level 2 runs one block per slice on the slice's contiguous
+// records (L1/L2 resident): bounding box, grid header, bin histogram and cursors in shared memory, and the final
+// (y-bin, z-bin) order written to yz / orig_idx / slice_of together with the slice's piece of bin_start.
+// Bins are laid out by an upper bound that depends on the slice counts alone (bins_per_cluster * count + 129 per
+// slice), so the grid dimensions -- which need the bounding box -- can be chosen inside level 2.
 #define A1_THREADS 256
 #define A1_ITEMS 8
+#define A1_TILE (A1_THREADS * A1_ITEMS)
+
+// (a1) clusters per slice
 __global__ void __launch_bounds__(A1_THREADS) k_slice_count(Dev d, SecOff so) {
   __shared__ int s_cnt[TPCCA_MAX_ROWS];
-  __shared__ uint32_t s_box[TPCCA_MAX_ROWS * 4];
-  const int base = blockIdx.x * (A1_THREADS * A1_ITEMS);
-  const int sec0 = sector_of(so, d.n_sectors, min(base, d.n - 1));  // sector privatised in shared memory
-  for (int r = threadIdx.x; r < d.n_rows; r += A1_THREADS) {
-    s_cnt[r] = 0;
-    s_box[4 * r] = 0xFFFFFFFFu; s_box[4 * r + 1] = 0u; s_box[4 * r + 2] = 0xFFFFFFFFu; s_box[4 * r + 3] = 0u;
-  }
+  const int base = blockIdx.x * A1_TILE;
+  const int sec0 = sector_of(so, d.n_sectors, min(base, d.n - 1));  // the block's first sector is privatised
+  for (int r = threadIdx.x; r < d.n_rows; r += A1_THREADS) s_cnt[r] = 0;
   __syncthreads();
   bool bad = false;
 #pragma unroll
   for (int k = 0; k < A1_ITEMS; k++) {
     const int i = base + k * A1_THREADS + threadIdx.x;
     if (i >= d.n) continue;
-    const float4 c = __ldg(&d.clusters[i]);
-    const int row = __float_as_int(c.w);
+    const int row = __float_as_int(__ldg(&d.clusters[i]).w);
     if (row < 0 || row >= d.n_rows) { bad = true; continue; }
-    const int sec = (i < so.v[sec0 + 1]) ? sec0 : sector_of(so, d.n_sectors, i);
-    const uint32_t oy = ordf(c.y), oz = ordf(c.z);
-    if (sec == sec0) {
-      atomicAdd(&s_cnt[row], 1);
-      atomicMin(&s_box[4 * row], oy); atomicMax(&s_box[4 * row + 1], oy);
-      atomicMin(&s_box[4 * row + 2], oz); atomicMax(&s_box[4 * row + 3], oz);
-    } else {
-      const int sl = sec * d.n_rows + row;
-      atomicAdd(&d.slice_count[sl], 1);
-      atomicMin(&d.slice_bbox[4 * sl], oy); atomicMax(&d.slice_bbox[4 * sl + 1], oy);
-      atomicMin(&d.slice_bbox[4 * sl + 2], oz); atomicMax(&d.slice_bbox[4 * sl + 3], oz);
-    }
+    if (i < so.v[sec0 + 1]) atomicAdd(&s_cnt[row], 1);
+    else atomicAdd(&d.slice_count[sector_of(so, d.n_sectors, i) * d.n_rows + row], 1);
   }
   if (bad) atomicOr(&d.cnt->status, TPCCA_STAT_BAD_CLUSTER);
   __syncthreads();
-  for (int r = threadIdx.x; r < d.n_rows; r += A1_THREADS) {
-    const int c = s_cnt[r];
-    if (c) {
-      const int sl = sec0 * d.n_rows + r;
-      atomicAdd(&d.slice_count[sl], c);
-      atomicMin(&d.slice_bbox[4 * sl], s_box[4 * r]); atomicMax(&d.slice_bbox[4 * sl + 1], s_box[4 * r + 1]);
-      atomicMin(&d.slice_bbox[4 * sl + 2], s_box[4 * r + 2]); atomicMax(&d.slice_bbox[4 * sl + 3], s_box[4 * r + 3]);
-    }
-  }
+  for (int r = threadIdx.x; r < d.n_rows; r += A1_THREADS)
+    if (s_cnt[r]) atomicAdd(&d.slice_count[sec0 * d.n_rows + r], s_cnt[r]);
 }
 
-// ---------------------------------------------------------------- (a2) slice offsets + grid headers
-__global__ void __launch_bounds__(1024) k_slice_setup(Dev d) {
+// (a2) slice offsets, bin offsets (upper-bound layout), fill cursors, per-row constants of the neighbours finder
+__global__ void __launch_bounds__(1024) k_slice_offsets(Dev d) {
   __shared__ int sm[32];
   int carry_c = 0, carry_b = 0;
   for (int b0 = 0; b0 < d.n_slices; b0 += 1024) {
     const int sl = b0 + threadIdx.x;
-    int cnt = 0, nb = 0;
-    GridHdr g;
-    g.ymin = g.zmin = 0.0f; g.inv_by = g.inv_bz = 0.0f; g.ny = g.nz = 1; g.bin_base = 0; g.pad = 0;
+    int cnt = 0, cap = 0;
     if (sl < d.n_slices) {
       cnt = d.slice_count[sl];
-      if (cnt > 0) {
-        const float ymin = unordf(d.slice_bbox[4 * sl]), ymax = unordf(d.slice_bbox[4 * sl + 1]);
-        const float zmin = unordf(d.slice_bbox[4 * sl + 2]), zmax = unordf(d.slice_bbox[4 * sl + 3]);
-        const float ye = fmaxf(ymax - ymin, 1e-3f), ze = fmaxf(zmax - zmin, 1e-3f);
-        int ny = (int)(ye / d.P.grid_bin_y) + 1;
-        ny = min(ny, 128);
-        float want = (float)cnt * d.P.grid_bins_per_cluster / (float)ny;
-        int nz = (int)want + 1;
-        const int nz_cap = (int)fminf(ze / d.P.grid_bin_z_min, 1.0e6f) + 1;
-        nz = max(1, min(nz, nz_cap));
-        g.ymin = ymin; g.zmin = zmin;
-        g.inv_by = ((float)ny / ye) * 0.9999f;
-        g.inv_bz = ((float)nz / ze) * 0.9999f;
-        g.ny = ny; g.nz = nz; g.pad = cnt;
-        nb = ny * nz;
-      }
+      cap = (int)((float)cnt * d.P.grid_bins_per_cluster) + 129;
     }
     int tot_c, tot_b;
     const int ec = block_scan_excl(cnt, &tot_c, sm);
-    const int eb = block_scan_excl(nb, &tot_b, sm);
+    const int eb = block_scan_excl(cap, &tot_b, sm);
     if (sl < d.n_slices) {
       d.row_start[sl] = carry_c + ec;
-      g.bin_base = carry_b + eb;
-      if (g.bin_base + nb > d.max_bins) {  // cannot happen with the default sizing; degrade to one bin
-        g.ny = g.nz = 1; g.pad = 0; g.bin_base = min(g.bin_base, d.max_bins - 1);
-        atomicOr(&d.cnt->status, TPCCA_STAT_BIN_OVERFLOW);
-      }
-      d.grid[sl] = g;
+      d.slice_fill[sl] = carry_c + ec;
+      d.bin_base[sl] = carry_b + eb;
       // per-row constants of the neighbours finder (O2): up/down row with one skip
       const int sec = sl / d.n_rows, r = sl - sec * d.n_rows;
       NbrHdr nb;
@@ -276,72 +246,165 @@ __global__ void __launch_bounds__(1024) k_slice_setup(Dev d) {
   }
   if (threadIdx.x == 0) {
     d.row_start[d.n_slices] = carry_c;
-    d.cnt->n_bins = min(carry_b, d.max_bins);
+    d.bin_base[d.n_slices] = carry_b;
   }
 }
 
-__global__ void k_zero_bins(Dev d) {
-  const int n = d.cnt->n_bins;
-  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i <= n; i += gridDim.x * blockDim.x) d.bin_start[i] = 0;
-  // hit weights of the selector: cleared here with coalesced stores rather than in the scatter
-  ulonglong2* hw = reinterpret_cast<ulonglong2*>(d.hit_weight);
-  const int n2 = (d.n + 1) >> 1;  // the array is 256-byte aligned and padded
-  for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n2; i += gridDim.x * blockDim.x) hw[i] = make_ulonglong2(0ull, 0ull);
+// (a3) scatter into slice order: records (y, z, input index); clears the selector's hit weights on the way
+__global__ void __launch_bounds__(A1_THREADS) k_slice_scatter(Dev d, SecOff so) {
+  __shared__ int s_cnt[TPCCA_MAX_ROWS], s_base[TPCCA_MAX_ROWS];
+  const int base = blockIdx.x * A1_TILE;
+  const int sec0 = sector_of(so, d.n_sectors, min(base, d.n - 1));
+  for (int r = threadIdx.x; r < d.n_rows; r += A1_THREADS) s_cnt[r] = 0;
+  __syncthreads();
+  float4 c[A1_ITEMS];
+  int rank[A1_ITEMS];  // >= 0: rank inside the block's (sec0, row) run; -1: other sector; -2: skipped
+#pragma unroll
+  for (int k = 0; k < A1_ITEMS; k++) {
+    const int i = base + k * A1_THREADS + threadIdx.x;
+    rank[k] = -2;
+    if (i >= d.n) continue;
+    d.hit_weight[i] = 0ull;
+    c[k] = __ldg(&d.clusters[i]);
+    const int row = __float_as_int(c[k].w);
+    if (row < 0 || row >= d.n_rows) { d.out_assign[i] = -1; continue; }
+    rank[k] = (i < so.v[sec0 + 1]) ? atomicAdd(&s_cnt[row], 1) : -1;
+  }
+  __syncthreads();
+  for (int r = threadIdx.x; r < d.n_rows; r += A1_THREADS)
+    if (s_cnt[r]) s_base[r] = atomicAdd(&d.slice_fill[sec0 * d.n_rows + r], s_cnt[r]);
+  __syncthreads();
+#pragma unroll
+  for (int k = 0; k < A1_ITEMS; k++) {
+    if (rank[k] == -2) continue;
+    const int i = base + k * A1_THREADS + threadIdx.x;
+    const int row = __float_as_int(c[k].w);
+    int pos;
+    if (rank[k] >= 0) pos = s_base[row] + rank[k];
+    else pos = atomicAdd(&d.slice_fill[sector_of(so, d.n_sectors, i) * d.n_rows + row], 1);
+    d.srec[pos] = make_float4(c[k].y, c[k].z, __int_as_float(i), 0.0f);
+  }
 }
 
-// ---------------------------------------------------------------- (a3) bin histogram (rank = arrival order)
-__global__ void __launch_bounds__(256) k_bin_count(Dev d, SecOff so) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= d.n) return;
-  const float4 c = __ldg(&d.clusters[i]);
-  const int row = __float_as_int(c.w);
-  if (row < 0 || row >= d.n_rows) { d.cluster_bin[i] = -1; return; }
-  const int sl = sector_of(so, d.n_sectors, i) * d.n_rows + row;
-  const GridHdr g = d.grid[sl];
-  int by = (int)((c.y - g.ymin) * g.inv_by);
-  int bz = (int)((c.z - g.zmin) * g.inv_bz);
+// (a4) one block per slice: bounding box -> grid header -> bin histogram -> exclusive scan -> scatter
+#define A4_THREADS 256
+#define A4_SMEM_BINS 16384  // bins held in shared memory (64 KB); a larger slice keeps its counters in bin_start itself
+
+__device__ __forceinline__ int bin_of(const GridHdr& g, float y, float z) {
+  int by = (int)((y - g.ymin) * g.inv_by);
+  int bz = (int)((z - g.zmin) * g.inv_bz);
   by = max(0, min(by, g.ny - 1));
   bz = max(0, min(bz, g.nz - 1));
-  const int gb = g.bin_base + by * g.nz + bz;
-  d.cluster_bin[i] = gb;
-  d.cluster_rank[i] = atomicAdd(&d.bin_start[gb], 1);
+  return by * g.nz + bz;
 }
 
-// ---------------------------------------------------------------- (a4) scatter into sorted SoA
-__global__ void __launch_bounds__(256) k_scatter(Dev d, SecOff so) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= d.n) return;
-  const int gb = d.cluster_bin[i];
-  if (gb < 0) { d.out_assign[i] = -1; return; }
-  const float4 c = __ldg(&d.clusters[i]);
-  const int pos = d.bin_start[gb] + d.cluster_rank[i];
-  d.yz[pos] = make_float2(c.y, c.z);
-  d.orig_idx[pos] = i;
-}
-
-// slice id of every sorted position: one block per slice, coalesced stores (instead of a 2-byte scatter)
-__global__ void __launch_bounds__(128) k_fill_slice_of(Dev d) {
-  const int sl = blockIdx.x;
-  const int b = d.row_start[sl], e = d.row_start[sl + 1];
-  for (int i = b + threadIdx.x; i < e; i += blockDim.x) d.slice_of[i] = (uint16_t)sl;
+__global__ void __launch_bounds__(A4_THREADS) k_slice_sort(Dev d) {
+  extern __shared__ int s_hist[];
+  __shared__ int sm[32];
+  __shared__ uint32_t s_box[4];
+  const int sl = blockIdx.x, tid = threadIdx.x;
+  const int b = d.row_start[sl], e = d.row_start[sl + 1], cnt = e - b;
+  const int bbase = d.bin_base[sl];
+  GridHdr g;
+  g.ymin = g.zmin = 0.0f; g.inv_by = g.inv_bz = 0.0f; g.ny = g.nz = 1; g.bin_base = bbase; g.pad = 0;
+  if (cnt == 0) {
+    if (tid == 0) d.grid[sl] = g;
+    return;
+  }
+  // ---- bounding box (ordered-uint min / max)
+  if (tid < 4) s_box[tid] = (tid & 1) ? 0u : 0xFFFFFFFFu;
+  __syncthreads();
+  {
+    uint32_t ylo = 0xFFFFFFFFu, yhi = 0u, zlo = 0xFFFFFFFFu, zhi = 0u;
+    for (int i = b + tid; i < e; i += A4_THREADS) {
+      const float4 c = d.srec[i];
+      const uint32_t oy = ordf(c.x), oz = ordf(c.y);
+      ylo = min(ylo, oy); yhi = max(yhi, oy); zlo = min(zlo, oz); zhi = max(zhi, oz);
+    }
+    ylo = __reduce_min_sync(0xffffffffu, ylo); yhi = __reduce_max_sync(0xffffffffu, yhi);
+    zlo = __reduce_min_sync(0xffffffffu, zlo); zhi = __reduce_max_sync(0xffffffffu, zhi);
+    if ((tid & 31) == 0) {
+      atomicMin(&s_box[0], ylo); atomicMax(&s_box[1], yhi); atomicMin(&s_box[2], zlo); atomicMax(&s_box[3], zhi);
+    }
+  }
+  __syncthreads();
+  // ---- grid header (every thread computes the same values)
+  {
+    const float ymin = unordf(s_box[0]), ymax = unordf(s_box[1]), zmin = unordf(s_box[2]), zmax = unordf(s_box[3]);
+    const float ye = fmaxf(ymax - ymin, 1e-3f), ze = fmaxf(zmax - zmin, 1e-3f);
+    int ny = (int)(ye / d.P.grid_bin_y) + 1;
+    ny = min(ny, 128);
+    const float want = (float)cnt * d.P.grid_bins_per_cluster / (float)ny;
+    int nz = (int)want + 1;
+    const int nz_cap = (int)fminf(ze / d.P.grid_bin_z_min, 1.0e6f) + 1;
+    nz = max(1, min(nz, nz_cap));
+    if (ny * nz + 1 > d.bin_base[sl + 1] - bbase) { ny = 1; nz = 1; }  // cannot happen: ny*nz <= bins_per_cluster*cnt + 128
+    g.ymin = ymin; g.zmin = zmin;
+    g.inv_by = ((float)ny / ye) * 0.9999f;
+    g.inv_bz = ((float)nz / ze) * 0.9999f;
+    g.ny = ny; g.nz = nz; g.pad = cnt;
+  }
+  const int nb = g.ny * g.nz;
+  // counters: hist[k] = count -> start -> end of bin k; bin_start[bbase + 1 + k] receives end(k) = start(k + 1)
+  int* hist = (nb <= A4_SMEM_BINS) ? s_hist : (d.bin_start + bbase + 1);
+  for (int k = tid; k < nb; k += A4_THREADS) hist[k] = 0;
+  __syncthreads();
+  for (int i = b + tid; i < e; i += A4_THREADS) {
+    const float4 c = d.srec[i];
+    atomicAdd(&hist[bin_of(g, c.x, c.y)], 1);
+  }
+  __syncthreads();
+  {  // exclusive scan in place (+ b): thread t owns an odd-length run of bins
+    const int chunk = ((nb + A4_THREADS - 1) / A4_THREADS) | 1;
+    const int k0 = min(tid * chunk, nb), k1 = min(k0 + chunk, nb);
+    int s = 0;
+    for (int k = k0; k < k1; k++) s += hist[k];
+    int tot;
+    int ex = block_scan_excl(s, &tot, sm) + b;
+    for (int k = k0; k < k1; k++) {
+      const int v = hist[k];
+      hist[k] = ex;
+      ex += v;
+    }
+  }
+  __syncthreads();
+  for (int i = b + tid; i < e; i += A4_THREADS) {
+    const float4 c = d.srec[i];
+    const int pos = atomicAdd(&hist[bin_of(g, c.x, c.y)], 1);
+    d.yz[pos] = make_float2(c.x, c.y);
+    d.orig_idx[pos] = __float_as_int(c.z);
+    d.slice_of[pos] = (uint16_t)sl;
+  }
+  __syncthreads();
+  if (nb <= A4_SMEM_BINS)
+    for (int k = tid; k < nb; k += A4_THREADS) d.bin_start[bbase + 1 + k] = hist[k];
+  if (tid == 0) {
+    d.bin_start[bbase] = b;
+    d.grid[sl] = g;
+    d.slice_bbox[4 * sl + 0] = s_box[0]; d.slice_bbox[4 * sl + 1] = s_box[1];
+    d.slice_bbox[4 * sl + 2] = s_box[2]; d.slice_bbox[4 * sl + 3] = s_box[3];
+    atomicAdd(&d.cnt->n_bins, nb);
+  }
 }
 
 void launch_grid(const Dev& d, const SecOff& so, Launch& L) {
-  k_reset<<<(max(d.n_slices, 4 * 1024) + 256) / 256, 256, 0, L.st>>>(d);
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaFuncSetAttribute(k_slice_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, A4_SMEM_BINS * (int)sizeof(int));
+    attr_set = true;
+  }
+  k_reset<<<32, 256, 0, L.st>>>(d);
   L.count++;
   if (d.n > 0) {
-    k_slice_count<<<(d.n + A1_THREADS * A1_ITEMS - 1) / (A1_THREADS * A1_ITEMS), A1_THREADS, 0, L.st>>>(d, so);
+    k_slice_count<<<(d.n + A1_TILE - 1) / A1_TILE, A1_THREADS, 0, L.st>>>(d, so);
     L.count++;
   }
-  k_slice_setup<<<1, 1024, 0, L.st>>>(d);
-  k_zero_bins<<<148 * 4, 256, 0, L.st>>>(d);
-  L.count += 2;
+  k_slice_offsets<<<1, 1024, 0, L.st>>>(d);
+  L.count++;
   if (d.n > 0) {
-    k_bin_count<<<(d.n + 255) / 256, 256, 0, L.st>>>(d, so);
+    k_slice_scatter<<<(d.n + A1_TILE - 1) / A1_TILE, A1_THREADS, 0, L.st>>>(d, so);
     L.count++;
-    launch_scan_i32(d.bin_start, &d.cnt->n_bins, d.max_bins, d.scan_tmp, L);
-    k_scatter<<<(d.n + 255) / 256, 256, 0, L.st>>>(d, so);
-    k_fill_slice_of<<<d.n_slices, 128, 0, L.st>>>(d);
-    L.count += 2;
   }
+  k_slice_sort<<<d.n_slices, A4_THREADS, A4_SMEM_BINS * sizeof(int), L.st>>>(d);
+  L.count++;
 }
