@@ -287,8 +287,14 @@ __global__ void __launch_bounds__(A1_THREADS) k_slice_scatter(Dev d, SecOff so) 
 }
 
 // (a4) one block per slice: bounding box -> grid header -> bin histogram -> exclusive scan -> scatter
-#define A4_THREADS 256
-#define A4_SMEM_BINS 16384  // bins held in shared memory (64 KB); a larger slice keeps its counters in bin_start itself
+#ifndef A4_THREADS
+#define A4_THREADS 512
+#endif
+#ifndef A4_SMEM_BINS
+#define A4_SMEM_BINS 12288
+#endif
+// A4_SMEM_BINS bins are held in shared memory (48 KB: four 512-thread blocks per SM); a larger slice keeps its
+// counters in bin_start itself
 
 __device__ __forceinline__ int bin_of(const GridHdr& g, float y, float z) {
   int by = (int)((y - g.ymin) * g.inv_by);
@@ -354,7 +360,7 @@ __global__ void __launch_bounds__(A4_THREADS) k_slice_sort(Dev d) {
     atomicAdd(&hist[bin_of(g, c.x, c.y)], 1);
   }
   __syncthreads();
-  {  // exclusive scan in place (+ b): thread t owns an odd-length run of bins
+  if (nb <= A4_SMEM_BINS) {  // exclusive scan in place (+ b); shared memory: thread t owns an odd-length run of bins
     const int chunk = ((nb + A4_THREADS - 1) / A4_THREADS) | 1;
     const int k0 = min(tid * chunk, nb), k1 = min(k0 + chunk, nb);
     int s = 0;
@@ -365,6 +371,16 @@ __global__ void __launch_bounds__(A4_THREADS) k_slice_sort(Dev d) {
       const int v = hist[k];
       hist[k] = ex;
       ex += v;
+    }
+  } else {  // global memory: one tile of A4_THREADS bins per step (coalesced)
+    int carry = b;
+    for (int k0 = 0; k0 < nb; k0 += A4_THREADS) {
+      const int k = k0 + tid;
+      const int v = (k < nb) ? hist[k] : 0;
+      int tot;
+      const int ex = block_scan_excl(v, &tot, sm);
+      if (k < nb) hist[k] = carry + ex;
+      carry += tot;
     }
   }
   __syncthreads();

@@ -131,10 +131,14 @@ def test_parity_dense_noise_overflows_candidate_lists(row_x):
     """Noise far above the track density: the neighbour windows hold more candidates than the shared-memory lists
     (NB_CAP), so the nested-loop fallback of k_neighbours and multi-pass pick-up searches are exercised."""
     cfg = synth.config(1, scale=0.5, seed=43)
-    cfg["noise_frac"] = 40.0
+    cfg["noise_frac"] = 60.0
     fr = synth.generate(cfg)
     t, orc, exact = compare(fr, row_x)
-    assert fr.n > 300000 and exact
+    assert fr.n > 500000 and exact
+    # the same frame with > 12288 bins per slice: the slice sort keeps its counters in global memory
+    t2 = run_gpu(fr, row_x, grid_bins_per_cluster=4.0, grid_bin_z_min=0.05)
+    assert t2.stats()["n_bins"] > 12288 * 152
+    assert np.array_equal(t2.assignment(), t.assignment()) and t2.tracks().tobytes() == t.tracks().tobytes()
 
 
 def test_parity_duplicate_clusters_tie_breaks(row_x):
