@@ -11,8 +11,12 @@
 // (NB_CAP entries each; the bins of up to two y-bin rows form one flat index space walked NB_UNROLL at a time
 // with independent loads), then the (up, down) pairs are evaluated from shared memory.  A list that overflows
 // (dense noise) falls back to the plain nested loops -- same result either way.
-#define NB_THREADS 128
+#ifndef NB_THREADS
+#define NB_THREADS 64
+#endif
+#ifndef NB_CAP
 #define NB_CAP 8
+#endif
 #ifndef NB_UNROLL
 #define NB_UNROLL 2
 #endif
