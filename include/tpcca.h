@@ -66,7 +66,7 @@ typedef struct {
   float qual_scale;
   float grid_bin_y, grid_bin_z_min;         /* cm */
   float grid_bins_per_cluster;              /* target bins per cluster in a row slice, <= 4 */
-  int64_t max_clusters;                     /* capacity per call */
+  int64_t max_clusters;                     /* capacity per call, <= 4e8 (32-bit positions and bin ids) */
   int32_t max_tracklets, max_tracks;
   void* workspace;                          /* device, >= tpcca_workspace_bytes(), 256-byte aligned; caller-owned */
   size_t workspace_bytes;

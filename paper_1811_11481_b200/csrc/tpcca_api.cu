@@ -103,7 +103,7 @@ static bool check_geo_params(const tpcca_geometry* g, const tpcca_params* p) {
   if (g->n_sectors < 1 || g->n_sectors > TPCCA_MAX_SECTORS) { set_err("n_sectors out of range [1,64]"); return false; }
   if (g->n_rows < 2 || g->n_rows > TPCCA_MAX_ROWS) { set_err("n_rows out of range [2,256]"); return false; }
   if ((size_t)g->n_sectors * g->n_rows > 65535) { set_err("n_sectors*n_rows must fit 16 bits"); return false; }
-  if (p->max_clusters < 0 || p->max_clusters > 1000000000LL || p->max_tracklets < 0 || p->max_tracks < 0) {
+  if (p->max_clusters < 0 || p->max_clusters > 400000000LL || p->max_tracklets < 0 || p->max_tracks < 0) {
     set_err("capacities out of range"); return false;
   }
   if (p->min_track_hits < 2 || p->min_tracklet_hits < 2 || p->min_seed_hits < 2) { set_err("min_*_hits must be >= 2"); return false; }

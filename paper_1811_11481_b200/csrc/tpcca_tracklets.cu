@@ -59,7 +59,9 @@ __global__ void __launch_bounds__(256) k_seed_compact(Dev d) {
 // per warp refill; ballot + popc give the lanes their ranks), so a warp never idles on its longest seed.
 // The Kalman state travels between the kernels through tl_state[w][24].  row_hit is [w][row]: a lane's
 // consecutive rows share a 32-byte sector, which L2 merges.
+#ifndef E_THREADS
 #define E_THREADS 128
+#endif
 #define E_STATE 40  // floats per seed in tl_state (layout: see k_tl_e3a)
 #define FULL 0xffffffffu
 #ifndef E_REFILL_MIN
