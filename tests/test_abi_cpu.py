@@ -33,7 +33,7 @@ def test_struct_layouts_match_header():
     assert binding.CLUSTER_DTYPE.itemsize == 16
     p = binding.default_params()
     assert abs(p.triplet_cut - 18.0) < 1e-6 and p.min_track_hits == 10 and abs(p.cov0[4] - 100.0) < 1e-6
-    assert p.max_gap == 5 and abs(p.grid_bins_per_cluster - 1.0) < 1e-6
+    assert p.max_gap == 5 and abs(p.grid_bins_per_cluster - 2.0) < 1e-6 and abs(p.grid_bin_y - 6.0) < 1e-6
 
 
 def test_defaults_equal_oracle_defaults():
