@@ -97,7 +97,8 @@ class Tracker:
 
     def __init__(self, row_x: np.ndarray, n_sectors: int = 36, bz: float = 0.5, max_clusters: int = 1 << 20,
                  max_tracklets: int | None = None, max_tracks: int | None = None,
-                 tan_half_angle: float = float(np.tan(np.deg2rad(10.0))), device: str = "cuda:0", **params):
+                 tan_half_angle: float = float(np.tan(np.deg2rad(10.0))), device: str = "cuda:0",
+                 poison: int | None = None, **params):
         import torch
         self.torch = torch
         self.lib = load()
@@ -123,6 +124,8 @@ class Tracker:
         if nbytes == 0:
             raise TpccaError(self.lib.tpcca_last_error().decode())
         self.workspace = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+        if poison is not None:  # tests: scratch must never be read before it is written
+            self.workspace.fill_(int(poison))
         base = (self.workspace.data_ptr() + 255) & ~255
         p.workspace, p.workspace_bytes = base, nbytes
         self.params = p

@@ -202,3 +202,17 @@ def test_concurrent_handles_on_two_streams(row_x):
         th.join()
     for i in range(2):
         assert np.array_equal(out[i][0], ref[i][0]) and out[i][1] == ref[i][1]
+
+
+@pytest.mark.parametrize("poison", [0xFF, 0x7B])
+def test_poisoned_workspace(row_x, poison):
+    """The caller's workspace may hold anything: every scratch array is written before it is read (frames with 36
+    sectors and with one sector, capacities well above the frame, two calls per handle)."""
+    for cfg, scale, ns in ((2, 0.1, 36), (1, 0.5, 1)):
+        fr = synth.generate(synth.config(cfg, scale=scale, seed=61))
+        t = B.Tracker(row_x, n_sectors=ns, max_clusters=2 * fr.n + 1000, max_tracklets=fr.n, max_tracks=fr.n // 2,
+                      poison=poison)
+        t.out_tracks.fill_(poison)
+        t.out_assign.fill_(poison)
+        run_gpu(fr, row_x, t)
+        compare(fr, row_x, tracker=t)
