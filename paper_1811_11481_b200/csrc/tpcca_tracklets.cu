@@ -3,7 +3,7 @@
 //              adjacent hits are collected without following multiple track hypotheses, and the fit is refined";
 // PAPER.md:65-68  outward first, then inward through the seed rejecting outliers;
 // PAPER.md:57  parallel over tracks;  PAPER.md:121  fp32, z kept relative to the start hit.
-// One thread per start hit.  E1 seed fit along the links, E2 outward pick-up, E3 inward pass.
+// One lane per seed.  E1 seed fit along the links, E2 outward pick-up, E3a inward through the seed, E3b pick-up below it.
 #include "tpcca_dev.cuh"
 
 __device__ __forceinline__ unsigned long long pack_weight(const Dev& d, int n_hits, float chi2, uint32_t tid) {
@@ -50,14 +50,16 @@ __global__ void __launch_bounds__(256) k_seed_compact(Dev d) {
 }
 
 // ---------------------------------------------------------------- (e) constructor
-// Three persistent kernels, one per phase of DESIGN.md O5, so that every warp runs ONE uniform step body:
+// Four persistent kernels, one per kind of row step of DESIGN.md O5, so that every warp runs ONE uniform step body:
 //   k_tl_e1  seed fit along the links            (transport + update)
 //   k_tl_e2  outward extrapolation and pick-up   (transport + search + update)
 //   k_tl_e3a inward pass through the seed        (transport + keep/reject of the existing hit + update)
 //   k_tl_e3b pick-up below the seed               (transport + search + update)
 // Every lane runs one seed at a time and, when it is done, takes the next one from a global queue (one atomic
 // per warp refill; ballot + popc give the lanes their ranks), so a warp never idles on its longest seed.
-// The Kalman state travels between the kernels through tl_state[w][24].  row_hit is [w][row]: a lane's
+// E2, E3a and E3b take the seeds longest first (counting sort by expected row steps, launch_order_desc): with only a
+// few seeds per resident lane the tail decides the time.  E1 keeps the id order: its link -> cluster gathers are local in it.
+// The Kalman state travels between the kernels through tl_state[w][E_STATE].  row_hit is [w][row]: a lane's
 // consecutive rows share a 32-byte sector, which L2 merges.
 #ifndef E_THREADS
 #define E_THREADS 128
