@@ -312,7 +312,12 @@ def run_gpu(args):
         cv, ct, cn = oracle_timed(1.0, 5, 1, 0, fr=fr)
         cpu_baseline = {"value": cv, "unit": UNIT, "cores": 1, "kind": "oracle",
                         "sample": f"one pass over the same config-5 frame, {cn} clusters, {ct:.1f} s"}
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+    try:
+        baseline_metric = json.load(open(os.path.join(ROOT, "BASELINE.json")))["metric"]
+    except Exception:
+        baseline_metric = None
+    line = {"metric": METRIC, "baseline_metric": baseline_metric, "value": value, "unit": UNIT, "n_gpus": world,
+            "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": "config5_timeframe_50_collisions", "clusters_per_frame": n,
