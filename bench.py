@@ -126,14 +126,21 @@ def oracle_timed(scale: float, seed: int, steps: int, warmup: int, fr=None):
     if fr is None:
         fr = synth.generate(synth.config(5, scale=scale, seed=seed))
     rx = synth.row_x()
-    times = []
+    times, res = [], None
     for i in range(warmup + steps):
         t0 = time.perf_counter()
-        oracle.track(fr.clusters, fr.sector_offsets, rx)
+        res = oracle.track(fr.clusters, fr.sector_offsets, rx)
         if i >= warmup:
             times.append(time.perf_counter() - t0)
     t = float(np.mean(times))
-    return fr.n / t, t, fr.n
+    return fr.n / t, t, fr.n, res
+
+
+def quality(assignment, n_tracks, fr):
+    """Efficiency / clone / fake rate against the generator's truth, per (track, sector) segment."""
+    from paper_1811_11481_b200 import score
+    q = score.score(assignment, fr.truth, score.sector_of_cluster(fr.sector_offsets, fr.n), n_tracks)
+    return {k: (round(v, 5) if isinstance(v, float) else v) for k, v in q.items()}
 
 
 def run_reference(args):
@@ -141,7 +148,7 @@ def run_reference(args):
     if rank != 0:
         return 0
     scale = 0.2
-    v, t, n = oracle_timed(scale, 5, args.steps, args.warmup)
+    v, t, n, _ = oracle_timed(scale, 5, args.steps, args.warmup)
     sample = f"config 5 at {int(round(50 * scale))} collisions in {1000 * scale:.0f} us (same occupancy), {n} clusters/step"
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak",
@@ -279,6 +286,8 @@ def run_gpu(args):
 
     if rank != 0:
         return 0
+    gpu_assignment = oa.numpy().copy()
+    gpu_quality = quality(gpu_assignment, nt, fr)
     # ---- roofline of the dominant kernel (per-stage CUDA events recorded inside the timed loop)
     peak, peak_src = peaks()
     dom = max(stage, key=stage.get)
@@ -309,9 +318,11 @@ def run_gpu(args):
     # ---- CPU baseline: the oracle as it stands, one pass over the same frame (rank 0, N = 1 only)
     cpu_baseline = None
     if world == 1:
-        cv, ct, cn = oracle_timed(1.0, 5, 1, 0, fr=fr)
+        cv, ct, cn, ores = oracle_timed(1.0, 5, 1, 0, fr=fr)
         cpu_baseline = {"value": cv, "unit": UNIT, "cores": 1, "kind": "oracle",
-                        "sample": f"one pass over the same config-5 frame, {cn} clusters, {ct:.1f} s"}
+                        "sample": f"one pass over the same config-5 frame, {cn} clusters, {ct:.1f} s",
+                        "quality": quality(ores.assignment, len(ores.tracks), fr),
+                        "assignment_equals_cuda_path": bool(np.array_equal(ores.assignment, gpu_assignment))}
     try:
         baseline_metric = json.load(open(os.path.join(ROOT, "BASELINE.json")))["metric"]
     except Exception:
@@ -323,6 +334,7 @@ def run_gpu(args):
             "config": {"workload": "config5_timeframe_50_collisions", "clusters_per_frame": n,
                        "frames_per_step": world, "ms_per_time_frame": ms_per_step, "n_tracks": hd["n_tracks"],
                        "n_start_hits": hd["n_start_hits"], "row_steps": stats["row_steps"],
+                       "quality": gpu_quality,
                        "l2": "inputs larger than L2 (cluster array %.0f MB, working set > 1 GB)" % (n * 16 / 1e6),
                        "parallelism": f"frames x{world} (no collective)"},
             "clocks": clocks, "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
