@@ -216,3 +216,15 @@ def test_poisoned_workspace(row_x, poison):
         t.out_assign.fill_(poison)
         run_gpu(fr, row_x, t)
         compare(fr, row_x, tracker=t)
+
+
+def test_parity_hand_built_scenarios(row_x):
+    """The hand-built inputs of the oracle's mechanics pins (gap of 5 and 6 rows, displaced hit with default and tight
+    reject_cut, two crossing helices) through the CUDA path: tiny single-sector frames, every table compared."""
+    from tests import scenarios
+    for cl, params in ((scenarios.gap_helix(row_x, 5), None), (scenarios.gap_helix(row_x, 6), None),
+                       (scenarios.displaced_hit_helix(row_x), None),
+                       (scenarios.displaced_hit_helix(row_x), dict(reject_cut=4.0)),
+                       (scenarios.crossing_helices(row_x)[0], None)):
+        t, orc, exact = compare(scenarios.frame(cl), row_x, params=params)
+        assert len(orc.tracks) >= 1 and exact

@@ -405,13 +405,7 @@ def test_golden_oracle_regression():
 
 
 # ---------------------------------------------------------------- mechanics of following, rejection and selection
-def _one_helix(row_x, rows=None, **kw):
-    rows = np.arange(len(row_x)) if rows is None else np.asarray(rows)
-    par = dict(x0=85.0, y0=0.5, z0=20.0, sinphi0=0.08, tanl=0.4, qpt=1.2, bz=0.5)
-    par.update(kw)
-    y, z, _ = helix_points(row_x[rows].astype(np.float64), par["x0"], par["y0"], par["z0"], par["sinphi0"],
-                           par["tanl"], par["qpt"], par["bz"])
-    return rows, y, z
+from tests import scenarios  # noqa: E402
 
 
 @pytest.mark.parametrize("missing,expect_tracks", [(5, 1), (6, 2)])
@@ -419,9 +413,8 @@ def test_gap_rule(row_x, missing, expect_tracks):
     """PAPER.md:51 "extrapolated through the TPC volume": `max_gap` = 5 consecutive rows without a cluster are
     bridged (both seeds then collect the same hits and the selector keeps one track); 6 are not (two tracks)."""
     R = len(row_x)
-    rows = np.r_[np.arange(0, 60), np.arange(60 + missing, R)]
-    rows, y, z = _one_helix(row_x, rows)
-    r = oracle.track(_mk(rows, y, z, row_x), np.array([0, len(rows)], np.int32), row_x)
+    cl = scenarios.gap_helix(row_x, missing)
+    r = oracle.track(cl, np.array([0, len(cl)], np.int32), row_x)
     assert len(r.tracks) == expect_tracks
     if expect_tracks == 1:
         assert r.tracks["n_hits"][0] == R - missing and (r.assignment == 0).all()
@@ -435,10 +428,7 @@ def test_outlier_rejection_on_the_inward_pass(row_x):
     """on the inward pass a hit of the seed that does not fit is rejected.  One hit displaced by 0.3 cm
     keeps its links (triplet cost 9 <= 18) and survives reject_cut = 25 (d ~ 9), but is dropped at reject_cut = 4."""
     R = len(row_x)
-    rows, y, z = _one_helix(row_x)
-    y = y.copy()
-    y[80] += 0.3
-    cl = _mk(rows, y, z, row_x)
+    cl = scenarios.displaced_hit_helix(row_x)
     so = np.array([0, R], np.int32)
     keep = oracle.track(cl, so, row_x)
     assert len(keep.tracks) == 1 and keep.tracks["n_hits"][0] == R and keep.assignment[80] == 0
@@ -452,22 +442,11 @@ def test_shared_cluster_goes_to_the_longer_track(row_x):
     """north_star (f) / PAPER.md:70: a cluster claimed by two tracklets goes to the one with more hits.  Two helices
     cross at row 90 and share that one cluster; the short one (rows 40-130) loses it."""
     R = len(row_x)
-    rows_a, ya, za = _one_helix(row_x)
-    x90 = float(row_x[90])
-    rows_b = np.arange(40, 131)
-    # second helix through the first one's point at row 90, with another direction
-    yb, zb, _ = helix_points(row_x[rows_b].astype(np.float64), x90, ya[90], za[90], -0.25, -0.6, -0.8, 0.5)
-    keep = rows_b != 90  # the crossing cluster exists once
-    rows = np.r_[rows_a, rows_b[keep]]
-    cl = _mk(rows, np.r_[ya, yb[keep]], np.r_[za, zb[keep]], row_x)
-    order = np.argsort(rows, kind="stable")
-    cl = cl[order]
+    cl, is_a = scenarios.crossing_helices(row_x)
     r = oracle.track(cl, np.array([0, len(cl)], np.int32), row_x)
     assert len(r.tracks) == 2
-    is_a = np.r_[np.ones(R, bool), np.zeros(keep.sum(), bool)][order]
     ta = r.assignment[is_a]
     tb = r.assignment[~is_a]
     assert (ta == ta[0]).all() and ta[0] >= 0, "the long track keeps every cluster, the shared one included"
     assert (tb[tb >= 0] == tb[tb >= 0][0]).all() and tb[tb >= 0][0] != ta[0]
-    nh = dict(zip(r.tracks["n_hits"], range(2)))
-    assert R in nh and max(n for n in nh if n != R) <= len(rows_b) - 1
+    assert R in r.tracks["n_hits"] and min(r.tracks["n_hits"]) <= 90
