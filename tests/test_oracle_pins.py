@@ -450,3 +450,23 @@ def test_shared_cluster_goes_to_the_longer_track(row_x):
     assert (ta == ta[0]).all() and ta[0] >= 0, "the long track keeps every cluster, the shared one included"
     assert (tb[tb >= 0] == tb[tb >= 0][0]).all() and tb[tb >= 0][0] != ta[0]
     assert R in r.tracks["n_hits"] and min(r.tracks["n_hits"]) <= 90
+
+
+def test_canonical_orders(cfg2_small, row_x):
+    """DESIGN.md A4 / O4 / O6: tracklet ids follow (sector, row, ord z, ord y, input index) of the start hit, track ids
+    follow tracklet ids; both are what makes the output independent of the input order."""
+    fr, r = cfg2_small
+    sh = r.start_hits
+    sec = score.sector_of_cluster(fr.sector_offsets, fr.n)[sh]
+    c = fr.clusters[sh]
+
+    def ordf(f):
+        b = f.astype(np.float32).view(np.uint32).astype(np.uint64)
+        return np.where(b & 0x80000000, (~b) & 0xFFFFFFFF, b | 0x80000000)
+
+    keys = list(zip(sec.tolist(), c["row"].tolist(), ordf(c["z"]).tolist(), ordf(c["y"]).tolist(), sh.tolist()))
+    assert keys == sorted(keys) and len(set(keys)) == len(keys)
+    assert (np.diff(r.track_tracklet) > 0).all()
+    # a start hit has an up-link and no down-link; every such cluster is a start hit
+    is_start = (r.link_down < 0) & (r.link_up >= 0)
+    assert np.array_equal(np.sort(sh), np.flatnonzero(is_start))
