@@ -549,6 +549,9 @@ __global__ void __launch_bounds__(128) k_tracklet_weights(Dev d) {
   }
 }
 
+#ifndef W_GRID
+#define W_GRID 8  // CTAs per SM of k_tracklet_weights: the L2 atomic units saturate with 32 warps per SM (16: +0.07 ms)
+#endif
 #ifndef E2_GRID
 #define E2_GRID E2_BLOCKS
 #endif
@@ -569,6 +572,6 @@ void launch_tracklets(const Dev& d, Launch& L) {
   k_tl_e3a<<<148 * E3_GRID, E_THREADS, 0, L.st>>>(d);
   launch_order_desc(d, 3, d.e_key + 2 * (size_t)T, &d.cnt->n_work, T, d.e_order + 2 * (size_t)T, L);
   k_tl_e3b<<<148 * E3B_BLOCKS, E_THREADS, 0, L.st>>>(d);
-  k_tracklet_weights<<<148 * 16, 128, 0, L.st>>>(d);
+  k_tracklet_weights<<<148 * W_GRID, 128, 0, L.st>>>(d);
   L.count += 6;
 }
