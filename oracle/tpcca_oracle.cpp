@@ -57,75 +57,84 @@ inline uint32_t ordf(float f) {  // monotone float -> uint map
   return (b & 0x80000000u) ? ~b : (b | 0x80000000u);
 }
 
-// ---- O5 model: transport x -> xnew ----
+inline int tri(int i, int j) { return i >= j ? i * (i + 1) / 2 + j : j * (j + 1) / 2 + i; }
+
+// ---- O5 model: transport x -> xnew (DESIGN.md section 3 "Transport") ----
+// The step is written as the textbook extended-Kalman prediction: move the state along the helix, fill the dense
+// 5x5 Jacobian F = d(y, z~, s, t, q)' / d(y, z~, s, t, q), then C <- F C F^T by the two matrix products of the
+// definition.  DESIGN.md section 3 fixes the summation order: every entry is summed over k = 0..4 in increasing k,
+// and a term whose Jacobian entry is structurally zero (see `nz`) is left out rather than added as 0 * c.
 bool transport(KF& k, float xnew, float kq, float max_sinphi) {
   const float dx = xnew - k.x;
-  if (dx == 0.0f) return true;
-  const float s = k.p[2], t = k.p[3], q = k.p[4];
-  const float kk = q * kq;
-  const float s1 = s + dx * kk;
-  if (!(std::fabs(s) <= max_sinphi) || !(std::fabs(s1) <= max_sinphi)) return false;
-  const float c0 = std::sqrt(1.0f - s * s);
-  const float c1 = std::sqrt(1.0f - s1 * s1);
-  const float cc = c0 + c1;
-  const float f = (s + s1) / cc;
+  if (dx == 0.0f) return true;  // identity (first step of E3 and of every refit pass)
+  const float s0 = k.p[2], tl = k.p[3];
+  const float curv = k.p[4] * kq;  // d sin(phi) / dx
+  const float s1 = s0 + dx * curv;
+  if (!(std::fabs(s0) <= max_sinphi)) return false;
+  if (!(std::fabs(s1) <= max_sinphi)) return false;
+  // helix step: chord direction f = tan of the mean angle, chord length L (signed like dx), arc = L * asin(u)/u
+  const float cos0 = std::sqrt(1.0f - s0 * s0);
+  const float cos1 = std::sqrt(1.0f - s1 * s1);
+  const float csum = cos0 + cos1;
+  const float f = (s0 + s1) / csum;
   const float dy = dx * f;
   float L = std::sqrt(dx * dx + dy * dy);
   if (dx < 0.0f) L = -L;
-  const float u = (0.5f * kk) * L;
+  const float u = (0.5f * curv) * L;
   const float u2 = u * u;
-  const float g = 1.0f + u2 * (0.16666667f + u2 * 0.075f);  // asin(u)/u series
-  const float dS = L * g;
-  const float fs0 = (1.0f + (f * s) / c0) / cc;
-  const float fs1 = (1.0f + (f * s1) / c1) / cc;
-  const float h = dx * kq;
-  const float fss = fs0 + fs1;
-  const float a02 = dx * fss;
-  const float a04 = (dx * fs1) * h;
-  const float w = (t * g) * ((dx * dy) / L);
-  const float a12 = w * fss;
-  const float a13 = dS;
-  const float a14 = (w * fs1) * h;
-  const float a24 = h;
+  const float g = 1.0f + u2 * (0.16666667f + u2 * 0.075f);  // asin(u)/u = 1 + u^2/6 + 3u^4/40 + ...
+  const float arc = L * g;
+  // Jacobian (d g neglected): d f / d s0 and d f / d s1, then the chain rule through s1 = s0 + dx * kq * q
+  const float df_ds0 = (1.0f + (f * s0) / cos0) / csum;
+  const float df_ds1 = (1.0f + (f * s1) / cos1) / csum;
+  const float ds1_dq = dx * kq;
+  const float df_ds = df_ds0 + df_ds1;
+  const float darc_df = (tl * g) * ((dx * dy) / L);  // d(z~)/df = t * g * dL/df, dL/df = dx*dy/L
+  float F[5][5];
+  bool nz[5][5];
+  for (int i = 0; i < 5; i++)
+    for (int j = 0; j < 5; j++) { F[i][j] = (i == j) ? 1.0f : 0.0f; nz[i][j] = (i == j); }
+  F[0][2] = dx * df_ds;               nz[0][2] = true;
+  F[0][4] = (dx * df_ds1) * ds1_dq;   nz[0][4] = true;
+  F[1][2] = darc_df * df_ds;          nz[1][2] = true;
+  F[1][3] = arc;                      nz[1][3] = true;
+  F[1][4] = (darc_df * df_ds1) * ds1_dq; nz[1][4] = true;
+  F[2][4] = ds1_dq;                   nz[2][4] = true;
+  // state
   k.p[0] = k.p[0] + dy;
-  k.p[1] = k.p[1] + t * dS;
+  k.p[1] = k.p[1] + tl * arc;
   k.p[2] = s1;
   k.x = xnew;
-  float* C = k.C;
-  const float c00 = C[0], c10 = C[1], c11 = C[2], c20 = C[3], c21 = C[4], c22 = C[5], c30 = C[6], c31 = C[7],
-              c32 = C[8], c33 = C[9], c40 = C[10], c41 = C[11], c42 = C[12], c43 = C[13], c44 = C[14];
-  const float m00 = (c00 + a02 * c20) + a04 * c40;
-  const float m02 = (c20 + a02 * c22) + a04 * c42;
-  const float m04 = (c40 + a02 * c42) + a04 * c44;
-  const float m10 = ((c10 + a12 * c20) + a13 * c30) + a14 * c40;
-  const float m11 = ((c11 + a12 * c21) + a13 * c31) + a14 * c41;
-  const float m12 = ((c21 + a12 * c22) + a13 * c32) + a14 * c42;
-  const float m13 = ((c31 + a12 * c32) + a13 * c33) + a14 * c43;
-  const float m14 = ((c41 + a12 * c42) + a13 * c43) + a14 * c44;
-  const float m20 = c20 + a24 * c40;
-  const float m21 = c21 + a24 * c41;
-  const float m22 = c22 + a24 * c42;
-  const float m23 = c32 + a24 * c43;
-  const float m24 = c42 + a24 * c44;
-  C[0] = (m00 + a02 * m02) + a04 * m04;
-  C[1] = (m10 + a02 * m12) + a04 * m14;
-  C[2] = ((m11 + a12 * m12) + a13 * m13) + a14 * m14;
-  C[3] = (m20 + a02 * m22) + a04 * m24;
-  C[4] = ((m21 + a12 * m22) + a13 * m23) + a14 * m24;
-  C[5] = m22 + a24 * m24;
-  C[6] = (c30 + a02 * c32) + a04 * c43;
-  C[7] = ((c31 + a12 * c32) + a13 * c33) + a14 * c43;
-  C[8] = c32 + a24 * c43;
-  C[9] = c33;
-  C[10] = (c40 + a02 * c42) + a04 * c44;
-  C[11] = ((c41 + a12 * c42) + a13 * c43) + a14 * c44;
-  C[12] = c42 + a24 * c44;
-  C[13] = c43;
-  C[14] = c44;
+  // covariance: full symmetric C, M = F C, C' = M F^T (lower triangle kept)
+  float Cf[5][5], M[5][5];
+  for (int i = 0; i < 5; i++)
+    for (int j = 0; j < 5; j++) Cf[i][j] = k.C[tri(i, j)];
+  for (int i = 0; i < 5; i++)
+    for (int j = 0; j < 5; j++) {
+      float acc = 0.0f;
+      bool first = true;
+      for (int l = 0; l < 5; l++) {
+        if (!nz[i][l]) continue;
+        const float term = (l == i) ? Cf[l][j] : F[i][l] * Cf[l][j];  // F_ii = 1
+        acc = first ? term : acc + term;
+        first = false;
+      }
+      M[i][j] = acc;
+    }
+  for (int i = 0; i < 5; i++)
+    for (int j = 0; j <= i; j++) {
+      float acc = 0.0f;
+      bool first = true;
+      for (int l = 0; l < 5; l++) {
+        if (!nz[j][l]) continue;
+        const float term = (l == j) ? M[i][l] : F[j][l] * M[i][l];
+        acc = first ? term : acc + term;
+        first = false;
+      }
+      k.C[tri(i, j)] = acc;
+    }
   return true;
 }
-
-inline int tri(int i, int j) { return i >= j ? i * (i + 1) / 2 + j : j * (j + 1) / 2 + i; }
 
 // ---- O5 model: scalar measurement update of component i (0: y, 1: z~) ----
 void update1(KF& k, int i, float m, float v) {

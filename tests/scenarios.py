@@ -54,3 +54,69 @@ def crossing_helices(row_x):
 
 def frame(cl):
     return synth.Frame(cl, np.array([0, len(cl)], np.int32), np.full(len(cl), -1, np.int32), np.zeros((0, 8)), 1, "scenario")
+
+
+# ---------------------------------------------------------------- round-2 scenarios (selector weight, sector edge, E3)
+def equal_length_crossing(row_x, displaced=None, mirror_z=False, dy=0.25):
+    """Two helices over the SAME rows 30..120 that cross at row 75 and share that one cluster (it exists once).
+    A: the gentle one; B: the steep one.  `displaced` = "A" / "B" moves one hit of that helix (row 50) by `dy` in y, which
+    raises its chi2 and nothing else.  `mirror_z` flips the sign of every z (swaps which helix has the lower z at the
+    first rows, i.e. the lower tracklet id).  Returns (clusters, index of the shared cluster, mask of A's own clusters,
+    mask of B's own clusters); the shared cluster is in neither mask."""
+    rows = np.arange(30, 121)
+    ya, za, _ = helix_points(row_x[rows].astype(np.float64), float(row_x[75]), 2.0, 40.0, 0.05, 0.3, 0.9, 0.5)
+    yb, zb, _ = helix_points(row_x[rows].astype(np.float64), float(row_x[75]), 2.0, 40.0, -0.22, -0.5, -0.7, 0.5)
+    ya, yb = ya.copy(), yb.copy()
+    if displaced == "A":
+        ya[50 - 30] += dy
+    elif displaced == "B":
+        yb[50 - 30] += dy
+    keep = rows != 75
+    r = np.r_[rows, rows[keep]]
+    y = np.r_[ya, yb[keep]]
+    z = np.r_[za, zb[keep]]
+    if mirror_z:
+        z = -z
+    is_a = np.r_[rows != 75, np.zeros(int(keep.sum()), bool)]
+    is_b = np.r_[np.zeros(len(rows), bool), np.ones(int(keep.sum()), bool)]
+    shared = np.r_[rows == 75, np.zeros(int(keep.sum()), bool)]
+    order = np.argsort(r, kind="stable")
+    cl = mk(r[order], y[order], z[order], row_x)
+    return cl, int(np.flatnonzero(shared[order])[0]), is_a[order], is_b[order]
+
+
+EDGE_OUT = dict(x0=85.0, y0=0.0, z0=15.0, sinphi0=0.26, tanl=0.35, qpt=-1.6, bz=0.5)    # leaves the sector upwards
+EDGE_IN = dict(x0=245.0, y0=0.0, z0=15.0, sinphi0=-0.38, tanl=0.35, qpt=1.7, bz=0.5)    # enters it from the side
+
+
+def edge_helix(row_x, inward=False, decoy_step=3):
+    """A helix that crosses the sector's side (|y| = x tan 10 deg) at mid radius.  Real clusters exist on every row where
+    the helix is inside the sector; beyond the side, on-helix "decoy" clusters sit on every `decoy_step`-th row only
+    (too sparse to form links -- one row skip at most, A5 -- and dense enough that the gap rule never fires).
+    outward (default): inside at the low rows, leaves upwards (pins the E2 stop).  inward: inside at the high rows, the
+    decoys are below (pins the E3 stop).  The parameters keep every row beyond the side at least 0.14 cm away from the
+    line |y| = x tan 10 deg + 3 cm.  Returns (clusters, float64 y of the helix on every row, in-sector mask per row)."""
+    R = len(row_x)
+    xs = row_x.astype(np.float64)
+    par = EDGE_IN if inward else EDGE_OUT
+    y, z, _ = helix_points(xs, par["x0"], par["y0"], par["z0"], par["sinphi0"], par["tanl"], par["qpt"], par["bz"])
+    inside = np.abs(y) <= xs * np.tan(np.deg2rad(10.0))
+    rows = np.arange(R)
+    if inward:
+        first_in = int(np.flatnonzero(inside)[0])
+        decoy = (~inside) & ((first_in - rows) % decoy_step == 0) & (rows < first_in)
+    else:
+        last_in = int(np.flatnonzero(inside)[-1])
+        decoy = (~inside) & ((rows - last_in) % decoy_step == 0) & (rows > last_in)
+    use = inside | decoy
+    return mk(rows[use], y[use], z[use], row_x), y, inside
+
+
+def e3_gap_above_start(row_x):
+    """Rows 99..103 removed (5 rows: E2 bridges them) and the last chain hit, row 98, displaced by 0.3 cm: on the inward
+    pass with reject_cut = pick_cut = 6 that hit is rejected, which makes SIX consecutive misses above the start row."""
+    R = len(row_x)
+    rows, y, z = one_helix(row_x, np.r_[np.arange(0, 99), np.arange(104, R)])
+    y = y.copy()
+    y[98] += 0.3
+    return mk(rows, y, z, row_x)

@@ -222,9 +222,43 @@ def test_parity_hand_built_scenarios(row_x):
     """The hand-built inputs of the oracle's mechanics pins (gap of 5 and 6 rows, displaced hit with default and tight
     reject_cut, two crossing helices) through the CUDA path: tiny single-sector frames, every table compared."""
     from tests import scenarios
-    for cl, params in ((scenarios.gap_helix(row_x, 5), None), (scenarios.gap_helix(row_x, 6), None),
-                       (scenarios.displaced_hit_helix(row_x), None),
-                       (scenarios.displaced_hit_helix(row_x), dict(reject_cut=4.0)),
-                       (scenarios.crossing_helices(row_x)[0], None)):
+    cases = [(scenarios.gap_helix(row_x, 5), None), (scenarios.gap_helix(row_x, 6), None),
+             (scenarios.displaced_hit_helix(row_x), None),
+             (scenarios.displaced_hit_helix(row_x), dict(reject_cut=4.0)),
+             (scenarios.crossing_helices(row_x)[0], None)]
+    # round 2: selector weight (quality, then id), sector-edge stops of E2 / E3, E3 gap rule above the start row
+    for displaced in (None, "A", "B"):
+        for mirror in (False, True):
+            cases.append((scenarios.equal_length_crossing(row_x, displaced, mirror)[0], None))
+    for inward in (False, True):
+        for margin in (3.0, 0.0, 60.0):
+            cases.append((scenarios.edge_helix(row_x, inward)[0], dict(edge_margin=margin)))
+    cases.append((scenarios.e3_gap_above_start(row_x), dict(reject_cut=4.0)))
+    for cl, params in cases:
         t, orc, exact = compare(scenarios.frame(cl), row_x, params=params)
         assert len(orc.tracks) >= 1 and exact
+
+
+def test_parity_exact_cost_ties(row_x):
+    """Mirror-image neighbour candidates have bit-equal triplet costs: the (ord z, ord y, input index) key order of
+    DESIGN.md A4 decides, in every input order (tests/test_oracle_pins.py::test_exact_ties_follow_the_key_order)."""
+    from tests import scenarios
+    f = np.float32
+    variants = ([(51, 0.05, +0.25), (51, 0.05, -0.25), (49, 0.0, 0.0)], [(51, +0.125, 0.1), (51, -0.125, 0.1), (49, 0.0, 0.0)],
+                [(51, 0.0, 0.0), (49, 0.05, +0.25), (49, 0.05, -0.25)], [(51, 0.05, 0.25), (51, 0.05, 0.25), (49, 0.0, 0.0)])
+    for pts in variants:
+        pts = [(50, 0.0, 0.0)] + pts
+        for order in ([0, 1, 2, 3], [3, 2, 1, 0], [2, 0, 3, 1]):
+            q = [pts[i] for i in order]
+            cl = scenarios.mk(np.array([a[0] for a in q]), np.array([a[1] for a in q], f), np.array([a[2] for a in q], f), row_x)
+            fr = scenarios.frame(cl)
+            orc = oracle_links(fr, row_x)
+            t = run_gpu(fr, row_x)
+            assert np.array_equal(t.intermediate(B.LINK_UP_RAW), orc.link_up_raw)
+            assert np.array_equal(t.intermediate(B.LINK_DOWN_RAW), orc.link_down_raw)
+            assert (orc.link_up_raw >= 0).sum() == 1
+
+
+def oracle_links(fr, row_x):
+    import oracle
+    return oracle.track(fr.clusters, fr.sector_offsets, row_x)
