@@ -39,7 +39,7 @@ enum tpcca_status {
 enum {
   TPCCA_STAT_TRACKLET_OVERFLOW = 1, /* more start hits than max_tracklets: highest ids dropped */
   TPCCA_STAT_TRACK_OVERFLOW = 2,    /* more tracks than max_tracks: highest ids dropped */
-  TPCCA_STAT_BAD_CLUSTER = 4,       /* a cluster with row outside [0,n_rows) was ignored */
+  TPCCA_STAT_BAD_CLUSTER = 4,       /* a cluster with row outside [0,n_rows) or a non-finite y / z was ignored */
   TPCCA_STAT_BIN_OVERFLOW = 8       /* internal grid capacity hit (never with the default sizing) */
 };
 
@@ -127,7 +127,13 @@ enum tpcca_intermediate {
   TPCCA_TRACKLET_FLOATS = 7,/* float[n_start_hits][8]: x, y, z-z_ref, sinphi, dzds, qpt, chi2, z_ref */
   TPCCA_TRACK_TRACKLET = 8  /* int32[n_tracks]: tracklet id of each track */
 };
+/* dst_device: 16-byte aligned, `bytes` long.  The call reads the live counts of the last frame (it synchronises
+ * `stream`) and returns TPCCA_ERR_ARGUMENT, writing nothing, if `bytes` is smaller than the table. */
 int tpcca_get_intermediate(tpcca_handle* h, int what, void* dst_device, size_t bytes, void* stream);
+
+/* Debugging aid: with on != 0 every tpcca_track on this handle synchronises after each stage and names the stage
+ * that faulted in tpcca_last_error().  Off by default; never use it in a timed run. */
+int tpcca_set_debug(tpcca_handle* h, int on);
 
 /* Per-stage device times, averaged over the tpcca_track calls (at most the last 32) made since profiling
  * was switched on (CUDA events recorded on each call's stream; synchronises those events).  ms: host float[TPCCA_N_STAGES]. */

@@ -70,6 +70,7 @@ def load():
         lib.tpcca_get_intermediate.restype = C.c_int
         lib.tpcca_get_intermediate.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_size_t, C.c_void_p]
         lib.tpcca_set_profiling.argtypes = [C.c_void_p, C.c_int]
+        lib.tpcca_set_debug.argtypes = [C.c_void_p, C.c_int]
         lib.tpcca_get_stage_ms.restype = C.c_int
         lib.tpcca_get_stage_ms.argtypes = [C.c_void_p, C.c_void_p]
         lib.tpcca_get_stats.restype = C.c_int
@@ -207,6 +208,9 @@ class Tracker:
         dst = torch.empty(max(4, numel), dtype=dt, device=self.device)
         self._check(self.lib.tpcca_get_intermediate(self.h, what, dst.data_ptr(), dst.numel() * 4, self._stream()))
         return dst[:numel].reshape(shape).cpu().numpy()
+
+    def set_debug(self, on: bool):
+        self.lib.tpcca_set_debug(self.h, int(on))
 
     def set_profiling(self, on: bool):
         self.lib.tpcca_set_profiling(self.h, int(on))

@@ -24,8 +24,9 @@ struct tpcca_handle {
   // last call
   int64_t last_n;
   int launches;
-  bool profiling, have_times;
+  bool profiling, have_times, debug_sync;
   int prof_calls;
+  int device;
   cudaEvent_t ev[PROF_RING][TPCCA_N_STAGES + 1];
 };
 
@@ -165,6 +166,17 @@ tpcca_handle* tpcca_init(const tpcca_geometry* g, float bz_tesla, const tpcca_pa
   d.inv_sy2 = 1.0f / d.sy2;
   d.inv_sz2 = 1.0f / d.sz2;
   d.max_tracklets = p->max_tracklets; d.max_tracks = p->max_tracks;
+  if (cudaGetDevice(&h->device) != cudaSuccess ||
+      cudaDeviceGetAttribute(&d.n_sm, cudaDevAttrMultiProcessorCount, h->device) != cudaSuccess || d.n_sm < 1) {
+    set_err("device query failed: %s", cudaGetErrorString(cudaGetLastError()));
+    delete h;
+    return nullptr;
+  }
+  if (setup_grid_kernels() != cudaSuccess) {  // per device: a second device in this process gets its own attribute
+    set_err("kernel attribute setup failed: %s", cudaGetErrorString(cudaGetLastError()));
+    delete h;
+    return nullptr;
+  }
   if (cudaMemcpy((void*)d.row_x, g->row_x, sizeof(float) * g->n_rows, cudaMemcpyHostToDevice) != cudaSuccess) {
     set_err("row_x upload failed: %s", cudaGetErrorString(cudaGetLastError()));
     delete h;
@@ -172,7 +184,12 @@ tpcca_handle* tpcca_init(const tpcca_geometry* g, float bz_tesla, const tpcca_pa
   }
   for (int k = 0; k < PROF_RING; k++)
     for (int i = 0; i <= TPCCA_N_STAGES; i++)
-      if (cudaEventCreate(&h->ev[k][i]) != cudaSuccess) { set_err("cudaEventCreate failed"); delete h; return nullptr; }
+      if (cudaEventCreate(&h->ev[k][i]) != cudaSuccess) {
+        set_err("cudaEventCreate failed: %s", cudaGetErrorString(cudaGetLastError()));
+        h->ev[k][i] = nullptr;
+        tpcca_free(h);  // destroys the events created so far
+        return nullptr;
+      }
   return h;
 }
 
@@ -195,8 +212,8 @@ static int track_impl(tpcca_handle* h, const tpcca_cluster* clusters, int64_t n,
   h->last_n = n;
   const bool prof = h->profiling;
   cudaEvent_t* ev = h->ev[h->prof_calls % PROF_RING];
-  // TPCCA_DEBUG_SYNC=1: synchronise after every stage and name the stage that faulted (debugging aid)
-  static const bool dbg = getenv("TPCCA_DEBUG_SYNC") != nullptr;
+  // tpcca_set_debug(h, 1): synchronise after every stage and name the stage that faulted (debugging aid)
+  const bool dbg = h->debug_sync;
 #define DBG_STAGE(name)                                                                          \
   if (dbg) {                                                                                     \
     const cudaError_t de = cudaStreamSynchronize(st);                                            \
@@ -283,18 +300,32 @@ int tpcca_track_host(tpcca_handle* h, const tpcca_cluster* clusters, int64_t n, 
 int tpcca_get_intermediate(tpcca_handle* h, int what, void* dst, size_t bytes, void* stream) {
   if (!h) { set_err("handle is null (not initialised)"); return TPCCA_ERR_NOT_INIT; }
   if (!dst || what < 0 || what > TPCCA_TRACK_TRACKLET) { set_err("bad intermediate id or null dst"); return TPCCA_ERR_ARGUMENT; }
+  if ((uintptr_t)dst & 15) { set_err("dst must be 16-byte aligned"); return TPCCA_ERR_ARGUMENT; }
   const Dev& d = h->d;
+  // the sizes of the tracklet / track tables are data dependent: read the live counters (synchronises `stream`;
+  // this is a parity / debugging interface, not part of the hot path)
+  DevCounters c;
+  cudaError_t e = cudaMemcpyAsync(&c, d.cnt, sizeof(c), cudaMemcpyDeviceToHost, (cudaStream_t)stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);
+  if (e != cudaSuccess) { set_err("counter copy failed: %s", cudaGetErrorString(e)); cudaGetLastError(); return TPCCA_ERR_CUDA; }
   size_t need;
   if (what <= TPCCA_LINK_DOWN) need = (size_t)d.n * 4;
-  else if (what == TPCCA_START_HITS) need = (size_t)d.max_tracklets * 4;
-  else if (what == TPCCA_TRACKLET_ROW_HITS) need = 0;  // data-dependent: caller sizes with n_start_hits
-  else need = 0;
-  if (what <= TPCCA_LINK_DOWN && bytes < need) { set_err("dst too small"); return TPCCA_ERR_ARGUMENT; }
-  (void)bytes;
+  else if (what == TPCCA_START_HITS) need = (size_t)c.n_start * 4;
+  else if (what == TPCCA_TRACKLET_ROW_HITS) need = (size_t)c.n_start * d.n_rows * 4;
+  else if (what == TPCCA_TRACKLET_INTS) need = (size_t)c.n_start * 16;
+  else if (what == TPCCA_TRACKLET_FLOATS) need = (size_t)c.n_start * 32;
+  else need = (size_t)c.n_tracks * 4;
+  if (bytes < need) { set_err("dst too small%s (need %lld bytes)", "", (long long)need); return TPCCA_ERR_ARGUMENT; }
   Launch L{(cudaStream_t)stream, 0};
   launch_export(d, what, dst, L);
-  const cudaError_t e = cudaGetLastError();
+  e = cudaGetLastError();
   if (e != cudaSuccess) { set_err("export launch failed: %s", cudaGetErrorString(e)); return TPCCA_ERR_CUDA; }
+  return TPCCA_OK;
+}
+
+int tpcca_set_debug(tpcca_handle* h, int on) {
+  if (!h) return TPCCA_ERR_NOT_INIT;
+  h->debug_sync = on != 0;
   return TPCCA_OK;
 }
 

@@ -40,6 +40,7 @@ struct SecOff { int32_t v[TPCCA_MAX_SECTORS + 1]; };
 struct Dev {
   // geometry / parameters
   int32_t n_sectors, n_rows, n_slices;
+  int32_t n_sm;  // multiprocessors of the handle's device (persistent grids are sized in multiples of it)
   float tan_half_angle, kq, sy2, sz2, inv_sy2, inv_sz2;
   tpcca_params P;
   const float* row_x;
@@ -283,6 +284,7 @@ struct Launch {
   cudaStream_t st;
   int count;  // kernels launched
 };
+cudaError_t setup_grid_kernels();  // per-device function attributes; called by tpcca_init on the handle's device
 void launch_grid(const Dev& d, const SecOff& so, Launch& L);
 void launch_neighbours(const Dev& d, Launch& L);
 void launch_clean_start(const Dev& d, Launch& L);

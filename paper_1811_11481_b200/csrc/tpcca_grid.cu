@@ -178,6 +178,11 @@ __global__ void k_reset(Dev d) {
 #define A1_ITEMS 8
 #define A1_TILE (A1_THREADS * A1_ITEMS)
 
+// a cluster with a non-finite y or z is ignored like one with a bad row (A21)
+__device__ __forceinline__ bool cluster_finite(const float4& c) {
+  return fabsf(c.y) <= 3.0e38f && fabsf(c.z) <= 3.0e38f;  // false for NaN and +-inf
+}
+
 // (a1) clusters per slice
 __global__ void __launch_bounds__(A1_THREADS) k_slice_count(Dev d, SecOff so) {
   __shared__ int s_cnt[TPCCA_MAX_ROWS];
@@ -190,8 +195,9 @@ __global__ void __launch_bounds__(A1_THREADS) k_slice_count(Dev d, SecOff so) {
   for (int k = 0; k < A1_ITEMS; k++) {
     const int i = base + k * A1_THREADS + threadIdx.x;
     if (i >= d.n) continue;
-    const int row = __float_as_int(__ldg(&d.clusters[i]).w);
-    if (row < 0 || row >= d.n_rows) { bad = true; continue; }
+    const float4 c = __ldg(&d.clusters[i]);
+    const int row = __float_as_int(c.w);
+    if (row < 0 || row >= d.n_rows || !cluster_finite(c)) { bad = true; continue; }
     if (i < so.v[sec0 + 1]) atomicAdd(&s_cnt[row], 1);
     else atomicAdd(&d.slice_count[sector_of(so, d.n_sectors, i) * d.n_rows + row], 1);
   }
@@ -267,7 +273,7 @@ __global__ void __launch_bounds__(A1_THREADS) k_slice_scatter(Dev d, SecOff so) 
     d.hit_weight[i] = 0ull;
     c[k] = __ldg(&d.clusters[i]);
     const int row = __float_as_int(c[k].w);
-    if (row < 0 || row >= d.n_rows) { d.out_assign[i] = -1; continue; }
+    if (row < 0 || row >= d.n_rows || !cluster_finite(c[k])) { d.out_assign[i] = -1; continue; }
     rank[k] = (i < so.v[sec0 + 1]) ? atomicAdd(&s_cnt[row], 1) : -1;
   }
   __syncthreads();
@@ -338,8 +344,7 @@ __global__ void __launch_bounds__(A4_THREADS) k_slice_sort(Dev d) {
   {
     const float ymin = unordf(s_box[0]), ymax = unordf(s_box[1]), zmin = unordf(s_box[2]), zmax = unordf(s_box[3]);
     const float ye = fmaxf(ymax - ymin, 1e-3f), ze = fmaxf(zmax - zmin, 1e-3f);
-    int ny = (int)(ye / d.P.grid_bin_y) + 1;
-    ny = min(ny, 128);
+    int ny = (int)fminf(ye / d.P.grid_bin_y, 127.0f) + 1;  // clamped before the cast: a huge y extent cannot overflow
     const float want = (float)cnt * d.P.grid_bins_per_cluster / (float)ny;
     int nz = (int)want + 1;
     const int nz_cap = (int)fminf(ze / d.P.grid_bin_z_min, 1.0e6f) + 1;
@@ -403,12 +408,11 @@ __global__ void __launch_bounds__(A4_THREADS) k_slice_sort(Dev d) {
   }
 }
 
+cudaError_t setup_grid_kernels() {
+  return cudaFuncSetAttribute(k_slice_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, A4_SMEM_BINS * (int)sizeof(int));
+}
+
 void launch_grid(const Dev& d, const SecOff& so, Launch& L) {
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaFuncSetAttribute(k_slice_sort, cudaFuncAttributeMaxDynamicSharedMemorySize, A4_SMEM_BINS * (int)sizeof(int));
-    attr_set = true;
-  }
   k_reset<<<32, 256, 0, L.st>>>(d);
   L.count++;
   if (d.n > 0) {

@@ -289,11 +289,11 @@ void launch_clean_start(const Dev& d, Launch& L) {
   L.count++;
   if (d.n > 0 && d.max_tracklets > 0) {
     const int T = d.max_tracklets;
-    k_sb_zero<<<148 * 2, 256, 0, L.st>>>(d);
-    k_sb_count<<<148 * 8, 256, 0, L.st>>>(d);
+    k_sb_zero<<<d.n_sm * 2, 256, 0, L.st>>>(d);
+    k_sb_count<<<d.n_sm * 8, 256, 0, L.st>>>(d);
     L.count += 2;
     launch_scan_i32(d.sb_count, &d.cnt->n_start, T, d.scan_tmp, L);
-    k_sb_scatter<<<148 * 8, 256, 0, L.st>>>(d);
+    k_sb_scatter<<<d.n_sm * 8, 256, 0, L.st>>>(d);
     k_sb_rank<<<(T + 255) / 256, 256, 0, L.st>>>(d);
     L.count += 2;
   }

@@ -91,7 +91,7 @@ __global__ void __launch_bounds__(256) k_assign(Dev d) {
 void launch_select(const Dev& d, Launch& L) {
   if (d.n <= 0 || d.max_tracklets <= 0) return;
   const int T = d.max_tracklets;
-  k_select_own<<<148 * 16, SEL_THREADS, 0, L.st>>>(d);
+  k_select_own<<<d.n_sm * 16, SEL_THREADS, 0, L.st>>>(d);
   L.count++;
   launch_scan_i32(d.sel_scan, &d.cnt->n_start, T, d.scan_tmp, L);
   k_select_ids<<<(T + 255) / 256, 256, 0, L.st>>>(d);

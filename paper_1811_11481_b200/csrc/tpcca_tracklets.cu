@@ -565,13 +565,13 @@ void launch_tracklets(const Dev& d, Launch& L) {
   L.count++;
   launch_scan_i32(d.seed_w, &d.cnt->n_start, T, d.scan_tmp, L);
   k_seed_compact<<<(T + 255) / 256, 256, 0, L.st>>>(d);
-  k_tl_e1<<<148 * E1_BLOCKS, E_THREADS, 0, L.st>>>(d);
+  k_tl_e1<<<d.n_sm * E1_BLOCKS, E_THREADS, 0, L.st>>>(d);
   launch_order_desc(d, 1, d.e_key, &d.cnt->n_work, T, d.e_order, L);
-  k_tl_e2<<<148 * E2_GRID, E_THREADS, 0, L.st>>>(d);
+  k_tl_e2<<<d.n_sm * E2_GRID, E_THREADS, 0, L.st>>>(d);
   launch_order_desc(d, 2, d.e_key + T, &d.cnt->n_work, T, d.e_order + T, L);
-  k_tl_e3a<<<148 * E3_GRID, E_THREADS, 0, L.st>>>(d);
+  k_tl_e3a<<<d.n_sm * E3_GRID, E_THREADS, 0, L.st>>>(d);
   launch_order_desc(d, 3, d.e_key + 2 * (size_t)T, &d.cnt->n_work, T, d.e_order + 2 * (size_t)T, L);
-  k_tl_e3b<<<148 * E3B_BLOCKS, E_THREADS, 0, L.st>>>(d);
-  k_tracklet_weights<<<148 * W_GRID, 128, 0, L.st>>>(d);
+  k_tl_e3b<<<d.n_sm * E3B_BLOCKS, E_THREADS, 0, L.st>>>(d);
+  k_tracklet_weights<<<d.n_sm * W_GRID, 128, 0, L.st>>>(d);
   L.count += 6;
 }

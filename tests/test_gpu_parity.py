@@ -78,10 +78,62 @@ def test_edge_cases(row_x):
     fb = synth.Frame(bad, fr.sector_offsets, fr.truth, fr.track_par, 36, "bad")
     run_gpu(fb, row_x, t)
     assert t.header()["status"] & 4 and t.assignment()[5] == -1
+    # non-finite coordinates: ignored like a bad row (A21), the rest of the frame is tracked as if they were absent
+    nf = fr.clusters.copy()
+    nf["y"][7] = np.inf
+    nf["z"][11] = np.nan
+    nf["y"][13] = -np.inf
+    run_gpu(synth.Frame(nf, fr.sector_offsets, fr.truth, fr.track_par, 36, "nonfinite"), row_x, t)
+    assert t.header()["status"] & 4 and (t.assignment()[[7, 11, 13]] == -1).all()
+    a_nf = t.assignment()
+    keep = np.ones(fr.n, bool)
+    keep[[7, 11, 13]] = False
+    so2 = np.searchsorted(np.flatnonzero(keep), fr.sector_offsets).astype(np.int32)
+    t2, orc2, _ = compare(synth.Frame(fr.clusters[keep], so2, fr.truth[keep], fr.track_par, 36, "without"), row_x, tracker=t)
+    assert np.array_equal(a_nf[keep], orc2.assignment)
     # n > max_clusters is refused
     big = synth.generate(synth.config(2, scale=0.05, seed=3))
     with pytest.raises(B.TpccaError):
         run_gpu(big, row_x, t)
+
+
+def test_boundary_argument_checks(row_x):
+    """Every tpcca_get_intermediate id honours `bytes` (a short dst is refused, nothing is written), misaligned pointers
+    are refused by tpcca_track and tpcca_get_intermediate (include/tpcca.h)."""
+    import torch
+    fr = synth.generate(synth.config(2, scale=0.05, seed=3))
+    t = run_gpu(fr, row_x)
+    hd = t.header()
+    ns, nt = hd["n_start_hits"], hd["n_tracks"]
+    assert ns > 100 and nt > 50
+    need = {B.LINK_UP_RAW: fr.n * 4, B.LINK_DOWN: fr.n * 4, B.START_HITS: ns * 4, B.TRACKLET_ROW_HITS: ns * 152 * 4,
+            B.TRACKLET_INTS: ns * 16, B.TRACKLET_FLOATS: ns * 32, B.TRACK_TRACKLET: nt * 4}
+    st = t._stream()
+    for what, nb in need.items():
+        dst = torch.full((nb // 4 + 64,), 0x5A5A5A5A, dtype=torch.int32, device="cuda")
+        assert t.lib.tpcca_get_intermediate(t.h, what, dst.data_ptr(), nb - 4, st) == -1, what
+        assert b"too small" in t.lib.tpcca_last_error()
+        torch.cuda.synchronize()
+        assert bool((dst == 0x5A5A5A5A).all()), what
+        assert t.lib.tpcca_get_intermediate(t.h, what, dst.data_ptr(), nb, st) == 0, what
+        torch.cuda.synchronize()
+        assert bool((dst[nb // 4:] == 0x5A5A5A5A).all()) and not bool((dst[:nb // 4] == 0x5A5A5A5A).all()), what
+        assert t.lib.tpcca_get_intermediate(t.h, what, dst.data_ptr() + 4, nb, st) == -1  # misaligned dst
+    assert t.lib.tpcca_get_intermediate(t.h, 99, dst.data_ptr(), 1 << 20, st) == -1
+    dev = t.upload(fr.clusters)
+    so = np.ascontiguousarray(fr.sector_offsets, np.int32)
+    args = (fr.n, so.ctypes.data, st)
+    assert t.lib.tpcca_track(t.h, dev.data_ptr() + 4, *args, t.out_tracks.data_ptr(), t.out_assign.data_ptr()) == -1
+    assert b"misaligned" in t.lib.tpcca_last_error()
+    assert t.lib.tpcca_track(t.h, dev.data_ptr(), *args, t.out_tracks.data_ptr() + 8, t.out_assign.data_ptr()) == -1
+    assert t.lib.tpcca_track(t.h, dev.data_ptr(), *args, t.out_tracks.data_ptr(), t.out_assign.data_ptr() + 2) == -1
+    bad = so.copy()
+    bad[5] = bad[6] + 1  # not monotone
+    assert t.lib.tpcca_track(t.h, dev.data_ptr(), fr.n, bad.ctypes.data, st, t.out_tracks.data_ptr(), t.out_assign.data_ptr()) == -1
+    # the handle is still usable and the debug mode gives the same result
+    t.set_debug(True)
+    compare(fr, row_x, tracker=t)
+    t.set_debug(False)
 
 
 def test_capacity_overflow_is_flagged(row_x):
