@@ -6,7 +6,9 @@
 // centred on the hit; :121 fp32, z kept relative).  It follows the algorithm step by step in
 // the order of DESIGN.md section "Arithmetic" (steps O1-O7) and shares no code with the CUDA path.
 // Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
-// load it.  Build: g++ -O2 -ffp-contract=off (no fast-math): every decision is fp32, no FMA.
+// load it.  Build: g++ -O2 -ffp-contract=off (no fast-math): every decision is fp32; the compiler never contracts a
+// multiply-add on its own -- the fused operations are exactly the fma() calls DESIGN.md section 3 states (std::fma is
+// correctly rounded on every platform, with or without hardware support).
 //
 // Pins (tests/test_oracle_pins.py): brute-force all-triplet search (P1), noiseless helix (P2),
 // mutual links (P3), exclusive assignment (P4), permutation invariance (P5), transport closed
@@ -51,6 +53,8 @@ struct KF {
   float chi2;
 };
 
+inline float fma32(float a, float b, float c) { return std::fma(a, b, c); }  // one rounding: the "fma(a,b,c)" of DESIGN.md
+
 inline uint32_t ordf(float f) {  // monotone float -> uint map
   uint32_t b;
   std::memcpy(&b, &f, 4);
@@ -62,27 +66,28 @@ inline int tri(int i, int j) { return i >= j ? i * (i + 1) / 2 + j : j * (j + 1)
 // ---- O5 model: transport x -> xnew (DESIGN.md section 3 "Transport") ----
 // The step is written as the textbook extended-Kalman prediction: move the state along the helix, fill the dense
 // 5x5 Jacobian F = d(y, z~, s, t, q)' / d(y, z~, s, t, q), then C <- F C F^T by the two matrix products of the
-// definition.  DESIGN.md section 3 fixes the summation order: every entry is summed over k = 0..4 in increasing k,
-// and a term whose Jacobian entry is structurally zero (see `nz`) is left out rather than added as 0 * c.
+// definition.  DESIGN.md section 3 fixes the summation order: every entry starts from the unit-diagonal term and
+// accumulates the remaining terms in increasing k by fma(F_ik, C_kj, acc); a term whose Jacobian entry is structurally
+// zero (see `nz`) is left out rather than added as 0 * c.
 bool transport(KF& k, float xnew, float kq, float max_sinphi) {
   const float dx = xnew - k.x;
   if (dx == 0.0f) return true;  // identity (first step of E3 and of every refit pass)
   const float s0 = k.p[2], tl = k.p[3];
   const float curv = k.p[4] * kq;  // d sin(phi) / dx
-  const float s1 = s0 + dx * curv;
+  const float s1 = fma32(dx, curv, s0);
   if (!(std::fabs(s0) <= max_sinphi)) return false;
   if (!(std::fabs(s1) <= max_sinphi)) return false;
   // helix step: chord direction f = tan of the mean angle, chord length L (signed like dx), arc = L * asin(u)/u
-  const float cos0 = std::sqrt(1.0f - s0 * s0);
-  const float cos1 = std::sqrt(1.0f - s1 * s1);
+  const float cos0 = std::sqrt(fma32(-s0, s0, 1.0f));
+  const float cos1 = std::sqrt(fma32(-s1, s1, 1.0f));
   const float csum = cos0 + cos1;
   const float f = (s0 + s1) / csum;
   const float dy = dx * f;
-  float L = std::sqrt(dx * dx + dy * dy);
+  float L = std::sqrt(fma32(dx, dx, dy * dy));
   if (dx < 0.0f) L = -L;
   const float u = (0.5f * curv) * L;
   const float u2 = u * u;
-  const float g = 1.0f + u2 * (0.16666667f + u2 * 0.075f);  // asin(u)/u = 1 + u^2/6 + 3u^4/40 + ...
+  const float g = fma32(u2, fma32(u2, 0.075f, 0.16666667f), 1.0f);  // asin(u)/u = 1 + u^2/6 + 3u^4/40 + ...
   const float arc = L * g;
   // Jacobian (d g neglected): d f / d s0 and d f / d s1, then the chain rule through s1 = s0 + dx * kq * q
   const float df_ds0 = (1.0f + (f * s0) / cos0) / csum;
@@ -102,7 +107,7 @@ bool transport(KF& k, float xnew, float kq, float max_sinphi) {
   F[2][4] = ds1_dq;                   nz[2][4] = true;
   // state
   k.p[0] = k.p[0] + dy;
-  k.p[1] = k.p[1] + tl * arc;
+  k.p[1] = fma32(tl, arc, k.p[1]);
   k.p[2] = s1;
   k.x = xnew;
   // covariance: full symmetric C, M = F C, C' = M F^T (lower triangle kept)
@@ -115,8 +120,7 @@ bool transport(KF& k, float xnew, float kq, float max_sinphi) {
       bool first = true;
       for (int l = 0; l < 5; l++) {
         if (!nz[i][l]) continue;
-        const float term = (l == i) ? Cf[l][j] : F[i][l] * Cf[l][j];  // F_ii = 1
-        acc = first ? term : acc + term;
+        acc = first ? Cf[l][j] : fma32(F[i][l], Cf[l][j], acc);  // first non-zero of row i is F_ii = 1
         first = false;
       }
       M[i][j] = acc;
@@ -127,8 +131,7 @@ bool transport(KF& k, float xnew, float kq, float max_sinphi) {
       bool first = true;
       for (int l = 0; l < 5; l++) {
         if (!nz[j][l]) continue;
-        const float term = (l == j) ? M[i][l] : F[j][l] * M[i][l];
-        acc = first ? term : acc + term;
+        acc = first ? M[i][l] : fma32(F[j][l], M[i][l], acc);
         first = false;
       }
       k.C[tri(i, j)] = acc;
@@ -145,10 +148,10 @@ void update1(KF& k, int i, float m, float v) {
   const float w = 1.0f / S;
   float K[5];
   for (int j = 0; j < 5; j++) K[j] = ci[j] * w;
-  for (int j = 0; j < 5; j++) k.p[j] = k.p[j] + K[j] * r;
+  for (int j = 0; j < 5; j++) k.p[j] = fma32(K[j], r, k.p[j]);
   for (int j = 0; j < 5; j++)
-    for (int l = 0; l <= j; l++) k.C[tri(j, l)] = k.C[tri(j, l)] - K[j] * ci[l];
-  k.chi2 = k.chi2 + (r * r) * w;
+    for (int l = 0; l <= j; l++) k.C[tri(j, l)] = fma32(-K[j], ci[l], k.C[tri(j, l)]);
+  k.chi2 = fma32(r * r, w, k.chi2);
 }
 
 void update(KF& k, float ym, float zm_rel, float sy2, float sz2) {
@@ -228,10 +231,10 @@ void find_neighbours(const Ctx& c, const Sector& S, std::vector<int32_t>& up, st
     const float dxu = c.row_x[ru] - c.row_x[r];
     const float dxd = c.row_x[r] - c.row_x[rd];
     const float t = dxd / (dxu + dxd);
-    const float wyu = dxu * P.nbr_dydx + P.nbr_margin_y;
-    const float wzu = dxu * P.nbr_dzdx + P.nbr_margin_z;
-    const float wyd = dxd * P.nbr_dydx + P.nbr_margin_y;
-    const float wzd = dxd * P.nbr_dzdx + P.nbr_margin_z;
+    const float wyu = fma32(dxu, P.nbr_dydx, P.nbr_margin_y);
+    const float wzu = fma32(dxu, P.nbr_dzdx, P.nbr_margin_z);
+    const float wyd = fma32(dxd, P.nbr_dydx, P.nbr_margin_y);
+    const float wzd = fma32(dxd, P.nbr_dzdx, P.nbr_margin_z);
     for (int32_t h : S.rows[r]) {
       const float y0 = cl[h].y, z0 = cl[h].z;
       U.clear(); D.clear();
@@ -251,9 +254,9 @@ void find_neighbours(const Ctx& c, const Sector& S, std::vector<int32_t>& up, st
       for (int32_t u : U)
         for (int32_t d : D) {
           const float yu = cl[u].y, zu = cl[u].z, yd = cl[d].y, zd = cl[d].z;
-          const float ey = y0 - (yd + t * (yu - yd));
-          const float ez = z0 - (zd + t * (zu - zd));
-          const float cost = (ey * ey) * c.inv_sy2 + (ez * ez) * c.inv_sz2;
+          const float ey = y0 - fma32(t, yu - yd, yd);
+          const float ez = z0 - fma32(t, zu - zd, zd);
+          const float cost = fma32(ez * ez, c.inv_sz2, (ey * ey) * c.inv_sy2);
           if (!(cost <= P.triplet_cut)) continue;
           bool better;
           if (bu < 0) better = true;
@@ -286,7 +289,7 @@ int32_t search_row(const Ctx& c, const std::vector<int32_t>& row, const KF& k, f
     const float dy = cl[h].y - k.p[0];
     const float dz = (cl[h].z - z_ref) - k.p[1];
     if (!(std::fabs(dy) <= wy) || !(std::fabs(dz) <= wz)) continue;
-    const float d = (dy * dy) * iy + (dz * dz) * iz;
+    const float d = fma32(dz * dz, iz, (dy * dy) * iy);
     if (!(d <= cut)) continue;
     bool better;
     if (best < 0) better = true;
@@ -301,7 +304,7 @@ inline float hit_dist(const Ctx& c, const KF& k, const Cl& h, float z_ref) {
   const float iy = 1.0f / (k.C[0] + c.sy2), iz = 1.0f / (k.C[2] + c.sz2);
   const float dy = h.y - k.p[0];
   const float dz = (h.z - z_ref) - k.p[1];
-  return (dy * dy) * iy + (dz * dz) * iz;
+  return fma32(dz * dz, iz, (dy * dy) * iy);
 }
 
 // ---- O5 tracklet construction for one start hit ----
@@ -320,7 +323,7 @@ void build_tracklet(const Ctx& c, const Sector& S, const std::vector<int32_t>& l
   KF k;
   {
     const float dx = cl[h1].x - cl[h0].x, dy = cl[h1].y - cl[h0].y, dz = cl[h1].z - cl[h0].z;
-    const float ds = std::sqrt(dx * dx + dy * dy);
+    const float ds = std::sqrt(fma32(dx, dx, dy * dy));
     k.x = cl[h0].x;
     k.p[0] = cl[h0].y; k.p[1] = 0.0f; k.p[2] = dy / ds; k.p[3] = dz / ds; k.p[4] = 0.0f;
     reset_cov(k, P);
@@ -342,7 +345,7 @@ void build_tracklet(const Ctx& c, const Sector& S, const std::vector<int32_t>& l
   int top_row = last_row, gap = 0;
   for (int r = last_row + 1; r < R; r++) {
     if (!transport(k, c.row_x[r], c.kq, P.max_sinphi)) break;
-    if (std::fabs(k.p[0]) > c.row_x[r] * P.tan_half_angle + P.edge_margin) break;
+    if (std::fabs(k.p[0]) > fma32(c.row_x[r], P.tan_half_angle, P.edge_margin)) break;
     const int32_t hb = search_row(c, S.rows[r], k, z_ref, P.pick_cut);
     if (hb >= 0) {
       update(k, cl[hb].y, cl[hb].z - z_ref, c.sy2, c.sz2);
@@ -361,7 +364,7 @@ void build_tracklet(const Ctx& c, const Sector& S, const std::vector<int32_t>& l
   int r = top_row;
   for (; r >= 0; r--) {
     if (!transport(k, c.row_x[r], c.kq, P.max_sinphi)) break;
-    if (std::fabs(k.p[0]) > c.row_x[r] * P.tan_half_angle + P.edge_margin) break;
+    if (std::fabs(k.p[0]) > fma32(c.row_x[r], P.tan_half_angle, P.edge_margin)) break;
     bool hit = false;
     if (row_hit[r] >= 0) {
       const Cl& hc = cl[row_hit[r]];
@@ -405,7 +408,7 @@ bool refit(const Ctx& c, const std::vector<int32_t>& hits, float q0, KF& k, floa
   const Cl& hM = cl[hits[n - 2]];
   z_ref = hN.z;
   const float dx = hN.x - hM.x, dy = hN.y - hM.y, dz = hN.z - hM.z;
-  const float ds = std::sqrt(dx * dx + dy * dy);
+  const float ds = std::sqrt(fma32(dx, dx, dy * dy));
   k.x = hN.x;
   k.p[0] = hN.y; k.p[1] = 0.0f; k.p[2] = dy / ds; k.p[3] = dz / ds; k.p[4] = q0;
   for (int pass = 0; pass < 3; pass++) {

@@ -46,6 +46,9 @@ def _brute_links_py(cl, rx, P):
     def key(i):
         return (float(cl["z"][i]), float(cl["y"][i]), int(i))
 
+    def fma(a, b, c):  # the fused multiply-add of DESIGN.md section 3: float32 x float32 is exact in float64
+        return f(np.float64(a) * np.float64(b) + np.float64(c))
+
     for r in range(R):
         ru = r + 1 if r + 1 < R and len(occupied[r + 1]) else (r + 2 if r + 2 < R and len(occupied[r + 2]) else -1)
         rd = r - 1 if r - 1 >= 0 and len(occupied[r - 1]) else (r - 2 if r - 2 >= 0 and len(occupied[r - 2]) else -1)
@@ -53,8 +56,8 @@ def _brute_links_py(cl, rx, P):
             continue
         dxu, dxd = f(rx[ru]) - f(rx[r]), f(rx[r]) - f(rx[rd])
         t = dxd / (dxu + dxd)
-        wyu, wzu = dxu * f(P["nbr_dydx"]) + f(P["nbr_margin_y"]), dxu * f(P["nbr_dzdx"]) + f(P["nbr_margin_z"])
-        wyd, wzd = dxd * f(P["nbr_dydx"]) + f(P["nbr_margin_y"]), dxd * f(P["nbr_dzdx"]) + f(P["nbr_margin_z"])
+        wyu, wzu = fma(dxu, f(P["nbr_dydx"]), f(P["nbr_margin_y"])), fma(dxu, f(P["nbr_dzdx"]), f(P["nbr_margin_z"]))
+        wyd, wzd = fma(dxd, f(P["nbr_dydx"]), f(P["nbr_margin_y"])), fma(dxd, f(P["nbr_dzdx"]), f(P["nbr_margin_z"]))
         for h in occupied[r]:
             y0, z0 = cl["y"][h], cl["z"][h]
             best = None
@@ -66,9 +69,9 @@ def _brute_links_py(cl, rx, P):
                     yd, zd = cl["y"][d], cl["z"][d]
                     if not (abs(yd - y0) <= wyd and abs(zd - z0) <= wzd):
                         continue
-                    ey = y0 - (yd + t * (yu - yd))
-                    ez = z0 - (zd + t * (zu - zd))
-                    cost = (ey * ey) * inv_sy2 + (ez * ez) * inv_sz2
+                    ey = y0 - fma(t, yu - yd, yd)
+                    ez = z0 - fma(t, zu - zd, zd)
+                    cost = fma(ez * ez, inv_sz2, (ey * ey) * inv_sy2)
                     if not cost <= f(P["triplet_cut"]):
                         continue
                     cand = (float(cost), key(u), key(d), u, d)
