@@ -137,23 +137,25 @@ __device__ __forceinline__ void kf_reset_cov(KF& k, const float* cov0) {
 }
 
 // Transport x -> xnew.  false: |sin(phi)| would exceed max_sinphi (state unchanged).
+// DESIGN.md section 3 "Transport": every fmaf below is a fused operation the section states (nothing else fuses:
+// the translation units are compiled with -fmad=false).  C <- F C F^T is the 51-fma expansion of M = F C, C' = M F^T.
 __device__ __forceinline__ bool kf_transport(KF& k, float xnew, float kq, float max_sinphi) {
   const float dx = xnew - k.x;
   if (dx == 0.0f) return true;
-  const float s = k.s, t = k.t, q = k.q;
-  const float kk = q * kq;
-  const float s1 = s + dx * kk;
+  const float s = k.s, t = k.t;
+  const float kk = k.q * kq;
+  const float s1 = fmaf(dx, kk, s);
   if (!(fabsf(s) <= max_sinphi) || !(fabsf(s1) <= max_sinphi)) return false;
-  const float c0 = sqrtf(1.0f - s * s);
-  const float c1 = sqrtf(1.0f - s1 * s1);
+  const float c0 = sqrtf(fmaf(-s, s, 1.0f));
+  const float c1 = sqrtf(fmaf(-s1, s1, 1.0f));
   const float cc = c0 + c1;
   const float f = (s + s1) / cc;
   const float dy = dx * f;
-  float L = sqrtf(dx * dx + dy * dy);
+  float L = sqrtf(fmaf(dx, dx, dy * dy));
   if (dx < 0.0f) L = -L;
   const float u = (0.5f * kk) * L;
   const float u2 = u * u;
-  const float g = 1.0f + u2 * (0.16666667f + u2 * 0.075f);
+  const float g = fmaf(u2, fmaf(u2, 0.075f, 0.16666667f), 1.0f);
   const float dS = L * g;
   const float fs0 = (1.0f + (f * s) / c0) / cc;
   const float fs1 = (1.0f + (f * s1) / c1) / cc;
@@ -167,71 +169,60 @@ __device__ __forceinline__ bool kf_transport(KF& k, float xnew, float kq, float 
   const float a14 = (w * fs1) * h;
   const float a24 = h;
   k.y = k.y + dy;
-  k.z = k.z + t * dS;
+  k.z = fmaf(t, dS, k.z);
   k.s = s1;
   k.x = xnew;
   const float c00 = k.c00, c10 = k.c10, c11 = k.c11, c20 = k.c20, c21 = k.c21, c22 = k.c22, c30 = k.c30,
               c31 = k.c31, c32 = k.c32, c33 = k.c33, c40 = k.c40, c41 = k.c41, c42 = k.c42, c43 = k.c43, c44 = k.c44;
-  const float m00 = (c00 + a02 * c20) + a04 * c40;
-  const float m02 = (c20 + a02 * c22) + a04 * c42;
-  const float m04 = (c40 + a02 * c42) + a04 * c44;
-  const float m10 = ((c10 + a12 * c20) + a13 * c30) + a14 * c40;
-  const float m11 = ((c11 + a12 * c21) + a13 * c31) + a14 * c41;
-  const float m12 = ((c21 + a12 * c22) + a13 * c32) + a14 * c42;
-  const float m13 = ((c31 + a12 * c32) + a13 * c33) + a14 * c43;
-  const float m14 = ((c41 + a12 * c42) + a13 * c43) + a14 * c44;
-  const float m20 = c20 + a24 * c40;
-  const float m21 = c21 + a24 * c41;
-  const float m22 = c22 + a24 * c42;
-  const float m23 = c32 + a24 * c43;
-  const float m24 = c42 + a24 * c44;
-  k.c00 = (m00 + a02 * m02) + a04 * m04;
-  k.c10 = (m10 + a02 * m12) + a04 * m14;
-  k.c11 = ((m11 + a12 * m12) + a13 * m13) + a14 * m14;
-  k.c20 = (m20 + a02 * m22) + a04 * m24;
-  k.c21 = ((m21 + a12 * m22) + a13 * m23) + a14 * m24;
-  k.c22 = m22 + a24 * m24;
-  k.c30 = (c30 + a02 * c32) + a04 * c43;
-  k.c31 = ((c31 + a12 * c32) + a13 * c33) + a14 * c43;
-  k.c32 = c32 + a24 * c43;
-  k.c40 = (c40 + a02 * c42) + a04 * c44;
-  k.c41 = ((c41 + a12 * c42) + a13 * c43) + a14 * c44;
-  k.c42 = c42 + a24 * c44;
+  // M = F C  (rows 3 and 4 of F are unit rows: M_3j = C_3j, M_4j = C_4j)
+  const float m00 = fmaf(a04, c40, fmaf(a02, c20, c00));
+  const float m02 = fmaf(a04, c42, fmaf(a02, c22, c20));
+  const float m04 = fmaf(a04, c44, fmaf(a02, c42, c40));
+  const float m10 = fmaf(a14, c40, fmaf(a13, c30, fmaf(a12, c20, c10)));
+  const float m11 = fmaf(a14, c41, fmaf(a13, c31, fmaf(a12, c21, c11)));
+  const float m12 = fmaf(a14, c42, fmaf(a13, c32, fmaf(a12, c22, c21)));
+  const float m13 = fmaf(a14, c43, fmaf(a13, c33, fmaf(a12, c32, c31)));
+  const float m14 = fmaf(a14, c44, fmaf(a13, c43, fmaf(a12, c42, c41)));
+  const float m20 = fmaf(a24, c40, c20);
+  const float m21 = fmaf(a24, c41, c21);
+  const float m22 = fmaf(a24, c42, c22);
+  const float m23 = fmaf(a24, c43, c32);
+  const float m24 = fmaf(a24, c44, c42);
+  // C' = M F^T, lower triangle
+  k.c00 = fmaf(a04, m04, fmaf(a02, m02, m00));
+  k.c10 = fmaf(a04, m14, fmaf(a02, m12, m10));
+  k.c11 = fmaf(a14, m14, fmaf(a13, m13, fmaf(a12, m12, m11)));
+  k.c20 = fmaf(a04, m24, fmaf(a02, m22, m20));
+  k.c21 = fmaf(a14, m24, fmaf(a13, m23, fmaf(a12, m22, m21)));
+  k.c22 = fmaf(a24, m24, m22);
+  k.c30 = fmaf(a04, c43, fmaf(a02, c32, c30));
+  k.c31 = fmaf(a14, c43, fmaf(a13, c33, fmaf(a12, c32, c31)));
+  k.c32 = fmaf(a24, c43, c32);
+  k.c40 = fmaf(a04, c44, fmaf(a02, c42, c40));
+  k.c41 = fmaf(a14, c44, fmaf(a13, c43, fmaf(a12, c42, c41)));
+  k.c42 = fmaf(a24, c44, c42);
   return true;
 }
 
-// Sequential scalar updates, y then z~ (DESIGN.md "Update").
+// One scalar measurement update of component with pre-update column (i0..i4), state value xi, variance v
+// (x_j <- fma(K_j, r, x_j), C_jl <- fma(-K_j, ci_l, C_jl), chi2 <- fma(r*r, w, chi2)).
+__device__ __forceinline__ void kf_update1(KF& k, float i0, float i1, float i2, float i3, float i4, float r, float S) {
+  const float w = 1.0f / S;
+  const float K0 = i0 * w, K1 = i1 * w, K2 = i2 * w, K3 = i3 * w, K4 = i4 * w;
+  k.y = fmaf(K0, r, k.y); k.z = fmaf(K1, r, k.z); k.s = fmaf(K2, r, k.s); k.t = fmaf(K3, r, k.t); k.q = fmaf(K4, r, k.q);
+  k.c00 = fmaf(-K0, i0, k.c00);
+  k.c10 = fmaf(-K1, i0, k.c10); k.c11 = fmaf(-K1, i1, k.c11);
+  k.c20 = fmaf(-K2, i0, k.c20); k.c21 = fmaf(-K2, i1, k.c21); k.c22 = fmaf(-K2, i2, k.c22);
+  k.c30 = fmaf(-K3, i0, k.c30); k.c31 = fmaf(-K3, i1, k.c31); k.c32 = fmaf(-K3, i2, k.c32); k.c33 = fmaf(-K3, i3, k.c33);
+  k.c40 = fmaf(-K4, i0, k.c40); k.c41 = fmaf(-K4, i1, k.c41); k.c42 = fmaf(-K4, i2, k.c42); k.c43 = fmaf(-K4, i3, k.c43);
+  k.c44 = fmaf(-K4, i4, k.c44);
+  k.chi2 = fmaf(r * r, w, k.chi2);
+}
+
+// Sequential scalar updates, y then z~.
 __device__ __forceinline__ void kf_update(KF& k, float ym, float zm, float sy2, float sz2) {
-  {  // component 0 (y): column (c00, c10, c20, c30, c40)
-    const float i0 = k.c00, i1 = k.c10, i2 = k.c20, i3 = k.c30, i4 = k.c40;
-    const float r = ym - k.y;
-    const float S = i0 + sy2;
-    const float w = 1.0f / S;
-    const float K0 = i0 * w, K1 = i1 * w, K2 = i2 * w, K3 = i3 * w, K4 = i4 * w;
-    k.y = k.y + K0 * r; k.z = k.z + K1 * r; k.s = k.s + K2 * r; k.t = k.t + K3 * r; k.q = k.q + K4 * r;
-    k.c00 = k.c00 - K0 * i0;
-    k.c10 = k.c10 - K1 * i0; k.c11 = k.c11 - K1 * i1;
-    k.c20 = k.c20 - K2 * i0; k.c21 = k.c21 - K2 * i1; k.c22 = k.c22 - K2 * i2;
-    k.c30 = k.c30 - K3 * i0; k.c31 = k.c31 - K3 * i1; k.c32 = k.c32 - K3 * i2; k.c33 = k.c33 - K3 * i3;
-    k.c40 = k.c40 - K4 * i0; k.c41 = k.c41 - K4 * i1; k.c42 = k.c42 - K4 * i2; k.c43 = k.c43 - K4 * i3;
-    k.c44 = k.c44 - K4 * i4;
-    k.chi2 = k.chi2 + (r * r) * w;
-  }
-  {  // component 1 (z~): column (c10, c11, c21, c31, c41)
-    const float i0 = k.c10, i1 = k.c11, i2 = k.c21, i3 = k.c31, i4 = k.c41;
-    const float r = zm - k.z;
-    const float S = i1 + sz2;
-    const float w = 1.0f / S;
-    const float K0 = i0 * w, K1 = i1 * w, K2 = i2 * w, K3 = i3 * w, K4 = i4 * w;
-    k.y = k.y + K0 * r; k.z = k.z + K1 * r; k.s = k.s + K2 * r; k.t = k.t + K3 * r; k.q = k.q + K4 * r;
-    k.c00 = k.c00 - K0 * i0;
-    k.c10 = k.c10 - K1 * i0; k.c11 = k.c11 - K1 * i1;
-    k.c20 = k.c20 - K2 * i0; k.c21 = k.c21 - K2 * i1; k.c22 = k.c22 - K2 * i2;
-    k.c30 = k.c30 - K3 * i0; k.c31 = k.c31 - K3 * i1; k.c32 = k.c32 - K3 * i2; k.c33 = k.c33 - K3 * i3;
-    k.c40 = k.c40 - K4 * i0; k.c41 = k.c41 - K4 * i1; k.c42 = k.c42 - K4 * i2; k.c43 = k.c43 - K4 * i3;
-    k.c44 = k.c44 - K4 * i4;
-    k.chi2 = k.chi2 + (r * r) * w;
-  }
+  kf_update1(k, k.c00, k.c10, k.c20, k.c30, k.c40, ym - k.y, k.c00 + sy2);  // component 0: column (c00, c10, c20, c30, c40)
+  kf_update1(k, k.c10, k.c11, k.c21, k.c31, k.c41, zm - k.z, k.c11 + sz2);  // component 1: column (c10, c11, c21, c31, c41)
 }
 
 // same-row key order (ord z, ord y, input index): true if a < b

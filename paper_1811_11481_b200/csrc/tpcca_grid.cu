@@ -240,10 +240,10 @@ __global__ void __launch_bounds__(1024) k_slice_offsets(Dev d) {
         const float dxd = xr - d.row_x[rd];
         nb.su = sec * d.n_rows + ru; nb.sd = sec * d.n_rows + rd;
         nb.t = dxd / (dxu + dxd);
-        nb.wyu = dxu * d.P.nbr_dydx + d.P.nbr_margin_y;
-        nb.wzu = dxu * d.P.nbr_dzdx + d.P.nbr_margin_z;
-        nb.wyd = dxd * d.P.nbr_dydx + d.P.nbr_margin_y;
-        nb.wzd = dxd * d.P.nbr_dzdx + d.P.nbr_margin_z;
+        nb.wyu = fmaf(dxu, d.P.nbr_dydx, d.P.nbr_margin_y);
+        nb.wzu = fmaf(dxu, d.P.nbr_dzdx, d.P.nbr_margin_z);
+        nb.wyd = fmaf(dxd, d.P.nbr_dydx, d.P.nbr_margin_y);
+        nb.wzd = fmaf(dxd, d.P.nbr_dzdx, d.P.nbr_margin_z);
       }
       d.nbr[sl] = nb;
     }

@@ -103,9 +103,9 @@ __device__ __forceinline__ void nested_pairs(const Dev& d, const NbrHdr& nb, con
         for (int dd = db; dd < de; dd++) {
           const float2 pd = d.yz[dd];
           if (!(fabsf(pd.x - y0) <= nb.wyd) || !(fabsf(pd.y - z0) <= nb.wzd)) continue;
-          const float ey = y0 - (pd.x + t * (pu.x - pd.x));
-          const float ez = z0 - (pd.y + t * (pu.y - pd.y));
-          const float cost = (ey * ey) * d.inv_sy2 + (ez * ez) * d.inv_sz2;
+          const float ey = y0 - fmaf(t, pu.x - pd.x, pd.x);
+          const float ez = z0 - fmaf(t, pu.y - pd.y, pd.y);
+          const float cost = fmaf(ez * ez, d.inv_sz2, (ey * ey) * d.inv_sy2);
           consider(d, best, cost, u, pu.x, pu.y, dd, pd.x, pd.y);
         }
       }
@@ -144,9 +144,9 @@ __global__ void __launch_bounds__(NB_THREADS) k_neighbours(Dev d) {
         int u = liu[0];
         for (int q = 0; q < np; q++) {
           const float2 pd = lpd[jd * NB_THREADS];
-          const float ey = y0 - (pd.x + t * (pu.x - pd.x));
-          const float ez = z0 - (pd.y + t * (pu.y - pd.y));
-          const float cost = (ey * ey) * d.inv_sy2 + (ez * ez) * d.inv_sz2;
+          const float ey = y0 - fmaf(t, pu.x - pd.x, pd.x);
+          const float ez = z0 - fmaf(t, pu.y - pd.y, pd.y);
+          const float cost = fmaf(ez * ez, d.inv_sz2, (ey * ey) * d.inv_sy2);
           consider(d, best, cost, u, pu.x, pu.y, lid[jd * NB_THREADS], pd.x, pd.y);
           if (++jd == nd) {
             jd = 0;

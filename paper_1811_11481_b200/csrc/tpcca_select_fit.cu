@@ -121,7 +121,7 @@ __global__ void __launch_bounds__(64) k_refit(Dev d) {
   KF k;
   {
     const float dx = d.row_x[rN] - d.row_x[rM], dy = pN.x - pM.x, dz = pN.y - pM.y;
-    const float ds = sqrtf(dx * dx + dy * dy);
+    const float ds = sqrtf(fmaf(dx, dx, dy * dy));
     k.x = d.row_x[rN];
     k.y = pN.x; k.z = 0.0f; k.s = dy / ds; k.t = dz / ds; k.q = q0;
   }

@@ -148,7 +148,7 @@ __device__ __forceinline__ int search_row(const Dev& d, const GridHdr& g, const 
       for (int j = 0; j < SEARCH_UNROLL; j++) {
         const float dy = p[j].x - k.y;
         const float dz = (p[j].y - z_ref) - k.z;
-        const float dist = (dy * dy) * iy + (dz * dz) * iz;
+        const float dist = fmaf(dz * dz, iz, (dy * dy) * iy);
         if ((fabsf(dy) <= wy) && (fabsf(dz) <= wz) && (dist <= cut) && c[j] != best) {
           bool better = (best < 0) || (dist < bd);
           if (!better && dist == bd) better = tie_less(d, c[j], p[j], best);
@@ -206,7 +206,7 @@ __global__ void __launch_bounds__(E_THREADS, E1_BOUNDS) k_tl_e1(Dev d) {
           r = (h >= d.row_start[sbase + r0 + 2]) ? r0 + 2 : r0 + 1;
           const float2 p1 = d.yz[h];
           const float dx = d.row_x[r] - d.row_x[r0], dy = p1.x - p0.x, dz = p1.y - p0.y;
-          const float ds = sqrtf(dx * dx + dy * dy);
+          const float ds = sqrtf(fmaf(dx, dx, dy * dy));
           k.x = d.row_x[r0];
           k.y = p0.x; k.z = 0.0f; k.s = dy / ds; k.t = dz / ds; k.q = 0.0f;
           kf_reset_cov(k, d.P.cov0);
@@ -296,7 +296,7 @@ __global__ void __launch_bounds__(E_THREADS, E2_BLOCKS) k_tl_e2(Dev d) {
     const GridHdr g = d.grid[sbase + r];
     if (r + 1 < R) prefetch_l1(&d.grid[sbase + r + 1]);
     const float xr = d.row_x[r];
-    if (!kf_transport(k, xr, d.kq, d.P.max_sinphi) || fabsf(k.y) > xr * d.tan_half_angle + d.P.edge_margin) {
+    if (!kf_transport(k, xr, d.kq, d.P.max_sinphi) || fabsf(k.y) > fmaf(xr, d.tan_half_angle, d.P.edge_margin)) {
       busy = false;
       continue;
     }
@@ -402,7 +402,7 @@ __global__ void __launch_bounds__(E_THREADS, E3_BLOCKS) k_tl_e3a(Dev d) {
     float2 pb = make_float2(0.f, 0.f);
     if (cur >= 0) pb = d.yz[cur];
     const float xr = d.row_x[r];
-    if (!kf_transport(k, xr, d.kq, d.P.max_sinphi) || fabsf(k.y) > xr * d.tan_half_angle + d.P.edge_margin) {
+    if (!kf_transport(k, xr, d.kq, d.P.max_sinphi) || fabsf(k.y) > fmaf(xr, d.tan_half_angle, d.P.edge_margin)) {
       busy = false; stopped = true;
       continue;
     }
@@ -411,7 +411,7 @@ __global__ void __launch_bounds__(E_THREADS, E3_BLOCKS) k_tl_e3a(Dev d) {
       const float iy = 1.0f / (k.c00 + d.sy2), iz = 1.0f / (k.c11 + d.sz2);
       const float dy = pb.x - k.y;
       const float dz = (pb.y - z_ref) - k.z;
-      const float dist = (dy * dy) * iy + (dz * dz) * iz;
+      const float dist = fmaf(dz * dz, iz, (dy * dy) * iy);
       cand = (dist <= d.P.reject_cut) ? cur : -1;
     } else {  // gap row inside the range (rare): pick-up search
       n_search++;
@@ -504,7 +504,7 @@ __global__ void __launch_bounds__(E_THREADS, E3B_BLOCKS) k_tl_e3b(Dev d) {
     const GridHdr g = d.grid[sbase + r];
     if (r > 0) prefetch_l1(&d.grid[sbase + r - 1]);
     const float xr = d.row_x[r];
-    if (!kf_transport(k, xr, d.kq, d.P.max_sinphi) || fabsf(k.y) > xr * d.tan_half_angle + d.P.edge_margin) {
+    if (!kf_transport(k, xr, d.kq, d.P.max_sinphi) || fabsf(k.y) > fmaf(xr, d.tan_half_angle, d.P.edge_margin)) {
       busy = false;
       continue;
     }
