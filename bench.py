@@ -2,9 +2,13 @@
 """bench.py -- TPC clusters/s tracked (CA find + KF fit) on seeded synthetic time frames.
 
 One "step" = one pass of the whole hot path (a)-(g) over one time frame (BASELINE.json config 5:
-50 overlapped collisions, 1 ms frame).  `value` is device-resident throughput, `e2e` goes through
-tpcca_track_host with pinned host buffers (H2D + D2H inside the timed region).
-"Measurement".  `--impl reference` times the CPU oracle (the only reference this tier has).
+50 overlapped collisions, 1 ms frame).  `value` is device-resident throughput, `e2e` goes through the
+library's pipelined host call (tpcca_track_host_async / tpcca_wait: pinned host buffers, H2D + D2H inside
+the timed region, two frames in flight in ONE workspace).  `--gpus N` starts N ranks itself (torchrun
+re-exec) unless it already runs under torchrun; `--shard frames` (default, weak scaling: one frame per
+rank) or `--shard sectors` (one frame split into contiguous sector ranges, strong
+scaling).  `--config k` times another BASELINE.json config (parity-test cases; the bench line is config 5).
+See DESIGN.md "Measurement".  `--impl reference` times the CPU oracle (the only reference this tier has).
 """
 from __future__ import annotations
 
@@ -29,13 +33,13 @@ FALLBACK_HBM_GBS = 6650.0  # /opt/skills/guides/B200_PROFILING.md fallback
 BYTES_PER_CLUSTER_NEIGHBOURS = 24.0      # 8 own yz + 8 links out + ~8 bin_start/neighbour share
 BYTES_PER_ROW_STEP_TRACKLETS = 22.0      # 8 bin range + ~1.2*8 candidates + 4 row_hit
 BYTES_PER_TRACKLET = 112.0               # record
-BYTES_PER_TRACKLET_HIT = 8.0             # weight atomic
-FP32_OPS_PER_ROW_STEP = 270.0            # transport 48 + covariance 102 + update 102 + search ~18
+BYTES_PER_TRACKLET_HIT = 8.0             # weight atomic (every hit of every valid tracklet)
+FP32_OPS_PER_ROW_STEP = 161.0            # DESIGN.md section 3 with the stated fma: transport 38 + covariance 51 + update 54 + search ~18
 
 
 def ncu_traffic(stage: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the stage's kernels, from the committed ncu
-    --set full summary of this round (profiles/traffic.json.txt), or None."""
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of a kernel (or of a stage's kernels), from the committed
+    ncu --set full summary of this round (profiles/traffic.json.txt), or None."""
     p = os.path.join(ROOT, "profiles", "traffic.json.txt")
     try:
         return float(json.load(open(p))[stage])
@@ -119,12 +123,12 @@ class ClockSampler:
                 "source": "nvml" if self._nvml is not None else "nvidia-smi"}
 
 
-def oracle_timed(scale: float, seed: int, steps: int, warmup: int, fr=None):
-    """The CPU oracle as it stands on `fr`, or on a bounded sample of the workload (config 5 at `scale` collisions)."""
+def oracle_timed(cfg: int, scale: float, seed: int, steps: int, warmup: int, fr=None):
+    """The CPU oracle as it stands on `fr`, or on a bounded sample of the workload (config `cfg` at `scale`)."""
     import oracle
     from paper_1811_11481_b200 import synth
     if fr is None:
-        fr = synth.generate(synth.config(5, scale=scale, seed=seed))
+        fr = synth.generate(synth.config(cfg, scale=scale, seed=seed))
     rx = synth.row_x()
     times, res = [], None
     for i in range(warmup + steps):
@@ -143,21 +147,40 @@ def quality(assignment, n_tracks, fr):
     return {k: (round(v, 5) if isinstance(v, float) else v) for k, v in q.items()}
 
 
+WORKLOADS = {1: "config1_single_sector_200_primaries", 2: "config2_central_event_4000_primaries",
+             3: "config3_low_pt_loopers", 4: "config4_5_collisions_100us", 5: "config5_timeframe_50_collisions"}
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    scale = 0.2
-    v, t, n, _ = oracle_timed(scale, 5, args.steps, args.warmup)
-    sample = f"config 5 at {int(round(50 * scale))} collisions in {1000 * scale:.0f} us (same occupancy), {n} clusters/step"
+    # bounded sample of the SAME workload: config 5 at 10 collisions in 200 us has the occupancy of the full frame
+    scale = 0.2 if args.config == 5 else (0.25 if args.config == 4 else 1.0)
+    v, t, n, _ = oracle_timed(args.config, scale, args.config, args.steps, args.warmup)
+    sample = (f"config {args.config} at scale {scale} "
+              + ("(10 collisions in 200 us: the occupancy of the full frame), " if args.config == 5 else "")
+              + f"{n} clusters/step")
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": "config5_timeframe_50_collisions (bounded sample)", "clusters_per_step": n},
+            "config": {"workload": WORKLOADS[args.config] + " (bounded sample)", "clusters_per_step": n},
             "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
             "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
     return 0
+
+
+def respawn_under_torchrun(args) -> int:
+    """`python bench.py --gpus N` with N > 1 outside torchrun: start the N ranks (one process per GPU)."""
+    import socket
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
 
 
 def run_gpu(args):
@@ -168,18 +191,33 @@ def run_gpu(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the tpcca path has no CPU fallback")
+    if world > 1 and torch.cuda.device_count() < world:
+        raise SystemExit(f"{world} ranks need {world} GPUs, {torch.cuda.device_count()} visible")
     torch.cuda.set_device(local)
+    if world > 1:
+        os.environ.setdefault("NCCL_DEBUG", "INFO")       # the communicator log (nranks) stays readable
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
     dist = distributed.init(world, rank, "nccl") if world > 1 else None
     if rank == 0:
         tbuild.build()
     if dist is not None:
         dist.barrier()
-    # weak scaling: every rank tracks its own time frame (one time frame per GPU)
-    fr = synth.generate(synth.config(5, seed=5 + 1000 * rank))
+    cfg = args.config
     rx = synth.row_x()
+    if args.shard == "sectors" and world > 1:
+        # strong scaling: ONE frame, rank r tracks sectors shard_sectors(36, world, r)
+        whole = synth.generate(synth.config(cfg, seed=cfg))
+        cl, so, lo = distributed.shard_frame(whole.clusters, whole.sector_offsets, world, rank)
+        fr = synth.Frame(np.ascontiguousarray(cl), so, whole.truth[lo:lo + len(cl)], whole.track_par, whole.n_sectors,
+                         f"config{cfg}/shard{rank}")
+        scaling, parallelism = "strong", f"sectors x{world} of one frame (no data-path collective)"
+    else:
+        # weak scaling: every rank tracks its own time frame (one time frame per GPU)
+        fr = synth.generate(synth.config(cfg, seed=cfg + 1000 * rank))
+        scaling, parallelism = "weak", f"frames x{world} (no collective)"
     n = fr.n
     extra = {k: float(v) for k, v in (kv.split("=") for kv in args.params.split(",") if kv)}
-    trk = binding.Tracker(rx, n_sectors=36, max_clusters=n, max_tracklets=max(1 << 16, n // 8),
+    trk = binding.Tracker(rx, n_sectors=fr.n_sectors, max_clusters=max(n, 1024), max_tracklets=max(1 << 16, n // 8),
                           max_tracks=max(1 << 16, n // 24), device=f"cuda:{local}", **extra)
     dev_clusters = trk.upload(fr.clusters)
     stream = torch.cuda.current_stream()
@@ -191,7 +229,7 @@ def run_gpu(args):
     hd = trk.header()
     if hd["status"] != 0:
         raise SystemExit(f"capacity overflow in warm-up: {hd}")
-    trk.set_profiling(True)
+    trk.set_profiling(1)
     sampler = ClockSampler(local)
     if dist is not None:
         dist.barrier()
@@ -209,18 +247,30 @@ def run_gpu(args):
     ms_local = e0.elapsed_time(e1)
     clocks = sampler.stop() if rank == 0 else None
     stage = trk.stage_ms()
-    trk.set_profiling(False)
+    trk.set_profiling(0)
     launches = trk.launch_count() * args.steps
     stats = trk.stats()
     hd = trk.header()
     ms_total, n_total = distributed.aggregate(dist, ms_local, n)
     ms_per_step = ms_total / args.steps
     value = n_total / (ms_per_step * 1e-3)
+    # global track ids of a sector split: exclusive scan of the per-rank counts (one 8-byte all-gather, outside the timed loop)
+    counts = distributed.gather_counts(dist, hd["n_tracks"])
+    id_offset = int(distributed.track_id_offsets(counts)[rank])
 
-    # ---- end to end through tpcca_track_host (pinned host buffers, H2D + D2H inside the timed region)
+    # ---- per-kernel device times (profiling level 2: two events around each main kernel), separate short pass
+    trk.set_profiling(2)
+    for _ in range(3):
+        trk.track(dev_clusters, n, fr.sector_offsets)
+    torch.cuda.synchronize()
+    kms = trk.kernel_ms()
+    trk.set_profiling(0)
+
+    # ---- end to end through the library's host calls (pinned host buffers, H2D + D2H inside the timed region)
     hc = torch.from_numpy(fr.clusters.view(np.uint8).reshape(-1)).pin_memory()
-    ot = torch.empty(16 + 128 * trk.max_tracks, dtype=torch.uint8).pin_memory()
-    oa = torch.empty(n, dtype=torch.int32).pin_memory()
+    outs = [(torch.empty(16 + 128 * trk.max_tracks, dtype=torch.uint8).pin_memory(),
+             torch.empty(max(n, 1), dtype=torch.int32).pin_memory()) for _ in range(2)]
+    ot, oa = outs[0]
     for _ in range(max(1, args.warmup // 2)):
         trk.track_host(hc, n, fr.sector_offsets, ot, oa)
     if dist is not None:
@@ -229,7 +279,7 @@ def run_gpu(args):
     f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     f0.record(stream)
     for _ in range(args.steps):
-        trk.track_host(hc, n, fr.sector_offsets, ot, oa)
+        trk.track_host(hc, n, fr.sector_offsets, ot, oa)   # strictly serial: copy in, track, copy out, wait
     f1.record(stream)
     torch.cuda.synchronize()
     if dist is not None:
@@ -238,89 +288,98 @@ def run_gpu(args):
     e2e_serial = n_total / (e2e_ms / args.steps * 1e-3)
     nt = int(ot[:16].numpy().view(binding.HEADER_DTYPE)["n_tracks"][0])
     h2d, d2h = n * 16, 16 + n * 4 + nt * 128
-
-    # ---- the same calls with several frames in flight: one handle, stream and host thread per frame in
-    # flight, so that one frame's copies overlap another frame's kernels.  Every step still copies its own inputs and results.
-    F = max(2, args.in_flight)
-    lanes = [(trk, ot, oa, torch.cuda.Stream())]
-    for _ in range(F - 1):
-        lanes.append((binding.Tracker(rx, n_sectors=36, max_clusters=n, max_tracklets=trk.max_tracklets,
-                                      max_tracks=trk.max_tracks, device=f"cuda:{local}", **extra),
-                      torch.empty(16 + 128 * trk.max_tracks, dtype=torch.uint8).pin_memory(),
-                      torch.empty(n, dtype=torch.int32).pin_memory(), torch.cuda.Stream()))
-    steps2 = max(F, args.steps - args.steps % F)
-
-    def worker(tr, o_t, o_a, st, k, ev):
-        torch.cuda.set_device(local)
-        with torch.cuda.stream(st):
-            if ev is not None:
-                st.wait_event(ev)
-            for _ in range(k):
-                tr.track_host(hc, n, fr.sector_offsets, o_t, o_a)
-
-    def run_pipelined(k, ev):
-        ths = [threading.Thread(target=worker, args=(tr, o_t, o_a, st, k, ev)) for tr, o_t, o_a, st in lanes]
-        for th in ths:
-            th.start()
-        for th in ths:
-            th.join()
-
-    run_pipelined(1, None)
+    # pipelined: tpcca_track_host_async / tpcca_wait, two frames in flight on ONE handle and ONE workspace:
+    # the upload of frame k+1 and the download of frame k-1 overlap the kernels of frame k.  Every step still copies its
+    # own input and its own results.
+    for i in range(2):
+        trk.track_host_async(hc, n, fr.sector_offsets, *outs[i])
+    trk.wait()
+    trk.wait()
     if dist is not None:
         dist.barrier()
     torch.cuda.synchronize()
+    t0 = time.perf_counter()
     g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     g0.record(stream)
-    run_pipelined(steps2 // F, g0)
-    for _, _, _, st in lanes:
-        stream.wait_stream(st)
+    trk.track_host_async(hc, n, fr.sector_offsets, *outs[0])
+    for i in range(1, args.steps):
+        trk.track_host_async(hc, n, fr.sector_offsets, *outs[i & 1])
+        trk.wait()
+    trk.wait()
     g1.record(stream)
     torch.cuda.synchronize()
+    wall_ms = (time.perf_counter() - t0) * 1e3
     if dist is not None:
         dist.barrier()
-    pipe_ms, _ = distributed.aggregate(dist, g0.elapsed_time(g1), n)
-    e2e_value = n_total / (pipe_ms / steps2 * 1e-3)
-    for _, _, o_a, _ in lanes[1:]:
-        assert np.array_equal(o_a.numpy(), oa.numpy()), "the in-flight handles disagree"
-    del lanes[1:]
+    # the last wait returns after the last D2H on the internal copy streams: take the larger of the device span on the
+    # caller's stream and the host wall clock around the loop
+    pipe_ms, _ = distributed.aggregate(dist, max(g0.elapsed_time(g1), wall_ms), n)
+    e2e_value = n_total / (pipe_ms / args.steps * 1e-3)
+    assert np.array_equal(outs[0][1].numpy(), outs[1][1].numpy()), "the two staging slots disagree"
 
     if rank != 0:
         return 0
-    gpu_assignment = oa.numpy().copy()
+    gpu_assignment = outs[0][1].numpy()[:n].copy()
     gpu_quality = quality(gpu_assignment, nt, fr)
-    # ---- roofline of the dominant kernel (per-stage CUDA events recorded inside the timed loop)
+    # ---- roofline (algorithmic bytes of DESIGN.md section 7 x live device counters)
     peak, peak_src = peaks()
-    dom = max(stage, key=stage.get)
-    alg = {
+    T = hd["n_start_hits"]
+    alg_stage = {
         "neighbours": BYTES_PER_CLUSTER_NEIGHBOURS * n,
-        "tracklets": BYTES_PER_ROW_STEP_TRACKLETS * stats["row_steps"] + BYTES_PER_TRACKLET * hd["n_start_hits"]
-        + BYTES_PER_TRACKLET_HIT * stats["track_hits"],
+        "tracklets": BYTES_PER_ROW_STEP_TRACKLETS * stats["row_steps"] + BYTES_PER_TRACKLET * T
+        + BYTES_PER_TRACKLET_HIT * stats["tracklet_hits"],
         "grid": 36.0 * n + 12.0 * stats["n_bins"],
         "clean_start": 32.0 * n,
-        "select": 12.0 * stats["track_hits"] + 12.0 * n,
+        "select": 12.0 * stats["tracklet_hits"] + 12.0 * n,
         "refit": 12.0 * 3 * stats["track_hits"] + 128.0 * hd["n_tracks"],
     }
-    per_stage = {k: {"ms": stage[k], "alg_GBps": alg[k] / (stage[k] * 1e-3) / 1e9 if stage[k] > 0 else None,
-                     "frac": alg[k] / (stage[k] * 1e-3) / 1e9 / peak if stage[k] > 0 else None} for k in stage}
-    ach = alg[dom] / (stage[dom] * 1e-3) / 1e9
-    # the Kalman stages are fp32-issue bound: useful fp32 operations of the section-3
-    # arithmetic per row step against 148 SM x 128 lanes x SM clock (no FMA: one operation per lane and clock)
+    alg_kernel = {
+        "k_slice_scatter": 32.0 * n, "k_slice_sort": 30.0 * n + 4.0 * stats["n_bins"],
+        "k_neighbours": alg_stage["neighbours"], "k_clean": 24.0 * n,
+        "k_tl_e1": BYTES_PER_ROW_STEP_TRACKLETS * stats["steps_e1"],
+        "k_tl_e2": BYTES_PER_ROW_STEP_TRACKLETS * stats["steps_e2"],
+        "k_tl_e3a": BYTES_PER_ROW_STEP_TRACKLETS * stats["steps_e3a"],
+        "k_tl_e3b": BYTES_PER_ROW_STEP_TRACKLETS * stats["steps_e3b"] + BYTES_PER_TRACKLET * T,
+        "k_tracklet_weights": (4.0 + BYTES_PER_TRACKLET_HIT) * stats["tracklet_hits"],
+        "k_select_own": 12.0 * stats["tracklet_hits"], "k_assign": 12.0 * n, "k_refit": alg_stage["refit"],
+    }
+
+    def rate(b, ms):
+        return b / (ms * 1e-3) / 1e9 if ms and ms > 0 else None
+
+    per_stage = {k: {"ms": stage[k], "alg_GBps": rate(alg_stage[k], stage[k]),
+                     "frac": (rate(alg_stage[k], stage[k]) or 0.0) / peak} for k in stage}
+    per_kernel = {k: {"ms": kms[k], "alg_GBps": rate(alg_kernel[k], kms[k]),
+                      "frac": (rate(alg_kernel[k], kms[k]) or 0.0) / peak} for k in kms}
+    dom = max(kms, key=kms.get)
+    # k_neighbours and k_refit are the only kernels of their stage (k_write_header aside): their time inside the timed
+    # region is the stage time; any other kernel takes the per-kernel pass
+    single = {"k_neighbours": "neighbours", "k_refit": "refit"}
+    dom_ms = stage[single[dom]] if dom in single else kms[dom]
+    dom_src = ("stage events inside the timed region (the stage is this one kernel)" if dom in single
+               else "per-kernel events, separate pass after the timed region")
+    ach = rate(alg_kernel[dom], dom_ms)
+    # the Kalman kernels are issue bound: useful fp32 instructions of the section-3 arithmetic per
+    # row step (an fma counts once) against 148 SM x 128 lanes x SM clock
     sm_mhz = (clocks or {}).get("sm_mhz") or 1965.0
     alu_peak = 148 * 128 * sm_mhz * 1e6 / 1e9
     alu_ops = FP32_OPS_PER_ROW_STEP * (stats["row_steps"] + 3 * stats["track_hits"])
     alu_ms = stage["tracklets"] + stage["refit"]
-    alu = {"achieved": alu_ops / (alu_ms * 1e-3) / 1e9, "peak": alu_peak, "unit": "Gop/s",
+    alu = {"achieved": alu_ops / (alu_ms * 1e-3) / 1e9, "peak": alu_peak, "unit": "Ginstr/s",
            "frac": alu_ops / (alu_ms * 1e-3) / 1e9 / alu_peak, "kernels": "tracklets+refit",
-           "ops_per_row_step": FP32_OPS_PER_ROW_STEP}
+           "instr_per_row_step": FP32_OPS_PER_ROW_STEP}
+    whole = sum(alg_stage.values())
     roofline = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": ncu_traffic(dom), "peak_source": peak_src, "algorithmic_bytes": alg[dom],
-                "kernel_ms": stage[dom], "stages": per_stage, "alu": alu}
+                "traffic": ncu_traffic(dom), "peak_source": peak_src, "algorithmic_bytes": alg_kernel[dom],
+                "kernel_ms": dom_ms, "kernel_ms_source": dom_src, "stages": per_stage, "kernels": per_kernel,
+                "whole_call": {"algorithmic_bytes": whole, "GBps": rate(whole, ms_local / args.steps),
+                               "frac": rate(whole, ms_local / args.steps) / peak}, "alu": alu}
     # ---- CPU baseline: the oracle as it stands, one pass over the same frame (rank 0, N = 1 only)
     cpu_baseline = None
-    if world == 1:
-        cv, ct, cn, ores = oracle_timed(1.0, 5, 1, 0, fr=fr)
+    if world == 1 and not args.no_cpu_baseline:
+        cv, ct, cn, ores = oracle_timed(cfg, 1.0, cfg, 1, 0, fr=fr)
         cpu_baseline = {"value": cv, "unit": UNIT, "cores": 1, "kind": "oracle",
-                        "sample": f"one pass over the same config-5 frame, {cn} clusters, {ct:.1f} s",
+                        "sample": f"one pass over the same config-{cfg} frame, {cn} clusters, {ct:.1f} s",
                         "quality": quality(ores.assignment, len(ores.tracks), fr),
                         "assignment_equals_cuda_path": bool(np.array_equal(ores.assignment, gpu_assignment))}
     try:
@@ -329,17 +388,20 @@ def run_gpu(args):
         baseline_metric = None
     line = {"metric": METRIC, "baseline_metric": baseline_metric, "value": value, "unit": UNIT, "n_gpus": world,
             "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": scaling,
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": "config5_timeframe_50_collisions", "clusters_per_frame": n,
-                       "frames_per_step": world, "ms_per_time_frame": ms_per_step, "n_tracks": hd["n_tracks"],
-                       "n_start_hits": hd["n_start_hits"], "row_steps": stats["row_steps"],
-                       "quality": gpu_quality,
-                       "l2": "inputs larger than L2 (cluster array %.0f MB, working set > 1 GB)" % (n * 16 / 1e6),
-                       "parallelism": f"frames x{world} (no collective)"},
-            "clocks": clocks, "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "ms_per_step": pipe_ms / steps2, "steps": steps2, "frames_in_flight": F,
-                    "one_in_flight": {"value": e2e_serial, "ms_per_step": e2e_ms / args.steps}},
+            "config": {"workload": WORKLOADS[cfg], "clusters_per_frame": n, "clusters_per_step": n_total,
+                       "frames_per_step": world if scaling == "weak" else 1, "ms_per_time_frame": ms_per_step,
+                       "n_tracks": hd["n_tracks"], "n_tracks_all_ranks": int(counts.sum()), "track_id_offset": id_offset,
+                       "n_start_hits": hd["n_start_hits"], "row_steps": stats["row_steps"], "quality": gpu_quality,
+                       "l2": "inputs larger than L2 (cluster array %.0f MB, working set > 1 GB)" % (n * 16 / 1e6)
+                       if n * 16 > 126e6 else "frame fits the 126 MB L2: a parity-test case, not the bench line",
+                       "parallelism": parallelism, "shard": args.shard},
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "ms_per_step": pipe_ms / args.steps, "steps": args.steps, "frames_in_flight": 2, "handles": 1,
+                    "workspaces": 1, "api": "tpcca_track_host_async + tpcca_wait",
+                    "one_in_flight": {"value": e2e_serial, "ms_per_step": e2e_ms / args.steps, "api": "tpcca_track_host"}},
             "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu_baseline}
     print(json.dumps(line))
     return 0
@@ -351,11 +413,19 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="tpcca", choices=["tpcca", "reference"])
-    ap.add_argument("--in-flight", type=int, default=3, help="frames in flight of the pipelined end-to-end leg")
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5],
+                    help="BASELINE.json config (5 = the bench line; 1-4 are parity-test cases)")
+    ap.add_argument("--shard", default="frames", choices=["frames", "sectors"],
+                    help="N > 1: one frame per rank (weak) or one frame split by sector ranges (strong)")
+    ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle leg (sweeps)")
     ap.add_argument("--params", default="", help="k=v,k=v overrides of tpcca_params (tuning experiments)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "tpcca" else args.warmup
-    return run_reference(args) if args.impl == "reference" else run_gpu(args)
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.gpus > 1 and "RANK" not in os.environ:
+        return respawn_under_torchrun(args)
+    return run_gpu(args)
 
 
 if __name__ == "__main__":

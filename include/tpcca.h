@@ -109,10 +109,26 @@ int tpcca_track(tpcca_handle* h, const tpcca_cluster* clusters, int64_t n, const
                 void* stream, void* out_tracks, int32_t* out_hit_assignment);
 
 /* Same, end to end from HOST buffers (pinned for best speed): copies clusters host->device into the
- * workspace, tracks, copies header, tracks and assignment device->host and synchronises `stream`.
- * out_tracks: host, sizeof(header) + max_tracks*128 bytes (only n_tracks records are written). */
+ * workspace, tracks, copies header, tracks and assignment device->host and waits for them.
+ * out_tracks: host, sizeof(header) + max_tracks*128 bytes (only n_tracks records are written).
+ * Equivalent to tpcca_track_host_async + tpcca_wait; refused while async frames are in flight. */
 int tpcca_track_host(tpcca_handle* h, const tpcca_cluster* clusters, int64_t n, const int32_t* sector_offsets,
                      void* stream, void* out_tracks, int32_t* out_hit_assignment);
+
+/* Pipelined host call ("processing two events concurrently on one GPU"; PAPER.md:177 host<->GPU
+ * transfers).  Same arguments as tpcca_track_host; returns after ENQUEUEING the host->device copy (internal copy
+ * stream), the kernels (`stream`) and the device->host copy of header and assignment (second internal stream).  At
+ * most TWO frames may be in flight per handle (two staging slots inside the one workspace): while the kernels of
+ * frame k run, the input of frame k+1 is uploaded and the results of frame k-1 are downloaded.  The host buffers
+ * of a frame must stay valid and untouched until its tpcca_wait returns.  Returns TPCCA_ERR_ARGUMENT if two frames
+ * are already in flight. */
+int tpcca_track_host_async(tpcca_handle* h, const tpcca_cluster* clusters, int64_t n, const int32_t* sector_offsets,
+                           void* stream, void* out_tracks, int32_t* out_hit_assignment);
+
+/* Blocks until the OLDEST frame submitted with tpcca_track_host_async is complete: its header and assignment have
+ * arrived, then its n_tracks track records are copied (third internal stream) -- frames complete in submission
+ * order.  TPCCA_ERR_ARGUMENT if no frame is in flight. */
+int tpcca_wait(tpcca_handle* h);
 
 /* Intermediates of the last tpcca_track on this handle, translated to INPUT-index space so that they
  * can be compared with an independent implementation.  dst: device.  Enqueued on `stream`. */
@@ -139,14 +155,23 @@ int tpcca_set_debug(tpcca_handle* h, int on);
  * was switched on (CUDA events recorded on each call's stream; synchronises those events).  ms: host float[TPCCA_N_STAGES]. */
 enum { TPCCA_STAGE_GRID = 0, TPCCA_STAGE_NEIGHBOURS, TPCCA_STAGE_CLEAN_START, TPCCA_STAGE_TRACKLETS,
        TPCCA_STAGE_SELECT, TPCCA_STAGE_REFIT, TPCCA_N_STAGES };
-int tpcca_set_profiling(tpcca_handle* h, int on);
+int tpcca_set_profiling(tpcca_handle* h, int on);  /* 0 off, 1 stage events, 2 stage + per-kernel events */
 int tpcca_get_stage_ms(tpcca_handle* h, float* ms);
+
+/* Device time of the main kernels of the LAST tpcca_track made with profiling level 2 (two CUDA events around each
+ * launch on the call's stream; synchronises them).  ms: host float[TPCCA_N_KERNELS]. */
+enum tpcca_kernel_id { TPCCA_K_SLICE_SCATTER = 0, TPCCA_K_SLICE_SORT, TPCCA_K_NEIGHBOURS, TPCCA_K_CLEAN, TPCCA_K_TL_E1,
+                       TPCCA_K_TL_E2, TPCCA_K_TL_E3A, TPCCA_K_TL_E3B, TPCCA_K_WEIGHTS, TPCCA_K_SELECT_OWN, TPCCA_K_ASSIGN,
+                       TPCCA_K_REFIT, TPCCA_N_KERNELS };
+int tpcca_get_kernel_ms(tpcca_handle* h, float* ms);
 
 /* Device-side work counters of the last tpcca_track (synchronises `stream`): host int64[TPCCA_N_WORK]. */
 enum { TPCCA_WORK_N_BINS = 0,      /* grid bins of the frame */
        TPCCA_WORK_ROW_STEPS,       /* Kalman row steps (transport attempts) taken by the tracklet constructor */
        TPCCA_WORK_SEARCHES,        /* pick-up searches (grid look-ups) by the tracklet constructor */
        TPCCA_WORK_TRACK_HITS,      /* hits owned by accepted tracks */
+       TPCCA_WORK_TRACKLET_HITS,   /* hits of all valid tracklets (one weight atomic each) */
+       TPCCA_WORK_STEPS_E1, TPCCA_WORK_STEPS_E2, TPCCA_WORK_STEPS_E3A, TPCCA_WORK_STEPS_E3B, /* row steps per constructor kernel */
        TPCCA_N_WORK };
 int tpcca_get_stats(tpcca_handle* h, int64_t* stats, void* stream);
 

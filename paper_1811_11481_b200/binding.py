@@ -17,6 +17,8 @@ _SO = os.path.join(_HERE, "libtpcca.so")
 LINK_UP_RAW, LINK_DOWN_RAW, LINK_UP, LINK_DOWN, START_HITS, TRACKLET_ROW_HITS, TRACKLET_INTS, TRACKLET_FLOATS, \
     TRACK_TRACKLET = range(9)
 STAGES = ("grid", "neighbours", "clean_start", "tracklets", "select", "refit")
+KERNELS = ("k_slice_scatter", "k_slice_sort", "k_neighbours", "k_clean", "k_tl_e1", "k_tl_e2", "k_tl_e3a", "k_tl_e3b",
+           "k_tracklet_weights", "k_select_own", "k_assign", "k_refit")
 
 CLUSTER_DTYPE = np.dtype([("x", "<f4"), ("y", "<f4"), ("z", "<f4"), ("row", "<i4")])
 TRACK_DTYPE = np.dtype([
@@ -63,16 +65,20 @@ def load():
         lib.tpcca_workspace_bytes.argtypes = [C.POINTER(Geometry), C.POINTER(Params)]
         lib.tpcca_init.restype = C.c_void_p
         lib.tpcca_init.argtypes = [C.POINTER(Geometry), C.c_float, C.POINTER(Params)]
-        for name in ("tpcca_track", "tpcca_track_host"):
+        for name in ("tpcca_track", "tpcca_track_host", "tpcca_track_host_async"):
             fn = getattr(lib, name)
             fn.restype = C.c_int
             fn.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.tpcca_wait.restype = C.c_int
+        lib.tpcca_wait.argtypes = [C.c_void_p]
         lib.tpcca_get_intermediate.restype = C.c_int
         lib.tpcca_get_intermediate.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_size_t, C.c_void_p]
         lib.tpcca_set_profiling.argtypes = [C.c_void_p, C.c_int]
         lib.tpcca_set_debug.argtypes = [C.c_void_p, C.c_int]
         lib.tpcca_get_stage_ms.restype = C.c_int
         lib.tpcca_get_stage_ms.argtypes = [C.c_void_p, C.c_void_p]
+        lib.tpcca_get_kernel_ms.restype = C.c_int
+        lib.tpcca_get_kernel_ms.argtypes = [C.c_void_p, C.c_void_p]
         lib.tpcca_get_stats.restype = C.c_int
         lib.tpcca_get_stats.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         lib.tpcca_last_launch_count.restype = C.c_int
@@ -188,6 +194,18 @@ class Tracker:
         self._check(self.lib.tpcca_track_host(self.h, clusters_host.data_ptr() if n else None, n, so.ctypes.data,
                                               self._stream(), out_tracks_host.data_ptr(), out_assign_host.data_ptr()))
 
+    def track_host_async(self, clusters_host, n: int, sector_offsets: np.ndarray, out_tracks_host, out_assign_host):
+        """tpcca_track_host_async: enqueue only; at most two frames in flight; pair every call with wait()."""
+        so = np.ascontiguousarray(sector_offsets, dtype=np.int32)
+        self._so = so
+        self.n = int(n)
+        self._check(self.lib.tpcca_track_host_async(self.h, clusters_host.data_ptr() if n else None, n, so.ctypes.data,
+                                                    self._stream(), out_tracks_host.data_ptr(),
+                                                    out_assign_host.data_ptr()))
+
+    def wait(self):
+        self._check(self.lib.tpcca_wait(self.h))
+
     def intermediate(self, what: int) -> np.ndarray:
         torch = self.torch
         hd = self.header()
@@ -212,8 +230,14 @@ class Tracker:
     def set_debug(self, on: bool):
         self.lib.tpcca_set_debug(self.h, int(on))
 
-    def set_profiling(self, on: bool):
+    def set_profiling(self, on):
+        """0 / False off, 1 / True stage events, 2 stage + per-kernel events."""
         self.lib.tpcca_set_profiling(self.h, int(on))
+
+    def kernel_ms(self) -> dict:
+        ms = (C.c_float * len(KERNELS))()
+        self._check(self.lib.tpcca_get_kernel_ms(self.h, ms))
+        return dict(zip(KERNELS, [float(v) for v in ms]))
 
     def stage_ms(self) -> dict:
         ms = (C.c_float * len(STAGES))()
@@ -221,9 +245,11 @@ class Tracker:
         return dict(zip(STAGES, [float(v) for v in ms]))
 
     def stats(self) -> dict:
-        st = (C.c_int64 * 4)()
+        st = (C.c_int64 * 9)()
         self._check(self.lib.tpcca_get_stats(self.h, st, self._stream()))
-        return dict(n_bins=int(st[0]), row_steps=int(st[1]), searches=int(st[2]), track_hits=int(st[3]))
+        return dict(n_bins=int(st[0]), row_steps=int(st[1]), searches=int(st[2]), track_hits=int(st[3]),
+                    tracklet_hits=int(st[4]), steps_e1=int(st[5]), steps_e2=int(st[6]), steps_e3a=int(st[7]),
+                    steps_e3b=int(st[8]))
 
     def launch_count(self) -> int:
         return int(self.lib.tpcca_last_launch_count(self.h))

@@ -17,14 +17,20 @@ struct tpcca_handle {
   Dev d;
   tpcca_geometry geo;
   int64_t max_clusters;
-  // host-API staging (inside the workspace)
-  float4* stage_clusters;
-  int32_t* stage_assign;
-  char* stage_tracks;
+  // host-API staging (inside the workspace): two slots, so that the copies of one frame overlap the kernels of the next
+  float4* stage_clusters[2];
+  int32_t* stage_assign[2];
+  char* stage_tracks[2];
+  // pipelined host call (tpcca_track_host_async / tpcca_wait): internal copy streams and per-slot events
+  cudaStream_t st_in, st_out, st_rec;
+  cudaEvent_t ev_in[2], ev_k[2], ev_out[2];
+  struct Pending { bool busy; int64_t n; void* out_tracks; } pend[2];
+  uint64_t seq_submit, seq_wait;
   // last call
   int64_t last_n;
   int launches;
-  bool profiling, have_times, debug_sync;
+  bool profiling, have_times, debug_sync, kprofiling, have_ktimes;
+  cudaEvent_t kev[2 * TPCCA_N_KERNELS];
   int prof_calls;
   int device;
   cudaEvent_t ev[PROF_RING][TPCCA_N_STAGES + 1];
@@ -91,9 +97,11 @@ static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params
   CARVE(d.w_list, int2, T);
   CARVE(d.th_yz, float2, N);
   CARVE(d.th_row, uint8_t, N);
-  CARVE(stage_clusters, float4, N);
-  CARVE(stage_assign, int32_t, N);
-  CARVE(stage_tracks, char, sizeof(tpcca_out_header) + K * sizeof(tpcca_track_rec));
+  for (int sl = 0; sl < 2; sl++) {
+    CARVE(stage_clusters[sl], float4, N);
+    CARVE(stage_assign[sl], int32_t, N);
+    CARVE(stage_tracks[sl], char, sizeof(tpcca_out_header) + K * sizeof(tpcca_track_rec));
+  }
 #undef CARVE
   if (base) { h->d.max_bins = (int32_t)NB; h->d.sb_key = h->d.cluster_rank; }
   return off;
@@ -190,6 +198,18 @@ tpcca_handle* tpcca_init(const tpcca_geometry* g, float bz_tesla, const tpcca_pa
         tpcca_free(h);  // destroys the events created so far
         return nullptr;
       }
+  bool ok = cudaStreamCreateWithFlags(&h->st_in, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaStreamCreateWithFlags(&h->st_out, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaStreamCreateWithFlags(&h->st_rec, cudaStreamNonBlocking) == cudaSuccess;
+  for (int sl = 0; sl < 2 && ok; sl++)
+    ok = cudaEventCreateWithFlags(&h->ev_in[sl], cudaEventDisableTiming) == cudaSuccess &&
+         cudaEventCreateWithFlags(&h->ev_k[sl], cudaEventDisableTiming) == cudaSuccess &&
+         cudaEventCreateWithFlags(&h->ev_out[sl], cudaEventDisableTiming) == cudaSuccess;
+  if (!ok) {
+    set_err("stream / event creation failed: %s", cudaGetErrorString(cudaGetLastError()));
+    tpcca_free(h);
+    return nullptr;
+  }
   return h;
 }
 
@@ -219,6 +239,7 @@ static int track_impl(tpcca_handle* h, const tpcca_cluster* clusters, int64_t n,
     const cudaError_t de = cudaStreamSynchronize(st);                                            \
     if (de != cudaSuccess) { set_err("stage %s failed: %lld", name, (long long)de); fprintf(stderr, "tpcca: stage %s: %s\n", name, cudaGetErrorString(de)); return TPCCA_ERR_CUDA; } \
   }
+  L.kev = (h->kprofiling && h->kev[0]) ? h->kev : nullptr;
   if (prof) cudaEventRecord(ev[0], st);
   launch_grid(d, so, L);
   DBG_STAGE("grid");
@@ -241,6 +262,7 @@ static int track_impl(tpcca_handle* h, const tpcca_cluster* clusters, int64_t n,
   if (prof) cudaEventRecord(ev[6], st);
   if (prof) h->prof_calls++;
   h->have_times = prof && h->prof_calls > 0;
+  h->have_ktimes = L.kev != nullptr && d.n > 0 && d.max_tracklets > 0 && d.max_tracks > 0;
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) { set_err("kernel launch failed: %s", cudaGetErrorString(e)); return TPCCA_ERR_CUDA; }
   return TPCCA_OK;
@@ -262,39 +284,76 @@ int tpcca_track(tpcca_handle* h, const tpcca_cluster* clusters, int64_t n, const
                 void* out_tracks, int32_t* out_hit_assignment) {
   int rc = check_call(h, clusters, n, sector_offsets, out_tracks, out_hit_assignment);
   if (rc) return rc;
-  Launch L{(cudaStream_t)stream, 0};
+  Launch L{(cudaStream_t)stream, 0, nullptr};
   rc = track_impl(h, clusters, n, sector_offsets, L.st, out_tracks, out_hit_assignment, L);
   h->launches = L.count;
   return rc;
 }
 
-int tpcca_track_host(tpcca_handle* h, const tpcca_cluster* clusters, int64_t n, const int32_t* sector_offsets,
-                     void* stream, void* out_tracks, int32_t* out_hit_assignment) {
+// Pipelined host call.  Frame k uses staging slot k % 2.  Streams: H2D on st_in, kernels on the caller's stream, D2H of
+// header + assignment on st_out, D2H of the n_tracks records on st_rec (issued by tpcca_wait once the header is known).
+// Events order the three; nothing here blocks the host.
+int tpcca_track_host_async(tpcca_handle* h, const tpcca_cluster* clusters, int64_t n, const int32_t* sector_offsets,
+                           void* stream, void* out_tracks, int32_t* out_hit_assignment) {
   int rc = check_call(h, clusters, n, sector_offsets, out_tracks, out_hit_assignment);
   if (rc) return rc;
+  const int sl = (int)(h->seq_submit & 1);
+  if (h->pend[sl].busy) { set_err("two frames are already in flight: call tpcca_wait first"); return TPCCA_ERR_ARGUMENT; }
   cudaStream_t st = (cudaStream_t)stream;
-  Launch L{st, 0};
-  if (n > 0 && cudaMemcpyAsync(h->stage_clusters, clusters, (size_t)n * 16, cudaMemcpyHostToDevice, st) != cudaSuccess) {
-    set_err("H2D copy failed: %s", cudaGetErrorString(cudaGetLastError())); return TPCCA_ERR_CUDA;
+  Launch L{st, 0, nullptr};
+  cudaError_t e = cudaSuccess;
+  if (n > 0) {
+    // the kernels of the frame that used this slot last (two frames ago) read stage_clusters[sl]: they were waited for by
+    // tpcca_wait; the event keeps the order explicit for callers that switch streams between frames
+    e = cudaStreamWaitEvent(h->st_in, h->ev_k[sl], 0);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h->stage_clusters[sl], clusters, (size_t)n * 16, cudaMemcpyHostToDevice, h->st_in);
   }
-  rc = track_impl(h, reinterpret_cast<const tpcca_cluster*>(h->stage_clusters), n, sector_offsets, st, h->stage_tracks,
-                  h->stage_assign, L);
+  if (e == cudaSuccess) e = cudaEventRecord(h->ev_in[sl], h->st_in);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(st, h->ev_in[sl], 0);
+  if (e != cudaSuccess) { set_err("H2D copy failed: %s", cudaGetErrorString(e)); cudaGetLastError(); return TPCCA_ERR_CUDA; }
+  rc = track_impl(h, reinterpret_cast<const tpcca_cluster*>(h->stage_clusters[sl]), n, sector_offsets, st,
+                  h->stage_tracks[sl], h->stage_assign[sl], L);
   h->launches = L.count;
   if (rc) return rc;
-  cudaError_t e = cudaMemcpyAsync(out_tracks, h->stage_tracks, sizeof(tpcca_out_header), cudaMemcpyDeviceToHost, st);
+  e = cudaEventRecord(h->ev_k[sl], st);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(h->st_out, h->ev_k[sl], 0);
+  if (e == cudaSuccess)
+    e = cudaMemcpyAsync(out_tracks, h->stage_tracks[sl], sizeof(tpcca_out_header), cudaMemcpyDeviceToHost, h->st_out);
   if (e == cudaSuccess && n > 0)
-    e = cudaMemcpyAsync(out_hit_assignment, h->stage_assign, (size_t)n * 4, cudaMemcpyDeviceToHost, st);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    e = cudaMemcpyAsync(out_hit_assignment, h->stage_assign[sl], (size_t)n * 4, cudaMemcpyDeviceToHost, h->st_out);
+  if (e == cudaSuccess) e = cudaEventRecord(h->ev_out[sl], h->st_out);
+  if (e != cudaSuccess) { set_err("D2H enqueue failed: %s", cudaGetErrorString(e)); cudaGetLastError(); return TPCCA_ERR_CUDA; }
+  h->pend[sl].busy = true; h->pend[sl].n = n; h->pend[sl].out_tracks = out_tracks;
+  h->seq_submit++;
+  return TPCCA_OK;
+}
+
+// Waits for the OLDEST frame in flight: header and assignment have arrived, then the n_tracks records are copied.
+int tpcca_wait(tpcca_handle* h) {
+  if (!h) { set_err("handle is null (not initialised)"); return TPCCA_ERR_NOT_INIT; }
+  if (h->seq_wait == h->seq_submit) { set_err("no frame in flight"); return TPCCA_ERR_ARGUMENT; }
+  const int sl = (int)(h->seq_wait & 1);
+  tpcca_handle::Pending& p = h->pend[sl];
+  cudaError_t e = cudaEventSynchronize(h->ev_out[sl]);
   if (e == cudaSuccess) {
-    const tpcca_out_header* hd = reinterpret_cast<const tpcca_out_header*>(out_tracks);
+    const tpcca_out_header* hd = reinterpret_cast<const tpcca_out_header*>(p.out_tracks);
     if (hd->n_tracks > 0) {
-      e = cudaMemcpyAsync((char*)out_tracks + sizeof(tpcca_out_header), h->stage_tracks + sizeof(tpcca_out_header),
-                          (size_t)hd->n_tracks * sizeof(tpcca_track_rec), cudaMemcpyDeviceToHost, st);
-      if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+      e = cudaMemcpyAsync((char*)p.out_tracks + sizeof(tpcca_out_header), h->stage_tracks[sl] + sizeof(tpcca_out_header),
+                          (size_t)hd->n_tracks * sizeof(tpcca_track_rec), cudaMemcpyDeviceToHost, h->st_rec);
+      if (e == cudaSuccess) e = cudaStreamSynchronize(h->st_rec);
     }
   }
+  p.busy = false;
+  h->seq_wait++;
   if (e != cudaSuccess) { set_err("D2H copy / execution failed: %s", cudaGetErrorString(e)); cudaGetLastError(); return TPCCA_ERR_CUDA; }
   return TPCCA_OK;
+}
+
+int tpcca_track_host(tpcca_handle* h, const tpcca_cluster* clusters, int64_t n, const int32_t* sector_offsets,
+                     void* stream, void* out_tracks, int32_t* out_hit_assignment) {
+  if (h && h->seq_wait != h->seq_submit) { set_err("frames of tpcca_track_host_async are in flight: call tpcca_wait first"); return TPCCA_ERR_ARGUMENT; }
+  const int rc = tpcca_track_host_async(h, clusters, n, sector_offsets, stream, out_tracks, out_hit_assignment);
+  return rc ? rc : tpcca_wait(h);
 }
 
 int tpcca_get_intermediate(tpcca_handle* h, int what, void* dst, size_t bytes, void* stream) {
@@ -316,7 +375,7 @@ int tpcca_get_intermediate(tpcca_handle* h, int what, void* dst, size_t bytes, v
   else if (what == TPCCA_TRACKLET_FLOATS) need = (size_t)c.n_start * 32;
   else need = (size_t)c.n_tracks * 4;
   if (bytes < need) { set_err("dst too small%s (need %lld bytes)", "", (long long)need); return TPCCA_ERR_ARGUMENT; }
-  Launch L{(cudaStream_t)stream, 0};
+  Launch L{(cudaStream_t)stream, 0, nullptr};
   launch_export(d, what, dst, L);
   e = cudaGetLastError();
   if (e != cudaSuccess) { set_err("export launch failed: %s", cudaGetErrorString(e)); return TPCCA_ERR_CUDA; }
@@ -332,7 +391,24 @@ int tpcca_set_debug(tpcca_handle* h, int on) {
 int tpcca_set_profiling(tpcca_handle* h, int on) {
   if (!h) return TPCCA_ERR_NOT_INIT;
   h->profiling = on != 0;
+  h->kprofiling = on >= 2;
   if (on) { h->have_times = false; h->prof_calls = 0; }
+  h->have_ktimes = false;
+  if (h->kprofiling && !h->kev[0])
+    for (int i = 0; i < 2 * TPCCA_N_KERNELS; i++)
+      if (cudaEventCreate(&h->kev[i]) != cudaSuccess) { set_err("cudaEventCreate failed"); h->kprofiling = false; return TPCCA_ERR_CUDA; }
+  return TPCCA_OK;
+}
+
+int tpcca_get_kernel_ms(tpcca_handle* h, float* ms) {
+  if (!h) return TPCCA_ERR_NOT_INIT;
+  if (!ms || !h->have_ktimes) { set_err("no kernel times recorded (tpcca_set_profiling(h, 2) before tpcca_track)"); return TPCCA_ERR_ARGUMENT; }
+  for (int i = 0; i < TPCCA_N_KERNELS; i++) {
+    if (cudaEventSynchronize(h->kev[2 * i + 1]) != cudaSuccess ||
+        cudaEventElapsedTime(&ms[i], h->kev[2 * i], h->kev[2 * i + 1]) != cudaSuccess) {
+      set_err("kernel event read failed"); cudaGetLastError(); return TPCCA_ERR_CUDA;
+    }
+  }
   return TPCCA_OK;
 }
 
@@ -364,6 +440,8 @@ int tpcca_get_stats(tpcca_handle* h, int64_t* stats, void* stream) {
   stats[TPCCA_WORK_ROW_STEPS] = (int64_t)c.row_steps;
   stats[TPCCA_WORK_SEARCHES] = (int64_t)c.searches;
   stats[TPCCA_WORK_TRACK_HITS] = (int64_t)c.track_hits;
+  stats[TPCCA_WORK_TRACKLET_HITS] = (int64_t)c.tracklet_hits;
+  for (int q = 0; q < 4; q++) stats[TPCCA_WORK_STEPS_E1 + q] = (int64_t)c.phase_steps[q];
   return TPCCA_OK;
 }
 
@@ -376,6 +454,16 @@ void tpcca_free(tpcca_handle* h) {
   for (int k = 0; k < PROF_RING; k++)
     for (int i = 0; i <= TPCCA_N_STAGES; i++)
       if (h->ev[k][i]) cudaEventDestroy(h->ev[k][i]);
+  for (int sl = 0; sl < 2; sl++) {
+    if (h->ev_in[sl]) cudaEventDestroy(h->ev_in[sl]);
+    if (h->ev_k[sl]) cudaEventDestroy(h->ev_k[sl]);
+    if (h->ev_out[sl]) cudaEventDestroy(h->ev_out[sl]);
+  }
+  for (int i = 0; i < 2 * TPCCA_N_KERNELS; i++)
+    if (h->kev[i]) cudaEventDestroy(h->kev[i]);
+  if (h->st_in) cudaStreamDestroy(h->st_in);
+  if (h->st_out) cudaStreamDestroy(h->st_out);
+  if (h->st_rec) cudaStreamDestroy(h->st_rec);
   delete h;
 }
 

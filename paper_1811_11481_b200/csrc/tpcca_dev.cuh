@@ -31,7 +31,8 @@ struct DevCounters {  // device-resident scalars
   int32_t n_work;      // seeds that reach the constructor (chain >= min_seed_hits)
   int32_t work_next[4];  // queue heads of the four tracklet-constructor kernels
   unsigned long long row_steps, searches, track_hits;  // work counters (roofline units)
-  unsigned long long pad2;
+  unsigned long long phase_steps[4];   // row steps of k_tl_e1 / e2 / e3a / e3b
+  unsigned long long tracklet_hits;    // hits of all valid tracklets (one weight atomic each)
 };
 
 struct SecOff { int32_t v[TPCCA_MAX_SECTORS + 1]; };
@@ -273,8 +274,16 @@ __device__ __forceinline__ int block_scan_excl(int v, int* total, int* smem /* >
 // launchers (one per pipeline step; defined in the .cu of that step)
 struct Launch {
   cudaStream_t st;
-  int count;  // kernels launched
+  int count;          // kernels launched
+  cudaEvent_t* kev;   // per-kernel profiling (tpcca_set_profiling(h, 2)): 2 events per timed kernel, or null
 };
+// Brackets one kernel launch with events when per-kernel profiling is on (id: enum tpcca_kernel_id).
+#define KTIMED(L, id, launch)                                   \
+  do {                                                          \
+    if ((L).kev) cudaEventRecord((L).kev[2 * (id)], (L).st);      \
+    launch;                                                     \
+    if ((L).kev) cudaEventRecord((L).kev[2 * (id) + 1], (L).st);  \
+  } while (0)
 cudaError_t setup_grid_kernels();  // per-device function attributes; called by tpcca_init on the handle's device
 void launch_grid(const Dev& d, const SecOff& so, Launch& L);
 void launch_neighbours(const Dev& d, Launch& L);

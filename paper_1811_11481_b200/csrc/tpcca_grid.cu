@@ -162,7 +162,8 @@ __global__ void k_reset(Dev d) {
     d.cnt->n_start = 0; d.cnt->n_tracks = 0; d.cnt->n_valid = 0; d.cnt->status = 0; d.cnt->n_bins = 0;
     d.cnt->n_start_raw = 0; d.cnt->n_work = 0;
     for (int q = 0; q < 4; q++) d.cnt->work_next[q] = 0;
-    d.cnt->row_steps = 0ull; d.cnt->searches = 0ull; d.cnt->track_hits = 0ull;
+    d.cnt->row_steps = 0ull; d.cnt->searches = 0ull; d.cnt->track_hits = 0ull; d.cnt->tracklet_hits = 0ull;
+    for (int q = 0; q < 4; q++) d.cnt->phase_steps[q] = 0ull;
   }
 }
 
@@ -422,9 +423,9 @@ void launch_grid(const Dev& d, const SecOff& so, Launch& L) {
   k_slice_offsets<<<1, 1024, 0, L.st>>>(d);
   L.count++;
   if (d.n > 0) {
-    k_slice_scatter<<<(d.n + A1_TILE - 1) / A1_TILE, A1_THREADS, 0, L.st>>>(d, so);
+    KTIMED(L, TPCCA_K_SLICE_SCATTER, (k_slice_scatter<<<(d.n + A1_TILE - 1) / A1_TILE, A1_THREADS, 0, L.st>>>(d, so)));
     L.count++;
   }
-  k_slice_sort<<<d.n_slices, A4_THREADS, A4_SMEM_BINS * sizeof(int), L.st>>>(d);
+  KTIMED(L, TPCCA_K_SLICE_SORT, (k_slice_sort<<<d.n_slices, A4_THREADS, A4_SMEM_BINS * sizeof(int), L.st>>>(d)));
   L.count++;
 }

@@ -166,7 +166,7 @@ __global__ void __launch_bounds__(NB_THREADS) k_neighbours(Dev d) {
 
 void launch_neighbours(const Dev& d, Launch& L) {
   if (d.n <= 0) return;
-  k_neighbours<<<(d.n + NB_THREADS - 1) / NB_THREADS, NB_THREADS, 0, L.st>>>(d);
+  KTIMED(L, TPCCA_K_NEIGHBOURS, (k_neighbours<<<(d.n + NB_THREADS - 1) / NB_THREADS, NB_THREADS, 0, L.st>>>(d)));
   L.count++;
 }
 
@@ -282,7 +282,7 @@ __global__ void __launch_bounds__(256) k_sb_rank(Dev d) {
 
 void launch_clean_start(const Dev& d, Launch& L) {
   if (d.n > 0) {
-    k_clean<<<(d.n + 255) / 256, 256, 0, L.st>>>(d);
+    KTIMED(L, TPCCA_K_CLEAN, (k_clean<<<(d.n + 255) / 256, 256, 0, L.st>>>(d)));
     L.count++;
   }
   k_start_offsets<<<1, 1024, 0, L.st>>>(d);

@@ -91,11 +91,11 @@ __global__ void __launch_bounds__(256) k_assign(Dev d) {
 void launch_select(const Dev& d, Launch& L) {
   if (d.n <= 0 || d.max_tracklets <= 0) return;
   const int T = d.max_tracklets;
-  k_select_own<<<d.n_sm * 16, SEL_THREADS, 0, L.st>>>(d);
+  KTIMED(L, TPCCA_K_SELECT_OWN, (k_select_own<<<d.n_sm * 16, SEL_THREADS, 0, L.st>>>(d)));
   L.count++;
   launch_scan_i32(d.sel_scan, &d.cnt->n_start, T, d.scan_tmp, L);
   k_select_ids<<<(T + 255) / 256, 256, 0, L.st>>>(d);
-  k_assign<<<(d.n + 255) / 256, 256, 0, L.st>>>(d);
+  KTIMED(L, TPCCA_K_ASSIGN, (k_assign<<<(d.n + 255) / 256, 256, 0, L.st>>>(d)));
   L.count += 2;
   // refit order: tracks by decreasing hit count, so that the lanes of a refit warp run the same number of steps
   launch_order_desc(d, 0, d.track_len, &d.cnt->n_tracks, d.max_tracks, d.track_order, L);
@@ -161,7 +161,7 @@ __global__ void k_write_header(Dev d) {
 
 void launch_refit(const Dev& d, Launch& L) {
   if (d.n > 0 && d.max_tracks > 0) {
-    k_refit<<<(d.max_tracks + 63) / 64, 64, 0, L.st>>>(d);
+    KTIMED(L, TPCCA_K_REFIT, (k_refit<<<(d.max_tracks + 63) / 64, 64, 0, L.st>>>(d)));
     L.count++;
   }
   k_write_header<<<1, 1, 0, L.st>>>(d);

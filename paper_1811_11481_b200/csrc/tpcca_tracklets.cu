@@ -233,7 +233,10 @@ __global__ void __launch_bounds__(E_THREADS, E1_BOUNDS) k_tl_e1(Dev d) {
     else r = (h >= rs2) ? r + 2 : r + 1;
   }
   const int ws = __reduce_add_sync(FULL, n_steps);
-  if (lane == 0 && ws) atomicAdd(&d.cnt->row_steps, (unsigned long long)ws);
+  if (lane == 0 && ws) {
+    atomicAdd(&d.cnt->row_steps, (unsigned long long)ws);
+    atomicAdd(&d.cnt->phase_steps[0], (unsigned long long)ws);
+  }
 }
 
 // ---- E2: outward extrapolation, one best cluster per row
@@ -317,6 +320,7 @@ __global__ void __launch_bounds__(E_THREADS, E2_BLOCKS) k_tl_e2(Dev d) {
   const int ws = __reduce_add_sync(FULL, n_steps);
   if (lane == 0 && ws) {
     atomicAdd(&d.cnt->row_steps, (unsigned long long)ws);
+    atomicAdd(&d.cnt->phase_steps[1], (unsigned long long)ws);
     atomicAdd(&d.cnt->searches, (unsigned long long)ws);
   }
 }
@@ -433,6 +437,7 @@ __global__ void __launch_bounds__(E_THREADS, E3_BLOCKS) k_tl_e3a(Dev d) {
   const int ws = __reduce_add_sync(FULL, n_steps), wq = __reduce_add_sync(FULL, n_search);
   if (lane == 0 && ws) {
     atomicAdd(&d.cnt->row_steps, (unsigned long long)ws);
+    atomicAdd(&d.cnt->phase_steps[2], (unsigned long long)ws);
     atomicAdd(&d.cnt->searches, (unsigned long long)wq);
   }
 }
@@ -440,7 +445,7 @@ __global__ void __launch_bounds__(E_THREADS, E3_BLOCKS) k_tl_e3a(Dev d) {
 __global__ void __launch_bounds__(E_THREADS, E3B_BLOCKS) k_tl_e3b(Dev d) {
   const int R = d.n_rows, n_work = d.cnt->n_work;
   const unsigned lane = threadIdx.x & 31;
-  int n_steps = 0, n_val = 0;
+  int n_steps = 0, n_val = 0, n_vhits = 0;
   int w = -1, t = -1, sbase = 0, r = 0, gap = 0, status = 0;
   int32_t* rh = nullptr;
   float z_ref = 0.f;
@@ -463,6 +468,7 @@ __global__ void __launch_bounds__(E_THREADS, E3B_BLOCKS) k_tl_e3b(Dev d) {
           tf1 = make_float4(it, iq, ichi, z_ref);
           W = pack_weight(d, n_hits, ichi, (uint32_t)t);
           n_val++;
+          n_vhits += n_hits;
         }
         reinterpret_cast<int4*>(d.tl_ints)[t] = ti;
         reinterpret_cast<float4*>(d.tl_floats)[2 * t] = tf0;
@@ -524,10 +530,13 @@ __global__ void __launch_bounds__(E_THREADS, E3B_BLOCKS) k_tl_e3b(Dev d) {
     if (r < 0) busy = false;
   }
   const int ws = __reduce_add_sync(FULL, n_steps), wv = __reduce_add_sync(FULL, n_val);
+  const int wh = __reduce_add_sync(FULL, n_vhits);
   if (lane == 0 && (ws || wv)) {
     atomicAdd(&d.cnt->row_steps, (unsigned long long)ws);
+    atomicAdd(&d.cnt->phase_steps[3], (unsigned long long)ws);
     atomicAdd(&d.cnt->searches, (unsigned long long)ws);
     atomicAdd(&d.cnt->n_valid, wv);
+    atomicAdd(&d.cnt->tracklet_hits, (unsigned long long)wh);
   }
 }
 
@@ -565,13 +574,13 @@ void launch_tracklets(const Dev& d, Launch& L) {
   L.count++;
   launch_scan_i32(d.seed_w, &d.cnt->n_start, T, d.scan_tmp, L);
   k_seed_compact<<<(T + 255) / 256, 256, 0, L.st>>>(d);
-  k_tl_e1<<<d.n_sm * E1_BLOCKS, E_THREADS, 0, L.st>>>(d);
+  KTIMED(L, TPCCA_K_TL_E1, (k_tl_e1<<<d.n_sm * E1_BLOCKS, E_THREADS, 0, L.st>>>(d)));
   launch_order_desc(d, 1, d.e_key, &d.cnt->n_work, T, d.e_order, L);
-  k_tl_e2<<<d.n_sm * E2_GRID, E_THREADS, 0, L.st>>>(d);
+  KTIMED(L, TPCCA_K_TL_E2, (k_tl_e2<<<d.n_sm * E2_GRID, E_THREADS, 0, L.st>>>(d)));
   launch_order_desc(d, 2, d.e_key + T, &d.cnt->n_work, T, d.e_order + T, L);
-  k_tl_e3a<<<d.n_sm * E3_GRID, E_THREADS, 0, L.st>>>(d);
+  KTIMED(L, TPCCA_K_TL_E3A, (k_tl_e3a<<<d.n_sm * E3_GRID, E_THREADS, 0, L.st>>>(d)));
   launch_order_desc(d, 3, d.e_key + 2 * (size_t)T, &d.cnt->n_work, T, d.e_order + 2 * (size_t)T, L);
-  k_tl_e3b<<<d.n_sm * E3B_BLOCKS, E_THREADS, 0, L.st>>>(d);
-  k_tracklet_weights<<<d.n_sm * W_GRID, 128, 0, L.st>>>(d);
+  KTIMED(L, TPCCA_K_TL_E3B, (k_tl_e3b<<<d.n_sm * E3B_BLOCKS, E_THREADS, 0, L.st>>>(d)));
+  KTIMED(L, TPCCA_K_WEIGHTS, (k_tracklet_weights<<<d.n_sm * W_GRID, 128, 0, L.st>>>(d)));
   L.count += 6;
 }

@@ -314,3 +314,74 @@ def test_parity_exact_cost_ties(row_x):
 def oracle_links(fr, row_x):
     import oracle
     return oracle.track(fr.clusters, fr.sector_offsets, row_x)
+
+
+def test_pipelined_host_call(row_x):
+    """tpcca_track_host_async / tpcca_wait (two events concurrently on one GPU): two frames in flight on ONE
+    handle and one workspace give, frame by frame, the results of the device-resident call; a third submission without
+    a wait and a wait without a frame are refused."""
+    import torch
+    frs = [synth.generate(synth.config(2, scale=0.2, seed=71)), synth.generate(synth.config(3, scale=0.2, seed=72)),
+           synth.generate(synth.config(4, scale=0.05, seed=73))]
+    nmax = max(f.n for f in frs)
+    t = B.Tracker(row_x, max_clusters=nmax, max_tracklets=max(1024, nmax // 4))
+    ref = []
+    for fr in frs:
+        run_gpu(fr, row_x, t)
+        ref.append((t.assignment(), t.tracks().tobytes()))
+    bufs = []
+    for fr in frs:
+        bufs.append((torch.from_numpy(fr.clusters.view(np.uint8).reshape(-1).copy()).pin_memory(),
+                     torch.empty(16 + 128 * t.max_tracks, dtype=torch.uint8).pin_memory(),
+                     torch.empty(fr.n, dtype=torch.int32).pin_memory()))
+    assert t.lib.tpcca_wait(t.h) == -1 and b"no frame" in t.lib.tpcca_last_error()
+    seq = [0, 1, 2, 0, 1, 2, 2, 0]
+    done = []
+    t.track_host_async(bufs[seq[0]][0], frs[seq[0]].n, frs[seq[0]].sector_offsets, bufs[seq[0]][1], bufs[seq[0]][2])
+    for k in range(1, len(seq) + 1):
+        if k < len(seq):
+            i = seq[k]
+            if seq[k] == seq[k - 1]:  # the same host buffers may not be reused while their frame is in flight
+                t.wait()
+                done.append(k - 1)
+            t.track_host_async(bufs[i][0], frs[i].n, frs[i].sector_offsets, bufs[i][1], bufs[i][2])
+            if k == 1:  # two in flight: a third is refused and changes nothing
+                with pytest.raises(B.TpccaError):
+                    t.track_host_async(bufs[2][0], frs[2].n, frs[2].sector_offsets, bufs[2][1], bufs[2][2])
+        if (k - 1) not in done:
+            t.wait()
+            done.append(k - 1)
+        j = seq[k - 1]
+        nt = int(bufs[j][1][:16].numpy().view(B.HEADER_DTYPE)["n_tracks"][0])
+        assert np.array_equal(bufs[j][2].numpy(), ref[j][0]), k
+        assert bufs[j][1][16:16 + 128 * nt].numpy().tobytes() == ref[j][1], k
+    # the synchronous call still works afterwards and is refused while a frame is in flight
+    t.track_host_async(bufs[0][0], frs[0].n, frs[0].sector_offsets, bufs[0][1], bufs[0][2])
+    with pytest.raises(B.TpccaError):
+        t.track_host(bufs[1][0], frs[1].n, frs[1].sector_offsets, bufs[1][1], bufs[1][2])
+    t.wait()
+    t.track_host(bufs[1][0], frs[1].n, frs[1].sector_offsets, bufs[1][1], bufs[1][2])
+    assert np.array_equal(bufs[1][2].numpy(), ref[1][0])
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_sector_shards_reproduce_the_whole_frame(row_x, world):
+    """one frame tracked as `world` contiguous sector ranges (one handle per range, as one rank per
+    GPU would) equals the whole-frame result once the track ids are offset by the exclusive scan of the per-shard counts."""
+    from paper_1811_11481_b200 import distributed as D
+    fr = synth.generate(synth.config(2, scale=0.3, seed=81))
+    whole = run_gpu(fr, row_x)
+    a_ref, tr_ref = whole.assignment(), whole.tracks()
+    parts, counts = [], []
+    for r in range(world):
+        cl, so, lo = D.shard_frame(fr.clusters, fr.sector_offsets, world, r)
+        t = run_gpu(synth.Frame(cl.copy(), so, fr.truth[lo:lo + len(cl)], fr.track_par, 36, f"shard{r}"), row_x)
+        assert t.header()["status"] == 0
+        parts.append((t.assignment(), t.tracks(), lo))
+        counts.append(len(parts[-1][1]))
+    off = D.track_id_offsets(counts)
+    a = np.full(fr.n, -1, np.int32)
+    for r, (ar, trr, lo) in enumerate(parts):
+        a[lo:lo + len(ar)] = D.globalise_assignment(ar, off[r])
+    assert sum(counts) == len(tr_ref) and np.array_equal(a, a_ref)
+    assert np.concatenate([p[1] for p in parts]).tobytes() == tr_ref.tobytes()
