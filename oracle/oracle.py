@@ -22,6 +22,17 @@ DEFAULT_PARAMS = dict(
 )
 
 
+# DESIGN.md section 12 Table B defaults of the merger (the product keeps its own copy in binding.py)
+DEFAULT_MERGE_PARAMS = dict(merge_chi2_cut=50.0, merge_dz_max=30.0, merge_edge_dist=10.0, merge_row_back=2,
+                            merge_row_fwd=8, fit_reject_cut=30.0, shared_err_scale=2.0, ring=18)
+
+
+class _MergeParams(C.Structure):
+    _fields_ = [("merge_chi2_cut", C.c_float), ("merge_dz_max", C.c_float), ("merge_edge_dist", C.c_float),
+                ("merge_row_back", C.c_int32), ("merge_row_fwd", C.c_int32),
+                ("fit_reject_cut", C.c_float), ("shared_err_scale", C.c_float), ("ring", C.c_int32)]
+
+
 class _Params(C.Structure):
     _fields_ = [
         ("sigma_y", C.c_float), ("sigma_z", C.c_float),
@@ -82,6 +93,15 @@ def _load(opt: str = "-O2"):
             getattr(lib, name).restype = C.c_void_p
             getattr(lib, name).argtypes = [C.c_void_p]
         lib.orc_tracklets.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.orc_merge.restype = C.c_int64
+        lib.orc_merge.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_float, C.POINTER(_Params), C.c_void_p,
+                                  C.POINTER(_MergeParams)]
+        for name in ("orc_merged", "orc_track_merged", "orc_link_next", "orc_shared"):
+            getattr(lib, name).restype = C.c_void_p
+            getattr(lib, name).argtypes = [C.c_void_p]
+        lib.orc_outer.argtypes = [C.c_void_p, C.c_void_p]
+        lib.orc_rotate.restype = C.c_int32
+        lib.orc_rotate.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_int32, C.c_float, C.c_float]
         lib.orc_kf_transport.restype = C.c_int32
         lib.orc_kf_transport.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_float]
         lib.orc_kf_update.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_float]
@@ -117,6 +137,11 @@ class OracleResult:
     assignment: np.ndarray
     tracks: np.ndarray           # TRACK_DTYPE
     track_tracklet: np.ndarray
+    shared: np.ndarray = None        # uint8 per cluster (O6 / B7)
+    outer: np.ndarray = None         # (n_tracks, 21): outer end x, y, z, sinphi, dzds, qpt, cov15 (O8)
+    merged: np.ndarray = None        # TRACK_DTYPE, merged tracks (O10); only with merge=...
+    track_merged: np.ndarray = None  # sector track -> merged track
+    link_next: np.ndarray = None     # sector track -> continuation or -1 (O9)
 
 
 def _arr(ptr, n, dtype):
@@ -127,8 +152,9 @@ def _arr(ptr, n, dtype):
 
 
 def track(clusters: np.ndarray, sector_offsets: np.ndarray, row_x: np.ndarray, bz: float = 0.5,
-          params: dict | None = None, brute: bool = False, opt: str = "-O2") -> OracleResult:
-    """Steps O1-O7 on one frame.  `clusters`: structured (x,y,z f32,row i32); returns input-index-space results."""
+          params: dict | None = None, brute: bool = False, opt: str = "-O2", merge: dict | bool | None = None) -> OracleResult:
+    """Steps O1-O7 on one frame.  `clusters`: structured (x,y,z f32,row i32); returns input-index-space results.
+    merge: True or a dict of DEFAULT_MERGE_PARAMS overrides -> also steps O8-O10 (sector-segment merger + final fit)."""
     lib = _load(opt)
     cl = np.ascontiguousarray(clusters)
     assert cl.dtype.itemsize == 16
@@ -143,7 +169,7 @@ def track(clusters: np.ndarray, sector_offsets: np.ndarray, row_x: np.ndarray, b
         tf = np.zeros((nt, 23), np.float32)
         if nt:
             lib.orc_tracklets(h, ti.ctypes.data, tf.ctypes.data)
-        return OracleResult(
+        res = OracleResult(
             _arr(lib.orc_link_up_raw(h), n, np.int32), _arr(lib.orc_link_down_raw(h), n, np.int32),
             _arr(lib.orc_link_up(h), n, np.int32), _arr(lib.orc_link_down(h), n, np.int32),
             _arr(lib.orc_start_hits(h), nt, np.int32),
@@ -151,6 +177,20 @@ def track(clusters: np.ndarray, sector_offsets: np.ndarray, row_x: np.ndarray, b
             ti, tf,
             _arr(lib.orc_assignment(h), n, np.int32),
             _arr(lib.orc_tracks(h), ntr, TRACK_DTYPE), _arr(lib.orc_track_tracklet(h), ntr, np.int32))
+        res.shared = _arr(lib.orc_shared(h), n, np.uint8)
+        res.outer = np.zeros((ntr, 21), np.float32)
+        if ntr:
+            lib.orc_outer(h, res.outer.ctypes.data)
+        if merge:
+            md = dict(DEFAULT_MERGE_PARAMS)
+            if isinstance(merge, dict):
+                md.update(merge)
+            mp = _MergeParams(**md)
+            nm = lib.orc_merge(h, nr, rx.ctypes.data, bz, C.byref(cp), cl.ctypes.data, C.byref(mp))
+            res.merged = _arr(lib.orc_merged(h), nm, TRACK_DTYPE)
+            res.track_merged = _arr(lib.orc_track_merged(h), ntr, np.int32)
+            res.link_next = _arr(lib.orc_link_next(h), ntr, np.int32)
+        return res
     finally:
         lib.orc_free(h)
 
@@ -161,6 +201,16 @@ def kf_transport(x, p5, cov15, xnew, bz=0.5, max_sinphi=0.95, opt="-O2"):
     p = np.array(p5, np.float32)
     c = np.array(cov15, np.float32)
     ok = lib.orc_kf_transport(xx.ctypes.data, p.ctypes.data, c.ctypes.data, xnew, bz, max_sinphi)
+    return bool(ok), float(xx[0]), p, c
+
+
+def rotate_frame(x, p5, cov15, sgn, tan_half_angle=DEFAULT_PARAMS["tan_half_angle"], bz=0.5, max_sinphi=0.95, opt="-O2"):
+    """Frame change into the next (sgn = +1) or previous (sgn = -1) sector (B3)."""
+    lib = _load(opt)
+    xx = np.array([x], np.float32)
+    p = np.array(p5, np.float32)
+    c = np.array(cov15, np.float32)
+    ok = lib.orc_rotate(xx.ctypes.data, p.ctypes.data, c.ctypes.data, tan_half_angle, sgn, bz, max_sinphi)
     return bool(ok), float(xx[0]), p, c
 
 

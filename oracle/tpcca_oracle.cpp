@@ -182,6 +182,15 @@ struct Result {
   std::vector<int32_t> assignment;
   std::vector<TrackRec> tracks;
   std::vector<int32_t> track_tracklet;
+  // kept for the merger (O8-O10)
+  std::vector<std::vector<int32_t>> track_hits;  // per sector track: input indices, increasing row
+  std::vector<KF> outer;                         // state at the outermost hit after the outward refit pass (z~ relative)
+  std::vector<float> outer_zref;
+  std::vector<uint8_t> shared;                   // per cluster: also collected by the tracklet of another accepted track
+  // merger output
+  std::vector<TrackRec> merged;
+  std::vector<int32_t> track_merged;             // sector track -> merged track
+  std::vector<int32_t> link_next;                // sector track -> sector track it continues into, or -1
 };
 
 struct Sector {
@@ -401,7 +410,7 @@ inline uint64_t pack_weight(const Params& P, int n_hits, float chi2, uint32_t ti
 
 // ---- O7 refit: inward, outward, inward over the track's hits ----
 // hits: input indices in increasing row order.  Returns false if a transport failed.
-bool refit(const Ctx& c, const std::vector<int32_t>& hits, float q0, KF& k, float& z_ref) {
+bool refit(const Ctx& c, const std::vector<int32_t>& hits, float q0, KF& k, float& z_ref, KF* outer = nullptr) {
   const Cl* cl = c.cl;
   const int n = (int)hits.size();
   const Cl& hN = cl[hits[n - 1]];
@@ -418,6 +427,7 @@ bool refit(const Ctx& c, const std::vector<int32_t>& hits, float q0, KF& k, floa
       if (!transport(k, h.x, c.kq, c.P.max_sinphi)) return false;
       update(k, h.y, h.z - z_ref, c.sy2, c.sz2);
     }
+    if (pass == 1 && outer) *outer = k;  // end of the outward pass: the state at the outermost hit (O8)
   }
   return true;
 }
@@ -431,6 +441,185 @@ Ctx make_ctx(const Cl* cl, const float* row_x, int n_rows, const Params& P, floa
   c.inv_sy2 = 1.0f / c.sy2;
   c.inv_sz2 = 1.0f / c.sz2;
   return c;
+}
+
+// ---- O8-O10: sector-segment merger and final fit (PAPER.md:51 second phase; :69-71) ----
+struct MergeParams {
+  float merge_chi2_cut, merge_dz_max, merge_edge_dist;
+  int32_t merge_row_back, merge_row_fwd;
+  float fit_reject_cut, shared_err_scale;
+  int32_t ring;  // sectors per z side that close the ring (18), 0: no neighbours
+};
+
+// Change of the sector frame by sgn * 20 degrees (sgn = +1: into the next sector).  cos / sin of the sector angle come
+// from tan(10 deg) by the double-angle formulas (no libm).  false: |sin(phi)| leaves [-max_sinphi, max_sinphi].
+bool rotate_frame(KF& k, float ca, float ss, float kq, float max_sinphi) {
+  const float s = k.p[2];
+  if (!(std::fabs(s) <= max_sinphi)) return false;
+  const float cphi = std::sqrt(fma32(-s, s, 1.0f));
+  const float s1 = fma32(s, ca, -(cphi * ss));
+  if (!(std::fabs(s1) <= max_sinphi)) return false;
+  const float c1 = std::sqrt(fma32(-s1, s1, 1.0f));
+  // Jacobian of "state on the plane x = const" -> "state on the plane x' = const through the same point":
+  // a shift of y moves the point off the new plane; sliding back along the track gives dy'/dy = cos(phi)/cos(phi'),
+  // dz'/dy = -t sin(a)/cos(phi'), d sin(phi')/dy = -(q kq) sin(a) (the slide changes sin(phi) by the curvature);
+  // d sin(phi')/d sin(phi) = cos(phi')/cos(phi).  F = diag(ry, 1, rr, 1, 1) + rz at (1,0) + rs at (2,0).
+  const float rr = c1 / cphi;
+  const float ry = cphi / c1;
+  const float rz = -((k.p[3] * ss) / c1);
+  const float rs = -((k.p[4] * kq) * ss);
+  const float x = k.x, y = k.p[0];
+  k.x = fma32(y, ss, x * ca);
+  k.p[0] = fma32(y, ca, -(x * ss));
+  k.p[2] = s1;
+  float Cf[5][5], Mx[5][5];
+  for (int i = 0; i < 5; i++)
+    for (int j = 0; j < 5; j++) Cf[i][j] = k.C[tri(i, j)];
+  for (int j = 0; j < 5; j++) {  // M = F C
+    Mx[0][j] = ry * Cf[0][j];
+    Mx[1][j] = fma32(rz, Cf[0][j], Cf[1][j]);
+    Mx[2][j] = fma32(rs, Cf[0][j], rr * Cf[2][j]);
+    Mx[3][j] = Cf[3][j];
+    Mx[4][j] = Cf[4][j];
+  }
+  for (int i = 0; i < 5; i++) {  // C' = M F^T, lower triangle
+    k.C[tri(i, 0)] = Mx[i][0] * ry;
+    if (i >= 1) k.C[tri(i, 1)] = fma32(rz, Mx[i][0], Mx[i][1]);
+    if (i >= 2) k.C[tri(i, 2)] = fma32(rs, Mx[i][0], Mx[i][2] * rr);
+    if (i >= 3) k.C[tri(i, 3)] = Mx[i][3];
+    if (i >= 4) k.C[tri(i, 4)] = Mx[i][4];
+  }
+  return true;
+}
+
+inline int ring_neighbour(int sector, int side, int ring) {  // side = +1 / -1; -1 if there is none
+  if (ring <= 0) return -1;
+  const int base = (sector / ring) * ring, l = sector - base;
+  return base + (l + side + ring) % ring;
+}
+
+void merge_tracks(Result* R, const Ctx& c, const MergeParams& M) {
+  const Cl* cl = c.cl;
+  const Params& P = c.P;
+  const int nt = (int)R->tracks.size();
+  const float th = P.tan_half_angle;
+  const float den = fma32(th, th, 1.0f);
+  const float ca = fma32(-th, th, 1.0f) / den, sa = (2.0f * th) / den;  // cos, sin of the sector angle
+  // O9: best partner of every outer end, best partner of every inner end
+  std::vector<int32_t> best_out(nt, -1), best_in(nt, -1);
+  std::vector<float> chi_out(nt, 0.0f), chi_in(nt, 0.0f);
+  std::vector<std::vector<int32_t>> by_sector(R->n_sectors);  // track ids per sector, increasing
+  for (int t = 0; t < nt; t++) by_sector[R->tracks[t].sector].push_back(t);
+  for (int a = 0; a < nt; a++) {
+    const TrackRec& A = R->tracks[a];
+    if (A.ndf < 0) continue;
+    const KF& oa = R->outer[a];
+    const float za = oa.p[1] + R->outer_zref[a];
+    const int side = oa.p[0] > 0.0f ? 1 : -1;
+    if (!(std::fabs(oa.p[0]) >= fma32(oa.x, th, -M.merge_edge_dist))) continue;
+    const int sb = ring_neighbour(A.sector, side, M.ring);
+    if (sb < 0 || sb >= R->n_sectors) continue;
+    for (int b : by_sector[sb]) {
+      const TrackRec& B = R->tracks[b];
+      if (B.ndf < 0) continue;
+      const int dr = B.first_row - A.last_row;
+      if (dr < -M.merge_row_back || dr > M.merge_row_fwd) continue;
+      if (!(std::fabs(B.z - za) <= M.merge_dz_max)) continue;
+      KF k = oa;
+      k.p[1] = 0.0f;  // z relative to the outer end of A
+      if (!rotate_frame(k, ca, (float)side * sa, c.kq, P.max_sinphi)) continue;
+      if (!transport(k, B.x, c.kq, P.max_sinphi)) continue;
+      const float pb[5] = {B.y, B.z - za, B.sinphi, B.dzds, B.qpt};
+      float chi = 0.0f;
+      for (int i = 0; i < 5; i++) {
+        const float d = k.p[i] - pb[i];
+        const float term = (d * d) / (k.C[tri(i, i)] + B.cov[tri(i, i)]);
+        chi = (i == 0) ? term : chi + term;
+      }
+      if (!(chi <= M.merge_chi2_cut)) continue;
+      if (best_out[a] < 0 || chi < chi_out[a]) { best_out[a] = b; chi_out[a] = chi; }       // equal chi2: lower id of B stays
+      if (best_in[b] < 0 || chi < chi_in[b]) { best_in[b] = a; chi_in[b] = chi; }           // equal chi2: lower id of A stays
+    }
+  }
+  R->link_next.assign(nt, -1);
+  std::vector<int32_t> prev(nt, -1);
+  for (int a = 0; a < nt; a++) {
+    const int b = best_out[a];
+    if (b >= 0 && best_in[b] == a) { R->link_next[a] = b; prev[b] = a; }
+  }
+  // O10: chains from the heads in id order, final three-pass fit with rejection
+  R->track_merged.assign(nt, -1);
+  R->merged.clear();
+  for (int head = 0; head < nt; head++) {
+    if (prev[head] >= 0) continue;
+    const int32_t mid = (int32_t)R->merged.size();
+    std::vector<int32_t> hits, hsec;  // inner -> outer
+    int n_seg = 0, last = head;
+    for (int t = head; t >= 0; t = R->link_next[t]) {
+      R->track_merged[t] = mid;
+      for (int32_t h : R->track_hits[t]) { hits.push_back(h); hsec.push_back(R->tracks[t].sector); }
+      n_seg++; last = t;
+    }
+    const int n = (int)hits.size();
+    TrackRec tr;
+    std::memset(&tr, 0, sizeof(tr));
+    tr.sector = R->tracks[head].sector; tr.first_row = cl[hits.front()].row; tr.last_row = cl[hits.back()].row;
+    tr.n_hits = n;
+    const Cl& hN = cl[hits[n - 1]];
+    const Cl& hM = cl[hits[n - 2]];  // same segment: a sector track has >= 2 hits
+    const float z_ref = hN.z;
+    KF k;
+    {
+      const float dx = hN.x - hM.x, dy = hN.y - hM.y, dz = hN.z - hM.z;
+      const float ds = std::sqrt(fma32(dx, dx, dy * dy));
+      k.x = hN.x;
+      k.p[0] = hN.y; k.p[1] = 0.0f; k.p[2] = dy / ds; k.p[3] = dz / ds; k.p[4] = R->tracks[last].qpt;
+    }
+    bool ok = true;
+    int n_used = 0, n_shared = 0;
+    int cur_sec = hsec[n - 1];
+    for (int pass = 0; pass < 3 && ok; pass++) {
+      reset_cov(k, P);
+      n_used = 0; n_shared = 0;
+      for (int j = 0; j < n && ok; j++) {
+        const int idx = (pass == 1) ? j : n - 1 - j;
+        const Cl& h = cl[hits[idx]];
+        if (hsec[idx] != cur_sec) {  // adjacent sectors by construction of the chain
+          const int sgn = (ring_neighbour(cur_sec, +1, M.ring) == hsec[idx]) ? 1 : -1;
+          if (!rotate_frame(k, ca, (float)sgn * sa, c.kq, P.max_sinphi)) { ok = false; break; }
+          cur_sec = hsec[idx];
+        }
+        if (!transport(k, h.x, c.kq, P.max_sinphi)) { ok = false; break; }
+        const bool sh = R->shared[hits[idx]] != 0;
+        const float ey = sh ? P.sigma_y * M.shared_err_scale : P.sigma_y;
+        const float ez = sh ? P.sigma_z * M.shared_err_scale : P.sigma_z;
+        const float vy = ey * ey, vz = ez * ez;
+        n_shared += sh ? 1 : 0;
+        const float iy = 1.0f / (k.C[0] + vy), iz = 1.0f / (k.C[2] + vz);
+        const float dy = h.y - k.p[0];
+        const float dz = (h.z - z_ref) - k.p[1];
+        const float d = fma32(dz * dz, iz, (dy * dy) * iy);
+        if (!(d <= M.fit_reject_cut)) continue;  // outlier for this pass
+        update(k, h.y, h.z - z_ref, vy, vz);
+        n_used++;
+      }
+    }
+    if (ok) {
+      tr.x = k.x; tr.y = k.p[0]; tr.z = k.p[1] + z_ref; tr.sinphi = k.p[2]; tr.dzds = k.p[3]; tr.qpt = k.p[4];
+      for (int i = 0; i < 15; i++) tr.cov[i] = k.C[i];
+      tr.chi2 = k.chi2;
+      tr.ndf = 2 * n_used - 5;
+    } else {  // a rotation or transport left |sin(phi)| <= max_sinphi: keep the innermost segment's own fit, flagged
+      const TrackRec& H = R->tracks[head];
+      tr.x = H.x; tr.y = H.y; tr.z = H.z; tr.sinphi = H.sinphi; tr.dzds = H.dzds; tr.qpt = H.qpt;
+      for (int i = 0; i < 15; i++) tr.cov[i] = H.cov[i];
+      tr.chi2 = H.chi2;
+      tr.ndf = -1;
+    }
+    tr.pad[0] = n_seg; tr.pad[1] = R->tracks[last].sector; tr.pad[2] = ok ? n - n_used : 0; tr.pad[3] = n_shared;
+    tr.pad[4] = head;
+    R->merged.push_back(tr);
+  }
 }
 
 }  // namespace
@@ -500,8 +689,14 @@ void* orc_track(int32_t n_sectors, int32_t n_rows, const float* row_x, float bz,
     std::memset(&tr, 0, sizeof(tr));
     tr.sector = T.sector; tr.first_row = cl[hits.front()].row; tr.last_row = cl[hits.back()].row;
     tr.n_hits = (int32_t)hits.size();
-    KF k; float z_ref = 0;
-    const bool ok = refit(c, hits, T.p[4], k, z_ref);
+    KF k, ko; float z_ref = 0;
+    ko.x = 0; ko.chi2 = 0;
+    for (int i = 0; i < 5; i++) ko.p[i] = 0;
+    for (int i = 0; i < 15; i++) ko.C[i] = 0;
+    const bool ok = refit(c, hits, T.p[4], k, z_ref, &ko);
+    R->track_hits.push_back(hits);
+    R->outer.push_back(ko);
+    R->outer_zref.push_back(z_ref);
     tr.x = k.x; tr.y = k.p[0]; tr.z = k.p[1] + z_ref; tr.sinphi = k.p[2]; tr.dzds = k.p[3]; tr.qpt = k.p[4];
     for (int i = 0; i < 15; i++) tr.cov[i] = k.C[i];
     tr.chi2 = k.chi2;
@@ -509,7 +704,38 @@ void* orc_track(int32_t n_sectors, int32_t n_rows, const float* row_x, float bz,
     R->tracks.push_back(tr);
     R->track_tracklet.push_back((int32_t)t);
   }
+  // shared clusters (B7): a hit that the tracklet of an accepted track collected but lost to another owner
+  R->shared.assign(n, 0);
+  for (size_t k = 0; k < R->tracks.size(); k++) {
+    const size_t t = (size_t)R->track_tracklet[k];
+    const Tracklet& T = R->tracklets[t];
+    const int32_t* rh = &R->row_hit[t * (size_t)n_rows];
+    for (int r = 0; r < n_rows; r++)
+      if (rh[r] >= 0 && weight[rh[r]] != T.W) R->shared[rh[r]] = 1;
+  }
   return R;
+}
+
+// O8-O10 on a result of orc_track (same clusters, geometry and parameters).  Returns the number of merged tracks.
+int64_t orc_merge(void* r, int32_t n_rows, const float* row_x, float bz, const Params* P, const Cl* cl, const MergeParams* M) {
+  Result* R = (Result*)r;
+  Ctx c = make_ctx(cl, row_x, n_rows, *P, bz, false);
+  merge_tracks(R, c, *M);
+  return (int64_t)R->merged.size();
+}
+const TrackRec* orc_merged(void* r) { return ((Result*)r)->merged.data(); }
+const int32_t* orc_track_merged(void* r) { return ((Result*)r)->track_merged.data(); }
+const int32_t* orc_link_next(void* r) { return ((Result*)r)->link_next.data(); }
+const uint8_t* orc_shared(void* r) { return ((Result*)r)->shared.data(); }
+// outer end of every sector track: x, y, z (absolute), sinphi, dzds, qpt, cov15 (21 floats per track)
+void orc_outer(void* r, float* out21) {
+  Result* R = (Result*)r;
+  for (size_t t = 0; t < R->outer.size(); t++) {
+    float* o = out21 + 21 * t;
+    const KF& k = R->outer[t];
+    o[0] = k.x; o[1] = k.p[0]; o[2] = k.p[1] + R->outer_zref[t]; o[3] = k.p[2]; o[4] = k.p[3]; o[5] = k.p[4];
+    for (int i = 0; i < 15; i++) o[6 + i] = k.C[i];
+  }
 }
 
 void orc_free(void* r) { delete (Result*)r; }
@@ -559,6 +785,20 @@ void orc_kf_update(float* p5, float* cov15, float* chi2, float ym, float zm, flo
   for (int i = 0; i < 5; i++) p5[i] = k.p[i];
   for (int i = 0; i < 15; i++) cov15[i] = k.C[i];
   *chi2 = k.chi2;
+}
+// frame rotation by sgn * (sector angle) for the pins: state6 = x, y, z, sinphi, dzds, qpt
+int32_t orc_rotate(float* x, float* p5, float* cov15, float tan_half_angle, int32_t sgn, float bz, float max_sinphi) {
+  KF k; k.x = *x; k.chi2 = 0;
+  for (int i = 0; i < 5; i++) k.p[i] = p5[i];
+  for (int i = 0; i < 15; i++) k.C[i] = cov15[i];
+  const float th = tan_half_angle;
+  const float den = fma32(th, th, 1.0f);
+  const float ca = fma32(-th, th, 1.0f) / den, sa = (2.0f * th) / den;
+  const bool ok = rotate_frame(k, ca, (float)sgn * sa, -((0.000299792458f * 10.0f) * bz), max_sinphi);
+  *x = k.x;
+  for (int i = 0; i < 5; i++) p5[i] = k.p[i];
+  for (int i = 0; i < 15; i++) cov15[i] = k.C[i];
+  return ok ? 1 : 0;
 }
 // O7 on a free-standing hit list (hits in increasing x).  out: x, y, z, sinphi, dzds, qpt, cov15, chi2 (22 floats)
 int32_t orc_refit_hits(int32_t n, const Cl* hits, float q0, float bz, const Params* P, float* out22) {

@@ -120,3 +120,65 @@ def e3_gap_above_start(row_x):
     y = y.copy()
     y[98] += 0.3
     return mk(rows, y, z, row_x)
+
+
+# ---------------------------------------------------------------- sector-boundary scenarios (merger)
+TAN10 = float(np.tan(np.deg2rad(10.0)))
+
+
+def helix_in_two_sectors(row_x, sector=3, side=+1, par=None, z_shift_b=0.0, drop_rows_b=0, rng=None, n_sectors=36,
+                         drop_rows_a_end=0, extend_a=0, qpt_b=None, copy_a_dz=None):
+    """One float64 helix that leaves `sector` through its +y (side = +1) or -y (side = -1) edge and continues in the
+    neighbouring sector.  The helix is given in the frame of `sector` (A); its continuation is the SAME circle expressed in
+    the neighbour's frame (B): reference point and direction rotated by side * 20 degrees.  Clusters exist on every row
+    where the helix is inside the respective sector (|y| <= x tan 10 deg).  Variations: z_shift_b displaces B's clusters
+    in z; drop_rows_b removes B's first rows; drop_rows_a_end removes A's last rows; extend_a keeps A's clusters on that
+    many rows beyond its edge (the two segments then overlap in rows); qpt_b continues in B with another curvature from
+    the point and direction the helix has on A's last in-sector row; copy_a_dz adds a second copy of A's clusters
+    displaced by that much in z; rng smears (0.1 cm, 0.15 cm).
+    Returns (frame, info) with info = dict(rows_a, rows_b, y_a, z_a, s_a: float64 truth on A's rows, sector_b)."""
+    par = dict(x0=85.0, y0=4.0, z0=25.0, sinphi0=0.12, tanl=0.5, qpt=-1.1, bz=0.5) if par is None else dict(par)
+    if side < 0:
+        par.update(y0=-par["y0"], sinphi0=-par["sinphi0"], qpt=-par["qpt"])
+        qpt_b = None if qpt_b is None else -qpt_b
+    xs = row_x.astype(np.float64)
+    ya, za, sa = helix_points(xs, par["x0"], par["y0"], par["z0"], par["sinphi0"], par["tanl"], par["qpt"], par["bz"])
+    in_a = np.abs(ya) <= xs * TAN10
+    last_in = int(np.flatnonzero(in_a)[-1])
+    a = np.deg2rad(20.0) * side
+    if qpt_b is None:
+        xr, yr, zr, sr, qb = par["x0"], par["y0"], par["z0"], par["sinphi0"], par["qpt"]
+    else:  # same point and direction on A's last in-sector row, other curvature beyond it
+        xr, yr, zr, sr, qb = xs[last_in], ya[last_in], za[last_in], sa[last_in], qpt_b
+    x0b = xr * np.cos(a) + yr * np.sin(a)
+    y0b = -xr * np.sin(a) + yr * np.cos(a)
+    s0b = np.sin(np.arcsin(sr) - a)
+    with np.errstate(invalid="ignore"):
+        yb, zb, sb = helix_points(xs, x0b, y0b, zr, s0b, par["tanl"], qb, par["bz"])
+    in_b = np.isfinite(yb) & (np.abs(sb) < 0.98) & (np.abs(yb) <= xs * TAN10)
+    rows_a = np.flatnonzero(in_a)
+    if extend_a:
+        rows_a = np.arange(rows_a[0], min(len(xs), last_in + 1 + extend_a))
+    if drop_rows_a_end:
+        rows_a = rows_a[:-drop_rows_a_end]
+    rows_b = np.flatnonzero(in_b)[drop_rows_b:]
+    ring = n_sectors // 2
+    base = (sector // ring) * ring
+    sector_b = base + (sector - base + side) % ring
+    ca = mk(rows_a, ya[rows_a], za[rows_a], row_x)
+    cb = mk(rows_b, yb[rows_b], zb[rows_b] + z_shift_b, row_x)
+    if copy_a_dz is not None:
+        c2 = ca.copy()
+        c2["z"] += np.float32(copy_a_dz)
+        ca = np.concatenate([ca, c2])
+    if rng is not None:
+        for c in (ca, cb):
+            c["y"] += rng.normal(0, 0.1, len(c)).astype(np.float32)
+            c["z"] += rng.normal(0, 0.15, len(c)).astype(np.float32)
+    parts = {sector: ca, sector_b: cb}
+    so = np.zeros(n_sectors + 1, np.int32)
+    for s in range(n_sectors):
+        so[s + 1] = so[s] + (len(parts[s]) if s in parts else 0)
+    cl = np.concatenate([parts[s] for s in sorted(parts)])
+    fr = synth.Frame(cl, so, np.full(len(cl), -1, np.int32), np.zeros((0, 8)), n_sectors, "two_sector_helix")
+    return fr, dict(rows_a=rows_a, rows_b=rows_b, y_a=ya, z_a=za, s_a=sa, sector_b=sector_b, par=par)
