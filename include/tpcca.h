@@ -141,7 +141,11 @@ enum tpcca_intermediate {
   TPCCA_TRACKLET_ROW_HITS = 5, /* int32[n_start_hits][n_rows], -1 = no hit (void tracklets: all -1) */
   TPCCA_TRACKLET_INTS = 6,  /* int32[n_start_hits][4]: valid, first_row, last_row, n_hits */
   TPCCA_TRACKLET_FLOATS = 7,/* float[n_start_hits][8]: x, y, z-z_ref, sinphi, dzds, qpt, chi2, z_ref */
-  TPCCA_TRACK_TRACKLET = 8  /* int32[n_tracks]: tracklet id of each track */
+  TPCCA_TRACK_TRACKLET = 8, /* int32[n_tracks]: tracklet id of each track */
+  TPCCA_TRACK_OUTER = 9,    /* float[n_tracks][24]: outer end of each track (state after the outward refit pass):
+                               x, y, z, sinphi, dzds, qpt, cov[15], 3 unused */
+  TPCCA_SHARED = 10,        /* int32[n]: 1 if the cluster was also collected by the tracklet of another accepted track */
+  TPCCA_MERGE_LINK_NEXT = 11 /* int32[n_tracks]: after tpcca_merge, the sector track this one continues into, or -1 */
 };
 /* dst_device: 16-byte aligned, `bytes` long.  The call reads the live counts of the last frame (it synchronises
  * `stream`) and returns TPCCA_ERR_ARGUMENT, writing nothing, if `bytes` is smaller than the table. */
@@ -150,6 +154,32 @@ int tpcca_get_intermediate(tpcca_handle* h, int what, void* dst_device, size_t b
 /* Debugging aid: with on != 0 every tpcca_track on this handle synchronises after each stage and names the stage
  * that faulted in tpcca_last_error().  Off by default; never use it in a timed run. */
 int tpcca_set_debug(tpcca_handle* h, int on);
+
+/* ---- Sector-segment merger and final fit ("The second phase merges the track segments found in the
+ * individual sectors and performs the final track fit with the full Kalman filter"; :69 outlier rejection by predicted
+ * chi2; :70 enlarged errors for shared clusters; :71 three passes, Table B). */
+typedef struct {
+  float merge_chi2_cut;        /* match: sum over the 5 parameters of diff^2 / (var_A + var_B) */
+  float merge_dz_max;          /* cm, |z_B - z_A| between the two ends */
+  float merge_edge_dist;       /* cm, the outer end must lie this close to the sector's side */
+  int32_t merge_row_back, merge_row_fwd; /* first_row(B) - last_row(A) in [-back, fwd] */
+  float fit_reject_cut;        /* 2-dof predicted distance above which a hit is left out of a pass of the final fit */
+  float shared_err_scale;      /* sigma_y, sigma_z multiplier of shared clusters in the final fit */
+  int32_t ring;                /* sectors per z side closing the ring (18); 0: no neighbours, nothing merges */
+} tpcca_merge_params;
+void tpcca_default_merge_params(tpcca_merge_params* p);
+
+/* Merge the sector tracks of the LAST tpcca_track / tpcca_track_host* on this handle and fit the merged tracks; enqueued
+ * on `stream` (the stream of that call, or one ordered after it), returns without waiting.  The out_tracks buffer of that
+ * call must still be valid and unchanged (it is read); everything else lives in the workspace.
+ * out_merged: device, 16-byte aligned, sizeof(tpcca_out_header) + max_tracks * 128 bytes: header {n_tracks = merged
+ *   tracks, n_tracklets = links, n_start_hits = merged fits that failed (ndf = -1), status}, then one tpcca_track_rec per
+ *   merged track in the order of their innermost segments' track ids: sector / first_row / state of the innermost
+ *   segment's frame, last_row of the outermost, n_hits of all segments, pad = {segments, outermost sector, hits rejected
+ *   in the last pass (-1: the fit failed, ndf = -1 and the state is the innermost segment's own fit), shared hits,
+ *   innermost sector-track id}.
+ * out_track_merged: device, max_tracks int32: merged track of every sector track (compose with out_hit_assignment). */
+int tpcca_merge(tpcca_handle* h, const tpcca_merge_params* mp, void* stream, void* out_merged, int32_t* out_track_merged);
 
 /* Per-stage device times, averaged over the tpcca_track calls (at most the last 32) made since profiling
  * was switched on (CUDA events recorded on each call's stream; synchronises those events).  ms: host float[TPCCA_N_STAGES]. */

@@ -616,7 +616,7 @@ void merge_tracks(Result* R, const Ctx& c, const MergeParams& M) {
       tr.chi2 = H.chi2;
       tr.ndf = -1;
     }
-    tr.pad[0] = n_seg; tr.pad[1] = R->tracks[last].sector; tr.pad[2] = ok ? n - n_used : 0; tr.pad[3] = n_shared;
+    tr.pad[0] = n_seg; tr.pad[1] = R->tracks[last].sector; tr.pad[2] = ok ? n - n_used : -1; tr.pad[3] = n_shared;
     tr.pad[4] = head;
     R->merged.push_back(tr);
   }

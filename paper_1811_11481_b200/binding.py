@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SO = os.path.join(_HERE, "libtpcca.so")
 
 LINK_UP_RAW, LINK_DOWN_RAW, LINK_UP, LINK_DOWN, START_HITS, TRACKLET_ROW_HITS, TRACKLET_INTS, TRACKLET_FLOATS, \
-    TRACK_TRACKLET = range(9)
+    TRACK_TRACKLET, TRACK_OUTER, SHARED, MERGE_LINK_NEXT = range(12)
 STAGES = ("grid", "neighbours", "clean_start", "tracklets", "select", "refit")
 KERNELS = ("k_slice_scatter", "k_slice_sort", "k_neighbours", "k_clean", "k_tl_e1", "k_tl_e2", "k_tl_e3a", "k_tl_e3b",
            "k_tracklet_weights", "k_select_own", "k_assign", "k_refit")
@@ -49,6 +49,12 @@ class Params(C.Structure):
     ]
 
 
+class MergeParams(C.Structure):
+    _fields_ = [("merge_chi2_cut", C.c_float), ("merge_dz_max", C.c_float), ("merge_edge_dist", C.c_float),
+                ("merge_row_back", C.c_int32), ("merge_row_fwd", C.c_int32),
+                ("fit_reject_cut", C.c_float), ("shared_err_scale", C.c_float), ("ring", C.c_int32)]
+
+
 _lib = None
 
 
@@ -69,6 +75,9 @@ def load():
             fn = getattr(lib, name)
             fn.restype = C.c_int
             fn.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.tpcca_default_merge_params.argtypes = [C.POINTER(MergeParams)]
+        lib.tpcca_merge.restype = C.c_int
+        lib.tpcca_merge.argtypes = [C.c_void_p, C.POINTER(MergeParams), C.c_void_p, C.c_void_p, C.c_void_p]
         lib.tpcca_wait.restype = C.c_int
         lib.tpcca_wait.argtypes = [C.c_void_p]
         lib.tpcca_get_intermediate.restype = C.c_int
@@ -87,6 +96,12 @@ def load():
         lib.tpcca_free.argtypes = [C.c_void_p]
         _lib = lib
     return _lib
+
+
+def default_merge_params() -> MergeParams:
+    p = MergeParams()
+    load().tpcca_default_merge_params(C.byref(p))
+    return p
 
 
 def default_params() -> Params:
@@ -210,8 +225,10 @@ class Tracker:
         torch = self.torch
         hd = self.header()
         ns, nt = hd["n_start_hits"], hd["n_tracks"]
-        if what <= LINK_DOWN:
+        if what <= LINK_DOWN or what == SHARED:
             shape, dt = (self.n,), torch.int32
+        elif what == TRACK_OUTER:
+            shape, dt = (nt, 24), torch.float32
         elif what == START_HITS:
             shape, dt = (ns,), torch.int32
         elif what == TRACKLET_ROW_HITS:
@@ -226,6 +243,32 @@ class Tracker:
         dst = torch.empty(max(4, numel), dtype=dt, device=self.device)
         self._check(self.lib.tpcca_get_intermediate(self.h, what, dst.data_ptr(), dst.numel() * 4, self._stream()))
         return dst[:numel].reshape(shape).cpu().numpy()
+
+    # ---- sector-segment merger + final fit on the results of the last track() (tpcca_merge)
+    def merge(self, **params):
+        torch = self.torch
+        mp = default_merge_params()
+        for k, v in params.items():
+            if not hasattr(mp, k):
+                raise TypeError(f"unknown merge parameter {k}")
+            setattr(mp, k, v)
+        if getattr(self, "out_merged", None) is None:
+            self.out_merged = torch.empty(16 + 128 * self.max_tracks, dtype=torch.uint8, device=self.device)
+            self.out_track_merged = torch.empty(max(1, self.max_tracks), dtype=torch.int32, device=self.device)
+        self._check(self.lib.tpcca_merge(self.h, C.byref(mp), self._stream(), self.out_merged.data_ptr(),
+                                         self.out_track_merged.data_ptr()))
+
+    def merged_header(self) -> dict:
+        h = self.out_merged[:16].cpu().numpy().view(HEADER_DTYPE)[0]
+        return dict(n_merged=int(h["n_tracks"]), n_links=int(h["n_tracklets"]), n_fit_failed=int(h["n_start_hits"]),
+                    status=int(h["status"]))
+
+    def merged(self) -> np.ndarray:
+        nm = self.merged_header()["n_merged"]
+        return self.out_merged[16:16 + 128 * nm].cpu().numpy().view(TRACK_DTYPE).copy()
+
+    def track_merged(self) -> np.ndarray:
+        return self.out_track_merged[:self.header()["n_tracks"]].cpu().numpy().copy()
 
     def set_debug(self, on: bool):
         self.lib.tpcca_set_debug(self.h, int(on))

@@ -71,7 +71,7 @@ static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params
   CARVE(d.link_up, int32_t, N);
   CARVE(d.link_down, int32_t, N);
   CARVE(d.link_up_clean, int32_t, N);
-  CARVE(d.start_flag, uint8_t, N);
+  CARVE(d.shared_flag, uint8_t, N);
   CARVE(d.hit_weight, unsigned long long, N);
   CARVE(d.start_tmp, int32_t, N);
   CARVE(d.sb_count, int32_t, T + 1);
@@ -79,7 +79,7 @@ static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params
   CARVE(d.sb_skey, int32_t, T);
   CARVE(d.start_hits, int32_t, T);
   CARVE(d.seed_w, int32_t, T + 1);
-  CARVE(d.ord, int32_t, 4 * 1024);
+  CARVE(d.ord, int32_t, 5 * 1024);
   CARVE(d.e_key, int32_t, 3 * T);
   CARVE(d.e_order, int32_t, 3 * T);
   CARVE(d.work_t, int32_t, T);
@@ -97,6 +97,17 @@ static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params
   CARVE(d.w_list, int2, T);
   CARVE(d.th_yz, float2, N);
   CARVE(d.th_row, uint8_t, N);
+  CARVE(d.th_hit, int32_t, N);
+  CARVE(d.th_shared, uint8_t, N);
+  CARVE(d.track_outer, float, K * 24);
+  CARVE(d.m_best_out, unsigned long long, K);
+  CARVE(d.m_best_in, unsigned long long, K);
+  CARVE(d.m_next, int32_t, K);
+  CARVE(d.m_prev, int32_t, K);
+  CARVE(d.m_scan, int32_t, K + 1);
+  CARVE(d.m_head, int32_t, K);
+  CARVE(d.m_len, int32_t, K);
+  CARVE(d.m_order, int32_t, K);
   for (int sl = 0; sl < 2; sl++) {
     CARVE(stage_clusters[sl], float4, N);
     CARVE(stage_assign[sl], int32_t, N);
@@ -134,6 +145,14 @@ void tpcca_default_params(tpcca_params* p) {
   p->pick_cut = 16.0f; p->reject_cut = 25.0f; p->max_gap = 5; p->edge_margin = 3.0f; p->max_sinphi = 0.95f;
   p->min_seed_hits = 4; p->min_tracklet_hits = 10; p->min_track_hits = 10; p->qual_scale = 1000.0f;
   p->grid_bin_y = 6.0f; p->grid_bin_z_min = 2.5f; p->grid_bins_per_cluster = 2.0f;
+}
+
+void tpcca_default_merge_params(tpcca_merge_params* p) {
+  if (!p) return;
+  memset(p, 0, sizeof(*p));
+  p->merge_chi2_cut = 50.0f; p->merge_dz_max = 30.0f; p->merge_edge_dist = 10.0f;
+  p->merge_row_back = 2; p->merge_row_fwd = 8;
+  p->fit_reject_cut = 30.0f; p->shared_err_scale = 2.0f; p->ring = 18;
 }
 
 size_t tpcca_workspace_bytes(const tpcca_geometry* g, const tpcca_params* p) {
@@ -356,9 +375,30 @@ int tpcca_track_host(tpcca_handle* h, const tpcca_cluster* clusters, int64_t n, 
   return rc ? rc : tpcca_wait(h);
 }
 
+int tpcca_merge(tpcca_handle* h, const tpcca_merge_params* mp, void* stream, void* out_merged, int32_t* out_track_merged) {
+  if (!h) { set_err("handle is null (not initialised)"); return TPCCA_ERR_NOT_INIT; }
+  if (!mp || !out_merged || !out_track_merged) { set_err("null merge parameters or output"); return TPCCA_ERR_ARGUMENT; }
+  if (((uintptr_t)out_merged & 15) || ((uintptr_t)out_track_merged & 3)) { set_err("misaligned merge output"); return TPCCA_ERR_ARGUMENT; }
+  if (!h->d.out_hdr) { set_err("tpcca_merge needs a preceding tpcca_track on this handle"); return TPCCA_ERR_ARGUMENT; }
+  if (mp->ring < 0 || mp->merge_row_back < 0 || mp->merge_row_fwd < 0 || !(mp->shared_err_scale > 0)) {
+    set_err("merge parameters out of range"); return TPCCA_ERR_ARGUMENT;
+  }
+  Dev d = h->d;
+  d.MP = *mp;
+  d.merged_hdr = reinterpret_cast<tpcca_out_header*>(out_merged);
+  d.merged_out = reinterpret_cast<tpcca_track_rec*>((char*)out_merged + sizeof(tpcca_out_header));
+  d.track_merged_out = out_track_merged;
+  Launch L{(cudaStream_t)stream, 0, nullptr};
+  launch_merge(d, L);
+  h->launches = L.count;
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) { set_err("merge launch failed: %s", cudaGetErrorString(e)); return TPCCA_ERR_CUDA; }
+  return TPCCA_OK;
+}
+
 int tpcca_get_intermediate(tpcca_handle* h, int what, void* dst, size_t bytes, void* stream) {
   if (!h) { set_err("handle is null (not initialised)"); return TPCCA_ERR_NOT_INIT; }
-  if (!dst || what < 0 || what > TPCCA_TRACK_TRACKLET) { set_err("bad intermediate id or null dst"); return TPCCA_ERR_ARGUMENT; }
+  if (!dst || what < 0 || what > TPCCA_MERGE_LINK_NEXT) { set_err("bad intermediate id or null dst"); return TPCCA_ERR_ARGUMENT; }
   if ((uintptr_t)dst & 15) { set_err("dst must be 16-byte aligned"); return TPCCA_ERR_ARGUMENT; }
   const Dev& d = h->d;
   // the sizes of the tracklet / track tables are data dependent: read the live counters (synchronises `stream`;
@@ -373,6 +413,8 @@ int tpcca_get_intermediate(tpcca_handle* h, int what, void* dst, size_t bytes, v
   else if (what == TPCCA_TRACKLET_ROW_HITS) need = (size_t)c.n_start * d.n_rows * 4;
   else if (what == TPCCA_TRACKLET_INTS) need = (size_t)c.n_start * 16;
   else if (what == TPCCA_TRACKLET_FLOATS) need = (size_t)c.n_start * 32;
+  else if (what == TPCCA_TRACK_OUTER) need = (size_t)c.n_tracks * 96;
+  else if (what == TPCCA_SHARED) need = (size_t)d.n * 4;
   else need = (size_t)c.n_tracks * 4;
   if (bytes < need) { set_err("dst too small%s (need %lld bytes)", "", (long long)need); return TPCCA_ERR_ARGUMENT; }
   Launch L{(cudaStream_t)stream, 0, nullptr};

@@ -30,6 +30,7 @@ struct DevCounters {  // device-resident scalars
   int32_t n_start_raw; // start hits before clamping to capacity
   int32_t n_work;      // seeds that reach the constructor (chain >= min_seed_hits)
   int32_t work_next[4];  // queue heads of the four tracklet-constructor kernels
+  int32_t n_merged, n_links, n_fit_failed, pad0;  // merger (tpcca_merge)
   unsigned long long row_steps, searches, track_hits;  // work counters (roofline units)
   unsigned long long phase_steps[4];   // row steps of k_tl_e1 / e2 / e3a / e3b
   unsigned long long tracklet_hits;    // hits of all valid tracklets (one weight atomic each)
@@ -69,7 +70,7 @@ struct Dev {
   int32_t* link_up;        // [n] sorted index space
   int32_t* link_down;
   int32_t* link_up_clean;
-  uint8_t* start_flag;     // [n]
+  uint8_t* shared_flag;    // [n] sorted index space: collected by the tracklet of an accepted track that does not own it
   int32_t* slice_nstart;   // [n_slices+1]
   int32_t* slice_sbase;    // [n_slices+1]
   int32_t* start_tmp;      // [n] start hits in arrival order
@@ -100,6 +101,22 @@ struct Dev {
   int2* w_list;            // [max_tracklets] w-space, accepted tracklets: (offset, count) of the owned-hit list
   float2* th_yz;           // [n] owned-hit lists (innermost first): (y, z)
   uint8_t* th_row;         // [n] their rows
+  int32_t* th_hit;         // [n] their sorted cluster indices
+  uint8_t* th_shared;      // [n] their shared flags (filled by tpcca_merge)
+  float* track_outer;      // [max_tracks][24] outer end of every track: x, y, z, sinphi, dzds, qpt, cov15 (after refit pass 2)
+  // merger
+  tpcca_merge_params MP;
+  unsigned long long* m_best_out;  // [max_tracks] (chi2 bits << 32 | partner id), ~0 = none
+  unsigned long long* m_best_in;
+  int32_t* m_next;         // [max_tracks] continuation of a sector track or -1
+  int32_t* m_prev;
+  int32_t* m_scan;         // [max_tracks+1] head flag -> exclusive scan = merged id
+  int32_t* m_head;         // [max_tracks] merged id -> head sector track
+  int32_t* m_len;          // [max_tracks] merged id -> total hits (fit work order key)
+  int32_t* m_order;        // [max_tracks] merged ids by decreasing length
+  tpcca_out_header* merged_hdr;
+  tpcca_track_rec* merged_out;
+  int32_t* track_merged_out;
   DevCounters* cnt;
   tpcca_out_header* out_hdr;
   tpcca_track_rec* out_tracks;
@@ -292,6 +309,7 @@ void launch_tracklets(const Dev& d, Launch& L);
 void launch_select(const Dev& d, Launch& L);
 void launch_refit(const Dev& d, Launch& L);
 void launch_export(const Dev& d, int what, void* dst, Launch& L);
+void launch_merge(const Dev& d, Launch& L);
 // exclusive scan of data[0..n) in place, n read from *n_dev (<= n_max); data[n] receives the total
 void launch_scan_i32(int32_t* data, const int32_t* n_dev, int32_t n_max, int32_t* tmp, Launch& L);
 // out[0..n) = indices 0..n-1 ordered by decreasing key[i] (keys in [0,256]; order inside a key is arbitrary);

@@ -144,7 +144,7 @@ void launch_order_desc(const Dev& d, int slot, const int32_t* key, const int32_t
 }
 
 // ---------------------------------------------------------------- (a0) reset per-call state
-#define ORD_SLOTS 4  // counting-sort scratch blocks of Dev::ord (refit, E2, E3a, E3b)
+#define ORD_SLOTS 5  // counting-sort scratch blocks of Dev::ord (refit, E2, E3a, E3b, merged fit)
 __global__ void k_reset(Dev d) {
   const int stride = gridDim.x * blockDim.x;
   for (int i = blockIdx.x * blockDim.x + threadIdx.x; i <= d.n_slices; i += stride) {
@@ -161,6 +161,7 @@ __global__ void k_reset(Dev d) {
   if (blockIdx.x == 0 && threadIdx.x == 0) {
     d.cnt->n_start = 0; d.cnt->n_tracks = 0; d.cnt->n_valid = 0; d.cnt->status = 0; d.cnt->n_bins = 0;
     d.cnt->n_start_raw = 0; d.cnt->n_work = 0;
+    d.cnt->n_merged = 0; d.cnt->n_links = 0; d.cnt->n_fit_failed = 0; d.cnt->pad0 = 0;
     for (int q = 0; q < 4; q++) d.cnt->work_next[q] = 0;
     d.cnt->row_steps = 0ull; d.cnt->searches = 0ull; d.cnt->track_hits = 0ull; d.cnt->tracklet_hits = 0ull;
     for (int q = 0; q < 4; q++) d.cnt->phase_steps[q] = 0ull;

@@ -183,6 +183,7 @@ __global__ void __launch_bounds__(256) k_clean(Dev d) {
     if (u >= 0 && d.link_down[u] != h) u = -1;
     if (dn >= 0 && d.link_up[dn] != h) dn = -1;
     d.link_up_clean[h] = u;
+    d.shared_flag[h] = 0;
     start = (dn < 0) && (u >= 0);
     if (start) atomicAdd(&d.slice_nstart[d.slice_of[h]], 1);
   }

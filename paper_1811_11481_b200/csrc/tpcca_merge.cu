@@ -1,0 +1,290 @@
+// tpcca_merge.cu -- sector-segment merger and final fit (steps O8-O10).
+// PAPER.md:51 "The second phase merges the track segments found in the individual sectors and performs the final track fit
+// with the full Kalman filter"; :69 rejection of outliers by predicted chi2; :70 enlarged errors for shared clusters;
+// :71 inward, outward, inward.  Works on what the last tpcca_track left in the workspace: the track records, the outer
+// ends written by k_refit, the owned-hit lists of k_select_own and the shared-cluster flags.
+#include "tpcca_dev.cuh"
+
+#define M_NONE 0xffffffffffffffffull
+
+struct Rot {  // cos and sin of the sector angle from tan(10 deg) by the double-angle formulas
+  float ca, sa;
+};
+__device__ __forceinline__ Rot sector_rotation(float th) {
+  const float den = fmaf(th, th, 1.0f);
+  Rot r;
+  r.ca = fmaf(-th, th, 1.0f) / den;
+  r.sa = (2.0f * th) / den;
+  return r;
+}
+
+// Frame change by sgn * (sector angle): ss = sgn * sin.  false: |sin(phi)| leaves the allowed range (state unchanged).
+__device__ __forceinline__ bool kf_rotate(KF& k, float ca, float ss, float kq, float max_sinphi) {
+  const float s = k.s;
+  if (!(fabsf(s) <= max_sinphi)) return false;
+  const float cphi = sqrtf(fmaf(-s, s, 1.0f));
+  const float s1 = fmaf(s, ca, -(cphi * ss));
+  if (!(fabsf(s1) <= max_sinphi)) return false;
+  const float c1 = sqrtf(fmaf(-s1, s1, 1.0f));
+  const float rr = c1 / cphi;
+  const float ry = cphi / c1;
+  const float rz = -((k.t * ss) / c1);
+  const float rs = -((k.q * kq) * ss);
+  const float x = k.x, y = k.y;
+  k.x = fmaf(y, ss, x * ca);
+  k.y = fmaf(y, ca, -(x * ss));
+  k.s = s1;
+  // M = F C with F = diag(ry, 1, rr, 1, 1) + rz at (1,0) + rs at (2,0); C' = M F^T
+  const float m00 = ry * k.c00;
+  const float m10 = fmaf(rz, k.c00, k.c10), m11 = fmaf(rz, k.c10, k.c11);
+  const float m20 = fmaf(rs, k.c00, rr * k.c20), m21 = fmaf(rs, k.c10, rr * k.c21), m22 = fmaf(rs, k.c20, rr * k.c22);
+  const float m30 = k.c30, m31 = k.c31, m32 = k.c32;
+  const float m40 = k.c40, m41 = k.c41, m42 = k.c42;
+  k.c00 = m00 * ry;
+  k.c10 = m10 * ry; k.c11 = fmaf(rz, m10, m11);
+  k.c20 = m20 * ry; k.c21 = fmaf(rz, m20, m21); k.c22 = fmaf(rs, m20, m22 * rr);
+  k.c30 = m30 * ry; k.c31 = fmaf(rz, m30, m31); k.c32 = fmaf(rs, m30, m32 * rr);
+  k.c40 = m40 * ry; k.c41 = fmaf(rz, m40, m41); k.c42 = fmaf(rs, m40, m42 * rr);
+  return true;
+}
+
+__device__ __forceinline__ int ring_neighbour(int sector, int side, int ring) {
+  if (ring <= 0) return -1;
+  const int base = (sector / ring) * ring, l = sector - base;
+  return base + (l + side + ring) % ring;
+}
+
+// ---------------------------------------------------------------- (m0) reset, per-sector track ranges, shared flags of the lists
+__global__ void __launch_bounds__(256) k_merge_reset(Dev d, int32_t* __restrict__ sec_begin) {
+  const int nt = d.cnt->n_tracks;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i == 0) { d.cnt->n_merged = 0; d.cnt->n_links = 0; d.cnt->n_fit_failed = 0; }
+  if (i < 1024) d.ord[4 * 1024 + i] = 0;  // counting-sort scratch of the fit order (slot 4)
+  if (i < nt) {
+    d.m_best_out[i] = M_NONE; d.m_best_in[i] = M_NONE;
+    d.m_next[i] = -1; d.m_prev[i] = -1;
+    // track ids are sector ordered (A4): sec_begin[s] = first track of sector s, sec_begin[S] = n_tracks
+    const int s = d.out_tracks[i].sector;
+    const int sp = i ? d.out_tracks[i - 1].sector : -1;
+    for (int q = sp + 1; q <= s; q++) sec_begin[q] = i;
+    if (i == nt - 1)
+      for (int q = s + 1; q <= d.n_sectors; q++) sec_begin[q] = nt;
+  }
+  if (nt == 0 && i <= d.n_sectors) sec_begin[i] = 0;
+}
+
+__global__ void __launch_bounds__(256) k_merge_shared(Dev d) {  // list entry -> shared flag of its cluster
+  const unsigned long long n = d.cnt->track_hits;
+  for (unsigned long long j = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; j < n;
+       j += (unsigned long long)gridDim.x * blockDim.x)
+    d.th_shared[j] = d.shared_flag[d.th_hit[j]];
+}
+
+// ---------------------------------------------------------------- (m1) matching: one warp per outer end
+// The lanes walk the tracks of the neighbouring sector (coalesced reads of first_row and z); a lane whose candidate passes
+// the row and z windows evaluates the match (frame change, transport, chi2).  best_out by a warp reduction, best_in by
+// atomicMin of (chi2 bits << 32 | id): min chi2, then lower id, as DESIGN.md B4 asks.
+__global__ void __launch_bounds__(128) k_merge_match(Dev d, const int32_t* __restrict__ sec_begin) {
+  const int lane = threadIdx.x & 31;
+  const int a = (blockIdx.x * 128 + threadIdx.x) >> 5;
+  if (a >= d.cnt->n_tracks) return;
+  const tpcca_track_rec* tr = d.out_tracks;
+  if (tr[a].ndf < 0) return;
+  const float4* oa = reinterpret_cast<const float4*>(d.track_outer + (size_t)a * 24);
+  const float4 o0 = oa[0];  // x, y, z, sinphi
+  const float th = d.tan_half_angle;
+  if (!(fabsf(o0.y) >= fmaf(o0.x, th, -d.MP.merge_edge_dist))) return;
+  const int side = o0.y > 0.0f ? 1 : -1;
+  const int sb = ring_neighbour(tr[a].sector, side, d.MP.ring);
+  if (sb < 0 || sb >= d.n_sectors) return;
+  const int last_row = tr[a].last_row;
+  const float za = o0.z;
+  const Rot R = sector_rotation(th);
+  unsigned long long best = M_NONE;
+  const int b0 = sec_begin[sb], b1 = sec_begin[sb + 1];
+  for (int bb = b0; bb < b1; bb += 32) {
+    const int b = bb + lane;
+    if (b >= b1) continue;
+    const int4 bi = *reinterpret_cast<const int4*>(&tr[b]);          // sector, first_row, last_row, n_hits
+    const int dr = bi.y - last_row;
+    if (dr < -d.MP.merge_row_back || dr > d.MP.merge_row_fwd) continue;
+    const float4 bp = reinterpret_cast<const float4*>(&tr[b])[1];     // x, y, z, sinphi
+    if (!(fabsf(bp.z - za) <= d.MP.merge_dz_max)) continue;
+    if (tr[b].ndf < 0) continue;
+    KF k;
+    const float4 o1 = oa[1], o2 = oa[2], o3 = oa[3], o4 = oa[4];
+    k.x = o0.x; k.y = o0.y; k.z = 0.0f; k.s = o0.w; k.t = o1.x; k.q = o1.y;
+    k.c00 = o1.z; k.c10 = o1.w; k.c11 = o2.x; k.c20 = o2.y; k.c21 = o2.z; k.c22 = o2.w;
+    k.c30 = o3.x; k.c31 = o3.y; k.c32 = o3.z; k.c33 = o3.w; k.c40 = o4.x; k.c41 = o4.y; k.c42 = o4.z; k.c43 = o4.w;
+    k.c44 = d.track_outer[(size_t)a * 24 + 20];
+    k.chi2 = 0.0f;
+    if (!kf_rotate(k, R.ca, (float)side * R.sa, d.kq, d.P.max_sinphi)) continue;
+    if (!kf_transport(k, bp.x, d.kq, d.P.max_sinphi)) continue;
+    const tpcca_track_rec& B = tr[b];
+    float dd = k.y - B.y;
+    float chi = (dd * dd) / (k.c00 + B.cov[0]);
+    dd = k.z - (B.z - za);
+    chi = chi + (dd * dd) / (k.c11 + B.cov[2]);
+    dd = k.s - B.sinphi;
+    chi = chi + (dd * dd) / (k.c22 + B.cov[5]);
+    dd = k.t - B.dzds;
+    chi = chi + (dd * dd) / (k.c33 + B.cov[9]);
+    dd = k.q - B.qpt;
+    chi = chi + (dd * dd) / (k.c44 + B.cov[14]);
+    if (!(chi <= d.MP.merge_chi2_cut)) continue;
+    const unsigned long long cb = (unsigned long long)__float_as_uint(chi) << 32;  // chi >= +0: bits order like values
+    best = min(best, cb | (unsigned)b);
+    atomicMin(&d.m_best_in[b], cb | (unsigned)a);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const unsigned long long v = __shfl_xor_sync(0xffffffffu, best, o);
+    best = min(best, v);
+  }
+  if (lane == 0) d.m_best_out[a] = best;
+}
+
+// ---------------------------------------------------------------- (m2) mutual links, heads
+__global__ void __launch_bounds__(256) k_merge_link(Dev d) {
+  const int a = blockIdx.x * blockDim.x + threadIdx.x;
+  if (a >= d.cnt->n_tracks) return;
+  const unsigned long long bo = d.m_best_out[a];
+  if (bo == M_NONE) return;
+  const int b = (int)(bo & 0xffffffffull);
+  const unsigned long long bi = d.m_best_in[b];
+  if (bi != M_NONE && (int)(bi & 0xffffffffull) == a) {
+    d.m_next[a] = b;
+    d.m_prev[b] = a;
+    atomicAdd(&d.cnt->n_links, 1);
+  }
+}
+__global__ void __launch_bounds__(256) k_merge_heads(Dev d) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  const int nt = d.cnt->n_tracks;
+  if (t < nt) d.m_scan[t] = d.m_prev[t] < 0 ? 1 : 0;
+}
+// (m3) after the scan: merged id of every head; the head walks its chain (<= 20 segments) and labels the segments
+__global__ void __launch_bounds__(256) k_merge_chains(Dev d) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  const int nt = d.cnt->n_tracks;
+  if (t == 0) d.cnt->n_merged = d.m_scan[nt];
+  if (t >= nt || d.m_prev[t] >= 0) return;
+  const int mid = d.m_scan[t];
+  d.m_head[mid] = t;
+  int len = 0;
+  for (int s = t; s >= 0; s = d.m_next[s]) {
+    d.track_merged_out[s] = mid;
+    len += d.out_tracks[s].n_hits;
+  }
+  d.m_len[mid] = len >> 1;  // work-order key of the fit (0..256 after clamping)
+}
+
+// ---------------------------------------------------------------- (m4) final fit: one lane per merged track, longest first
+#define MERGE_MAX_SEGS 24
+__global__ void __launch_bounds__(64) k_merge_fit(Dev d) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= d.cnt->n_merged) return;
+  const int mid = d.m_order[p];
+  const int head = d.m_head[mid];
+  const tpcca_track_rec* tr = d.out_tracks;
+  int segs[MERGE_MAX_SEGS];
+  int n_seg = 0, n = 0;
+  for (int s = head; s >= 0 && n_seg < MERGE_MAX_SEGS; s = d.m_next[s]) { segs[n_seg++] = s; n += tr[s].n_hits; }
+  const int last = segs[n_seg - 1];
+  const Rot R = sector_rotation(d.tan_half_angle);
+  // start: chord of the two outermost hits of the outermost segment, q/pT of its record
+  const int2 wl_last = d.w_list[d.track_w[last]];
+  const float2 pN = d.th_yz[wl_last.x + wl_last.y - 1], pM = d.th_yz[wl_last.x + wl_last.y - 2];
+  const int rN = d.th_row[wl_last.x + wl_last.y - 1], rM = d.th_row[wl_last.x + wl_last.y - 2];
+  const float z_ref = pN.y;
+  KF k;
+  {
+    const float dx = d.row_x[rN] - d.row_x[rM], dy = pN.x - pM.x, dz = pN.y - pM.y;
+    const float ds = sqrtf(fmaf(dx, dx, dy * dy));
+    k.x = d.row_x[rN];
+    k.y = pN.x; k.z = 0.0f; k.s = dy / ds; k.t = dz / ds; k.q = tr[last].qpt;
+  }
+  const float ey1 = d.P.sigma_y * d.MP.shared_err_scale, ez1 = d.P.sigma_z * d.MP.shared_err_scale;
+  const float vy_sh = ey1 * ey1, vz_sh = ez1 * ez1;
+  bool ok = true;
+  int n_used = 0, n_shared = 0;
+  int cur_sec = tr[last].sector;
+  for (int pass = 0; pass < 3 && ok; pass++) {
+    kf_reset_cov(k, d.P.cov0);
+    n_used = 0; n_shared = 0;
+    for (int si = 0; si < n_seg && ok; si++) {
+      const int seg = (pass == 1) ? segs[si] : segs[n_seg - 1 - si];
+      const int2 wl = d.w_list[d.track_w[seg]];
+      const int sec = tr[seg].sector;
+      if (sec != cur_sec) {  // adjacent sectors by construction of the chain
+        const int sgn = (ring_neighbour(cur_sec, +1, d.MP.ring) == sec) ? 1 : -1;
+        if (!kf_rotate(k, R.ca, (float)sgn * R.sa, d.kq, d.P.max_sinphi)) { ok = false; break; }
+        cur_sec = sec;
+      }
+      for (int i = 0; i < wl.y; i++) {
+        const int j = wl.x + ((pass == 1) ? i : wl.y - 1 - i);
+        const float2 pj = d.th_yz[j];
+        const int r = d.th_row[j];
+        const bool sh = d.th_shared[j] != 0;
+        if (!kf_transport(k, d.row_x[r], d.kq, d.P.max_sinphi)) { ok = false; break; }
+        const float vy = sh ? vy_sh : d.sy2, vz = sh ? vz_sh : d.sz2;
+        n_shared += sh ? 1 : 0;
+        const float iy = 1.0f / (k.c00 + vy), iz = 1.0f / (k.c11 + vz);
+        const float dy = pj.x - k.y;
+        const float dz = (pj.y - z_ref) - k.z;
+        const float dist = fmaf(dz * dz, iz, (dy * dy) * iy);
+        if (!(dist <= d.MP.fit_reject_cut)) continue;  // outlier for this pass
+        kf_update(k, pj.x, pj.y - z_ref, vy, vz);
+        n_used++;
+      }
+    }
+  }
+  tpcca_track_rec o;
+  const tpcca_track_rec H = tr[head];
+  if (ok) {
+    o.x = k.x; o.y = k.y; o.z = k.z + z_ref; o.sinphi = k.s; o.dzds = k.t; o.qpt = k.q;
+    o.cov[0] = k.c00; o.cov[1] = k.c10; o.cov[2] = k.c11; o.cov[3] = k.c20; o.cov[4] = k.c21; o.cov[5] = k.c22;
+    o.cov[6] = k.c30; o.cov[7] = k.c31; o.cov[8] = k.c32; o.cov[9] = k.c33; o.cov[10] = k.c40; o.cov[11] = k.c41;
+    o.cov[12] = k.c42; o.cov[13] = k.c43; o.cov[14] = k.c44;
+    o.chi2 = k.chi2;
+    o.ndf = 2 * n_used - 5;
+  } else {  // keep the innermost segment's own fit, flagged (B6)
+    o = H;
+    o.ndf = -1;
+    atomicAdd(&d.cnt->n_fit_failed, 1);
+  }
+  o.sector = H.sector; o.first_row = H.first_row; o.last_row = tr[last].last_row; o.n_hits = n;
+  o.pad[0] = n_seg; o.pad[1] = tr[last].sector; o.pad[2] = ok ? n - n_used : -1; o.pad[3] = n_shared; o.pad[4] = head;
+  float4* dst = reinterpret_cast<float4*>(&d.merged_out[mid]);
+  const float4* src = reinterpret_cast<const float4*>(&o);
+#pragma unroll
+  for (int i = 0; i < 8; i++) dst[i] = src[i];
+}
+
+__global__ void k_merge_header(Dev d) {
+  tpcca_out_header hd;
+  hd.n_tracks = d.cnt->n_merged; hd.n_tracklets = d.cnt->n_links; hd.n_start_hits = d.cnt->n_fit_failed;
+  hd.status = d.cnt->status;
+  *d.merged_hdr = hd;
+}
+
+void launch_merge(const Dev& d, Launch& L) {
+  const int K = d.max_tracks;
+  if (d.n > 0 && K > 0) {
+    int32_t* sec_begin = d.slice_sbase;  // scratch of the start-hit step, free after it: [n_sectors + 1] needed
+    k_merge_reset<<<(K + 255) / 256 + 1, 256, 0, L.st>>>(d, sec_begin);
+    k_merge_shared<<<d.n_sm * 8, 256, 0, L.st>>>(d);
+    k_merge_match<<<(K + 3) / 4, 128, 0, L.st>>>(d, sec_begin);
+    k_merge_link<<<(K + 255) / 256, 256, 0, L.st>>>(d);
+    k_merge_heads<<<(K + 255) / 256, 256, 0, L.st>>>(d);
+    L.count += 5;
+    launch_scan_i32(d.m_scan, &d.cnt->n_tracks, K, d.scan_tmp, L);
+    k_merge_chains<<<(K + 255) / 256, 256, 0, L.st>>>(d);
+    L.count++;
+    launch_order_desc(d, 4, d.m_len, &d.cnt->n_merged, K, d.m_order, L);
+    k_merge_fit<<<(K + 63) / 64, 64, 0, L.st>>>(d);
+    L.count++;
+  }
+  k_merge_header<<<1, 1, 0, L.st>>>(d);
+  L.count++;
+}

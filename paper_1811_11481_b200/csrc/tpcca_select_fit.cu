@@ -33,6 +33,15 @@ __global__ void __launch_bounds__(SEL_THREADS) k_select_own(Dev d) {
       owned += __popc(mm[c]);
     }
     if (owned < d.P.min_track_hits) continue;
+    // accepted: the hits this tracklet collected but lost to another owner are shared clusters (B7)
+#pragma unroll
+    for (int c = 0; c < SEL_CHUNKS; c++) {
+      const int r = ti.y + 32 * c + (int)lane;
+      if (hh[c] < 0 && r <= ti.z) {
+        const int h = rh[r];
+        if (h >= 0) d.shared_flag[h] = 1;
+      }
+    }
     int off = 0;
     if (lane == 0) off = (int)atomicAdd(&d.cnt->track_hits, (unsigned long long)owned);
     off = __shfl_sync(0xffffffffu, off, 0);
@@ -43,6 +52,7 @@ __global__ void __launch_bounds__(SEL_THREADS) k_select_own(Dev d) {
         const int j = base + __popc(mm[c] & ((1u << lane) - 1u));
         d.th_yz[j] = d.yz[hh[c]];
         d.th_row[j] = (uint8_t)(ti.y + 32 * c + (int)lane);
+        d.th_hit[j] = hh[c];
       }
       base += __popc(mm[c]);
     }
@@ -125,7 +135,7 @@ __global__ void __launch_bounds__(64) k_refit(Dev d) {
     k.x = d.row_x[rN];
     k.y = pN.x; k.z = 0.0f; k.s = dy / ds; k.t = dz / ds; k.q = q0;
   }
-  bool ok = true;
+  bool ok = true, outer_written = false;
   for (int pass = 0; pass < 3 && ok; pass++) {
     kf_reset_cov(k, d.P.cov0);
     for (int i = 0; i < n_hits; i++) {
@@ -135,6 +145,20 @@ __global__ void __launch_bounds__(64) k_refit(Dev d) {
       if (!kf_transport(k, d.row_x[r], d.kq, d.P.max_sinphi)) { ok = false; break; }
       kf_update(k, pj.x, pj.y - z_ref, d.sy2, d.sz2);
     }
+    if (pass == 1 && ok) {  // end of the outward pass: the outer end of the track (O8), kept for tpcca_merge
+      float4* od = reinterpret_cast<float4*>(d.track_outer + (size_t)id * 24);
+      od[0] = make_float4(k.x, k.y, k.z + z_ref, k.s);
+      od[1] = make_float4(k.t, k.q, k.c00, k.c10);
+      od[2] = make_float4(k.c11, k.c20, k.c21, k.c22);
+      od[3] = make_float4(k.c30, k.c31, k.c32, k.c33);
+      od[4] = make_float4(k.c40, k.c41, k.c42, k.c43);
+      od[5] = make_float4(k.c44, 0.f, 0.f, 0.f);
+      outer_written = true;
+    }
+  }
+  if (!outer_written) {  // the refit failed before the outward pass ended: no outer end (the merger skips ndf < 0)
+    float4* od = reinterpret_cast<float4*>(d.track_outer + (size_t)id * 24);
+    for (int i = 0; i < 6; i++) od[i] = make_float4(0.f, 0.f, 0.f, 0.f);
   }
   tpcca_track_rec o;
   o.sector = sector;
@@ -207,9 +231,20 @@ __global__ void k_export_tracklets(Dev d, int what, void* dst) {
     }
   }
 }
-__global__ void k_export_track_tracklet(Dev d, int32_t* dst) {
+__global__ void k_export_track_tracklet(Dev d, int what, int32_t* dst) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < d.cnt->n_tracks) dst[i] = d.track_tracklet[i];
+  if (i >= d.cnt->n_tracks) return;
+  if (what == TPCCA_TRACK_TRACKLET) dst[i] = d.track_tracklet[i];
+  else if (what == TPCCA_MERGE_LINK_NEXT) dst[i] = d.m_next[i];
+  else {
+    const float4* src = reinterpret_cast<const float4*>(d.track_outer + (size_t)i * 24);
+    float4* o = reinterpret_cast<float4*>(dst) + (size_t)i * 6;
+    for (int q = 0; q < 6; q++) o[q] = src[q];
+  }
+}
+__global__ void k_export_shared(Dev d, int32_t* dst) {
+  const int h = blockIdx.x * blockDim.x + threadIdx.x;
+  if (h < d.row_start[d.n_slices]) dst[d.orig_idx[h]] = d.shared_flag[h];
 }
 
 void launch_export(const Dev& d, int what, void* dst, Launch& L) {
@@ -217,8 +252,12 @@ void launch_export(const Dev& d, int what, void* dst, Launch& L) {
     if (d.n <= 0) return;
     k_export_fill<<<(d.n + 255) / 256, 256, 0, L.st>>>(d, (int32_t*)dst);
     k_export_links<<<(d.n + 255) / 256, 256, 0, L.st>>>(d, what, (int32_t*)dst);
-  } else if (what == TPCCA_TRACK_TRACKLET) {
-    if (d.max_tracks > 0) k_export_track_tracklet<<<(d.max_tracks + 255) / 256, 256, 0, L.st>>>(d, (int32_t*)dst);
+  } else if (what == TPCCA_TRACK_TRACKLET || what == TPCCA_MERGE_LINK_NEXT || what == TPCCA_TRACK_OUTER) {
+    if (d.max_tracks > 0) k_export_track_tracklet<<<(d.max_tracks + 255) / 256, 256, 0, L.st>>>(d, what, (int32_t*)dst);
+  } else if (what == TPCCA_SHARED) {
+    if (d.n <= 0) return;
+    k_export_fill<<<(d.n + 255) / 256, 256, 0, L.st>>>(d, (int32_t*)dst);  // ignored clusters: -1
+    k_export_shared<<<(d.n + 255) / 256, 256, 0, L.st>>>(d, (int32_t*)dst);
   } else {
     if (d.max_tracklets > 0) k_export_tracklets<<<(d.max_tracklets + 127) / 128, 128, 0, L.st>>>(d, what, dst);
   }

@@ -22,7 +22,8 @@ def test_exports_every_declared_symbol(lib):
     hdr = open(os.path.join(ROOT, "include", "tpcca.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
     names = set(re.findall(r"\b(tpcca_[a-z_]+)\s*\(", hdr))
-    assert {"tpcca_init", "tpcca_track", "tpcca_free", "tpcca_track_host", "tpcca_get_intermediate"} <= names
+    assert {"tpcca_init", "tpcca_track", "tpcca_free", "tpcca_track_host", "tpcca_get_intermediate", "tpcca_merge",
+            "tpcca_track_host_async", "tpcca_wait", "tpcca_default_merge_params", "tpcca_get_kernel_ms"} <= names
     for n in names:
         assert hasattr(lib, n), n
 
@@ -45,6 +46,14 @@ def test_defaults_equal_oracle_defaults():
             continue
         got = list(p.cov0) if k == "cov0" else getattr(p, k)
         assert np.allclose(got, v, rtol=1e-7), k
+
+
+def test_merge_defaults_equal_oracle_defaults(lib):
+    import oracle
+    mp = binding.default_merge_params()
+    for k, v in oracle.DEFAULT_MERGE_PARAMS.items():
+        assert np.isclose(getattr(mp, k), v), k
+    assert {f[0] for f in binding.MergeParams._fields_} == set(oracle.DEFAULT_MERGE_PARAMS)
 
 
 def test_workspace_bytes_and_argument_checks(lib, row_x):

@@ -290,8 +290,8 @@ def test_merge_invariants(event):
     nh = np.bincount(r.track_merged, weights=r.tracks["n_hits"], minlength=nm)
     assert np.array_equal(nh.astype(int), r.merged["n_hits"])
     assert np.array_equal(np.bincount(r.track_merged, minlength=nm), r.merged["pad"][:, 0])
-    ok = r.merged["ndf"] >= 0
-    assert ok.mean() > 0.85
+    ok = r.merged["pad"][:, 2] >= 0
+    assert ok.mean() > 0.85 and (r.merged["ndf"][~ok] == -1).all()
     assert np.array_equal(r.merged["ndf"][ok], 2 * (r.merged["n_hits"][ok] - r.merged["pad"][ok][:, 2]) - 5)
 
 
