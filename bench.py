@@ -266,6 +266,21 @@ def run_gpu(args):
     kms = trk.kernel_ms()
     trk.set_profiling(0)
 
+    # ---- the step after the path: sector-segment merger + final fit (tpcca_merge), timed on its own
+    trk.track(dev_clusters, n, fr.sector_offsets)
+    trk.merge()
+    torch.cuda.synchronize()
+    m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    m0.record(stream)
+    for _ in range(args.steps):
+        trk.merge()
+    m1.record(stream)
+    torch.cuda.synchronize()
+    merge_ms = m0.elapsed_time(m1) / args.steps
+    mh = trk.merged_header()
+    track_merged = trk.track_merged()
+    dev_assign = trk.assignment()
+
     # ---- end to end through the library's host calls (pinned host buffers, H2D + D2H inside the timed region)
     hc = torch.from_numpy(fr.clusters.view(np.uint8).reshape(-1)).pin_memory()
     outs = [(torch.empty(16 + 128 * trk.max_tracks, dtype=torch.uint8).pin_memory(),
@@ -321,6 +336,15 @@ def run_gpu(args):
         return 0
     gpu_assignment = outs[0][1].numpy()[:n].copy()
     gpu_quality = quality(gpu_assignment, nt, fr)
+    # clone rate per PARTICLE before and after the merger (a particle crossing k sectors gives k sector tracks)
+    from paper_1811_11481_b200 import score
+    one = np.zeros(n, np.int32)
+    q_sec = score.score(dev_assign, fr.truth, one, hd["n_tracks"])
+    am = np.where(dev_assign >= 0, track_merged[np.maximum(dev_assign, 0)], -1) if hd["n_tracks"] else dev_assign
+    q_mrg = score.score(am, fr.truth, one, mh["n_merged"])
+    merge_info = {"ms": merge_ms, "api": "tpcca_merge (after the timed path, not part of `value`)", **mh,
+                  "per_particle": {"sector_tracks": {k: round(float(v), 5) for k, v in q_sec.items()},
+                                   "merged_tracks": {k: round(float(v), 5) for k, v in q_mrg.items()}}}
     # ---- roofline (algorithmic bytes of DESIGN.md section 7 x live device counters)
     peak, peak_src = peaks()
     T = hd["n_start_hits"]
@@ -396,7 +420,7 @@ def run_gpu(args):
                        "n_start_hits": hd["n_start_hits"], "row_steps": stats["row_steps"], "quality": gpu_quality,
                        "l2": "inputs larger than L2 (cluster array %.0f MB, working set > 1 GB)" % (n * 16 / 1e6)
                        if n * 16 > 126e6 else "frame fits the 126 MB L2: a parity-test case, not the bench line",
-                       "parallelism": parallelism, "shard": args.shard},
+                       "parallelism": parallelism, "shard": args.shard, "merge": merge_info},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": pipe_ms / args.steps, "steps": args.steps, "frames_in_flight": 2, "handles": 1,

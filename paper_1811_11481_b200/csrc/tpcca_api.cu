@@ -108,6 +108,7 @@ static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params
   CARVE(d.m_head, int32_t, K);
   CARVE(d.m_len, int32_t, K);
   CARVE(d.m_order, int32_t, K);
+  CARVE(d.m_cand, int2, K);
   for (int sl = 0; sl < 2; sl++) {
     CARVE(stage_clusters[sl], float4, N);
     CARVE(stage_assign[sl], int32_t, N);

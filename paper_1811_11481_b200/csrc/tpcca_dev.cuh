@@ -114,6 +114,7 @@ struct Dev {
   int32_t* m_head;         // [max_tracks] merged id -> head sector track
   int32_t* m_len;          // [max_tracks] merged id -> total hits (fit work order key)
   int32_t* m_order;        // [max_tracks] merged ids by decreasing length
+  int2* m_cand;            // [max_tracks] inner ends bucketed by (sector, first_row): (z bits, track id)
   tpcca_out_header* merged_hdr;
   tpcca_track_rec* merged_out;
   int32_t* track_merged_out;

@@ -54,23 +54,47 @@ __device__ __forceinline__ int ring_neighbour(int sector, int side, int ring) {
   return base + (l + side + ring) % ring;
 }
 
-// ---------------------------------------------------------------- (m0) reset, per-sector track ranges, shared flags of the lists
-__global__ void __launch_bounds__(256) k_merge_reset(Dev d, int32_t* __restrict__ sec_begin) {
+// ---------------------------------------------------------------- (m0) reset, candidate buckets, shared flags of the lists
+// The inner ends are bucketed by (sector, first_row) with a counting sort (histogram -> scan -> scatter), so that the row
+// window of DESIGN.md B2 is ONE contiguous range of the sorted order.  Scratch: the per-slice arrays of the grid and
+// start-hit steps (slice_nstart / slice_sbase / slice_fill), free once tpcca_track is through.
+__global__ void __launch_bounds__(256) k_merge_reset(Dev d) {
   const int nt = d.cnt->n_tracks;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i == 0) { d.cnt->n_merged = 0; d.cnt->n_links = 0; d.cnt->n_fit_failed = 0; }
   if (i < 1024) d.ord[4 * 1024 + i] = 0;  // counting-sort scratch of the fit order (slot 4)
+  if (i <= d.n_slices) d.slice_nstart[i] = 0;
   if (i < nt) {
     d.m_best_out[i] = M_NONE; d.m_best_in[i] = M_NONE;
     d.m_next[i] = -1; d.m_prev[i] = -1;
-    // track ids are sector ordered (A4): sec_begin[s] = first track of sector s, sec_begin[S] = n_tracks
-    const int s = d.out_tracks[i].sector;
-    const int sp = i ? d.out_tracks[i - 1].sector : -1;
-    for (int q = sp + 1; q <= s; q++) sec_begin[q] = i;
-    if (i == nt - 1)
-      for (int q = s + 1; q <= d.n_sectors; q++) sec_begin[q] = nt;
   }
-  if (nt == 0 && i <= d.n_sectors) sec_begin[i] = 0;
+}
+__global__ void __launch_bounds__(256) k_merge_count(Dev d) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= d.cnt->n_tracks) return;
+  const int4 ti = *reinterpret_cast<const int4*>(&d.out_tracks[t]);  // sector, first_row, last_row, n_hits
+  if (d.out_tracks[t].ndf >= 0) atomicAdd(&d.slice_nstart[ti.x * d.n_rows + ti.y], 1);
+}
+__global__ void __launch_bounds__(1024) k_merge_offsets(Dev d) {
+  __shared__ int sm[32];
+  int carry = 0;
+  for (int b0 = 0; b0 < d.n_slices; b0 += 1024) {
+    const int sl = b0 + threadIdx.x;
+    const int v = (sl < d.n_slices) ? d.slice_nstart[sl] : 0;
+    int tot;
+    const int e = block_scan_excl(v, &tot, sm);
+    if (sl < d.n_slices) { d.slice_sbase[sl] = carry + e; d.slice_fill[sl] = carry + e; }
+    carry += tot;
+  }
+  if (threadIdx.x == 0) d.slice_sbase[d.n_slices] = carry;
+}
+__global__ void __launch_bounds__(256) k_merge_scatter(Dev d) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= d.cnt->n_tracks) return;
+  const tpcca_track_rec& T = d.out_tracks[t];
+  if (T.ndf < 0) return;
+  const int pos = atomicAdd(&d.slice_fill[T.sector * d.n_rows + T.first_row], 1);
+  d.m_cand[pos] = make_int2(__float_as_int(T.z), t);  // order inside a bucket is arbitrary: the match takes min (chi2, id)
 }
 
 __global__ void __launch_bounds__(256) k_merge_shared(Dev d) {  // list entry -> shared flag of its cluster
@@ -81,10 +105,10 @@ __global__ void __launch_bounds__(256) k_merge_shared(Dev d) {  // list entry ->
 }
 
 // ---------------------------------------------------------------- (m1) matching: one warp per outer end
-// The lanes walk the tracks of the neighbouring sector (coalesced reads of first_row and z); a lane whose candidate passes
-// the row and z windows evaluates the match (frame change, transport, chi2).  best_out by a warp reduction, best_in by
-// atomicMin of (chi2 bits << 32 | id): min chi2, then lower id, as DESIGN.md B4 asks.
-__global__ void __launch_bounds__(128) k_merge_match(Dev d, const int32_t* __restrict__ sec_begin) {
+// The lanes walk the inner ends of the neighbouring sector inside the row window (one contiguous range of m_cand, read
+// coalesced: z and id); a lane whose candidate passes the z window evaluates the match (frame change, transport, chi2).
+// best_out by a warp reduction, best_in by atomicMin of (chi2 bits << 32 | id): min chi2, then lower id (B4).
+__global__ void __launch_bounds__(128) k_merge_match(Dev d) {
   const int lane = threadIdx.x & 31;
   const int a = (blockIdx.x * 128 + threadIdx.x) >> 5;
   if (a >= d.cnt->n_tracks) return;
@@ -98,19 +122,19 @@ __global__ void __launch_bounds__(128) k_merge_match(Dev d, const int32_t* __res
   const int sb = ring_neighbour(tr[a].sector, side, d.MP.ring);
   if (sb < 0 || sb >= d.n_sectors) return;
   const int last_row = tr[a].last_row;
+  const int r_lo = max(0, last_row - d.MP.merge_row_back), r_hi = min(d.n_rows - 1, last_row + d.MP.merge_row_fwd);
+  if (r_lo > r_hi) return;
   const float za = o0.z;
   const Rot R = sector_rotation(th);
   unsigned long long best = M_NONE;
-  const int b0 = sec_begin[sb], b1 = sec_begin[sb + 1];
+  const int b0 = d.slice_sbase[sb * d.n_rows + r_lo], b1 = d.slice_sbase[sb * d.n_rows + r_hi + 1];
   for (int bb = b0; bb < b1; bb += 32) {
-    const int b = bb + lane;
-    if (b >= b1) continue;
-    const int4 bi = *reinterpret_cast<const int4*>(&tr[b]);          // sector, first_row, last_row, n_hits
-    const int dr = bi.y - last_row;
-    if (dr < -d.MP.merge_row_back || dr > d.MP.merge_row_fwd) continue;
-    const float4 bp = reinterpret_cast<const float4*>(&tr[b])[1];     // x, y, z, sinphi
-    if (!(fabsf(bp.z - za) <= d.MP.merge_dz_max)) continue;
-    if (tr[b].ndf < 0) continue;
+    const int pos = bb + lane;
+    if (pos >= b1) continue;
+    const int2 cz = d.m_cand[pos];
+    if (!(fabsf(__int_as_float(cz.x) - za) <= d.MP.merge_dz_max)) continue;
+    const int b = cz.y;
+    const tpcca_track_rec& B = tr[b];
     KF k;
     const float4 o1 = oa[1], o2 = oa[2], o3 = oa[3], o4 = oa[4];
     k.x = o0.x; k.y = o0.y; k.z = 0.0f; k.s = o0.w; k.t = o1.x; k.q = o1.y;
@@ -119,8 +143,7 @@ __global__ void __launch_bounds__(128) k_merge_match(Dev d, const int32_t* __res
     k.c44 = d.track_outer[(size_t)a * 24 + 20];
     k.chi2 = 0.0f;
     if (!kf_rotate(k, R.ca, (float)side * R.sa, d.kq, d.P.max_sinphi)) continue;
-    if (!kf_transport(k, bp.x, d.kq, d.P.max_sinphi)) continue;
-    const tpcca_track_rec& B = tr[b];
+    if (!kf_transport(k, B.x, d.kq, d.P.max_sinphi)) continue;
     float dd = k.y - B.y;
     float chi = (dd * dd) / (k.c00 + B.cov[0]);
     dd = k.z - (B.z - za);
@@ -271,13 +294,16 @@ __global__ void k_merge_header(Dev d) {
 void launch_merge(const Dev& d, Launch& L) {
   const int K = d.max_tracks;
   if (d.n > 0 && K > 0) {
-    int32_t* sec_begin = d.slice_sbase;  // scratch of the start-hit step, free after it: [n_sectors + 1] needed
-    k_merge_reset<<<(K + 255) / 256 + 1, 256, 0, L.st>>>(d, sec_begin);
+    const int nb = (max(K, d.n_slices + 1) + 255) / 256;
+    k_merge_reset<<<nb, 256, 0, L.st>>>(d);
+    k_merge_count<<<(K + 255) / 256, 256, 0, L.st>>>(d);
+    k_merge_offsets<<<1, 1024, 0, L.st>>>(d);
+    k_merge_scatter<<<(K + 255) / 256, 256, 0, L.st>>>(d);
     k_merge_shared<<<d.n_sm * 8, 256, 0, L.st>>>(d);
-    k_merge_match<<<(K + 3) / 4, 128, 0, L.st>>>(d, sec_begin);
+    k_merge_match<<<(K + 3) / 4, 128, 0, L.st>>>(d);
     k_merge_link<<<(K + 255) / 256, 256, 0, L.st>>>(d);
     k_merge_heads<<<(K + 255) / 256, 256, 0, L.st>>>(d);
-    L.count += 5;
+    L.count += 8;
     launch_scan_i32(d.m_scan, &d.cnt->n_tracks, K, d.scan_tmp, L);
     k_merge_chains<<<(K + 255) / 256, 256, 0, L.st>>>(d);
     L.count++;
