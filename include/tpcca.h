@@ -181,6 +181,19 @@ void tpcca_default_merge_params(tpcca_merge_params* p);
  * out_track_merged: device, max_tracks int32: merged track of every sector track (compose with out_hit_assignment). */
 int tpcca_merge(tpcca_handle* h, const tpcca_merge_params* mp, void* stream, void* out_merged, int32_t* out_track_merged);
 
+/* ---- z / time estimate of the tracks of a time frame ("After the Kalman fit of the initial seed, the
+ * position of closest approach to the beam line is computed and assumed as z-position (and thus time) of the primary
+ * vertex"; :109 refined after the merge; :119 "In case clusters of a fully merged secondary track are outside the real
+ * TPC volume, the track is shifted inside").  For every sector track of the last tpcca_track and,
+ * if out_merged is not NULL, every merged track of the last tpcca_merge: z of the helix at its closest approach to
+ * the beam line (z_dca), the shift that brings all its clusters inside the drift volume of their side
+ * (z_shift = z_dca clamped; side A: 0 <= z - shift <= z_max, side C mirrored), the collision time
+ * t0_us = side * z_shift / vdrift, and the signed transverse distance of closest approach (dca_xy).
+ * out_sector / out_merged: device, max_tracks records of 16 bytes, 16-byte aligned.  Enqueued on `stream`. */
+typedef struct { float z_dca, z_shift, t0_us, dca_xy; } tpcca_time_rec;
+int tpcca_estimate_time(tpcca_handle* h, float vdrift_cm_per_us, float z_max_cm, void* stream,
+                        tpcca_time_rec* out_sector, tpcca_time_rec* out_merged);
+
 /* Per-stage device times, averaged over the tpcca_track calls (at most the last 32) made since profiling
  * was switched on (CUDA events recorded on each call's stream; synchronises those events).  ms: host float[TPCCA_N_STAGES]. */
 enum { TPCCA_STAGE_GRID = 0, TPCCA_STAGE_NEIGHBOURS, TPCCA_STAGE_CLEAN_START, TPCCA_STAGE_TRACKLETS,

@@ -27,6 +27,9 @@ DEFAULT_MERGE_PARAMS = dict(merge_chi2_cut=50.0, merge_dz_max=30.0, merge_edge_d
                             merge_row_fwd=8, fit_reject_cut=30.0, shared_err_scale=2.0, ring=18)
 
 
+DEFAULT_TIME_PARAMS = dict(vdrift=2.58, z_max=250.0)  # cm/us, cm (BASELINE.json config 4; TPC half length)
+
+
 class _MergeParams(C.Structure):
     _fields_ = [("merge_chi2_cut", C.c_float), ("merge_dz_max", C.c_float), ("merge_edge_dist", C.c_float),
                 ("merge_row_back", C.c_int32), ("merge_row_fwd", C.c_int32),
@@ -100,6 +103,9 @@ def _load(opt: str = "-O2"):
             getattr(lib, name).restype = C.c_void_p
             getattr(lib, name).argtypes = [C.c_void_p]
         lib.orc_outer.argtypes = [C.c_void_p, C.c_void_p]
+        lib.orc_time_estimate.argtypes = [C.c_void_p, C.c_int32, C.c_float, C.c_void_p, C.c_float, C.c_float, C.c_void_p]
+        lib.orc_time_estimate_state.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_int32, C.c_float,
+                                                C.c_float, C.c_void_p]
         lib.orc_rotate.restype = C.c_int32
         lib.orc_rotate.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_float, C.c_int32, C.c_float, C.c_float]
         lib.orc_kf_transport.restype = C.c_int32
@@ -142,6 +148,8 @@ class OracleResult:
     merged: np.ndarray = None        # TRACK_DTYPE, merged tracks (O10); only with merge=...
     track_merged: np.ndarray = None  # sector track -> merged track
     link_next: np.ndarray = None     # sector track -> continuation or -1 (O9)
+    time_sector: np.ndarray = None   # (n_tracks, 4): z_dca, z_shift, t0_us, dca_xy (O11); only with time=...
+    time_merged: np.ndarray = None   # (n_merged, 4)
 
 
 def _arr(ptr, n, dtype):
@@ -152,9 +160,11 @@ def _arr(ptr, n, dtype):
 
 
 def track(clusters: np.ndarray, sector_offsets: np.ndarray, row_x: np.ndarray, bz: float = 0.5,
-          params: dict | None = None, brute: bool = False, opt: str = "-O2", merge: dict | bool | None = None) -> OracleResult:
+          params: dict | None = None, brute: bool = False, opt: str = "-O2", merge: dict | bool | None = None,
+          time: dict | bool | None = None) -> OracleResult:
     """Steps O1-O7 on one frame.  `clusters`: structured (x,y,z f32,row i32); returns input-index-space results.
-    merge: True or a dict of DEFAULT_MERGE_PARAMS overrides -> also steps O8-O10 (sector-segment merger + final fit)."""
+    merge: True or a dict of DEFAULT_MERGE_PARAMS overrides -> also steps O8-O10 (sector-segment merger + final fit).
+    time: True or dict(vdrift=..., z_max=...) -> also O11 (z / time estimate) for the sector and, with merge, merged tracks."""
     lib = _load(opt)
     cl = np.ascontiguousarray(clusters)
     assert cl.dtype.itemsize == 16
@@ -190,6 +200,17 @@ def track(clusters: np.ndarray, sector_offsets: np.ndarray, row_x: np.ndarray, b
             res.merged = _arr(lib.orc_merged(h), nm, TRACK_DTYPE)
             res.track_merged = _arr(lib.orc_track_merged(h), ntr, np.int32)
             res.link_next = _arr(lib.orc_link_next(h), ntr, np.int32)
+        if time:
+            td = dict(DEFAULT_TIME_PARAMS)
+            if isinstance(time, dict):
+                td.update(time)
+            res.time_sector = np.zeros((ntr, 4), np.float32)
+            if ntr:
+                lib.orc_time_estimate(h, 0, bz, cl.ctypes.data, td["vdrift"], td["z_max"], res.time_sector.ctypes.data)
+            if merge:
+                res.time_merged = np.zeros((len(res.merged), 4), np.float32)
+                if len(res.merged):
+                    lib.orc_time_estimate(h, 1, bz, cl.ctypes.data, td["vdrift"], td["z_max"], res.time_merged.ctypes.data)
         return res
     finally:
         lib.orc_free(h)
@@ -212,6 +233,15 @@ def rotate_frame(x, p5, cov15, sgn, tan_half_angle=DEFAULT_PARAMS["tan_half_angl
     c = np.array(cov15, np.float32)
     ok = lib.orc_rotate(xx.ctypes.data, p.ctypes.data, c.ctypes.data, tan_half_angle, sgn, bz, max_sinphi)
     return bool(ok), float(xx[0]), p, c
+
+
+def time_estimate_state(state6, zmin_hits, zmax_hits, side, bz=0.5, vdrift=2.58, z_max=250.0, opt="-O2"):
+    """O11 on one state (x, y, z, sinphi, dzds, qpt): returns (z_dca, z_shift, t0_us, dca_xy)."""
+    lib = _load(opt)
+    st = np.array(state6, np.float32)
+    out = np.zeros(4, np.float32)
+    lib.orc_time_estimate_state(st.ctypes.data, bz, zmin_hits, zmax_hits, side, vdrift, z_max, out.ctypes.data)
+    return out
 
 
 def kf_update(p5, cov15, chi2, ym, zm, sy2, sz2, opt="-O2"):

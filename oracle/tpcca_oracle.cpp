@@ -622,6 +622,38 @@ void merge_tracks(Result* R, const Ctx& c, const MergeParams& M) {
   }
 }
 
+// ---- O11: z / time estimate of a track in a time frame ----
+// Plain definition in double precision from the fp32 track record: the point of closest approach of the helix to the
+// beam line (x = y = 0 in every sector frame), its z, and the shift that brings the track's clusters inside the drift volume.
+struct TimeRec { float z_dca, z_shift, t0_us, dca_xy; };
+
+TimeRec time_estimate(const TrackRec& T, double kq, double zmin_hits, double zmax_hits, int side, double vdrift, double z_max) {
+  const double x = T.x, y = T.y, s = T.sinphi, c = std::sqrt(1.0 - s * s), k = (double)T.qpt * kq;
+  double ds, dca;  // path length from the state to the closest approach (negative: behind), signed distance there
+  if (std::fabs(k) < 1e-12) {
+    ds = -(c * x + s * y);
+    dca = y * c - x * s;
+  } else {
+    const double R = 1.0 / std::fabs(k), sg = k > 0 ? 1.0 : -1.0;
+    const double xc = x - s / k, yc = y + c / k;          // circle centre: left of the direction by 1/k
+    const double Rc = std::sqrt(xc * xc + yc * yc);
+    // turning angle from the state to the point of the circle nearest to the origin (on the line origin -> centre)
+    const double dphi = std::atan2(-sg * (c * x + s * y), R - sg * (s * x - c * y));
+    ds = dphi / k;
+    dca = sg * (Rc - R);  // same sign convention as the straight line: the state's offset along its left normal
+  }
+  TimeRec o;
+  const double zd = (double)T.z + (double)T.dzds * ds;
+  // shift so that the clusters lie inside the drift volume of their side: A: 0 <= z - shift <= z_max, C: -z_max <= z - shift <= 0
+  const double lo = side > 0 ? zmax_hits - z_max : zmax_hits;
+  const double hi = side > 0 ? zmin_hits : zmin_hits + z_max;
+  double sh = zd;
+  if (sh > hi) sh = hi;
+  if (sh < lo) sh = lo;
+  o.z_dca = (float)zd; o.z_shift = (float)sh; o.t0_us = (float)((double)side * sh / vdrift); o.dca_xy = (float)dca;
+  return o;
+}
+
 }  // namespace
 
 extern "C" {
@@ -736,6 +768,32 @@ void orc_outer(void* r, float* out21) {
     o[0] = k.x; o[1] = k.p[0]; o[2] = k.p[1] + R->outer_zref[t]; o[3] = k.p[2]; o[4] = k.p[3]; o[5] = k.p[4];
     for (int i = 0; i < 15; i++) o[6 + i] = k.C[i];
   }
+}
+
+// O11 for every sector track (merged = 0) or merged track (merged = 1) of a result.  out: 4 floats per track.
+void orc_time_estimate(void* r, int32_t merged, float bz, const Cl* cl, float vdrift, float z_max, float* out4) {
+  Result* R = (Result*)r;
+  const double kq = -((0.000299792458 * 10.0) * (double)bz);
+  const int half = R->n_sectors / 2;
+  const size_t n = merged ? R->merged.size() : R->tracks.size();
+  for (size_t i = 0; i < n; i++) {
+    const TrackRec& T = merged ? R->merged[i] : R->tracks[i];
+    double zmin = 1e300, zmax = -1e300;
+    for (int t = merged ? T.pad[4] : (int)i; t >= 0; t = merged ? R->link_next[t] : -1)
+      for (int32_t h : R->track_hits[t]) { zmin = std::min(zmin, (double)cl[h].z); zmax = std::max(zmax, (double)cl[h].z); }
+    const int side = (half > 0 && T.sector >= half) ? -1 : 1;
+    const TimeRec o = time_estimate(T, kq, zmin, zmax, side, vdrift, z_max);
+    out4[4 * i + 0] = o.z_dca; out4[4 * i + 1] = o.z_shift; out4[4 * i + 2] = o.t0_us; out4[4 * i + 3] = o.dca_xy;
+  }
+}
+// O11 on a free-standing state (pins): state6 = x, y, z, sinphi, dzds, qpt
+void orc_time_estimate_state(const float* state6, float bz, float zmin_hits, float zmax_hits, int32_t side, float vdrift,
+                             float z_max, float* out4) {
+  TrackRec T;
+  std::memset(&T, 0, sizeof(T));
+  T.x = state6[0]; T.y = state6[1]; T.z = state6[2]; T.sinphi = state6[3]; T.dzds = state6[4]; T.qpt = state6[5];
+  const TimeRec o = time_estimate(T, -((0.000299792458 * 10.0) * (double)bz), zmin_hits, zmax_hits, side, vdrift, z_max);
+  out4[0] = o.z_dca; out4[1] = o.z_shift; out4[2] = o.t0_us; out4[3] = o.dca_xy;
 }
 
 void orc_free(void* r) { delete (Result*)r; }

@@ -78,6 +78,8 @@ def load():
         lib.tpcca_default_merge_params.argtypes = [C.POINTER(MergeParams)]
         lib.tpcca_merge.restype = C.c_int
         lib.tpcca_merge.argtypes = [C.c_void_p, C.POINTER(MergeParams), C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.tpcca_estimate_time.restype = C.c_int
+        lib.tpcca_estimate_time.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
         lib.tpcca_wait.restype = C.c_int
         lib.tpcca_wait.argtypes = [C.c_void_p]
         lib.tpcca_get_intermediate.restype = C.c_int
@@ -269,6 +271,20 @@ class Tracker:
 
     def track_merged(self) -> np.ndarray:
         return self.out_track_merged[:self.header()["n_tracks"]].cpu().numpy().copy()
+
+    def estimate_time(self, vdrift: float = 2.58, z_max: float = 250.0, merged: bool = True):
+        """tpcca_estimate_time: (n_tracks, 4) and, after merge(), (n_merged, 4) arrays of z_dca, z_shift, t0_us, dca_xy."""
+        torch = self.torch
+        ts = torch.empty(4 * max(1, self.max_tracks), dtype=torch.float32, device=self.device)
+        tm = torch.empty(4 * max(1, self.max_tracks), dtype=torch.float32, device=self.device) if merged else None
+        self._check(self.lib.tpcca_estimate_time(self.h, vdrift, z_max, self._stream(), ts.data_ptr(),
+                                                 tm.data_ptr() if merged else None))
+        nt = self.header()["n_tracks"]
+        out_s = ts[:4 * nt].reshape(nt, 4).cpu().numpy()
+        if not merged:
+            return out_s, None
+        nm = self.merged_header()["n_merged"]
+        return out_s, tm[:4 * nm].reshape(nm, 4).cpu().numpy()
 
     def set_debug(self, on: bool):
         self.lib.tpcca_set_debug(self.h, int(on))

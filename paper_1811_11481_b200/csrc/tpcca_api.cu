@@ -25,6 +25,8 @@ struct tpcca_handle {
   cudaStream_t st_in, st_out, st_rec;
   cudaEvent_t ev_in[2], ev_k[2], ev_out[2];
   struct Pending { bool busy; int64_t n; void* out_tracks; } pend[2];
+  // last tpcca_merge (for tpcca_estimate_time)
+  void* last_merged;
   uint64_t seq_submit, seq_wait;
   // last call
   int64_t last_n;
@@ -250,6 +252,7 @@ static int track_impl(tpcca_handle* h, const tpcca_cluster* clusters, int64_t n,
   d.out_assign = out_assign;
   h->d.n = d.n; h->d.clusters = d.clusters; h->d.out_hdr = d.out_hdr; h->d.out_tracks = d.out_tracks; h->d.out_assign = out_assign;
   h->last_n = n;
+  h->last_merged = nullptr;  // a new frame: the merged tracks of the previous one are gone
   const bool prof = h->profiling;
   cudaEvent_t* ev = h->ev[h->prof_calls % PROF_RING];
   // tpcca_set_debug(h, 1): synchronise after every stage and name the stage that faulted (debugging aid)
@@ -392,8 +395,25 @@ int tpcca_merge(tpcca_handle* h, const tpcca_merge_params* mp, void* stream, voi
   Launch L{(cudaStream_t)stream, 0, nullptr};
   launch_merge(d, L);
   h->launches = L.count;
+  h->last_merged = out_merged;
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) { set_err("merge launch failed: %s", cudaGetErrorString(e)); return TPCCA_ERR_CUDA; }
+  return TPCCA_OK;
+}
+
+int tpcca_estimate_time(tpcca_handle* h, float vdrift, float z_max, void* stream, tpcca_time_rec* out_sector,
+                        tpcca_time_rec* out_merged) {
+  if (!h) { set_err("handle is null (not initialised)"); return TPCCA_ERR_NOT_INIT; }
+  if (!h->d.out_hdr) { set_err("tpcca_estimate_time needs a preceding tpcca_track on this handle"); return TPCCA_ERR_ARGUMENT; }
+  if ((!out_sector && !out_merged) || !(vdrift > 0) || !(z_max > 0)) { set_err("null outputs or bad drift parameters"); return TPCCA_ERR_ARGUMENT; }
+  if (((uintptr_t)out_sector & 15) || ((uintptr_t)out_merged & 15)) { set_err("misaligned output"); return TPCCA_ERR_ARGUMENT; }
+  if (out_merged && !h->last_merged) { set_err("merged estimates need a tpcca_merge after the last tpcca_track"); return TPCCA_ERR_ARGUMENT; }
+  Dev d = h->d;
+  if (out_merged) d.merged_out = reinterpret_cast<tpcca_track_rec*>((char*)h->last_merged + sizeof(tpcca_out_header));
+  Launch L{(cudaStream_t)stream, 0, nullptr};
+  launch_time_estimate(d, vdrift, z_max, out_sector, out_merged, L);
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) { set_err("time estimate launch failed: %s", cudaGetErrorString(e)); return TPCCA_ERR_CUDA; }
   return TPCCA_OK;
 }
 

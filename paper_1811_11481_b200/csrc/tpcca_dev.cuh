@@ -311,6 +311,8 @@ void launch_select(const Dev& d, Launch& L);
 void launch_refit(const Dev& d, Launch& L);
 void launch_export(const Dev& d, int what, void* dst, Launch& L);
 void launch_merge(const Dev& d, Launch& L);
+void launch_time_estimate(const Dev& d, float vdrift, float z_max, tpcca_time_rec* out_sector, tpcca_time_rec* out_merged,
+                          Launch& L);
 // exclusive scan of data[0..n) in place, n read from *n_dev (<= n_max); data[n] receives the total
 void launch_scan_i32(int32_t* data, const int32_t* n_dev, int32_t n_max, int32_t* tmp, Launch& L);
 // out[0..n) = indices 0..n-1 ordered by decreasing key[i] (keys in [0,256]; order inside a key is arbitrary);

@@ -314,3 +314,60 @@ void launch_merge(const Dev& d, Launch& L) {
   k_merge_header<<<1, 1, 0, L.st>>>(d);
   L.count++;
 }
+
+// ---------------------------------------------------------------- z / time estimate (step O11)
+// The helix of a fitted state is a circle in the xy plane (centre left of the direction by 1/k, k = q kq); the point of
+// the circle nearest to the beam line lies on the line origin -> centre.  Turning angle from the state to that point:
+// atan2(-sg (c x + s y), R - sg (s x - c y)) (no cancellation for stiff tracks), path length = angle / k.
+__device__ __forceinline__ tpcca_time_rec time_estimate(const tpcca_track_rec& T, float kq, float zmin_hits, float zmax_hits,
+                                                        int side, float vdrift, float z_max) {
+  const float x = T.x, y = T.y, s = T.sinphi, c = sqrtf(1.0f - s * s), k = T.qpt * kq;
+  float ds, dca;
+  if (fabsf(k) < 1e-9f) {
+    ds = -(c * x + s * y);
+    dca = y * c - x * s;
+  } else {
+    const float R = 1.0f / fabsf(k), sg = k > 0.0f ? 1.0f : -1.0f;
+    const float dphi = atan2f(-sg * (c * x + s * y), R - sg * (s * x - c * y));
+    ds = dphi / k;
+    const float xc = x - s / k, yc = y + c / k;
+    const float Rc = sqrtf(xc * xc + yc * yc);
+    dca = sg * ((x * x + y * y + 2.0f * sg * R * (y * c - x * s)) / (Rc + R));  // sg (Rc - R) without the cancellation
+  }
+  tpcca_time_rec o;
+  const float zd = T.z + T.dzds * ds;
+  const float lo = side > 0 ? zmax_hits - z_max : zmax_hits;
+  const float hi = side > 0 ? zmin_hits : zmin_hits + z_max;
+  float sh = zd;
+  if (sh > hi) sh = hi;
+  if (sh < lo) sh = lo;
+  o.z_dca = zd; o.z_shift = sh; o.t0_us = (float)side * sh / vdrift; o.dca_xy = dca;
+  return o;
+}
+
+__global__ void __launch_bounds__(128) k_time_estimate(Dev d, int merged, float vdrift, float z_max,
+                                                        tpcca_time_rec* __restrict__ out) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  const int n = merged ? d.cnt->n_merged : d.cnt->n_tracks;
+  if (i >= n) return;
+  const tpcca_track_rec T = merged ? d.merged_out[i] : d.out_tracks[i];
+  float zmin = 3.0e38f, zmax = -3.0e38f;
+  for (int t = merged ? T.pad[4] : i; t >= 0; t = merged ? d.m_next[t] : -1) {
+    const int2 wl = d.w_list[d.track_w[t]];
+    for (int j = 0; j < wl.y; j++) {
+      const float z = d.th_yz[wl.x + j].y;
+      zmin = fminf(zmin, z); zmax = fmaxf(zmax, z);
+    }
+  }
+  const int half = d.n_sectors / 2;
+  const int side = (half > 0 && T.sector >= half) ? -1 : 1;
+  out[i] = time_estimate(T, d.kq, zmin, zmax, side, vdrift, z_max);
+}
+
+void launch_time_estimate(const Dev& d, float vdrift, float z_max, tpcca_time_rec* out_sector, tpcca_time_rec* out_merged,
+                          Launch& L) {
+  if (d.n <= 0 || d.max_tracks <= 0) return;
+  const int nb = (d.max_tracks + 127) / 128;
+  if (out_sector) { k_time_estimate<<<nb, 128, 0, L.st>>>(d, 0, vdrift, z_max, out_sector); L.count++; }
+  if (out_merged) { k_time_estimate<<<nb, 128, 0, L.st>>>(d, 1, vdrift, z_max, out_merged); L.count++; }
+}
