@@ -10,12 +10,12 @@
 #define TPCCA_MAX_SECTORS 64
 #define TPCCA_MAX_ROWS 256
 
-struct GridHdr {  // 32 B per (sector,row) slice
+struct __align__(16) GridHdr {  // 32 B per (sector,row) slice (read as two 16-byte words)
   float ymin, zmin, inv_by, inv_bz;
   int32_t ny, nz, bin_base, pad;  // pad = clusters in the slice
 };
 
-struct NbrHdr {  // 32 B per slice: the per-row constants of the neighbours finder (O2)
+struct __align__(16) NbrHdr {  // 32 B per slice: the per-row constants of the neighbours finder (O2)
   int32_t su, sd;  // slices of the up / down row, -1 if none
   float t, wyu, wzu, wyd, wzd;
   int32_t pad;
@@ -259,6 +259,15 @@ __device__ __forceinline__ void bin_range(float lo, float hi, float vmin, float 
   b0 = (f0 > 0.0f) ? ((f0 < (float)nb) ? (int)f0 : nb - 1) : 0;
   b1 = (f1 >= 0.0f) ? ((f1 < (float)nb) ? (int)f1 : nb - 1) : -1;  // -1 => empty range
   if (!(lo <= hi)) { b0 = 1; b1 = 0; }                             // NaN window: nothing
+}
+
+// Conservative bin range with the clamps done in the float domain (any superset of the window is a valid search
+// structure, O1): b0 = bin of lo clamped to [0, nb-1]; b1 = bin of hi clamped to nb-1, or -1 below the grid.
+__device__ __forceinline__ void bin_range_fast(float lo, float hi, float vmin, float inv_b, int nb, int& b0, int& b1) {
+  const float top = (float)(nb - 1);
+  const float f0 = (lo - vmin) * inv_b, f1 = (hi - vmin) * inv_b;
+  b0 = (int)fminf(fmaxf(f0, 0.0f), top);            // NaN -> 0
+  b1 = (f1 >= 0.0f) ? (int)fminf(f1, top) : -1;      // NaN -> -1 (empty)
 }
 
 // exclusive block scan; every thread receives the block total.  smem: >= 32 ints.

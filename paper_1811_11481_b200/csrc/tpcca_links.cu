@@ -46,12 +46,13 @@ __device__ __forceinline__ void consider(const Dev& d, Best& b, float cost, int 
 }
 
 // Window candidates of one neighbour row: appended to the calling thread's shared-memory list; returns their number
-// (entries beyond NB_CAP are counted, not stored).
+// (entries beyond NB_CAP are counted, not stored).  The bins of up to two y-bin rows form one flat index space
+// [0, ntot): index i < na is cluster a0 + i, the others b0 + (i - na); the body is predicated, not branched.
 __device__ __forceinline__ int collect(const Dev& d, const GridHdr& g, float y0, float z0, float wy, float wz, float mz,
                                        float2* __restrict__ lp, int* __restrict__ li) {
   int by0, by1, bz0, bz1;
-  bin_range(y0 - wy - 1e-3f, y0 + wy + 1e-3f, g.ymin, g.inv_by, g.ny, by0, by1);
-  bin_range(z0 - wz - mz, z0 + wz + mz, g.zmin, g.inv_bz, g.nz, bz0, bz1);
+  bin_range_fast(y0 - wy - 1e-3f, y0 + wy + 1e-3f, g.ymin, g.inv_by, g.ny, by0, by1);
+  bin_range_fast(z0 - wz - mz, z0 + wz + mz, g.zmin, g.inv_bz, g.nz, bz0, bz1);
   if (bz0 > bz1) return 0;
   int n = 0;
   for (int by = by0; by <= by1; by += 2) {
@@ -60,21 +61,25 @@ __device__ __forceinline__ int collect(const Dev& d, const GridHdr& g, float y0,
     int b0 = 0, b1 = 0;
     if (by + 1 <= by1) { b0 = bs[g.nz + bz0]; b1 = bs[g.nz + bz1 + 1]; }
     const int na = a1 - a0, ntot = na + (b1 - b0);
+    const int jump = b0 - a1;  // index i >= na is cluster a0 + i + jump
     for (int i = 0; i < ntot; i += NB_UNROLL) {
       float2 p[NB_UNROLL];
       int c[NB_UNROLL];
 #pragma unroll
       for (int j = 0; j < NB_UNROLL; j++) {
         const int ii = min(i + j, ntot - 1);
-        c[j] = (ii < na) ? a0 + ii : b0 + (ii - na);
+        c[j] = a0 + ii + ((ii >= na) ? jump : 0);
         p[j] = d.yz[c[j]];
       }
 #pragma unroll
       for (int j = 0; j < NB_UNROLL; j++) {
-        if ((i + j < ntot) && (fabsf(p[j].x - y0) <= wy) && (fabsf(p[j].y - z0) <= wz)) {
-          if (n < NB_CAP) { lp[n * NB_THREADS] = p[j]; li[n * NB_THREADS] = c[j]; }
-          n++;
+        const bool in = (i + j < ntot) && (fabsf(p[j].x - y0) <= wy) && (fabsf(p[j].y - z0) <= wz);
+        if (in) {
+          const int slot = min(n, NB_CAP - 1) * NB_THREADS;  // an overflowing list is never read (fallback path)
+          lp[slot] = p[j];
+          li[slot] = c[j];
         }
+        n += in ? 1 : 0;
       }
     }
   }
@@ -137,24 +142,37 @@ __global__ void __launch_bounds__(NB_THREADS) k_neighbours(Dev d) {
       const int nu = collect(d, gu, y0, z0, nb.wyu, nb.wzu, mz, lpu, liu);
       if (nd <= NB_CAP && nu <= NB_CAP) {
         const float t = nb.t;
-        // one flat loop over the nu x nd pairs: lanes with different list shapes stay together
+        // One flat loop over the nu x nd pairs, lanes with different list shapes stay together; the body is
+        // branch-free (selects) apart from the exact-tie test, which is rare.  The best pair is tracked by its list
+        // positions; min by (cost, key(u), key(d)) among cost <= triplet_cut (O2).
         const int np = nu * nd;
-        int ju = 0, jd = 0;
+        int ju = 0, jd = 0, bju = -1, bjd = 0;
+        float bc = d.P.triplet_cut;
         float2 pu = lpu[0];
-        int u = liu[0];
         for (int q = 0; q < np; q++) {
           const float2 pd = lpd[jd * NB_THREADS];
           const float ey = y0 - fmaf(t, pu.x - pd.x, pd.x);
           const float ez = z0 - fmaf(t, pu.y - pd.y, pd.y);
           const float cost = fmaf(ez * ez, d.inv_sz2, (ey * ey) * d.inv_sy2);
-          consider(d, best, cost, u, pu.x, pu.y, lid[jd * NB_THREADS], pd.x, pd.y);
-          if (++jd == nd) {
-            jd = 0;
-            ju = min(ju + 1, NB_CAP - 1);
-            pu = lpu[ju * NB_THREADS];
-            u = liu[ju * NB_THREADS];
+          bool take = cost < bc;
+          if (cost == bc) {  // cost == triplet_cut with no pair yet, or an exact tie between two pairs
+            take = bju < 0;
+            if (!take) {
+              const float2 qu = lpu[bju * NB_THREADS], qd = lpd[bjd * NB_THREADS];
+              const int u = liu[ju * NB_THREADS], bu = liu[bju * NB_THREADS];
+              if (u != bu) take = key_less(pu.y, pu.x, d.orig_idx[u], qu.y, qu.x, d.orig_idx[bu]);
+              else take = key_less(pd.y, pd.x, d.orig_idx[lid[jd * NB_THREADS]], qd.y, qd.x, d.orig_idx[lid[bjd * NB_THREADS]]);
+            }
           }
+          bju = take ? ju : bju;
+          bjd = take ? jd : bjd;
+          bc = take ? cost : bc;
+          const bool wrap = (jd + 1 == nd);
+          jd = wrap ? 0 : jd + 1;
+          ju = wrap ? min(ju + 1, NB_CAP - 1) : ju;
+          if (wrap) pu = lpu[ju * NB_THREADS];
         }
+        if (bju >= 0) { best.bu = liu[bju * NB_THREADS]; best.bd = lid[bjd * NB_THREADS]; best.bc = bc; }
       } else if (nu > 0) {
         nested_pairs(d, nb, gu, gd, y0, z0, mz, best);
       }

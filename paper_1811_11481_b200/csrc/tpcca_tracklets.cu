@@ -123,8 +123,8 @@ __device__ __forceinline__ int search_row(const Dev& d, const GridHdr& g, const 
   int y0, y1, z0, z1;
   const float zc = z_ref + k.z;  // search centre in frame coordinates (bin lookup only)
   const float mz = 2e-3f + (fabsf(zc) + fabsf(z_ref) + fabsf(k.z)) * 4e-7f;
-  bin_range(k.y - wy - 1e-3f, k.y + wy + 1e-3f, g.ymin, g.inv_by, g.ny, y0, y1);
-  bin_range(zc - wz - mz, zc + wz + mz, g.zmin, g.inv_bz, g.nz, z0, z1);
+  bin_range_fast(k.y - wy - 1e-3f, k.y + wy + 1e-3f, g.ymin, g.inv_by, g.ny, y0, y1);
+  bin_range_fast(zc - wz - mz, zc + wz + mz, g.zmin, g.inv_bz, g.nz, z0, z1);
   if (z0 > z1 || g.pad == 0) { y0 = 1; y1 = 0; }  // NaN / empty window, or empty row
   int best = -1;
   float bd = 0.0f;
@@ -135,13 +135,14 @@ __device__ __forceinline__ int search_row(const Dev& d, const GridHdr& g, const 
     int b0 = 0, b1 = 0;
     if (two) { b0 = bs[g.nz + z0]; b1 = bs[g.nz + z1 + 1]; }
     const int na = a1 - a0, ntot = na + (b1 - b0);
+    const int jump = b0 - a1;  // flat index i >= na is cluster a0 + i + jump
     for (int i = 0; i < ntot; i += SEARCH_UNROLL) {
       float2 p[SEARCH_UNROLL];
       int c[SEARCH_UNROLL];
 #pragma unroll
       for (int j = 0; j < SEARCH_UNROLL; j++) {
-        const int ii = min(i + j, ntot - 1);  // clamped: a repeated candidate cannot change the minimum
-        c[j] = (ii < na) ? a0 + ii : b0 + (ii - na);
+        const int ii = min(i + j, ntot - 1);  // clamped address; the evaluation below is predicated on i + j < ntot
+        c[j] = a0 + ii + ((ii >= na) ? jump : 0);
         p[j] = d.yz[c[j]];
       }
 #pragma unroll
@@ -149,11 +150,13 @@ __device__ __forceinline__ int search_row(const Dev& d, const GridHdr& g, const 
         const float dy = p[j].x - k.y;
         const float dz = (p[j].y - z_ref) - k.z;
         const float dist = fmaf(dz * dz, iz, (dy * dy) * iy);
-        if ((fabsf(dy) <= wy) && (fabsf(dz) <= wz) && (dist <= cut) && c[j] != best) {
-          bool better = (best < 0) || (dist < bd);
-          if (!better && dist == bd) better = tie_less(d, c[j], p[j], best);
-          if (better) { best = c[j]; bd = dist; pbest = p[j]; }
-        }
+        const bool in = (i + j < ntot) && (fabsf(dy) <= wy) && (fabsf(dz) <= wz) && (dist <= cut);
+        bool take = in && ((best < 0) || (dist < bd));
+        if (in && best >= 0 && dist == bd) take = tie_less(d, c[j], p[j], best);  // exact tie: key order (rare)
+        best = take ? c[j] : best;
+        bd = take ? dist : bd;
+        pbest.x = take ? p[j].x : pbest.x;
+        pbest.y = take ? p[j].y : pbest.y;
       }
     }
   }
