@@ -13,7 +13,10 @@
 // Pins (tests/test_oracle_pins.py): brute-force all-triplet search (P1), noiseless helix (P2),
 // mutual links (P3), exclusive assignment (P4), permutation invariance (P5), transport closed
 // form (P6), straight-line least squares (P7), pulls (P8), -O0 == -O2 (P10).
-// Parity unpinned: the numeric defaults of DESIGN.md Table A (cuts, windows, cov0) -- the paper
+// Merger and final fit O8-O10: tests/test_merge_pins.py; z / time estimate O11: tests/test_time_pins.py; looper legs and
+// cluster tags O12-O13: tests/test_looper_pins.py (float64 closed-form helices
+// over all sectors, the angle polynomial against arctan2, every term of the pair score, 41 one-line mutants all fail a pin).
+// Parity unpinned: the numeric defaults of DESIGN.md Tables A, B and D (cuts, windows, cov0) -- the paper
 // prints no value for them.
 #include <algorithm>
 #include <cmath>
@@ -191,6 +194,10 @@ struct Result {
   std::vector<TrackRec> merged;
   std::vector<int32_t> track_merged;             // sector track -> merged track
   std::vector<int32_t> link_next;                // sector track -> sector track it continues into, or -1
+  // looper legs and cluster tags (O12, O13)
+  std::vector<int32_t> leg_partner;              // merged track -> merged track joined at the outer turning point, or -1
+  std::vector<uint8_t> leg_first;                // merged track: 1 = first (or only) leg, 0 = additional leg
+  std::vector<uint8_t> cluster_tags;             // per cluster: TAG_* bits
 };
 
 struct Sector {
@@ -654,6 +661,177 @@ TimeRec time_estimate(const TrackRec& T, double kq, double zmin_hits, double zma
   return o;
 }
 
+// ---- O12-O13: legs of low-pT loopers and cluster tags ----
+struct LegParams {
+  float leg_min_qpt, leg_min_sinphi, leg_apex_margin;
+  int32_t leg_max_sector_gap;
+  float leg_max_turn, leg_centre_frac, leg_centre_abs, leg_radius_frac, leg_dz_max, leg_dzds_tol;
+  float tag_qpt_low, tag_qpt_leg, tag_sinphi;
+  int32_t ring;
+};
+
+// atan(r) for |r| <= 1: the degree-17 odd polynomial of Abramowitz & Stegun 4.4.49 (|error| <= 2e-8), Horner with fma.
+inline float atan_unit(float r) {
+  const float r2 = r * r;
+  float p = 0.0028662257f;
+  p = fma32(p, r2, -0.0161657367f);
+  p = fma32(p, r2, 0.0429096138f);
+  p = fma32(p, r2, -0.0752896400f);
+  p = fma32(p, r2, 0.1065626393f);
+  p = fma32(p, r2, -0.1420889944f);
+  p = fma32(p, r2, 0.1999355085f);
+  p = fma32(p, r2, -0.3333314528f);
+  p = fma32(p, r2, 1.0f);
+  return r * p;
+}
+
+// Angle of the vector (x, y) with y > 0, in (0, pi): octant reduction onto atan_unit.
+inline float angle_upper(float y, float x) {
+  const float half_pi = 1.57079632679f, pi = 3.14159265359f;
+  if (std::fabs(x) <= y) return half_pi - atan_unit(x / y);
+  if (x > 0.0f) return atan_unit(y / x);
+  return pi + atan_unit(y / x);
+}
+
+struct LegEnd {  // outer end of a merged track in the frame of its outermost sector segment
+  int32_t sector;
+  float x, y, z, s, t, q;
+  float c, R, xc, yc;  // cos(phi), radius, circle centre
+  bool cand;
+};
+
+inline LegEnd leg_end(int sector, float x, float y, float z, float s, float t, float q, bool valid, float kq, float x_last,
+                      const LegParams& L) {
+  LegEnd e;
+  e.sector = sector; e.x = x; e.y = y; e.z = z; e.s = s; e.t = t; e.q = q;
+  e.c = 0; e.R = 0; e.xc = 0; e.yc = 0; e.cand = false;
+  if (!valid || !(std::fabs(q) >= L.leg_min_qpt) || !(std::fabs(s) >= L.leg_min_sinphi) || !(std::fabs(s) < 1.0f)) return e;
+  const float k = q * kq;
+  e.c = std::sqrt(fma32(-s, s, 1.0f));
+  e.R = 1.0f / std::fabs(k);
+  e.xc = x - s / k;
+  e.yc = y + e.c / k;
+  e.cand = (e.xc + e.R) <= (x_last + L.leg_apex_margin);  // the helix turns back inside the TPC
+  return e;
+}
+
+// Score of the pair (A, B) -- A is the track with the lower id -- or a negative value if the ends do not belong to the two
+// legs of one turn.  Everything is evaluated in A's frame; B's frame lies j sector steps ahead in A's turning sense.
+inline float leg_pair_score(const LegEnd& A, const LegEnd& B, float kq, float ca, float sa, const LegParams& L) {
+  if (!A.cand || !B.cand) return -1.0f;
+  if (!(A.q * B.q < 0.0f)) return -1.0f;  // the two legs of a turn are fitted in opposite senses
+  if (L.ring <= 0) { if (A.sector != B.sector) return -1.0f; }
+  else if (A.sector / L.ring != B.sector / L.ring) return -1.0f;  // same z side
+  const int sgn = (A.q * kq > 0.0f) ? 1 : -1;  // curvature sign = sense in which sin(phi) grows along the fit direction
+  int j = 0;
+  if (L.ring > 0) j = (((B.sector - A.sector) * sgn) % L.ring + L.ring) % L.ring;
+  if (j > L.leg_max_sector_gap) return -1.0f;
+  // B's end point, centre and fit direction in A's frame: j rotations by the sector angle
+  const float ss = (float)sgn * sa;
+  float bx = B.x, by = B.y, bxc = B.xc, byc = B.yc, bdx = B.c, bdy = B.s;
+  for (int i = 0; i < j; i++) {
+    float u = fma32(-by, ss, bx * ca), v = fma32(bx, ss, by * ca);
+    bx = u; by = v;
+    u = fma32(-byc, ss, bxc * ca); v = fma32(bxc, ss, byc * ca);
+    bxc = u; byc = v;
+    u = fma32(-bdy, ss, bdx * ca); v = fma32(bdx, ss, bdy * ca);
+    bdx = u; bdy = v;
+  }
+  (void)bx; (void)by;
+  // turning angle from A's fit direction to the reversed fit direction of B, in A's turning sense
+  const float dot = -fma32(A.s, bdy, A.c * bdx);
+  const float cross = fma32(A.s, bdx, -(A.c * bdy));
+  const float yy = (float)sgn * cross;
+  if (!(yy > 0.0f)) return -1.0f;
+  const float theta = angle_upper(yy, dot);
+  if (!(theta <= L.leg_max_turn)) return -1.0f;
+  const float Rm = 0.5f * (A.R + B.R);
+  const float arc = theta * Rm;
+  const float dxc = A.xc - bxc, dyc = A.yc - byc;
+  const float dc2 = fma32(dyc, dyc, dxc * dxc);
+  const float tolc = fma32(L.leg_centre_frac, Rm, L.leg_centre_abs);
+  const float tolc2 = tolc * tolc;
+  if (!(dc2 <= tolc2)) return -1.0f;
+  const float dR = A.R - B.R, tolR = L.leg_radius_frac * Rm;
+  if (!(std::fabs(dR) <= tolR)) return -1.0f;
+  const float tm = 0.5f * (A.t - B.t);
+  const float dz = fma32(-tm, arc, B.z - A.z);
+  if (!(std::fabs(dz) <= L.leg_dz_max)) return -1.0f;
+  const float dt = A.t + B.t;
+  if (!(std::fabs(dt) <= L.leg_dzds_tol)) return -1.0f;
+  const float e1 = dc2 / tolc2, e2 = dR / tolR, e3 = dz / L.leg_dz_max, e4 = dt / L.leg_dzds_tol;
+  float score = e1;
+  score = fma32(e2, e2, score);
+  score = fma32(e3, e3, score);
+  score = fma32(e4, e4, score);
+  return score;
+}
+
+void find_legs(Result* R, const Ctx& c, const LegParams& L) {
+  const Params& P = c.P;
+  const int nm = (int)R->merged.size(), nt = (int)R->tracks.size();
+  const float th = P.tan_half_angle;
+  const float den = fma32(th, th, 1.0f);
+  const float ca = fma32(-th, th, 1.0f) / den, sa = (2.0f * th) / den;
+  const float x_last = c.row_x[c.n_rows - 1];
+  // outer end of every merged track = outer state (O8) of the last sector segment of its chain
+  std::vector<LegEnd> ends(nm);
+  for (int m = 0; m < nm; m++) {
+    int tail = R->merged[m].pad[4];
+    while (R->link_next[tail] >= 0) tail = R->link_next[tail];
+    const KF& o = R->outer[tail];
+    ends[m] = leg_end(R->tracks[tail].sector, o.x, o.p[0], o.p[1] + R->outer_zref[tail], o.p[2], o.p[3], o.p[4],
+                      R->tracks[tail].ndf >= 0, c.kq, x_last, L);
+  }
+  // O12: best partner of every end (min by (score, id)), mutual pairs are linked
+  std::vector<int32_t> best(nm, -1);
+  std::vector<float> bs(nm, 0.0f);
+  for (int a = 0; a < nm; a++) {
+    if (!ends[a].cand) continue;
+    for (int b = a + 1; b < nm; b++) {
+      if (!ends[b].cand) continue;
+      const float sc = leg_pair_score(ends[a], ends[b], c.kq, ca, sa, L);
+      if (!(sc >= 0.0f)) continue;
+      if (best[a] < 0 || sc < bs[a]) { best[a] = b; bs[a] = sc; }   // equal score: the lower id stays (b increases)
+      if (best[b] < 0 || sc < bs[b]) { best[b] = a; bs[b] = sc; }   // equal score: the lower id stays (a increases)
+    }
+  }
+  R->leg_partner.assign(nm, -1);
+  R->leg_first.assign(nm, 1);
+  for (int a = 0; a < nm; a++) {
+    const int b = best[a];
+    if (b >= 0 && best[b] == a) R->leg_partner[a] = b;
+  }
+  // the first leg of a pair is the one whose inner end lies at the smaller |z| (the vertex side of the drift volume)
+  for (int a = 0; a < nm; a++) {
+    const int b = R->leg_partner[a];
+    if (b < 0) continue;
+    const float za = std::fabs(R->merged[a].z), zb = std::fabs(R->merged[b].z);
+    const bool a_first = (za < zb) || (za == zb && a < b);
+    R->leg_first[a] = a_first ? 1 : 0;
+  }
+  // O13: cluster tags
+  R->cluster_tags.assign((size_t)R->n, 0);
+  for (int t = 0; t < nt; t++) {
+    const TrackRec& T = R->tracks[t];
+    const int m = R->track_merged[t];
+    const TrackRec& Mr = R->merged[m];
+    uint8_t base = 0;
+    if (std::fabs(Mr.qpt) > L.tag_qpt_low) base |= 1;
+    if (R->leg_first[m] == 0 && std::fabs(Mr.qpt) > L.tag_qpt_leg) base |= 2;
+    const float k = T.qpt * c.kq;
+    for (int32_t h : R->track_hits[t]) {
+      uint8_t f = base;
+      if (T.ndf < 0) f |= 4;
+      else {
+        const float sl = fma32(c.cl[h].x - T.x, k, T.sinphi);  // sin(phi) is linear in x along a helix
+        if (!(std::fabs(sl) <= L.tag_sinphi)) f |= 4;
+      }
+      R->cluster_tags[h] = f;
+    }
+  }
+}
+
 }  // namespace
 
 extern "C" {
@@ -794,6 +972,36 @@ void orc_time_estimate_state(const float* state6, float bz, float zmin_hits, flo
   T.x = state6[0]; T.y = state6[1]; T.z = state6[2]; T.sinphi = state6[3]; T.dzds = state6[4]; T.qpt = state6[5];
   const TimeRec o = time_estimate(T, -((0.000299792458 * 10.0) * (double)bz), zmin_hits, zmax_hits, side, vdrift, z_max);
   out4[0] = o.z_dca; out4[1] = o.z_shift; out4[2] = o.t0_us; out4[3] = o.dca_xy;
+}
+
+
+// O12-O13 on a result of orc_track + orc_merge.  Returns the number of leg links (pairs).
+int64_t orc_legs(void* r, int32_t n_rows, const float* row_x, float bz, const Params* P, const Cl* cl, const LegParams* L) {
+  Result* R = (Result*)r;
+  Ctx c = make_ctx(cl, row_x, n_rows, *P, bz, false);
+  find_legs(R, c, *L);
+  int64_t n = 0;
+  for (size_t m = 0; m < R->leg_partner.size(); m++) n += (R->leg_partner[m] > (int32_t)m) ? 1 : 0;
+  return n;
+}
+const int32_t* orc_leg_partner(void* r) { return ((Result*)r)->leg_partner.data(); }
+const uint8_t* orc_leg_first(void* r) { return ((Result*)r)->leg_first.data(); }
+const uint8_t* orc_cluster_tags(void* r) { return ((Result*)r)->cluster_tags.data(); }
+float orc_angle_upper(float y, float x) { return angle_upper(y, x); }
+// one end: state7 = sector, x, y, z, sinphi, dzds, qpt -> out5 = cand, R, xc, yc, c
+void orc_leg_end(const float* state7, float bz, float x_last, const LegParams* L, float* out5) {
+  const float kq = -((0.000299792458f * 10.0f) * bz);
+  const LegEnd e = leg_end((int)state7[0], state7[1], state7[2], state7[3], state7[4], state7[5], state7[6], true, kq, x_last, *L);
+  out5[0] = e.cand ? 1.0f : 0.0f; out5[1] = e.R; out5[2] = e.xc; out5[3] = e.yc; out5[4] = e.c;
+}
+// pair score of two ends (A = first argument, taken as the lower id), or a negative value
+float orc_leg_pair(const float* a7, const float* b7, float bz, float x_last, float tan_half_angle, const LegParams* L) {
+  const float kq = -((0.000299792458f * 10.0f) * bz);
+  const float den = fma32(tan_half_angle, tan_half_angle, 1.0f);
+  const float ca = fma32(-tan_half_angle, tan_half_angle, 1.0f) / den, sa = (2.0f * tan_half_angle) / den;
+  const LegEnd A = leg_end((int)a7[0], a7[1], a7[2], a7[3], a7[4], a7[5], a7[6], true, kq, x_last, *L);
+  const LegEnd B = leg_end((int)b7[0], b7[1], b7[2], b7[3], b7[4], b7[5], b7[6], true, kq, x_last, *L);
+  return leg_pair_score(A, B, kq, ca, sa, *L);
 }
 
 void orc_free(void* r) { delete (Result*)r; }
