@@ -194,6 +194,43 @@ typedef struct { float z_dca, z_shift, t0_us, dca_xy; } tpcca_time_rec;
 int tpcca_estimate_time(tpcca_handle* h, float vdrift_cm_per_us, float z_max_cm, void* stream,
                         tpcca_time_rec* out_sector, tpcca_time_rec* out_merged);
 
+/* ---- Legs of low-pT loopers and cluster tags ("additional legs of looping tracks do not point to the vertex
+ * ... special low-pT track merging"; :157 clusters to remove for the compression factor: "very low-pT looping tracks below
+ * 50 MeV/c, additional legs of tracks below 200 MeV/c, and track segments with high inclination angle"; DESIGN.md section 14,
+ * Table D).  The outer ends of two merged tracks that are the outgoing and the returning leg of one turn of a helix (same
+ * circle in the sector plane, opposite fitted curvature, z consistent with the arc between them) are linked at the turning
+ * point; clusters are tagged for removal. */
+typedef struct {
+  float leg_min_qpt;          /* (GeV/c)^-1: only ends with |q/pT| >= this are candidates */
+  float leg_min_sinphi;       /* and |sin(phi)| >= this at the outer end */
+  float leg_apex_margin;      /* cm: the turning point xc + R must lie below row_x[last] + margin */
+  int32_t leg_max_sector_gap; /* the partner's end lies 0..gap sectors ahead in the turning sense */
+  float leg_max_turn;         /* rad, < pi: turning angle between the two ends */
+  float leg_centre_frac, leg_centre_abs; /* centre distance <= frac * mean radius + abs (cm) */
+  float leg_radius_frac;      /* |R_A - R_B| <= frac * mean radius */
+  float leg_dz_max;           /* cm: z_B - z_A - mean slope * arc */
+  float leg_dzds_tol;         /* |dzds_A + dzds_B| (the legs are fitted in opposite senses) */
+  float tag_qpt_low;          /* TAG_LOW_PT: |q/pT| of the merged track above this (20 = 50 MeV/c) */
+  float tag_qpt_leg;          /* TAG_EXTRA_LEG: additional leg with |q/pT| above this (5 = 200 MeV/c) */
+  float tag_sinphi;           /* TAG_HIGH_INCLINATION: local |sin(phi)| above this */
+  int32_t ring;               /* sectors per z side closing the ring (18); 0: partners in the same sector only */
+} tpcca_leg_params;
+void tpcca_default_leg_params(tpcca_leg_params* p);
+enum { TPCCA_TAG_LOW_PT = 1, TPCCA_TAG_EXTRA_LEG = 2, TPCCA_TAG_HIGH_INCLINATION = 4 };
+typedef struct { int32_t n_links, n_tag_low_pt, n_tag_extra_leg, n_tag_high_inclination; } tpcca_leg_summary; /* 16 B */
+
+/* Link legs and tag clusters for the merged tracks of the LAST tpcca_merge on this handle (whose outputs, and those of the
+ * tpcca_track before it, must still be valid and unchanged); enqueued on `stream`, returns without waiting.
+ * out_leg_partner: device, max_tracks int32: merged track joined at the outer turning point, or -1 (mutual).
+ * out_leg_first: device, max_tracks bytes: 1 = first (or only) leg -- of a pair, the one whose inner end lies at the
+ *   smaller |z| --, 0 = additional leg.
+ * out_cluster_tags: device, n bytes in INPUT order (n of the last tpcca_track): TPCCA_TAG_* bits, 0 for clusters on no track.
+ * out_summary: device, 16-byte aligned: links and tagged clusters per bit.
+ * TPCCA_ERR_ARGUMENT without a preceding tpcca_merge, for null / misaligned pointers or parameters out of range
+ * (leg_max_turn must be < pi, leg_min_sinphi > sin(20 deg), tolerances > 0). */
+int tpcca_find_legs(tpcca_handle* h, const tpcca_leg_params* lp, void* stream, int32_t* out_leg_partner,
+                    uint8_t* out_leg_first, uint8_t* out_cluster_tags, tpcca_leg_summary* out_summary);
+
 /* Per-stage device times, averaged over the tpcca_track calls (at most the last 32) made since profiling
  * was switched on (CUDA events recorded on each call's stream; synchronises those events).  ms: host float[TPCCA_N_STAGES]. */
 enum { TPCCA_STAGE_GRID = 0, TPCCA_STAGE_NEIGHBOURS, TPCCA_STAGE_CLEAN_START, TPCCA_STAGE_TRACKLETS,

@@ -55,6 +55,16 @@ class MergeParams(C.Structure):
                 ("fit_reject_cut", C.c_float), ("shared_err_scale", C.c_float), ("ring", C.c_int32)]
 
 
+class LegParams(C.Structure):
+    _fields_ = [("leg_min_qpt", C.c_float), ("leg_min_sinphi", C.c_float), ("leg_apex_margin", C.c_float),
+                ("leg_max_sector_gap", C.c_int32), ("leg_max_turn", C.c_float), ("leg_centre_frac", C.c_float),
+                ("leg_centre_abs", C.c_float), ("leg_radius_frac", C.c_float), ("leg_dz_max", C.c_float),
+                ("leg_dzds_tol", C.c_float), ("tag_qpt_low", C.c_float), ("tag_qpt_leg", C.c_float),
+                ("tag_sinphi", C.c_float), ("ring", C.c_int32)]
+
+
+TAG_LOW_PT, TAG_EXTRA_LEG, TAG_HIGH_INCLINATION = 1, 2, 4
+
 _lib = None
 
 
@@ -78,6 +88,10 @@ def load():
         lib.tpcca_default_merge_params.argtypes = [C.POINTER(MergeParams)]
         lib.tpcca_merge.restype = C.c_int
         lib.tpcca_merge.argtypes = [C.c_void_p, C.POINTER(MergeParams), C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.tpcca_default_leg_params.argtypes = [C.POINTER(LegParams)]
+        lib.tpcca_find_legs.restype = C.c_int
+        lib.tpcca_find_legs.argtypes = [C.c_void_p, C.POINTER(LegParams), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                        C.c_void_p]
         lib.tpcca_estimate_time.restype = C.c_int
         lib.tpcca_estimate_time.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
         lib.tpcca_wait.restype = C.c_int
@@ -98,6 +112,12 @@ def load():
         lib.tpcca_free.argtypes = [C.c_void_p]
         _lib = lib
     return _lib
+
+
+def default_leg_params() -> LegParams:
+    p = LegParams()
+    load().tpcca_default_leg_params(C.byref(p))
+    return p
 
 
 def default_merge_params() -> MergeParams:
@@ -271,6 +291,32 @@ class Tracker:
 
     def track_merged(self) -> np.ndarray:
         return self.out_track_merged[:self.header()["n_tracks"]].cpu().numpy().copy()
+
+    # ---- looper legs and cluster tags on the results of the last merge() (tpcca_find_legs)
+    def find_legs(self, **params):
+        """Returns (leg_partner[n_merged], leg_first[n_merged], cluster_tags[n], summary dict)."""
+        torch = self.torch
+        lp = default_leg_params()
+        for k, v in params.items():
+            if not hasattr(lp, k):
+                raise TypeError(f"unknown leg parameter {k}")
+            setattr(lp, k, v)
+        n = max(1, int(self.n))
+        if getattr(self, "out_leg_partner", None) is None:
+            self.out_leg_partner = torch.empty(max(1, self.max_tracks), dtype=torch.int32, device=self.device)
+            self.out_leg_first = torch.empty(max(1, self.max_tracks), dtype=torch.uint8, device=self.device)
+            self.out_leg_summary = torch.empty(4, dtype=torch.int32, device=self.device)
+        if getattr(self, "out_tags", None) is None or self.out_tags.numel() < n:
+            self.out_tags = torch.empty(n, dtype=torch.uint8, device=self.device)
+        self._check(self.lib.tpcca_find_legs(self.h, C.byref(lp), self._stream(), self.out_leg_partner.data_ptr(),
+                                             self.out_leg_first.data_ptr(), self.out_tags.data_ptr(),
+                                             self.out_leg_summary.data_ptr()))
+        nm = self.merged_header()["n_merged"]
+        sm = self.out_leg_summary.cpu().numpy()
+        return (self.out_leg_partner[:nm].cpu().numpy().copy(), self.out_leg_first[:nm].cpu().numpy().copy(),
+                self.out_tags[:int(self.n)].cpu().numpy().copy(),
+                dict(n_links=int(sm[0]), n_tag_low_pt=int(sm[1]), n_tag_extra_leg=int(sm[2]),
+                     n_tag_high_inclination=int(sm[3])))
 
     def estimate_time(self, vdrift: float = 2.58, z_max: float = 250.0, merged: bool = True):
         """tpcca_estimate_time: (n_tracks, 4) and, after merge(), (n_merged, 4) arrays of z_dca, z_shift, t0_us, dca_xy."""

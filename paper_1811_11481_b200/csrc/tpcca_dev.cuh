@@ -118,6 +118,18 @@ struct Dev {
   tpcca_out_header* merged_hdr;
   tpcca_track_rec* merged_out;
   int32_t* track_merged_out;
+  // looper legs and cluster tags (tpcca_find_legs)
+  tpcca_leg_params LP;
+  float4* leg_ends;                // [max_tracks][3] outer end of every merged track (layout: tpcca_legs.cu)
+  unsigned long long* leg_best;    // [max_tracks] (score bits << 32 | partner id), ~0 = none
+  int32_t* leg_sec;                // [TPCCA_MAX_SECTORS+2] candidate ends per sector -> bucket starts
+  int32_t* leg_cur;                // [TPCCA_MAX_SECTORS] scatter cursors
+  int32_t* leg_list;               // [max_tracks] candidate ends grouped by sector
+  int32_t* leg_summary;            // [4] links, tagged clusters per bit
+  int32_t* leg_partner_out;
+  uint8_t* leg_first_out;
+  uint8_t* tags_out;
+  int32_t* leg_summary_out;
   DevCounters* cnt;
   tpcca_out_header* out_hdr;
   tpcca_track_rec* out_tracks;
@@ -320,6 +332,7 @@ void launch_select(const Dev& d, Launch& L);
 void launch_refit(const Dev& d, Launch& L);
 void launch_export(const Dev& d, int what, void* dst, Launch& L);
 void launch_merge(const Dev& d, Launch& L);
+void launch_legs(const Dev& d, Launch& L);
 void launch_time_estimate(const Dev& d, float vdrift, float z_max, tpcca_time_rec* out_sector, tpcca_time_rec* out_merged,
                           Launch& L);
 // exclusive scan of data[0..n) in place, n read from *n_dev (<= n_max); data[n] receives the total
