@@ -280,6 +280,16 @@ def run_gpu(args):
     mh = trk.merged_header()
     track_merged = trk.track_merged()
     dev_assign = trk.assignment()
+    # ---- looper legs and cluster tags on the merged tracks (tpcca_find_legs), timed on its own
+    leg_partner, leg_first, tags, leg_sum = trk.find_legs()
+    torch.cuda.synchronize()
+    l0, l1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0.record(stream)
+    for _ in range(args.steps):
+        trk.find_legs_enqueue()
+    l1.record(stream)
+    torch.cuda.synchronize()
+    legs_ms = l0.elapsed_time(l1) / args.steps
 
     # ---- end to end through the library's host calls (pinned host buffers, H2D + D2H inside the timed region)
     hc = torch.from_numpy(fr.clusters.view(np.uint8).reshape(-1)).pin_memory()
@@ -342,9 +352,16 @@ def run_gpu(args):
     q_sec = score.score(dev_assign, fr.truth, one, hd["n_tracks"])
     am = np.where(dev_assign >= 0, track_merged[np.maximum(dev_assign, 0)], -1) if hd["n_tracks"] else dev_assign
     q_mrg = score.score(am, fr.truth, one, mh["n_merged"])
+    # a pair of legs counts as one reconstructed particle: relabel the additional leg by its partner
+    leg_root = np.where((leg_partner >= 0) & (leg_first == 0), leg_partner, np.arange(len(leg_partner))) if len(leg_partner) else leg_partner
+    al = np.where(am >= 0, leg_root[np.maximum(am, 0)], -1) if len(leg_partner) else am
+    q_leg = score.score(al, fr.truth, one, mh["n_merged"])
     merge_info = {"ms": merge_ms, "api": "tpcca_merge (after the timed path, not part of `value`)", **mh,
                   "per_particle": {"sector_tracks": {k: round(float(v), 5) for k, v in q_sec.items()},
-                                   "merged_tracks": {k: round(float(v), 5) for k, v in q_mrg.items()}}}
+                                   "merged_tracks": {k: round(float(v), 5) for k, v in q_mrg.items()},
+                                   "merged_tracks_legs_joined": {k: round(float(v), 5) for k, v in q_leg.items()}}}
+    legs_info = {"ms": legs_ms, "api": "tpcca_find_legs (after tpcca_merge, not part of `value`)", **leg_sum,
+                 "tagged_fraction_of_clusters": round(float((tags > 0).mean()), 5) if n else 0.0}
     # ---- roofline (algorithmic bytes of DESIGN.md section 7 x live device counters)
     peak, peak_src = peaks()
     T = hd["n_start_hits"]
@@ -420,7 +437,7 @@ def run_gpu(args):
                        "n_start_hits": hd["n_start_hits"], "row_steps": stats["row_steps"], "quality": gpu_quality,
                        "l2": "inputs larger than L2 (cluster array %.0f MB, working set > 1 GB)" % (n * 16 / 1e6)
                        if n * 16 > 126e6 else "frame fits the 126 MB L2: a parity-test case, not the bench line",
-                       "parallelism": parallelism, "shard": args.shard, "merge": merge_info},
+                       "parallelism": parallelism, "shard": args.shard, "merge": merge_info, "legs": legs_info},
             "clocks": clocks,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "ms_per_step": pipe_ms / args.steps, "steps": args.steps, "frames_in_flight": 2, "handles": 1,

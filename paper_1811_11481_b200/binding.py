@@ -293,8 +293,8 @@ class Tracker:
         return self.out_track_merged[:self.header()["n_tracks"]].cpu().numpy().copy()
 
     # ---- looper legs and cluster tags on the results of the last merge() (tpcca_find_legs)
-    def find_legs(self, **params):
-        """Returns (leg_partner[n_merged], leg_first[n_merged], cluster_tags[n], summary dict)."""
+    def find_legs_enqueue(self, **params):
+        """tpcca_find_legs, enqueue only (results stay in out_leg_partner / out_leg_first / out_tags / out_leg_summary)."""
         torch = self.torch
         lp = default_leg_params()
         for k, v in params.items():
@@ -311,6 +311,10 @@ class Tracker:
         self._check(self.lib.tpcca_find_legs(self.h, C.byref(lp), self._stream(), self.out_leg_partner.data_ptr(),
                                              self.out_leg_first.data_ptr(), self.out_tags.data_ptr(),
                                              self.out_leg_summary.data_ptr()))
+
+    def find_legs(self, **params):
+        """Returns (leg_partner[n_merged], leg_first[n_merged], cluster_tags[n], summary dict)."""
+        self.find_legs_enqueue(**params)
         nm = self.merged_header()["n_merged"]
         sm = self.out_leg_summary.cpu().numpy()
         return (self.out_leg_partner[:nm].cpu().numpy().copy(), self.out_leg_first[:nm].cpu().numpy().copy(),
