@@ -151,6 +151,11 @@ enum tpcca_intermediate {
  * `stream`) and returns TPCCA_ERR_ARGUMENT, writing nothing, if `bytes` is smaller than the table. */
 int tpcca_get_intermediate(tpcca_handle* h, int what, void* dst_device, size_t bytes, void* stream);
 
+/* Debugging aid: the i-th array carved out of the workspace (byte offset from params.workspace, bytes in use; arrays start
+ * on 256-byte boundaries, so the bytes between the end of one and the start of the next are never touched by a correct
+ * kernel -- tests fill the workspace with a pattern and check those gaps afterwards).  TPCCA_ERR_ARGUMENT past the last. */
+int tpcca_debug_workspace_layout(tpcca_handle* h, int i, size_t* offset, size_t* bytes);
+
 /* Debugging aid: with on != 0 every tpcca_track on this handle synchronises after each stage and names the stage
  * that faulted in tpcca_last_error().  Off by default; never use it in a timed run. */
 int tpcca_set_debug(tpcca_handle* h, int on);

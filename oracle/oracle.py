@@ -90,13 +90,16 @@ def _host_has_fma() -> bool:
 
 
 def build(opt: str = "-O2", force: bool = False) -> str:
-    so = os.path.join(_HERE, f"libtpcca_oracle{opt.replace('-', '_')}.so")
+    # TPCCA_ORACLE_CXXFLAGS: extra compiler flags for a checking build of the oracle (e.g. -fsanitize=address,undefined,
+    # with libasan preloaded into python; profiles/r2_sanitizer.md has the command)
+    extra = os.environ.get("TPCCA_ORACLE_CXXFLAGS", "").split()
+    so = os.path.join(_HERE, f"libtpcca_oracle{opt.replace('-', '_')}{'_chk' if extra else ''}.so")
     if force or not os.path.exists(so) or os.path.getmtime(so) < os.path.getmtime(_SRC):
         # -mfma only makes std::fma a single instruction where the host has it (the result is the same correctly
         # rounded value either way); -ffp-contract=off: the compiler itself never fuses
         hw = ["-mfma"] if _host_has_fma() else []
         subprocess.check_call(["g++", opt, "-std=c++17", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC"] + hw
-                              + ["-o", so, _SRC])
+                              + extra + ["-o", so, _SRC])
     return so
 
 

@@ -98,6 +98,8 @@ def load():
         lib.tpcca_wait.argtypes = [C.c_void_p]
         lib.tpcca_get_intermediate.restype = C.c_int
         lib.tpcca_get_intermediate.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_size_t, C.c_void_p]
+        lib.tpcca_debug_workspace_layout.restype = C.c_int
+        lib.tpcca_debug_workspace_layout.argtypes = [C.c_void_p, C.c_int, C.POINTER(C.c_size_t), C.POINTER(C.c_size_t)]
         lib.tpcca_set_profiling.argtypes = [C.c_void_p, C.c_int]
         lib.tpcca_set_debug.argtypes = [C.c_void_p, C.c_int]
         lib.tpcca_get_stage_ms.restype = C.c_int
@@ -335,6 +337,15 @@ class Tracker:
             return out_s, None
         nm = self.merged_header()["n_merged"]
         return out_s, tm[:4 * nm].reshape(nm, 4).cpu().numpy()
+
+    def workspace_layout(self) -> list:
+        """[(offset, bytes)] of every array carved out of the workspace (tpcca_debug_workspace_layout)."""
+        out, i = [], 0
+        off, nb = C.c_size_t(), C.c_size_t()
+        while self.lib.tpcca_debug_workspace_layout(self.h, i, C.byref(off), C.byref(nb)) == 0:
+            out.append((int(off.value), int(nb.value)))
+            i += 1
+        return out
 
     def set_debug(self, on: bool):
         self.lib.tpcca_set_debug(self.h, int(on))

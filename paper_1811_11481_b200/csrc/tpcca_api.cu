@@ -13,8 +13,12 @@ static thread_local char g_err[512] = "";
 static void set_err(const char* fmt, const char* a = "", long long b = 0) { snprintf(g_err, sizeof(g_err), fmt, a, b); }
 
 #define PROF_RING 32
+#define MAX_LAYOUT 128
 struct tpcca_handle {
   Dev d;
+  // workspace layout as carved (offset, bytes used) -- tpcca_debug_workspace_layout
+  size_t lay_off[MAX_LAYOUT], lay_bytes[MAX_LAYOUT];
+  int n_layout;
   tpcca_geometry geo;
   int64_t max_clusters;
   // host-API staging (inside the workspace): two slots, so that the copies of one frame overlap the kernels of the next
@@ -48,9 +52,13 @@ static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params
   const size_t SL = (size_t)g->n_sectors * g->n_rows;
   const size_t NB = 4 * N + 130 * SL + 2;
   const size_t NSCAN = T + 8 + NB / 2048 + T / 2048 + 64;
+  if (base) h->n_layout = 0;
 #define CARVE(field, type, count)                                  \
   do {                                                             \
-    if (base) h->field = reinterpret_cast<type*>(base + off);      \
+    if (base) {                                                    \
+      h->field = reinterpret_cast<type*>(base + off);              \
+      if (h->n_layout < MAX_LAYOUT) { h->lay_off[h->n_layout] = off; h->lay_bytes[h->n_layout++] = sizeof(type) * (size_t)(count); } \
+    }                                                              \
     off += align_up(sizeof(type) * (size_t)(count));               \
   } while (0)
   CARVE(d.cnt, DevCounters, 1);
@@ -459,6 +467,14 @@ int tpcca_estimate_time(tpcca_handle* h, float vdrift, float z_max, void* stream
   launch_time_estimate(d, vdrift, z_max, out_sector, out_merged, L);
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) { set_err("time estimate launch failed: %s", cudaGetErrorString(e)); return TPCCA_ERR_CUDA; }
+  return TPCCA_OK;
+}
+
+int tpcca_debug_workspace_layout(tpcca_handle* h, int i, size_t* offset, size_t* bytes) {
+  if (!h) { set_err("handle is null (not initialised)"); return TPCCA_ERR_NOT_INIT; }
+  if (i < 0 || i >= h->n_layout || !offset || !bytes) return TPCCA_ERR_ARGUMENT;
+  *offset = h->lay_off[i];
+  *bytes = h->lay_bytes[i];
   return TPCCA_OK;
 }
 

@@ -385,3 +385,72 @@ def test_sector_shards_reproduce_the_whole_frame(row_x, world):
         a[lo:lo + len(ar)] = D.globalise_assignment(ar, off[r])
     assert sum(counts) == len(tr_ref) and np.array_equal(a, a_ref)
     assert np.concatenate([p[1] for p in parts]).tobytes() == tr_ref.tobytes()
+
+
+def _gaps_untouched(t, poison):
+    """Every byte between the end of one workspace array and the start of the next (arrays start on 256-byte boundaries)
+    still holds the fill pattern; returns the number of gap bytes checked."""
+    import torch
+    lay = t.workspace_layout()
+    assert len(lay) > 40
+    base_off = ((t.workspace.data_ptr() + 255) & ~255) - t.workspace.data_ptr()
+    checked = 0
+    for (off, nb), nxt in zip(lay, [o for o, _ in lay[1:]] + [None]):
+        end = off + nb
+        stop = nxt if nxt is not None else min(end + 256, t.workspace.numel() - base_off)
+        assert stop >= end, (off, nb, nxt)
+        if stop > end:
+            gap = t.workspace[base_off + end:base_off + stop]
+            assert bool((gap == poison).all()), f"workspace array at offset {off} (+{nb} bytes) was overrun"
+            checked += stop - end
+    return checked
+
+
+@pytest.mark.parametrize("case", ["config2", "dense_noise", "tight_capacity", "loopers"])
+def test_no_kernel_writes_outside_its_arrays(row_x, case):
+    """Bounds check of our own (compute-sanitizer is closed on the GPU pool): the workspace is filled with a pattern, the
+    whole chain track -> merge -> find_legs -> estimate_time runs, and the padding behind every one of the carved arrays,
+    the guard bands around the caller's output buffers and the unused tail of the outputs must be untouched."""
+    import torch
+    poison = 0xA5
+    if case == "config2":
+        fr, kw = synth.generate(synth.config(2, scale=0.25, seed=7)), {}
+    elif case == "dense_noise":
+        fr, kw = synth.generate(synth.config(1, scale=0.5, seed=3), noise_frac=30.0), {}
+    elif case == "tight_capacity":   # capacities hit: truncation must not write past the arrays either
+        fr = synth.generate(synth.config(2, scale=0.25, seed=7))
+        kw = dict(max_tracklets=700, max_tracks=150)
+    else:
+        fr, kw = synth.generate(synth.config(3, scale=0.3, seed=3)), {}
+    cap = dict(max_clusters=fr.n, max_tracklets=max(1024, fr.n // 4))
+    cap.update(kw)
+    t = B.Tracker(row_x, n_sectors=fr.n_sectors, poison=poison, **cap)
+    G = 4096
+    bufs = {}
+    for name, nbytes in (("tracks", 16 + 128 * t.max_tracks), ("assign", 4 * fr.n), ("merged", 16 + 128 * t.max_tracks),
+                         ("track_merged", 4 * max(1, t.max_tracks)), ("partner", 4 * max(1, t.max_tracks)),
+                         ("first", max(1, t.max_tracks)), ("tags", fr.n), ("summary", 16),
+                         ("time_s", 16 * max(1, t.max_tracks)), ("time_m", 16 * max(1, t.max_tracks))):
+        full = torch.full((nbytes + 2 * G,), poison, dtype=torch.uint8, device="cuda")
+        bufs[name] = (full, full[G:G + nbytes])
+    import ctypes as C
+    dev = t.upload(fr.clusters)
+    so = np.ascontiguousarray(fr.sector_offsets, dtype=np.int32)
+    p = lambda k: bufs[k][1].data_ptr()
+    for _ in range(2):
+        assert t.lib.tpcca_track(t.h, dev.data_ptr(), fr.n, so.ctypes.data, t._stream(), p("tracks"), p("assign")) == 0
+        mp, lp = B.default_merge_params(), B.default_leg_params()
+        assert t.lib.tpcca_merge(t.h, C.byref(mp), t._stream(), p("merged"), p("track_merged")) == 0
+        assert t.lib.tpcca_find_legs(t.h, C.byref(lp), t._stream(), p("partner"), p("first"), p("tags"), p("summary")) == 0
+        assert t.lib.tpcca_estimate_time(t.h, 2.58, 250.0, t._stream(), p("time_s"), p("time_m")) == 0
+    torch.cuda.synchronize()
+    hd = bufs["tracks"][1][:16].cpu().numpy().view(B.HEADER_DTYPE)[0]
+    assert (hd["status"] != 0) == (case == "tight_capacity")
+    assert _gaps_untouched(t, poison) > 2000
+    for name, (full, view) in bufs.items():
+        assert bool((full[:G] == poison).all()) and bool((full[-G:] == poison).all()), f"guard band of {name} overwritten"
+    nt = int(hd["n_tracks"])
+    assert nt <= t.max_tracks
+    assert bool((bufs["tracks"][1][16 + 128 * nt:] == poison).all()), "track records past n_tracks were written"
+    nm = int(bufs["merged"][1][:16].cpu().numpy().view(B.HEADER_DTYPE)[0]["n_tracks"])
+    assert bool((bufs["merged"][1][16 + 128 * nm:] == poison).all()), "merged records past n_merged were written"
