@@ -168,13 +168,15 @@ __device__ __forceinline__ int search_row(const Dev& d, const GridHdr& g, const 
 #define E1_BLOCKS 4  // CTAs per SM in the grid: fewer lanes = more seeds per lane = better balance
 #endif
 #ifndef E1_BOUNDS
-#define E1_BOUNDS 8
+#define E1_BOUNDS 6
 #endif
 __global__ void __launch_bounds__(E_THREADS, E1_BOUNDS) k_tl_e1(Dev d) {
   const int R = d.n_rows, n_work = d.cnt->n_work;
   const unsigned lane = threadIdx.x & 31;
   int n_steps = 0;
   int w = -1, sbase = 0, h = -1, r = 0, last_row = 0;
+  int hn_n = -1;                           // link of h, loaded one step ahead
+  float2 pc_n = make_float2(0.f, 0.f);     // cluster h, loaded one step ahead
   int32_t* rh = nullptr;
   float z_ref = 0.f;
   KF k;
@@ -208,6 +210,7 @@ __global__ void __launch_bounds__(E_THREADS, E1_BOUNDS) k_tl_e1(Dev d) {
           h = d.link_up_clean[h0];
           r = (h >= d.row_start[sbase + r0 + 2]) ? r0 + 2 : r0 + 1;
           const float2 p1 = d.yz[h];
+          pc_n = p1; hn_n = d.link_up_clean[h];
           const float dx = d.row_x[r] - d.row_x[r0], dy = p1.x - p0.x, dz = p1.y - p0.y;
           const float ds = sqrtf(fmaf(dx, dx, dy * dy));
           k.x = d.row_x[r0];
@@ -221,10 +224,12 @@ __global__ void __launch_bounds__(E_THREADS, E1_BOUNDS) k_tl_e1(Dev d) {
       if (__ballot_sync(FULL, !exhausted) == 0u) break;
     }
     if (!busy) continue;
-    // ---- one chain step (loads first: they do not depend on the filter state)
+    // ---- one chain step.  The chain h -> link[h] -> yz[link[h]] is two dependent gathers per step; they are taken one
+    // step ahead (pc, hn of THIS step were loaded during the previous one), so their latency hides behind the filter.
     n_steps++;
-    const float2 pc = d.yz[h];
-    const int hn = d.link_up_clean[h];
+    const float2 pc = pc_n;
+    const int hn = hn_n;
+    if (hn >= 0) { pc_n = d.yz[hn]; hn_n = d.link_up_clean[hn]; }
     const int rs2 = (r + 2 < R) ? d.row_start[sbase + r + 2] : 0x7fffffff;
     if (!kf_transport(k, d.row_x[r], d.kq, d.P.max_sinphi)) { valid = false; busy = false; continue; }
     kf_update(k, pc.x, pc.y - z_ref, d.sy2, d.sz2);
