@@ -372,7 +372,7 @@ def run_gpu(args):
         "grid": 36.0 * n + 12.0 * stats["n_bins"],
         "clean_start": 32.0 * n,
         "select": 12.0 * stats["tracklet_hits"] + 12.0 * n,
-        "refit": 12.0 * 3 * stats["track_hits"] + 128.0 * hd["n_tracks"],
+        "refit": 12.0 * stats["track_hits"] + 128.0 * hd["n_tracks"],  # the hits are moved once, three passes reuse them
     }
     alg_kernel = {
         "k_slice_scatter": 32.0 * n, "k_slice_sort": 30.0 * n + 4.0 * stats["n_bins"],
