@@ -31,15 +31,17 @@ DEFAULT_TIME_PARAMS = dict(vdrift=2.58, z_max=250.0)  # cm/us, cm (BASELINE.json
 
 
 # DESIGN.md section 14 Table D defaults of the looper-leg finder and the cluster tags (the product keeps its own copy)
-DEFAULT_LEG_PARAMS = dict(leg_min_qpt=4.0, leg_min_sinphi=0.5, leg_apex_margin=2.0, leg_max_sector_gap=5,
-                          leg_max_turn=2.9, leg_centre_frac=0.05, leg_centre_abs=1.5, leg_radius_frac=0.2,
+DEFAULT_LEG_PARAMS = dict(leg_min_qpt=4.0, leg_min_sinphi=0.5, leg_inner_min_sinphi=0.2, leg_apex_margin=2.0, leg_max_sector_gap=5,
+                          leg_inner_max_sector_gap=9, leg_max_turn=2.9, leg_inner_max_turn=5.0, leg_centre_frac=0.05, leg_centre_abs=1.5, leg_radius_frac=0.2,
                           leg_dz_max=4.0, leg_dzds_tol=0.1, tag_qpt_low=20.0, tag_qpt_leg=5.0, tag_sinphi=0.8, ring=18)
 TAG_LOW_PT, TAG_EXTRA_LEG, TAG_HIGH_INCLINATION = 1, 2, 4
 
 
 class _LegParams(C.Structure):
-    _fields_ = [("leg_min_qpt", C.c_float), ("leg_min_sinphi", C.c_float), ("leg_apex_margin", C.c_float),
-                ("leg_max_sector_gap", C.c_int32), ("leg_max_turn", C.c_float), ("leg_centre_frac", C.c_float),
+    _fields_ = [("leg_min_qpt", C.c_float), ("leg_min_sinphi", C.c_float), ("leg_inner_min_sinphi", C.c_float),
+                ("leg_apex_margin", C.c_float),
+                ("leg_max_sector_gap", C.c_int32), ("leg_inner_max_sector_gap", C.c_int32), ("leg_max_turn", C.c_float),
+                ("leg_inner_max_turn", C.c_float), ("leg_centre_frac", C.c_float),
                 ("leg_centre_abs", C.c_float), ("leg_radius_frac", C.c_float), ("leg_dz_max", C.c_float),
                 ("leg_dzds_tol", C.c_float), ("tag_qpt_low", C.c_float), ("tag_qpt_leg", C.c_float),
                 ("tag_sinphi", C.c_float), ("ring", C.c_int32)]
@@ -131,14 +133,14 @@ def _load(opt: str = "-O2"):
         lib.orc_legs.restype = C.c_int64
         lib.orc_legs.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_float, C.POINTER(_Params), C.c_void_p,
                                  C.POINTER(_LegParams)]
-        for name in ("orc_leg_partner", "orc_leg_first", "orc_cluster_tags"):
+        for name in ("orc_leg_partner", "orc_leg_partner_in", "orc_leg_first", "orc_cluster_tags"):
             getattr(lib, name).restype = C.c_void_p
             getattr(lib, name).argtypes = [C.c_void_p]
         lib.orc_angle_upper.restype = C.c_float
         lib.orc_angle_upper.argtypes = [C.c_float, C.c_float]
-        lib.orc_leg_end.argtypes = [C.c_void_p, C.c_float, C.c_float, C.POINTER(_LegParams), C.c_void_p]
+        lib.orc_leg_end.argtypes = [C.c_int32, C.c_void_p, C.c_float, C.c_float, C.POINTER(_LegParams), C.c_void_p]
         lib.orc_leg_pair.restype = C.c_float
-        lib.orc_leg_pair.argtypes = [C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_float, C.POINTER(_LegParams)]
+        lib.orc_leg_pair.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_float, C.c_float, C.c_float, C.POINTER(_LegParams)]
         lib.orc_time_estimate.argtypes = [C.c_void_p, C.c_int32, C.c_float, C.c_void_p, C.c_float, C.c_float, C.c_void_p]
         lib.orc_time_estimate_state.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_float, C.c_int32, C.c_float,
                                                 C.c_float, C.c_void_p]
@@ -185,6 +187,7 @@ class OracleResult:
     track_merged: np.ndarray = None  # sector track -> merged track
     link_next: np.ndarray = None     # sector track -> continuation or -1 (O9)
     leg_partner: np.ndarray = None   # merged track -> merged track joined at the outer turning point or -1 (O12); with legs=...
+    leg_partner_in: np.ndarray = None  # merged track -> merged track joined through the inner region or -1
     leg_first: np.ndarray = None     # merged track: 1 first / only leg, 0 additional leg
     cluster_tags: np.ndarray = None  # uint8 per cluster: TAG_* bits (O13)
     time_sector: np.ndarray = None   # (n_tracks, 4): z_dca, z_shift, t0_us, dca_xy (O11); only with time=...
@@ -245,6 +248,7 @@ def track(clusters: np.ndarray, sector_offsets: np.ndarray, row_x: np.ndarray, b
             lp = _leg_params(legs)
             lib.orc_legs(h, nr, rx.ctypes.data, bz, C.byref(cp), cl.ctypes.data, C.byref(lp))
             res.leg_partner = _arr(lib.orc_leg_partner(h), len(res.merged), np.int32)
+            res.leg_partner_in = _arr(lib.orc_leg_partner_in(h), len(res.merged), np.int32)
             res.leg_first = _arr(lib.orc_leg_first(h), len(res.merged), np.uint8)
             res.cluster_tags = _arr(lib.orc_cluster_tags(h), n, np.uint8)
         if time:
@@ -317,19 +321,19 @@ def angle_upper(y, x, opt="-O2"):
     return float(_load(opt).orc_angle_upper(float(y), float(x)))
 
 
-def leg_end(state7, bz=0.5, x_last=245.0, legs=None, opt="-O2"):
-    """O12 on one outer end (sector, x, y, z, sinphi, dzds, qpt): returns (candidate, R, xc, yc, cos phi)."""
+def leg_end(state7, bz=0.5, x_last=245.0, legs=None, opt="-O2", sig=1):
+    """O12 on one end (sector, x, y, z, sinphi, dzds, qpt), sig = +1 outer / -1 inner: returns (candidate, R, xc, yc, cos phi)."""
     lib = _load(opt)
     st = np.array(state7, np.float32)
     out = np.zeros(5, np.float32)
     lp = _leg_params(legs)
-    lib.orc_leg_end(st.ctypes.data, bz, x_last, C.byref(lp), out.ctypes.data)
+    lib.orc_leg_end(sig, st.ctypes.data, bz, x_last, C.byref(lp), out.ctypes.data)
     return bool(out[0]), float(out[1]), float(out[2]), float(out[3]), float(out[4])
 
 
-def leg_pair(a7, b7, bz=0.5, x_last=245.0, tan_half_angle=DEFAULT_PARAMS["tan_half_angle"], legs=None, opt="-O2"):
-    """O12 pair score of two outer ends (a7 plays the lower id), negative = no match."""
+def leg_pair(a7, b7, bz=0.5, x_last=245.0, tan_half_angle=DEFAULT_PARAMS["tan_half_angle"], legs=None, opt="-O2", sig=1):
+    """O12 pair score of two ends of one kind (sig = +1 outer, -1 inner; a7 plays the lower id), negative = no match."""
     lib = _load(opt)
     a, b = np.array(a7, np.float32), np.array(b7, np.float32)
     lp = _leg_params(legs)
-    return float(lib.orc_leg_pair(a.ctypes.data, b.ctypes.data, bz, x_last, tan_half_angle, C.byref(lp)))
+    return float(lib.orc_leg_pair(sig, a.ctypes.data, b.ctypes.data, bz, x_last, tan_half_angle, C.byref(lp)))

@@ -196,6 +196,7 @@ struct Result {
   std::vector<int32_t> link_next;                // sector track -> sector track it continues into, or -1
   // looper legs and cluster tags (O12, O13)
   std::vector<int32_t> leg_partner;              // merged track -> merged track joined at the outer turning point, or -1
+  std::vector<int32_t> leg_partner_in;           // merged track -> merged track joined through the inner region, or -1
   std::vector<uint8_t> leg_first;                // merged track: 1 = first (or only) leg, 0 = additional leg
   std::vector<uint8_t> cluster_tags;             // per cluster: TAG_* bits
 };
@@ -663,9 +664,9 @@ TimeRec time_estimate(const TrackRec& T, double kq, double zmin_hits, double zma
 
 // ---- O12-O13: legs of low-pT loopers and cluster tags ----
 struct LegParams {
-  float leg_min_qpt, leg_min_sinphi, leg_apex_margin;
-  int32_t leg_max_sector_gap;
-  float leg_max_turn, leg_centre_frac, leg_centre_abs, leg_radius_frac, leg_dz_max, leg_dzds_tol;
+  float leg_min_qpt, leg_min_sinphi, leg_inner_min_sinphi, leg_apex_margin;
+  int32_t leg_max_sector_gap, leg_inner_max_sector_gap;
+  float leg_max_turn, leg_inner_max_turn, leg_centre_frac, leg_centre_abs, leg_radius_frac, leg_dz_max, leg_dzds_tol;
   float tag_qpt_low, tag_qpt_leg, tag_sinphi;
   int32_t ring;
 };
@@ -693,43 +694,63 @@ inline float angle_upper(float y, float x) {
   return pi + atan_unit(y / x);
 }
 
-struct LegEnd {  // outer end of a merged track in the frame of its outermost sector segment
-  int32_t sector;
+struct LegEnd {  // an end of a merged track: the outer end in the frame of its outermost sector segment (sig = +1: the helix
+  int32_t sector;  // continues along the fit direction), or the inner end in the frame of its innermost segment (sig = -1: against it)
+  int32_t sig;
   float x, y, z, s, t, q;
   float c, R, xc, yc;  // cos(phi), radius, circle centre
   bool cand;
 };
 
-inline LegEnd leg_end(int sector, float x, float y, float z, float s, float t, float q, bool valid, float kq, float x_last,
-                      const LegParams& L) {
+inline LegEnd leg_end(int sig, int sector, float x, float y, float z, float s, float t, float q, bool valid, float kq,
+                      float x_last, const LegParams& L) {
   LegEnd e;
-  e.sector = sector; e.x = x; e.y = y; e.z = z; e.s = s; e.t = t; e.q = q;
+  e.sig = sig; e.sector = sector; e.x = x; e.y = y; e.z = z; e.s = s; e.t = t; e.q = q;
   e.c = 0; e.R = 0; e.xc = 0; e.yc = 0; e.cand = false;
-  if (!valid || !(std::fabs(q) >= L.leg_min_qpt) || !(std::fabs(s) >= L.leg_min_sinphi) || !(std::fabs(s) < 1.0f)) return e;
+  const float smin = sig > 0 ? L.leg_min_sinphi : L.leg_inner_min_sinphi;
+  if (!valid || !(std::fabs(q) >= L.leg_min_qpt) || !(std::fabs(s) >= smin) || !(std::fabs(s) < 1.0f)) return e;
   const float k = q * kq;
   e.c = std::sqrt(fma32(-s, s, 1.0f));
   e.R = 1.0f / std::fabs(k);
   e.xc = x - s / k;
   e.yc = y + e.c / k;
-  e.cand = (e.xc + e.R) <= (x_last + L.leg_apex_margin);  // the helix turns back inside the TPC
+  e.cand = sig < 0 || (e.xc + e.R) <= (x_last + L.leg_apex_margin);  // outer end: the helix turns back inside the TPC
   return e;
 }
 
-// Score of the pair (A, B) -- A is the track with the lower id -- or a negative value if the ends do not belong to the two
-// legs of one turn.  Everything is evaluated in A's frame; B's frame lies j sector steps ahead in A's turning sense.
+// Score of the pair (A, B) -- A is the track with the lower id, both ends of the same kind -- or a negative value if the
+// helix continued from A does not arrive at B.  Everything is evaluated in A's frame; B's frame lies j sector steps ahead
+// in A's turning sense.  For inner ends (sig = -1) the helix is continued AGAINST the fit direction: the turning sense and
+// the slope change sign, the products of the two direction vectors do not.
 inline float leg_pair_score(const LegEnd& A, const LegEnd& B, float kq, float ca, float sa, const LegParams& L) {
   if (!A.cand || !B.cand) return -1.0f;
   if (!(A.q * B.q < 0.0f)) return -1.0f;  // the two legs of a turn are fitted in opposite senses
   if (L.ring <= 0) { if (A.sector != B.sector) return -1.0f; }
   else if (A.sector / L.ring != B.sector / L.ring) return -1.0f;  // same z side
-  const int sgn = (A.q * kq > 0.0f) ? 1 : -1;  // curvature sign = sense in which sin(phi) grows along the fit direction
-  int j = 0;
-  if (L.ring > 0) j = (((B.sector - A.sector) * sgn) % L.ring + L.ring) % L.ring;
-  if (j > L.leg_max_sector_gap) return -1.0f;
-  // B's end point, centre and fit direction in A's frame: j rotations by the sector angle
-  const float ss = (float)sgn * sa;
+  if (A.sig != B.sig) return -1.0f;
+  const float sig = (float)A.sig;
+  const int sgn = ((sig * A.q) * kq > 0.0f) ? 1 : -1;  // sense in which the direction turns along the continuation
+  // B's frame relative to A's: jrot sector steps (B's axis = A's axis + jrot * sector angle).  Over a turning point the
+  // partner lies at most leg_max_sector_gap steps AHEAD in the turning sense; through the inner region the helix passes
+  // near the beam line, where the azimuth of the position jumps by half a turn, so any sector of the side within
+  // leg_inner_max_sector_gap steps either way is allowed.
+  int jrot = 0;
+  if (L.ring > 0) {
+    const int dsec = ((B.sector - A.sector) % L.ring + L.ring) % L.ring;
+    if (A.sig > 0) {
+      const int j = ((dsec * sgn) % L.ring + L.ring) % L.ring;
+      if (j > L.leg_max_sector_gap) return -1.0f;
+      jrot = sgn * j;
+    } else {
+      jrot = (2 * dsec <= L.ring) ? dsec : dsec - L.ring;
+      if (std::abs(jrot) > L.leg_inner_max_sector_gap) return -1.0f;
+    }
+  }
+  // B's end point, centre and fit direction in A's frame: |jrot| rotations by the sector angle
+  const float ss = (jrot >= 0) ? sa : -sa;
+  const int nrot = std::abs(jrot);
   float bx = B.x, by = B.y, bxc = B.xc, byc = B.yc, bdx = B.c, bdy = B.s;
-  for (int i = 0; i < j; i++) {
+  for (int i = 0; i < nrot; i++) {
     float u = fma32(-by, ss, bx * ca), v = fma32(bx, ss, by * ca);
     bx = u; by = v;
     u = fma32(-byc, ss, bxc * ca); v = fma32(bxc, ss, byc * ca);
@@ -742,9 +763,15 @@ inline float leg_pair_score(const LegEnd& A, const LegEnd& B, float kq, float ca
   const float dot = -fma32(A.s, bdy, A.c * bdx);
   const float cross = fma32(A.s, bdx, -(A.c * bdy));
   const float yy = (float)sgn * cross;
-  if (!(yy > 0.0f)) return -1.0f;
-  const float theta = angle_upper(yy, dot);
-  if (!(theta <= L.leg_max_turn)) return -1.0f;
+  // turning angle in (0, 2 pi) in the turning sense; over a turning point it stays below half a turn (leg_max_turn < pi),
+  // through the inner region it may be most of a turn
+  const float two_pi = 6.28318530718f, pi = 3.14159265359f;
+  float theta;
+  if (yy > 0.0f) theta = angle_upper(yy, dot);
+  else if (yy < 0.0f) theta = two_pi - angle_upper(-yy, dot);
+  else if (dot < 0.0f) theta = pi;
+  else return -1.0f;
+  if (!(theta <= (A.sig > 0 ? L.leg_max_turn : L.leg_inner_max_turn))) return -1.0f;
   const float Rm = 0.5f * (A.R + B.R);
   const float arc = theta * Rm;
   const float dxc = A.xc - bxc, dyc = A.yc - byc;
@@ -754,7 +781,7 @@ inline float leg_pair_score(const LegEnd& A, const LegEnd& B, float kq, float ca
   if (!(dc2 <= tolc2)) return -1.0f;
   const float dR = A.R - B.R, tolR = L.leg_radius_frac * Rm;
   if (!(std::fabs(dR) <= tolR)) return -1.0f;
-  const float tm = 0.5f * (A.t - B.t);
+  const float tm = sig * (0.5f * (A.t - B.t));  // mean slope along the continuation
   const float dz = fma32(-tm, arc, B.z - A.z);
   if (!(std::fabs(dz) <= L.leg_dz_max)) return -1.0f;
   const float dt = A.t + B.t;
@@ -774,41 +801,52 @@ void find_legs(Result* R, const Ctx& c, const LegParams& L) {
   const float den = fma32(th, th, 1.0f);
   const float ca = fma32(-th, th, 1.0f) / den, sa = (2.0f * th) / den;
   const float x_last = c.row_x[c.n_rows - 1];
-  // outer end of every merged track = outer state (O8) of the last sector segment of its chain
-  std::vector<LegEnd> ends(nm);
+  // ends of every merged track: outer = outer state (O8) of the last sector segment of its chain; inner = its own record
+  std::vector<LegEnd> outer(nm), inner(nm);
   for (int m = 0; m < nm; m++) {
-    int tail = R->merged[m].pad[4];
+    const TrackRec& Mr = R->merged[m];
+    const int head = Mr.pad[4];
+    int tail = head;
     while (R->link_next[tail] >= 0) tail = R->link_next[tail];
     const KF& o = R->outer[tail];
-    ends[m] = leg_end(R->tracks[tail].sector, o.x, o.p[0], o.p[1] + R->outer_zref[tail], o.p[2], o.p[3], o.p[4],
-                      R->tracks[tail].ndf >= 0, c.kq, x_last, L);
+    outer[m] = leg_end(+1, R->tracks[tail].sector, o.x, o.p[0], o.p[1] + R->outer_zref[tail], o.p[2], o.p[3], o.p[4],
+                       R->tracks[tail].ndf >= 0, c.kq, x_last, L);
+    inner[m] = leg_end(-1, Mr.sector, Mr.x, Mr.y, Mr.z, Mr.sinphi, Mr.dzds, Mr.qpt, R->tracks[head].ndf >= 0, c.kq, x_last, L);
   }
-  // O12: best partner of every end (min by (score, id)), mutual pairs are linked
-  std::vector<int32_t> best(nm, -1);
-  std::vector<float> bs(nm, 0.0f);
-  for (int a = 0; a < nm; a++) {
-    if (!ends[a].cand) continue;
-    for (int b = a + 1; b < nm; b++) {
-      if (!ends[b].cand) continue;
-      const float sc = leg_pair_score(ends[a], ends[b], c.kq, ca, sa, L);
-      if (!(sc >= 0.0f)) continue;
-      if (best[a] < 0 || sc < bs[a]) { best[a] = b; bs[a] = sc; }   // equal score: the lower id stays (b increases)
-      if (best[b] < 0 || sc < bs[b]) { best[b] = a; bs[b] = sc; }   // equal score: the lower id stays (a increases)
+  // O12: best partner of every end among the ends of its kind (min by (score, id)), mutual pairs are linked
+  auto match = [&](const std::vector<LegEnd>& ends, std::vector<int32_t>& partner) {
+    std::vector<int32_t> best(nm, -1);
+    std::vector<float> bs(nm, 0.0f);
+    for (int a = 0; a < nm; a++) {
+      if (!ends[a].cand) continue;
+      for (int b = a + 1; b < nm; b++) {
+        if (!ends[b].cand) continue;
+        const float sc = leg_pair_score(ends[a], ends[b], c.kq, ca, sa, L);
+        if (!(sc >= 0.0f)) continue;
+        if (best[a] < 0 || sc < bs[a]) { best[a] = b; bs[a] = sc; }   // equal score: the lower id stays (b increases)
+        if (best[b] < 0 || sc < bs[b]) { best[b] = a; bs[b] = sc; }   // equal score: the lower id stays (a increases)
+      }
     }
-  }
-  R->leg_partner.assign(nm, -1);
+    partner.assign(nm, -1);
+    for (int a = 0; a < nm; a++) {
+      const int b = best[a];
+      if (b >= 0 && best[b] == a) partner[a] = b;
+    }
+  };
+  match(outer, R->leg_partner);
+  match(inner, R->leg_partner_in);
+  // Legs joined at turning points (outer) and through the inner region (inner) form a chain along which |z| of the inner
+  // ends grows (the particle drifts away from the side it was born on; the shift of a time frame is common to all legs).
+  // The first leg is the one none of whose linked neighbours lies at a smaller |z| (equal |z|: the lower id).
   R->leg_first.assign(nm, 1);
   for (int a = 0; a < nm; a++) {
-    const int b = best[a];
-    if (b >= 0 && best[b] == a) R->leg_partner[a] = b;
-  }
-  // the first leg of a pair is the one whose inner end lies at the smaller |z| (the vertex side of the drift volume)
-  for (int a = 0; a < nm; a++) {
-    const int b = R->leg_partner[a];
-    if (b < 0) continue;
-    const float za = std::fabs(R->merged[a].z), zb = std::fabs(R->merged[b].z);
-    const bool a_first = (za < zb) || (za == zb && a < b);
-    R->leg_first[a] = a_first ? 1 : 0;
+    const float za = std::fabs(R->merged[a].z);
+    for (int kind = 0; kind < 2; kind++) {
+      const int b = kind == 0 ? R->leg_partner[a] : R->leg_partner_in[a];
+      if (b < 0) continue;
+      const float zb = std::fabs(R->merged[b].z);
+      if (zb < za || (zb == za && b < a)) R->leg_first[a] = 0;
+    }
   }
   // O13: cluster tags
   R->cluster_tags.assign((size_t)R->n, 0);
@@ -981,26 +1019,28 @@ int64_t orc_legs(void* r, int32_t n_rows, const float* row_x, float bz, const Pa
   Ctx c = make_ctx(cl, row_x, n_rows, *P, bz, false);
   find_legs(R, c, *L);
   int64_t n = 0;
-  for (size_t m = 0; m < R->leg_partner.size(); m++) n += (R->leg_partner[m] > (int32_t)m) ? 1 : 0;
+  for (size_t m = 0; m < R->leg_partner.size(); m++)
+    n += ((R->leg_partner[m] > (int32_t)m) ? 1 : 0) + ((R->leg_partner_in[m] > (int32_t)m) ? 1 : 0);
   return n;
 }
 const int32_t* orc_leg_partner(void* r) { return ((Result*)r)->leg_partner.data(); }
+const int32_t* orc_leg_partner_in(void* r) { return ((Result*)r)->leg_partner_in.data(); }
 const uint8_t* orc_leg_first(void* r) { return ((Result*)r)->leg_first.data(); }
 const uint8_t* orc_cluster_tags(void* r) { return ((Result*)r)->cluster_tags.data(); }
 float orc_angle_upper(float y, float x) { return angle_upper(y, x); }
-// one end: state7 = sector, x, y, z, sinphi, dzds, qpt -> out5 = cand, R, xc, yc, c
-void orc_leg_end(const float* state7, float bz, float x_last, const LegParams* L, float* out5) {
+// one end (sig = +1 outer, -1 inner): state7 = sector, x, y, z, sinphi, dzds, qpt -> out5 = cand, R, xc, yc, c
+void orc_leg_end(int32_t sig, const float* state7, float bz, float x_last, const LegParams* L, float* out5) {
   const float kq = -((0.000299792458f * 10.0f) * bz);
-  const LegEnd e = leg_end((int)state7[0], state7[1], state7[2], state7[3], state7[4], state7[5], state7[6], true, kq, x_last, *L);
+  const LegEnd e = leg_end(sig, (int)state7[0], state7[1], state7[2], state7[3], state7[4], state7[5], state7[6], true, kq, x_last, *L);
   out5[0] = e.cand ? 1.0f : 0.0f; out5[1] = e.R; out5[2] = e.xc; out5[3] = e.yc; out5[4] = e.c;
 }
-// pair score of two ends (A = first argument, taken as the lower id), or a negative value
-float orc_leg_pair(const float* a7, const float* b7, float bz, float x_last, float tan_half_angle, const LegParams* L) {
+// pair score of two ends of kind sig (A = first argument, taken as the lower id), or a negative value
+float orc_leg_pair(int32_t sig, const float* a7, const float* b7, float bz, float x_last, float tan_half_angle, const LegParams* L) {
   const float kq = -((0.000299792458f * 10.0f) * bz);
   const float den = fma32(tan_half_angle, tan_half_angle, 1.0f);
   const float ca = fma32(-tan_half_angle, tan_half_angle, 1.0f) / den, sa = (2.0f * tan_half_angle) / den;
-  const LegEnd A = leg_end((int)a7[0], a7[1], a7[2], a7[3], a7[4], a7[5], a7[6], true, kq, x_last, *L);
-  const LegEnd B = leg_end((int)b7[0], b7[1], b7[2], b7[3], b7[4], b7[5], b7[6], true, kq, x_last, *L);
+  const LegEnd A = leg_end(sig, (int)a7[0], a7[1], a7[2], a7[3], a7[4], a7[5], a7[6], true, kq, x_last, *L);
+  const LegEnd B = leg_end(sig, (int)b7[0], b7[1], b7[2], b7[3], b7[4], b7[5], b7[6], true, kq, x_last, *L);
   return leg_pair_score(A, B, kq, ca, sa, *L);
 }
 

@@ -192,6 +192,106 @@ def test_radius_term():
             assert abs(sc - ((1 - f) / (0.2 * 0.5 * (1 + f))) ** 2) < 0.01
 
 
+# ---------------------------------------------------------------- inner ends: the passage below the first pad row
+def _end_on_circle(cx, cy, R, w, a, z, tanl):
+    """Fitted-state view (sector, x, y, z, sin phi, dz/ds, q/pT) of the point at angle `a` of a float64 circle (centre
+    (cx, cy) in the global frame, sense of rotation w = +-1), side A: the fit runs with cos(phi) > 0 in the sector frame,
+    so a particle flying inward is described against its flight (sin phi, dz/ds and q/pT change sign)."""
+    gx, gy = cx + R * np.cos(a), cy + R * np.sin(a)
+    sec = int(np.floor((np.degrees(np.arctan2(gy, gx)) % 360.0) / 20.0))
+    al = np.deg2rad(20.0 * sec + 10.0)
+    x = gx * np.cos(al) + gy * np.sin(al)
+    y = -gx * np.sin(al) + gy * np.cos(al)
+    ta = a + w * np.pi / 2 - al                      # direction of flight in the sector frame
+    k = w / R
+    qpt = k / KQ
+    if np.cos(ta) > 0:
+        return [sec, x, y, z, np.sin(ta), tanl, qpt]
+    return [sec, x, y, z, -np.sin(ta), -tanl, -qpt]
+
+
+def _inner_pair(R, w, tanl=0.3, d=0.0, phi=0.4, r_in=85.0, z1=50.0):
+    """Two points at radius r_in of a circle that passes at distance d from the beam line: where the particle dives below
+    the first pad row (end of a returning leg) and where it comes out again (start of the next outgoing leg).
+    Returns (returning leg's inner end, outgoing leg's inner end, turning angle between them)."""
+    rc = R + d                                      # distance of the centre from the beam line
+    cx, cy = rc * np.cos(phi), rc * np.sin(phi)
+    # points of the circle at distance r_in from the origin: angle g from the direction centre -> origin
+    cosg = (R * R + rc * rc - r_in * r_in) / (2 * R * rc)
+    g = np.arccos(cosg)
+    a0 = phi + np.pi                                # point of the circle nearest to the beam line
+    a_in, a_out = a0 - w * g, a0 + w * g            # flight order: a_in, nearest point, a_out
+    turn = 2 * g
+    e_in = _end_on_circle(cx, cy, R, w, a_in, z1, tanl)
+    e_out = _end_on_circle(cx, cy, R, w, a_out, z1 + tanl * R * turn, tanl)
+    return e_in, e_out, turn
+
+
+@pytest.mark.parametrize("w", [+1, -1])
+@pytest.mark.parametrize("R,d", [(95.0, 0.0), (80.0, 0.0), (55.0, 0.0), (47.0, 0.0), (70.0, 6.0), (120.0, -4.0)])
+@pytest.mark.parametrize("phi", [0.4, 2.0, 5.9])
+def test_two_inner_ends_of_one_helix_match_with_score_zero(R, d, w, phi):
+    """Through the region below the first pad row the particle turns by 2*acos(...) -- more than half a turn for R < 60 cm
+    -- and, passing close to the beam line, comes out up to nine sectors away on either side."""
+    e_in, e_out, turn = _inner_pair(R, w, d=d, phi=phi)
+    assert 1.2 < turn < 5.0
+    for a7, b7 in ((e_in, e_out), (e_out, e_in)):   # either leg may carry the lower id
+        sc = oracle.leg_pair(a7, b7, sig=-1)
+        assert 0 <= sc < 5e-4, (sc, turn, e_in, e_out)
+    assert oracle.leg_pair(e_in, e_out, sig=+1) < 0          # as OUTER ends these two do not continue into each other
+
+
+def test_inner_pair_terms():
+    e_in, e_out, turn = _inner_pair(80.0, +1, tanl=0.3)
+    R = 80.0
+    # z: along the continuation of an inner end the slope has the opposite sign of the fitted one
+    b = list(e_out); b[3] += 2.0
+    assert abs(oracle.leg_pair(e_in, b, sig=-1) - 0.25) < 3e-3
+    b = list(e_out); b[3] -= 2 * 0.3 * R * turn      # the z a wrong slope sign would predict
+    assert oracle.leg_pair(e_in, b, sig=-1) < 0
+    # turn limit and sector limit of the inner kind are their own parameters
+    assert oracle.leg_pair(e_in, e_out, sig=-1, legs=dict(leg_inner_max_turn=float(turn) - 0.01)) < 0
+    assert oracle.leg_pair(e_in, e_out, sig=-1, legs=dict(leg_inner_max_turn=float(turn) + 0.01, leg_max_turn=0.1)) >= 0
+    dsec = (e_out[0] - e_in[0]) % 18
+    dsec = min(dsec, 18 - dsec)
+    assert dsec >= 4
+    assert oracle.leg_pair(e_in, e_out, sig=-1, legs=dict(leg_inner_max_sector_gap=dsec - 1)) < 0
+    assert oracle.leg_pair(e_in, e_out, sig=-1, legs=dict(leg_inner_max_sector_gap=dsec, leg_max_sector_gap=0)) >= 0
+    # candidates: the inner kind has its own sin(phi) threshold and no turning-point condition
+    st = [3, 85.0, 2.0, 10.0, 0.3, 0.2, 7.0]
+    assert oracle.leg_end(st, sig=-1)[0] and not oracle.leg_end(st, sig=+1)[0]
+    st[4] = 0.15
+    assert not oracle.leg_end(st, sig=-1)[0]
+    big = [3, 85.0, 2.0, 10.0, 0.3, 0.2, 4.5]      # R = 148 cm: the helix leaves the TPC on its way out, but it came from below
+    assert oracle.leg_end(big, sig=-1)[0] and not oracle.leg_end([3, 240.0, 2.0, 10.0, -0.9, 0.2, 4.5], sig=+1)[0]
+    # more than half a turn: the angle comes from the lower half plane (R = 47 cm: 258 degrees)
+    e_in, e_out, turn = _inner_pair(47.0, -1, tanl=0.2)
+    assert turn > np.pi + 0.5
+    b = list(e_out); b[3] += 1.0
+    assert abs(oracle.leg_pair(e_in, b, sig=-1) - 1.0 / 16) < 2e-3   # pins arc = turn * R beyond pi
+
+
+def test_two_turns_are_chained_through_the_inner_region(row_x):
+    """Two full turns of a 120 MeV/c particle: outgoing 1 -(turning point)- returning 1 -(inner region)- outgoing 2
+    -(turning point)- returning 2.  One chain, its first leg is outgoing 1, every other leg is tagged as additional."""
+    for q in (+1, -1):
+        p = looper.helix_clusters(row_x, 0.12, 0.7, 0.3, q, z0=10.0, turns=2.0, z_max=400.0)
+        fr, info = looper.frame_from([p])
+        res = _run(fr, row_x)
+        am = _merged_of_cluster(res)
+        nm = len(res.merged)
+        assert nm == 4
+        th = np.array([info["theta"][am == m].mean() for m in range(nm)])
+        order = np.argsort(th)                      # flight order of the four legs
+        o1, r1, o2, r2 = order
+        assert res.leg_partner[o1] == r1 and res.leg_partner[o2] == r2
+        assert res.leg_partner_in[r1] == o2 and res.leg_partner_in[o2] == r1
+        assert res.leg_partner_in[o1] == -1 and res.leg_partner_in[r2] == -1
+        assert list(res.leg_first[order]) == [1, 0, 0, 0]
+        extra = (res.cluster_tags & oracle.TAG_EXTRA_LEG) > 0
+        assert np.array_equal(extra, (am >= 0) & (am != o1))
+
+
 # ---------------------------------------------------------------- whole path on hand-built loopers
 def test_noiseless_looper_outgoing_and_returning_leg_are_linked(row_x):
     """One 120 MeV/c particle from the origin: the chain of sector segments up to the turning point and the chain coming
@@ -289,19 +389,41 @@ def event(row_x):
     return fr, _run(fr, row_x)
 
 
+def _chains(res):
+    """Union of both kinds of links: chain label of every merged track."""
+    nm = len(res.merged)
+    parent = np.arange(nm)
+
+    def find(x):
+        while parent[x] != x:
+            parent[x] = parent[parent[x]]
+            x = parent[x]
+        return x
+
+    for lp in (res.leg_partner, res.leg_partner_in):
+        for m in np.where(lp >= 0)[0]:
+            parent[find(m)] = find(lp[m])
+    return np.array([find(m) for m in range(nm)])
+
+
 def test_leg_invariants(event):
     fr, res = event
-    lp, lf = res.leg_partner, res.leg_first
+    lf = res.leg_first
     nm = len(res.merged)
-    linked = np.where(lp >= 0)[0]
-    assert len(linked) >= 400 and len(linked) % 2 == 0
-    assert np.array_equal(lp[lp[linked]], linked) and (lp[linked] != linked).all()      # an involution without fixed points
-    assert (lf[lp < 0] == 1).all() and (lf[linked] + lf[lp[linked]] == 1).all()           # exactly one first leg per pair
-    z = np.abs(res.merged["z"])
-    firsts = linked[lf[linked] == 1]
-    assert (z[firsts] <= z[lp[firsts]]).all()
     q = res.merged["qpt"]
-    assert (q[linked] * q[lp[linked]] < 0).all()
+    for lp, n_min in ((res.leg_partner, 400), (res.leg_partner_in, 300)):
+        linked = np.where(lp >= 0)[0]
+        assert len(linked) >= n_min and len(linked) % 2 == 0
+        assert np.array_equal(lp[lp[linked]], linked) and (lp[linked] != linked).all()   # an involution without fixed points
+        assert (q[linked] * q[lp[linked]] < 0).all()                                     # neighbouring legs are fitted in opposite senses
+    # exactly one first leg per chain, and it is the leg whose inner end lies at the smallest |z|
+    root = _chains(res)
+    z = np.abs(res.merged["z"])
+    for r in np.unique(root):
+        members = np.where(root == r)[0]
+        firsts = members[lf[members] == 1]
+        assert len(firsts) == 1
+        assert z[firsts[0]] == z[members].min()
     tags = res.cluster_tags
     assert (tags[res.assignment < 0] == 0).all() and (tags < 8).all()
     am = _merged_of_cluster(res)
@@ -325,10 +447,12 @@ def test_legs_join_the_same_particle(event):
         l = l[l >= 0]
         if len(l):
             lab[m] = np.bincount(l).argmax()
+    for lp in (res.leg_partner, res.leg_partner_in):
+        linked = np.where(lp > np.arange(nm))[0]
+        same = lab[linked] == lab[lp[linked]]
+        assert same.mean() >= 0.99, same.mean()
+        assert (fr.track_par[lab[linked], 0] < 0.25).all()
     linked = np.where(res.leg_partner > np.arange(nm))[0]
-    same = lab[linked] == lab[res.leg_partner[linked]]
-    assert same.mean() >= 0.99, same.mean()
-    assert (fr.track_par[lab[linked], 0] < 0.25).all()
     # a sizeable share of the loopers that reach the TPC have their first turn linked
     loopers = np.where((fr.track_par[:, 0] < 0.15) & (fr.track_par[:, 0] > 0.07))[0]
     found = np.isin(loopers, lab[linked]).mean()
@@ -340,6 +464,7 @@ def test_legs_permutation_invariance(event, row_x):
     fr2, p = synth.permute_within_sectors(fr, 11)
     res2 = _run(fr2, row_x)
     assert np.array_equal(res2.leg_partner, res.leg_partner) and np.array_equal(res2.leg_first, res.leg_first)
+    assert np.array_equal(res2.leg_partner_in, res.leg_partner_in)
     assert np.array_equal(res2.cluster_tags, res.cluster_tags[p])
 
 
@@ -348,3 +473,4 @@ def test_legs_optimisation_level_independent(row_x):
     a = _run(fr, row_x)
     b = _run(fr, row_x, opt="-O0")
     assert np.array_equal(a.leg_partner, b.leg_partner) and np.array_equal(a.cluster_tags, b.cluster_tags)
+    assert np.array_equal(a.leg_partner_in, b.leg_partner_in) and np.array_equal(a.leg_first, b.leg_first)
