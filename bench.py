@@ -281,7 +281,7 @@ def run_gpu(args):
     track_merged = trk.track_merged()
     dev_assign = trk.assignment()
     # ---- looper legs and cluster tags on the merged tracks (tpcca_find_legs), timed on its own
-    leg_partner, leg_first, tags, leg_sum = trk.find_legs()
+    leg_partner, leg_partner_in, leg_first, tags, leg_sum = trk.find_legs()
     torch.cuda.synchronize()
     l0, l1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     l0.record(stream)
@@ -352,8 +352,19 @@ def run_gpu(args):
     q_sec = score.score(dev_assign, fr.truth, one, hd["n_tracks"])
     am = np.where(dev_assign >= 0, track_merged[np.maximum(dev_assign, 0)], -1) if hd["n_tracks"] else dev_assign
     q_mrg = score.score(am, fr.truth, one, mh["n_merged"])
-    # a pair of legs counts as one reconstructed particle: relabel the additional leg by its partner
-    leg_root = np.where((leg_partner >= 0) & (leg_first == 0), leg_partner, np.arange(len(leg_partner))) if len(leg_partner) else leg_partner
+    # a chain of legs counts as one reconstructed particle: relabel every leg by the root of its chain (union of both kinds of link)
+    leg_root = np.arange(len(leg_partner))
+
+    def _find(x):
+        while leg_root[x] != x:
+            leg_root[x] = leg_root[leg_root[x]]
+            x = leg_root[x]
+        return x
+
+    for lp in (leg_partner, leg_partner_in):
+        for m in np.flatnonzero(lp >= 0):
+            leg_root[_find(m)] = _find(int(lp[m]))
+    leg_root = np.array([_find(m) for m in range(len(leg_root))], dtype=np.int64)
     al = np.where(am >= 0, leg_root[np.maximum(am, 0)], -1) if len(leg_partner) else am
     q_leg = score.score(al, fr.truth, one, mh["n_merged"])
     merge_info = {"ms": merge_ms, "api": "tpcca_merge (after the timed path, not part of `value`)", **mh,

@@ -202,15 +202,19 @@ int tpcca_estimate_time(tpcca_handle* h, float vdrift_cm_per_us, float z_max_cm,
 /* ---- Legs of low-pT loopers and cluster tags ("additional legs of looping tracks do not point to the vertex
  * ... special low-pT track merging"; :157 clusters to remove for the compression factor: "very low-pT looping tracks below
  * 50 MeV/c, additional legs of tracks below 200 MeV/c, and track segments with high inclination angle"; DESIGN.md section 14,
- * Table D).  The outer ends of two merged tracks that are the outgoing and the returning leg of one turn of a helix (same
- * circle in the sector plane, opposite fitted curvature, z consistent with the arc between them) are linked at the turning
- * point; clusters are tagged for removal. */
+ * Table D).  Two merged tracks that are consecutive legs of one helix (same circle in the sector plane, opposite fitted
+ * curvature, z consistent with the arc between them) are linked: outer end to outer end over the turning point, inner end
+ * to inner end through the region below the first pad row (the looper passes the beam line and comes out again one
+ * pitch further in z); clusters are tagged for removal. */
 typedef struct {
   float leg_min_qpt;          /* (GeV/c)^-1: only ends with |q/pT| >= this are candidates */
-  float leg_min_sinphi;       /* and |sin(phi)| >= this at the outer end */
-  float leg_apex_margin;      /* cm: the turning point xc + R must lie below row_x[last] + margin */
-  int32_t leg_max_sector_gap; /* the partner's end lies 0..gap sectors ahead in the turning sense */
-  float leg_max_turn;         /* rad, < pi: turning angle between the two ends */
+  float leg_min_sinphi;       /* and |sin(phi)| >= this at an outer end */
+  float leg_inner_min_sinphi; /* ... at an inner end */
+  float leg_apex_margin;      /* cm: outer ends only, the turning point xc + R must lie below row_x[last] + margin */
+  int32_t leg_max_sector_gap; /* outer: the partner's end lies 0..gap sectors AHEAD in the turning sense */
+  int32_t leg_inner_max_sector_gap; /* inner: at most this many sectors away, either way round */
+  float leg_max_turn;         /* rad, < pi: turning angle between two outer ends */
+  float leg_inner_max_turn;   /* rad, < 2 pi: turning angle between two inner ends */
   float leg_centre_frac, leg_centre_abs; /* centre distance <= frac * mean radius + abs (cm) */
   float leg_radius_frac;      /* |R_A - R_B| <= frac * mean radius */
   float leg_dz_max;           /* cm: z_B - z_A - mean slope * arc */
@@ -222,19 +226,23 @@ typedef struct {
 } tpcca_leg_params;
 void tpcca_default_leg_params(tpcca_leg_params* p);
 enum { TPCCA_TAG_LOW_PT = 1, TPCCA_TAG_EXTRA_LEG = 2, TPCCA_TAG_HIGH_INCLINATION = 4 };
-typedef struct { int32_t n_links, n_tag_low_pt, n_tag_extra_leg, n_tag_high_inclination; } tpcca_leg_summary; /* 16 B */
+typedef struct {
+  int32_t n_links_outer, n_links_inner, n_tag_low_pt, n_tag_extra_leg, n_tag_high_inclination, pad[3];
+} tpcca_leg_summary; /* 32 B */
 
 /* Link legs and tag clusters for the merged tracks of the LAST tpcca_merge on this handle (whose outputs, and those of the
  * tpcca_track before it, must still be valid and unchanged); enqueued on `stream`, returns without waiting.
  * out_leg_partner: device, max_tracks int32: merged track joined at the outer turning point, or -1 (mutual).
- * out_leg_first: device, max_tracks bytes: 1 = first (or only) leg -- of a pair, the one whose inner end lies at the
- *   smaller |z| --, 0 = additional leg.
+ * out_leg_partner_inner: device, max_tracks int32: merged track joined through the inner region, or -1 (mutual).
+ * out_leg_first: device, max_tracks bytes: 1 = first (or only) leg of its chain -- no linked neighbour has its inner end
+ *   at a smaller |z| --, 0 = additional leg.
  * out_cluster_tags: device, n bytes in INPUT order (n of the last tpcca_track): TPCCA_TAG_* bits, 0 for clusters on no track.
- * out_summary: device, 16-byte aligned: links and tagged clusters per bit.
+ * out_summary: device, 16-byte aligned, 32 bytes: links per kind and tagged clusters per bit.
  * TPCCA_ERR_ARGUMENT without a preceding tpcca_merge, for null / misaligned pointers or parameters out of range
- * (leg_max_turn must be < pi, leg_min_sinphi > sin(20 deg), tolerances > 0). */
+ * (leg_max_turn must be < pi, leg_inner_max_turn < 2 pi, thresholds and tolerances > 0). */
 int tpcca_find_legs(tpcca_handle* h, const tpcca_leg_params* lp, void* stream, int32_t* out_leg_partner,
-                    uint8_t* out_leg_first, uint8_t* out_cluster_tags, tpcca_leg_summary* out_summary);
+                    int32_t* out_leg_partner_inner, uint8_t* out_leg_first, uint8_t* out_cluster_tags,
+                    tpcca_leg_summary* out_summary);
 
 /* Per-stage device times, averaged over the tpcca_track calls (at most the last 32) made since profiling
  * was switched on (CUDA events recorded on each call's stream; synchronises those events).  ms: host float[TPCCA_N_STAGES]. */

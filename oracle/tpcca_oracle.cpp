@@ -15,7 +15,7 @@
 // form (P6), straight-line least squares (P7), pulls (P8), -O0 == -O2 (P10).
 // Merger and final fit O8-O10: tests/test_merge_pins.py; z / time estimate O11: tests/test_time_pins.py; looper legs and
 // cluster tags O12-O13: tests/test_looper_pins.py (float64 closed-form helices
-// over all sectors, the angle polynomial against arctan2, every term of the pair score, 41 one-line mutants all fail a pin).
+// over all sectors, the angle polynomial against arctan2, every term of the pair score, 54 one-line mutants all fail a pin).
 // Parity unpinned: the numeric defaults of DESIGN.md Tables A, B and D (cuts, windows, cov0) -- the paper
 // prints no value for them.
 #include <algorithm>

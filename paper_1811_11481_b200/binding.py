@@ -56,8 +56,9 @@ class MergeParams(C.Structure):
 
 
 class LegParams(C.Structure):
-    _fields_ = [("leg_min_qpt", C.c_float), ("leg_min_sinphi", C.c_float), ("leg_apex_margin", C.c_float),
-                ("leg_max_sector_gap", C.c_int32), ("leg_max_turn", C.c_float), ("leg_centre_frac", C.c_float),
+    _fields_ = [("leg_min_qpt", C.c_float), ("leg_min_sinphi", C.c_float), ("leg_inner_min_sinphi", C.c_float),
+                ("leg_apex_margin", C.c_float), ("leg_max_sector_gap", C.c_int32), ("leg_inner_max_sector_gap", C.c_int32),
+                ("leg_max_turn", C.c_float), ("leg_inner_max_turn", C.c_float), ("leg_centre_frac", C.c_float),
                 ("leg_centre_abs", C.c_float), ("leg_radius_frac", C.c_float), ("leg_dz_max", C.c_float),
                 ("leg_dzds_tol", C.c_float), ("tag_qpt_low", C.c_float), ("tag_qpt_leg", C.c_float),
                 ("tag_sinphi", C.c_float), ("ring", C.c_int32)]
@@ -91,7 +92,7 @@ def load():
         lib.tpcca_default_leg_params.argtypes = [C.POINTER(LegParams)]
         lib.tpcca_find_legs.restype = C.c_int
         lib.tpcca_find_legs.argtypes = [C.c_void_p, C.POINTER(LegParams), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
-                                        C.c_void_p]
+                                        C.c_void_p, C.c_void_p]
         lib.tpcca_estimate_time.restype = C.c_int
         lib.tpcca_estimate_time.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
         lib.tpcca_wait.restype = C.c_int
@@ -306,23 +307,24 @@ class Tracker:
         n = max(1, int(self.n))
         if getattr(self, "out_leg_partner", None) is None:
             self.out_leg_partner = torch.empty(max(1, self.max_tracks), dtype=torch.int32, device=self.device)
+            self.out_leg_partner_in = torch.empty(max(1, self.max_tracks), dtype=torch.int32, device=self.device)
             self.out_leg_first = torch.empty(max(1, self.max_tracks), dtype=torch.uint8, device=self.device)
-            self.out_leg_summary = torch.empty(4, dtype=torch.int32, device=self.device)
+            self.out_leg_summary = torch.empty(8, dtype=torch.int32, device=self.device)
         if getattr(self, "out_tags", None) is None or self.out_tags.numel() < n:
             self.out_tags = torch.empty(n, dtype=torch.uint8, device=self.device)
         self._check(self.lib.tpcca_find_legs(self.h, C.byref(lp), self._stream(), self.out_leg_partner.data_ptr(),
-                                             self.out_leg_first.data_ptr(), self.out_tags.data_ptr(),
-                                             self.out_leg_summary.data_ptr()))
+                                             self.out_leg_partner_in.data_ptr(), self.out_leg_first.data_ptr(),
+                                             self.out_tags.data_ptr(), self.out_leg_summary.data_ptr()))
 
     def find_legs(self, **params):
-        """Returns (leg_partner[n_merged], leg_first[n_merged], cluster_tags[n], summary dict)."""
+        """Returns (leg_partner[n_merged], leg_partner_inner[n_merged], leg_first[n_merged], cluster_tags[n], summary dict)."""
         self.find_legs_enqueue(**params)
         nm = self.merged_header()["n_merged"]
         sm = self.out_leg_summary.cpu().numpy()
-        return (self.out_leg_partner[:nm].cpu().numpy().copy(), self.out_leg_first[:nm].cpu().numpy().copy(),
-                self.out_tags[:int(self.n)].cpu().numpy().copy(),
-                dict(n_links=int(sm[0]), n_tag_low_pt=int(sm[1]), n_tag_extra_leg=int(sm[2]),
-                     n_tag_high_inclination=int(sm[3])))
+        return (self.out_leg_partner[:nm].cpu().numpy().copy(), self.out_leg_partner_in[:nm].cpu().numpy().copy(),
+                self.out_leg_first[:nm].cpu().numpy().copy(), self.out_tags[:int(self.n)].cpu().numpy().copy(),
+                dict(n_links_outer=int(sm[0]), n_links_inner=int(sm[1]), n_tag_low_pt=int(sm[2]), n_tag_extra_leg=int(sm[3]),
+                     n_tag_high_inclination=int(sm[4])))
 
     def estimate_time(self, vdrift: float = 2.58, z_max: float = 250.0, merged: bool = True):
         """tpcca_estimate_time: (n_tracks, 4) and, after merge(), (n_merged, 4) arrays of z_dca, z_shift, t0_us, dca_xy."""

@@ -120,12 +120,12 @@ static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params
   CARVE(d.m_len, int32_t, K);
   CARVE(d.m_order, int32_t, K);
   CARVE(d.m_cand, int2, K);
-  CARVE(d.leg_ends, float4, K * 3);
-  CARVE(d.leg_best, unsigned long long, K);
-  CARVE(d.leg_sec, int32_t, TPCCA_MAX_SECTORS + 2);
-  CARVE(d.leg_cur, int32_t, TPCCA_MAX_SECTORS);
-  CARVE(d.leg_list, int32_t, K);
-  CARVE(d.leg_summary, int32_t, 4);
+  CARVE(d.leg_ends, float4, K * 6);
+  CARVE(d.leg_best, unsigned long long, K * 2);
+  CARVE(d.leg_sec, int32_t, 2 * (TPCCA_MAX_SECTORS + 2));
+  CARVE(d.leg_cur, int32_t, 2 * TPCCA_MAX_SECTORS);
+  CARVE(d.leg_list, int32_t, K * 2);
+  CARVE(d.leg_summary, int32_t, 8);
   for (int sl = 0; sl < 2; sl++) {
     CARVE(stage_clusters[sl], float4, N);
     CARVE(stage_assign[sl], int32_t, N);
@@ -420,20 +420,23 @@ int tpcca_merge(tpcca_handle* h, const tpcca_merge_params* mp, void* stream, voi
 void tpcca_default_leg_params(tpcca_leg_params* p) {
   if (!p) return;
   memset(p, 0, sizeof(*p));
-  p->leg_min_qpt = 4.0f; p->leg_min_sinphi = 0.5f; p->leg_apex_margin = 2.0f; p->leg_max_sector_gap = 5;
-  p->leg_max_turn = 2.9f; p->leg_centre_frac = 0.05f; p->leg_centre_abs = 1.5f; p->leg_radius_frac = 0.2f;
+  p->leg_min_qpt = 4.0f; p->leg_min_sinphi = 0.5f; p->leg_inner_min_sinphi = 0.2f; p->leg_apex_margin = 2.0f;
+  p->leg_max_sector_gap = 5; p->leg_inner_max_sector_gap = 9;
+  p->leg_max_turn = 2.9f; p->leg_inner_max_turn = 5.0f; p->leg_centre_frac = 0.05f; p->leg_centre_abs = 1.5f; p->leg_radius_frac = 0.2f;
   p->leg_dz_max = 4.0f; p->leg_dzds_tol = 0.1f;
   p->tag_qpt_low = 20.0f; p->tag_qpt_leg = 5.0f; p->tag_sinphi = 0.8f; p->ring = 18;
 }
 
 int tpcca_find_legs(tpcca_handle* h, const tpcca_leg_params* lp, void* stream, int32_t* out_leg_partner,
-                    uint8_t* out_leg_first, uint8_t* out_cluster_tags, tpcca_leg_summary* out_summary) {
+                    int32_t* out_leg_partner_inner, uint8_t* out_leg_first, uint8_t* out_cluster_tags,
+                    tpcca_leg_summary* out_summary) {
   if (!h) { set_err("handle is null (not initialised)"); return TPCCA_ERR_NOT_INIT; }
-  if (!lp || !out_leg_partner || !out_leg_first || !out_cluster_tags || !out_summary) { set_err("null leg parameters or output"); return TPCCA_ERR_ARGUMENT; }
-  if (((uintptr_t)out_leg_partner & 3) || ((uintptr_t)out_summary & 15)) { set_err("misaligned leg output"); return TPCCA_ERR_ARGUMENT; }
+  if (!lp || !out_leg_partner || !out_leg_partner_inner || !out_leg_first || !out_cluster_tags || !out_summary) { set_err("null leg parameters or output"); return TPCCA_ERR_ARGUMENT; }
+  if (((uintptr_t)out_leg_partner & 3) || ((uintptr_t)out_leg_partner_inner & 3) || ((uintptr_t)out_summary & 15)) { set_err("misaligned leg output"); return TPCCA_ERR_ARGUMENT; }
   if (!h->d.out_hdr || !h->last_merged) { set_err("tpcca_find_legs needs a tpcca_merge after the last tpcca_track on this handle"); return TPCCA_ERR_ARGUMENT; }
-  if (lp->ring < 0 || lp->leg_max_sector_gap < 0 || !(lp->leg_max_turn > 0.0f) || !(lp->leg_max_turn < 3.14159f) ||
-      !(lp->leg_min_sinphi > 0.3421f) || !(lp->leg_min_qpt > 0.0f) || !(lp->leg_centre_abs >= 0.0f) || !(lp->leg_centre_frac >= 0.0f) ||
+  if (lp->ring < 0 || lp->leg_max_sector_gap < 0 || lp->leg_inner_max_sector_gap < 0 || !(lp->leg_max_turn > 0.0f) ||
+      !(lp->leg_max_turn < 3.14159f) || !(lp->leg_inner_max_turn > 0.0f) || !(lp->leg_inner_max_turn < 6.28318f) ||
+      !(lp->leg_min_sinphi > 0.0f) || !(lp->leg_inner_min_sinphi > 0.0f) || !(lp->leg_min_qpt > 0.0f) || !(lp->leg_centre_abs >= 0.0f) || !(lp->leg_centre_frac >= 0.0f) ||
       !(lp->leg_centre_abs + lp->leg_centre_frac > 0.0f) || !(lp->leg_radius_frac > 0.0f) || !(lp->leg_dz_max > 0.0f) ||
       !(lp->leg_dzds_tol > 0.0f)) {
     set_err("leg parameters out of range"); return TPCCA_ERR_ARGUMENT;
@@ -443,6 +446,7 @@ int tpcca_find_legs(tpcca_handle* h, const tpcca_leg_params* lp, void* stream, i
   d.merged_out = reinterpret_cast<tpcca_track_rec*>((char*)h->last_merged + sizeof(tpcca_out_header));
   d.track_merged_out = h->last_track_merged;
   d.leg_partner_out = out_leg_partner;
+  d.leg_partner_in_out = out_leg_partner_inner;
   d.leg_first_out = out_leg_first;
   d.tags_out = out_cluster_tags;
   d.leg_summary_out = reinterpret_cast<int32_t*>(out_summary);

@@ -120,13 +120,14 @@ struct Dev {
   int32_t* track_merged_out;
   // looper legs and cluster tags (tpcca_find_legs)
   tpcca_leg_params LP;
-  float4* leg_ends;                // [max_tracks][3] outer end of every merged track (layout: tpcca_legs.cu)
-  unsigned long long* leg_best;    // [max_tracks] (score bits << 32 | partner id), ~0 = none
-  int32_t* leg_sec;                // [TPCCA_MAX_SECTORS+2] candidate ends per sector -> bucket starts
-  int32_t* leg_cur;                // [TPCCA_MAX_SECTORS] scatter cursors
-  int32_t* leg_list;               // [max_tracks] candidate ends grouped by sector
-  int32_t* leg_summary;            // [4] links, tagged clusters per bit
+  float4* leg_ends;                // [2][max_tracks][3] outer / inner end of every merged track (layout: tpcca_legs.cu)
+  unsigned long long* leg_best;    // [2][max_tracks] (score bits << 32 | partner id), ~0 = none
+  int32_t* leg_sec;                // [2][TPCCA_MAX_SECTORS+2] candidate ends per sector -> bucket starts
+  int32_t* leg_cur;                // [2][TPCCA_MAX_SECTORS] scatter cursors
+  int32_t* leg_list;               // [2][max_tracks] candidate ends grouped by sector
+  int32_t* leg_summary;            // [8] links per kind, tagged clusters per bit
   int32_t* leg_partner_out;
+  int32_t* leg_partner_in_out;
   uint8_t* leg_first_out;
   uint8_t* tags_out;
   int32_t* leg_summary_out;

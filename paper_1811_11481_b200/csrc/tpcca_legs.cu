@@ -30,7 +30,9 @@ __device__ __forceinline__ float angle_upper(float y, float x) {
   return pi + atan_unit(y / x);
 }
 
-// Outer end of a merged track, 48 bytes in the workspace: {z, s, t, q} {c, R, xc, yc} {sector, cand, -, -}
+// An end of a merged track, 48 bytes in the workspace: {z, s, t, q} {c, R, xc, yc} {sector, cand, -, -}.  Two kinds
+// (D1): kind 0 = outer end (continued along the fit direction, sig = +1), kind 1 = inner end (against it, -1);
+// kind-major arrays: entry kind * max_tracks + m.
 struct LegEnd {
   float z, s, t, q, c, R, xc, yc;
   int sector, cand;
@@ -44,71 +46,83 @@ __device__ __forceinline__ LegEnd load_end(const float4* e, int m) {
 }
 
 // ---------------------------------------------------------------- (l0) ends (D1-D3), candidate count per sector
+#define LEG_SEC_STRIDE (TPCCA_MAX_SECTORS + 2)
 __global__ void __launch_bounds__(256) k_leg_reset(Dev d) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i <= TPCCA_MAX_SECTORS) d.leg_sec[i] = 0;
-  if (i < 4) d.leg_summary[i] = 0;
-  if (i < d.cnt->n_merged) d.leg_best[i] = LEG_NONE;
+  if (i < 2 * LEG_SEC_STRIDE) d.leg_sec[i] = 0;
+  if (i < 8) d.leg_summary[i] = 0;
+  if (i < d.cnt->n_merged) { d.leg_best[i] = LEG_NONE; d.leg_best[d.max_tracks + i] = LEG_NONE; }
 }
 
-__global__ void __launch_bounds__(128) k_leg_ends(Dev d) {
-  const int m = blockIdx.x * blockDim.x + threadIdx.x;
-  if (m >= d.cnt->n_merged) return;
-  int tail = d.merged_out[m].pad[4];
-  for (int nx = d.m_next[tail]; nx >= 0; nx = d.m_next[tail]) tail = nx;
-  const tpcca_track_rec* tr = d.out_tracks;
-  const float4* oa = reinterpret_cast<const float4*>(d.track_outer + (size_t)tail * 24);
-  const float4 o0 = oa[0];  // x, y, z, sinphi
-  const float4 o1 = oa[1];  // dzds, qpt, ..
-  const float x = o0.x, y = o0.y, s = o0.w, t = o1.x, q = o1.y;
-  const int sector = tr[tail].sector;
+__device__ __forceinline__ void store_end(const Dev& d, int kind, int m, int sector, float x, float y, float z, float s, float t,
+                                          float q, bool valid) {
   float c = 0.f, R = 0.f, xc = 0.f, yc = 0.f;
   int cand = 0;
-  if (tr[tail].ndf >= 0 && (fabsf(q) >= d.LP.leg_min_qpt) && (fabsf(s) >= d.LP.leg_min_sinphi) && (fabsf(s) < 1.0f)) {
+  const float smin = kind == 0 ? d.LP.leg_min_sinphi : d.LP.leg_inner_min_sinphi;
+  if (valid && (fabsf(q) >= d.LP.leg_min_qpt) && (fabsf(s) >= smin) && (fabsf(s) < 1.0f)) {
     const float k = q * d.kq;
     c = sqrtf(fmaf(-s, s, 1.0f));
     R = 1.0f / fabsf(k);
     xc = x - s / k;
     yc = y + c / k;
-    cand = ((xc + R) <= (d.row_x[d.n_rows - 1] + d.LP.leg_apex_margin)) ? 1 : 0;
+    cand = (kind == 1 || (xc + R) <= (d.row_x[d.n_rows - 1] + d.LP.leg_apex_margin)) ? 1 : 0;  // outer: turns back inside the TPC
   }
-  float4* e = d.leg_ends + 3 * (size_t)m;
-  e[0] = make_float4(o0.z, s, t, q);
+  float4* e = d.leg_ends + 3 * ((size_t)kind * d.max_tracks + m);
+  e[0] = make_float4(z, s, t, q);
   e[1] = make_float4(c, R, xc, yc);
   e[2] = make_float4(__int_as_float(sector), __int_as_float(cand), 0.f, 0.f);
-  if (cand) atomicAdd(&d.leg_sec[sector + 1], 1);
+  if (cand) atomicAdd(&d.leg_sec[kind * LEG_SEC_STRIDE + sector + 1], 1);
 }
 
-// one block: exclusive scan of the (<= 64) per-sector counts; leg_sec[s] = start of sector s, cursors behind them
+__global__ void __launch_bounds__(128) k_leg_ends(Dev d) {
+  const int m = blockIdx.x * blockDim.x + threadIdx.x;
+  if (m >= d.cnt->n_merged) return;
+  const tpcca_track_rec* tr = d.out_tracks;
+  const tpcca_track_rec* M = &d.merged_out[m];
+  const int head = M->pad[4];
+  int tail = head;
+  for (int nx = d.m_next[tail]; nx >= 0; nx = d.m_next[tail]) tail = nx;
+  const float4* oa = reinterpret_cast<const float4*>(d.track_outer + (size_t)tail * 24);
+  const float4 o0 = oa[0];  // x, y, z, sinphi
+  const float4 o1 = oa[1];  // dzds, qpt, ..
+  store_end(d, 0, m, tr[tail].sector, o0.x, o0.y, o0.z, o0.w, o1.x, o1.y, tr[tail].ndf >= 0);
+  store_end(d, 1, m, M->sector, M->x, M->y, M->z, M->sinphi, M->dzds, M->qpt, tr[head].ndf >= 0);
+}
+
+// one block per kind: exclusive scan of the (<= 64) per-sector counts; leg_sec[s] = start of sector s, cursors behind them
 __global__ void __launch_bounds__(128) k_leg_offsets(Dev d) {
   __shared__ int sm[32];
+  int32_t* sec = d.leg_sec + blockIdx.x * LEG_SEC_STRIDE;
+  int32_t* cur = d.leg_cur + blockIdx.x * TPCCA_MAX_SECTORS;
   const int s = threadIdx.x;
-  const int v = (s < TPCCA_MAX_SECTORS) ? d.leg_sec[s + 1] : 0;
+  const int v = (s < TPCCA_MAX_SECTORS) ? sec[s + 1] : 0;
   int tot;
   const int e = block_scan_excl(v, &tot, sm);
   __syncthreads();
-  if (s < TPCCA_MAX_SECTORS) { d.leg_sec[s] = e; d.leg_cur[s] = e; }
-  if (s == 0) d.leg_sec[TPCCA_MAX_SECTORS] = tot;
+  if (s < TPCCA_MAX_SECTORS) { sec[s] = e; cur[s] = e; }
+  if (s == 0) sec[TPCCA_MAX_SECTORS] = tot;
 }
 
 __global__ void __launch_bounds__(128) k_leg_scatter(Dev d) {
   const int m = blockIdx.x * blockDim.x + threadIdx.x;
+  const int kind = blockIdx.y;
   if (m >= d.cnt->n_merged) return;
-  const float4 c = d.leg_ends[3 * (size_t)m + 2];
+  const float4 c = d.leg_ends[3 * ((size_t)kind * d.max_tracks + m) + 2];
   if (!__float_as_int(c.y)) return;
-  const int pos = atomicAdd(&d.leg_cur[__float_as_int(c.x)], 1);
-  d.leg_list[pos] = m;  // order inside a sector is arbitrary: the match takes min (score, id)
+  const int pos = atomicAdd(&d.leg_cur[kind * TPCCA_MAX_SECTORS + __float_as_int(c.x)], 1);
+  d.leg_list[(size_t)kind * d.max_tracks + pos] = m;  // order inside a sector is arbitrary: the match takes min (score, id)
 }
 
 // ---------------------------------------------------------------- (l1) pair scores (D4-D8): one warp per end A
 // Every unordered pair is evaluated once, by the warp of the LOWER id, in A's frame; both ends receive the score through
 // atomicMin of (score bits << 32 | partner id): min score, then lower partner id.
-__device__ __forceinline__ float leg_pair_score(const Dev& d, const LegEnd& A, const LegEnd& B, int j, int sgn, float ca,
-                                                float sa) {
+__device__ __forceinline__ float leg_pair_score(const Dev& d, const LegEnd& A, const LegEnd& B, int jrot, int sgn, float sig,
+                                                float ca, float sa) {
   if (!(A.q * B.q < 0.0f)) return -1.0f;
-  const float ss = (float)sgn * sa;
+  const float ss = (jrot >= 0) ? sa : -sa;
+  const int nrot = abs(jrot);
   float bxc = B.xc, byc = B.yc, bdx = B.c, bdy = B.s;
-  for (int i = 0; i < j; i++) {
+  for (int i = 0; i < nrot; i++) {
     float u = fmaf(-byc, ss, bxc * ca), v = fmaf(bxc, ss, byc * ca);
     bxc = u; byc = v;
     u = fmaf(-bdy, ss, bdx * ca); v = fmaf(bdx, ss, bdy * ca);
@@ -117,9 +131,13 @@ __device__ __forceinline__ float leg_pair_score(const Dev& d, const LegEnd& A, c
   const float dot = -fmaf(A.s, bdy, A.c * bdx);
   const float cross = fmaf(A.s, bdx, -(A.c * bdy));
   const float yy = (float)sgn * cross;
-  if (!(yy > 0.0f)) return -1.0f;
-  const float theta = angle_upper(yy, dot);
-  if (!(theta <= d.LP.leg_max_turn)) return -1.0f;
+  const float two_pi = 6.28318530718f, pi = 3.14159265359f;
+  float theta;
+  if (yy > 0.0f) theta = angle_upper(yy, dot);
+  else if (yy < 0.0f) theta = two_pi - angle_upper(-yy, dot);
+  else if (dot < 0.0f) theta = pi;
+  else return -1.0f;
+  if (!(theta <= (sig > 0.0f ? d.LP.leg_max_turn : d.LP.leg_inner_max_turn))) return -1.0f;
   const float Rm = 0.5f * (A.R + B.R);
   const float arc = theta * Rm;
   const float dxc = A.xc - bxc, dyc = A.yc - byc;
@@ -129,7 +147,7 @@ __device__ __forceinline__ float leg_pair_score(const Dev& d, const LegEnd& A, c
   if (!(dc2 <= tolc2)) return -1.0f;
   const float dR = A.R - B.R, tolR = d.LP.leg_radius_frac * Rm;
   if (!(fabsf(dR) <= tolR)) return -1.0f;
-  const float tm = 0.5f * (A.t - B.t);
+  const float tm = sig * (0.5f * (A.t - B.t));
   const float dz = fmaf(-tm, arc, B.z - A.z);
   if (!(fabsf(dz) <= d.LP.leg_dz_max)) return -1.0f;
   const float dt = A.t + B.t;
@@ -145,30 +163,48 @@ __device__ __forceinline__ float leg_pair_score(const Dev& d, const LegEnd& A, c
 __global__ void __launch_bounds__(128) k_leg_match(Dev d) {
   const int lane = threadIdx.x & 31;
   const int a = (blockIdx.x * 128 + threadIdx.x) >> 5;
+  const int kind = blockIdx.y;
   if (a >= d.cnt->n_merged) return;
-  const LegEnd A = load_end(d.leg_ends, a);
+  const float4* ends = d.leg_ends + 3 * (size_t)kind * d.max_tracks;
+  const int32_t* sec = d.leg_sec + kind * LEG_SEC_STRIDE;
+  const int32_t* list = d.leg_list + (size_t)kind * d.max_tracks;
+  unsigned long long* bestv = d.leg_best + (size_t)kind * d.max_tracks;
+  const LegEnd A = load_end(ends, a);
   if (!A.cand) return;
   const float th = d.tan_half_angle;
   const float den = fmaf(th, th, 1.0f);
   const float ca = fmaf(-th, th, 1.0f) / den, sa = (2.0f * th) / den;
   const int ring = d.LP.ring;
-  const int sgn = (A.q * d.kq > 0.0f) ? 1 : -1;
+  const float sig = kind == 0 ? 1.0f : -1.0f;
+  const int sgn = ((sig * A.q) * d.kq > 0.0f) ? 1 : -1;
   const int base = ring > 0 ? (A.sector / ring) * ring : A.sector, l = A.sector - base;
-  const int jmax = ring > 0 ? min(d.LP.leg_max_sector_gap, ring - 1) : 0;
+  // sector offsets dsec = 0 .. ring-1 of the partner; jrot as in DESIGN.md D4
+  const int nsec = ring > 0 ? ring : 1;
   unsigned long long best = LEG_NONE;
-  for (int j = 0; j <= jmax; j++) {
-    const int sb = ring > 0 ? base + (((l + sgn * j) % ring) + ring) % ring : A.sector;
+  for (int dsec = 0; dsec < nsec; dsec++) {
+    int jrot = 0;
+    if (ring > 0) {
+      if (kind == 0) {
+        const int j = ((dsec * sgn) % ring + ring) % ring;
+        if (j > d.LP.leg_max_sector_gap) continue;
+        jrot = sgn * j;
+      } else {
+        jrot = (2 * dsec <= ring) ? dsec : dsec - ring;
+        if (abs(jrot) > d.LP.leg_inner_max_sector_gap) continue;
+      }
+    }
+    const int sb = ring > 0 ? base + (l + dsec) % ring : A.sector;
     if (sb >= d.n_sectors) continue;
-    const int b0 = d.leg_sec[sb], b1 = d.leg_sec[sb + 1];
+    const int b0 = sec[sb], b1 = sec[sb + 1];
     for (int pos = b0 + lane; pos < b1; pos += 32) {
-      const int b = d.leg_list[pos];
+      const int b = list[pos];
       if (b <= a) continue;
-      const LegEnd B = load_end(d.leg_ends, b);
-      const float sc = leg_pair_score(d, A, B, j, sgn, ca, sa);
+      const LegEnd B = load_end(ends, b);
+      const float sc = leg_pair_score(d, A, B, jrot, sgn, sig, ca, sa);
       if (!(sc >= 0.0f)) continue;
       const unsigned long long sb64 = (unsigned long long)__float_as_uint(sc) << 32;  // score >= +0: bits order like values
       best = min(best, sb64 | (unsigned)b);
-      atomicMin(&d.leg_best[b], sb64 | (unsigned)a);
+      atomicMin(&bestv[b], sb64 | (unsigned)a);
     }
   }
 #pragma unroll
@@ -176,27 +212,38 @@ __global__ void __launch_bounds__(128) k_leg_match(Dev d) {
     const unsigned long long v = __shfl_xor_sync(0xffffffffu, best, o);
     best = min(best, v);
   }
-  if (lane == 0 && best != LEG_NONE) atomicMin(&d.leg_best[a], best);
+  if (lane == 0 && best != LEG_NONE) atomicMin(&bestv[a], best);
 }
 
 // ---------------------------------------------------------------- (l2) mutual links, first leg (D9, D10)
+__device__ __forceinline__ int mutual_partner(const unsigned long long* bestv, int a) {
+  const unsigned long long ba = bestv[a];
+  if (ba == LEG_NONE) return -1;
+  const int b = (int)(ba & 0xffffffffull);
+  const unsigned long long bb = bestv[b];
+  return (bb != LEG_NONE && (int)(bb & 0xffffffffull) == a) ? b : -1;
+}
+
 __global__ void __launch_bounds__(256) k_leg_link(Dev d) {
   const int a = blockIdx.x * blockDim.x + threadIdx.x;
   if (a >= d.cnt->n_merged) return;
-  int partner = -1;
-  const unsigned long long ba = d.leg_best[a];
-  if (ba != LEG_NONE) {
-    const int b = (int)(ba & 0xffffffffull);
-    const unsigned long long bb = d.leg_best[b];
-    if (bb != LEG_NONE && (int)(bb & 0xffffffffull) == a) partner = b;
-  }
+  const int po = mutual_partner(d.leg_best, a);
+  const int pi = mutual_partner(d.leg_best + d.max_tracks, a);
+  // first leg: no linked neighbour at a smaller |z| of the inner end (equal: the lower id), D10
+  const float za = fabsf(d.merged_out[a].z);
   int first = 1;
-  if (partner >= 0) {
-    const float za = fabsf(d.merged_out[a].z), zb = fabsf(d.merged_out[partner].z);
-    first = ((za < zb) || (za == zb && a < partner)) ? 1 : 0;
-    if (a < partner) atomicAdd(&d.leg_summary[0], 1);
+  if (po >= 0) {
+    const float zb = fabsf(d.merged_out[po].z);
+    if (zb < za || (zb == za && po < a)) first = 0;
+    if (a < po) atomicAdd(&d.leg_summary[0], 1);
   }
-  d.leg_partner_out[a] = partner;
+  if (pi >= 0) {
+    const float zb = fabsf(d.merged_out[pi].z);
+    if (zb < za || (zb == za && pi < a)) first = 0;
+    if (a < pi) atomicAdd(&d.leg_summary[1], 1);
+  }
+  d.leg_partner_out[a] = po;
+  d.leg_partner_in_out[a] = pi;
   d.leg_first_out[a] = (uint8_t)first;
 }
 
@@ -228,14 +275,14 @@ __global__ void __launch_bounds__(128) k_leg_tags(Dev d) {
   }
   n1 = __reduce_add_sync(0xffffffffu, n1); n2 = __reduce_add_sync(0xffffffffu, n2); n4 = __reduce_add_sync(0xffffffffu, n4);
   if (lane == 0) {
-    if (n1) atomicAdd(&d.leg_summary[1], n1);
-    if (n2) atomicAdd(&d.leg_summary[2], n2);
-    if (n4) atomicAdd(&d.leg_summary[3], n4);
+    if (n1) atomicAdd(&d.leg_summary[2], n1);
+    if (n2) atomicAdd(&d.leg_summary[3], n2);
+    if (n4) atomicAdd(&d.leg_summary[4], n4);
   }
 }
 
 __global__ void k_leg_summary(Dev d) {
-  if (threadIdx.x < 4) d.leg_summary_out[threadIdx.x] = d.leg_summary[threadIdx.x];
+  if (threadIdx.x < 8) d.leg_summary_out[threadIdx.x] = d.leg_summary[threadIdx.x];
 }
 
 void launch_legs(const Dev& d, Launch& L) {
@@ -244,9 +291,9 @@ void launch_legs(const Dev& d, Launch& L) {
   if (d.n > 0 && K > 0) {
     k_leg_reset<<<(max(K, 128) + 255) / 256, 256, 0, L.st>>>(d);
     k_leg_ends<<<(K + 127) / 128, 128, 0, L.st>>>(d);
-    k_leg_offsets<<<1, 128, 0, L.st>>>(d);
-    k_leg_scatter<<<(K + 127) / 128, 128, 0, L.st>>>(d);
-    k_leg_match<<<(K + 3) / 4, 128, 0, L.st>>>(d);
+    k_leg_offsets<<<2, 128, 0, L.st>>>(d);
+    k_leg_scatter<<<dim3((K + 127) / 128, 2), 128, 0, L.st>>>(d);
+    k_leg_match<<<dim3((K + 3) / 4, 2), 128, 0, L.st>>>(d);
     k_leg_link<<<(K + 255) / 256, 256, 0, L.st>>>(d);
     k_leg_tags<<<(K + 3) / 4, 128, 0, L.st>>>(d);
     L.count += 7;

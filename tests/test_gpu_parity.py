@@ -429,7 +429,7 @@ def test_no_kernel_writes_outside_its_arrays(row_x, case):
     bufs = {}
     for name, nbytes in (("tracks", 16 + 128 * t.max_tracks), ("assign", 4 * fr.n), ("merged", 16 + 128 * t.max_tracks),
                          ("track_merged", 4 * max(1, t.max_tracks)), ("partner", 4 * max(1, t.max_tracks)),
-                         ("first", max(1, t.max_tracks)), ("tags", fr.n), ("summary", 16),
+                         ("partner_in", 4 * max(1, t.max_tracks)), ("first", max(1, t.max_tracks)), ("tags", fr.n), ("summary", 32),
                          ("time_s", 16 * max(1, t.max_tracks)), ("time_m", 16 * max(1, t.max_tracks))):
         full = torch.full((nbytes + 2 * G,), poison, dtype=torch.uint8, device="cuda")
         bufs[name] = (full, full[G:G + nbytes])
@@ -441,7 +441,8 @@ def test_no_kernel_writes_outside_its_arrays(row_x, case):
         assert t.lib.tpcca_track(t.h, dev.data_ptr(), fr.n, so.ctypes.data, t._stream(), p("tracks"), p("assign")) == 0
         mp, lp = B.default_merge_params(), B.default_leg_params()
         assert t.lib.tpcca_merge(t.h, C.byref(mp), t._stream(), p("merged"), p("track_merged")) == 0
-        assert t.lib.tpcca_find_legs(t.h, C.byref(lp), t._stream(), p("partner"), p("first"), p("tags"), p("summary")) == 0
+        assert t.lib.tpcca_find_legs(t.h, C.byref(lp), t._stream(), p("partner"), p("partner_in"), p("first"), p("tags"),
+                                     p("summary")) == 0
         assert t.lib.tpcca_estimate_time(t.h, 2.58, 250.0, t._stream(), p("time_s"), p("time_m")) == 0
     torch.cuda.synchronize()
     hd = bufs["tracks"][1][:16].cpu().numpy().view(B.HEADER_DTYPE)[0]
