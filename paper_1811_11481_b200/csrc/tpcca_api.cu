@@ -122,9 +122,10 @@ static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params
   CARVE(d.m_cand, int2, K);
   CARVE(d.leg_ends, float4, K * 6);
   CARVE(d.leg_best, unsigned long long, K * 2);
-  CARVE(d.leg_sec, int32_t, 2 * (TPCCA_MAX_SECTORS + 2));
-  CARVE(d.leg_cur, int32_t, 2 * TPCCA_MAX_SECTORS);
+  CARVE(d.leg_sec, int32_t, 2 * (TPCCA_MAX_SECTORS * 128 + 2));   // tpcca_legs.cu: LEG_SEC_STRIDE
+  CARVE(d.leg_cur, int32_t, 2 * TPCCA_MAX_SECTORS * 128);
   CARVE(d.leg_list, int32_t, K * 2);
+  CARVE(d.leg_bk, float4, K * 4);
   CARVE(d.leg_summary, int32_t, 8);
   for (int sl = 0; sl < 2; sl++) {
     CARVE(stage_clusters[sl], float4, N);

@@ -122,9 +122,10 @@ struct Dev {
   tpcca_leg_params LP;
   float4* leg_ends;                // [2][max_tracks][3] outer / inner end of every merged track (layout: tpcca_legs.cu)
   unsigned long long* leg_best;    // [2][max_tracks] (score bits << 32 | partner id), ~0 = none
-  int32_t* leg_sec;                // [2][TPCCA_MAX_SECTORS+2] candidate ends per sector -> bucket starts
-  int32_t* leg_cur;                // [2][TPCCA_MAX_SECTORS] scatter cursors
-  int32_t* leg_list;               // [2][max_tracks] candidate ends grouped by sector
+  int32_t* leg_sec;                // [2][TPCCA_MAX_SECTORS*128+2] candidate ends per (sector, z bin) -> bucket starts
+  int32_t* leg_cur;                // [2][TPCCA_MAX_SECTORS*128] scatter cursors
+  int32_t* leg_list;               // [2][max_tracks] candidate ends grouped by (sector, z bin)
+  float4* leg_bk;                  // [2][2][max_tracks] first 32 bytes of the candidates' records, in leg_list order
   int32_t* leg_summary;            // [8] links per kind, tagged clusters per bit
   int32_t* leg_partner_out;
   int32_t* leg_partner_in_out;

@@ -46,10 +46,20 @@ __device__ __forceinline__ LegEnd load_end(const float4* e, int m) {
 }
 
 // ---------------------------------------------------------------- (l0) ends (D1-D3), candidate count per sector
-#define LEG_SEC_STRIDE (TPCCA_MAX_SECTORS + 2)
+// Candidates are bucketed by (sector, z bin of |z|): LEG_NZB bins of LEG_ZBIN cm per sector (the last one open-ended), so
+// that an end only meets the partners inside a conservative z window (a search structure: any superset of the pairs that
+// pass the cuts gives the same links).
+#define LEG_NZB 128
+#define LEG_ZBIN 32.0f
+#define LEG_NKEY (TPCCA_MAX_SECTORS * LEG_NZB)
+#define LEG_SEC_STRIDE (LEG_NKEY + 2)
+__device__ __forceinline__ int leg_zbin(float z) {
+  const float f = fabsf(z) * (1.0f / LEG_ZBIN);
+  return (f < (float)(LEG_NZB - 1)) ? (int)f : LEG_NZB - 1;  // NaN -> last bin
+}
 __global__ void __launch_bounds__(256) k_leg_reset(Dev d) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < 2 * LEG_SEC_STRIDE) d.leg_sec[i] = 0;
+  for (int j = i; j < 2 * LEG_SEC_STRIDE; j += gridDim.x * blockDim.x) d.leg_sec[j] = 0;
   if (i < 8) d.leg_summary[i] = 0;
   if (i < d.cnt->n_merged) { d.leg_best[i] = LEG_NONE; d.leg_best[d.max_tracks + i] = LEG_NONE; }
 }
@@ -71,7 +81,7 @@ __device__ __forceinline__ void store_end(const Dev& d, int kind, int m, int sec
   e[0] = make_float4(z, s, t, q);
   e[1] = make_float4(c, R, xc, yc);
   e[2] = make_float4(__int_as_float(sector), __int_as_float(cand), 0.f, 0.f);
-  if (cand) atomicAdd(&d.leg_sec[kind * LEG_SEC_STRIDE + sector + 1], 1);
+  if (cand) atomicAdd(&d.leg_sec[kind * LEG_SEC_STRIDE + sector * LEG_NZB + leg_zbin(z) + 1], 1);
 }
 
 __global__ void __launch_bounds__(128) k_leg_ends(Dev d) {
@@ -89,28 +99,39 @@ __global__ void __launch_bounds__(128) k_leg_ends(Dev d) {
   store_end(d, 1, m, M->sector, M->x, M->y, M->z, M->sinphi, M->dzds, M->qpt, tr[head].ndf >= 0);
 }
 
-// one block per kind: exclusive scan of the (<= 64) per-sector counts; leg_sec[s] = start of sector s, cursors behind them
-__global__ void __launch_bounds__(128) k_leg_offsets(Dev d) {
+// one block per kind: exclusive scan of the per-(sector, z bin) counts; leg_sec[key] = start of bucket key, cursors behind
+__global__ void __launch_bounds__(1024) k_leg_offsets(Dev d) {
   __shared__ int sm[32];
   int32_t* sec = d.leg_sec + blockIdx.x * LEG_SEC_STRIDE;
-  int32_t* cur = d.leg_cur + blockIdx.x * TPCCA_MAX_SECTORS;
-  const int s = threadIdx.x;
-  const int v = (s < TPCCA_MAX_SECTORS) ? sec[s + 1] : 0;
-  int tot;
-  const int e = block_scan_excl(v, &tot, sm);
-  __syncthreads();
-  if (s < TPCCA_MAX_SECTORS) { sec[s] = e; cur[s] = e; }
-  if (s == 0) sec[TPCCA_MAX_SECTORS] = tot;
+  int32_t* cur = d.leg_cur + blockIdx.x * LEG_NKEY;
+  int carry = 0;
+  for (int k0 = 0; k0 < LEG_NKEY; k0 += 1024) {
+    const int k = k0 + threadIdx.x;
+    const int v = sec[k + 1];  // count of bucket k (read by all threads before anyone overwrites: the scan synchronises)
+    int tot;
+    const int e = block_scan_excl(v, &tot, sm);
+    __syncthreads();
+    sec[k] = carry + e;
+    cur[k] = carry + e;
+    carry += tot;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) sec[LEG_NKEY] = carry;
 }
 
 __global__ void __launch_bounds__(128) k_leg_scatter(Dev d) {
   const int m = blockIdx.x * blockDim.x + threadIdx.x;
   const int kind = blockIdx.y;
   if (m >= d.cnt->n_merged) return;
-  const float4 c = d.leg_ends[3 * ((size_t)kind * d.max_tracks + m) + 2];
+  const float4* e = d.leg_ends + 3 * ((size_t)kind * d.max_tracks + m);
+  const float4 c = e[2];
   if (!__float_as_int(c.y)) return;
-  const int pos = atomicAdd(&d.leg_cur[kind * TPCCA_MAX_SECTORS + __float_as_int(c.x)], 1);
-  d.leg_list[(size_t)kind * d.max_tracks + pos] = m;  // order inside a sector is arbitrary: the match takes min (score, id)
+  const float4 e0 = e[0];
+  const int pos = atomicAdd(&d.leg_cur[kind * LEG_NKEY + __float_as_int(c.x) * LEG_NZB + leg_zbin(e0.x)], 1);
+  d.leg_list[(size_t)kind * d.max_tracks + pos] = m;  // order inside a bucket is arbitrary: the match takes min (score, id)
+  // the first 32 bytes of the record again, in bucket order: the lanes of k_leg_match read consecutive entries
+  d.leg_bk[(size_t)(2 * kind) * d.max_tracks + pos] = e0;
+  d.leg_bk[(size_t)(2 * kind + 1) * d.max_tracks + pos] = e[1];
 }
 
 // ---------------------------------------------------------------- (l1) pair scores (D4-D8): one warp per end A
@@ -168,6 +189,8 @@ __global__ void __launch_bounds__(128) k_leg_match(Dev d) {
   const float4* ends = d.leg_ends + 3 * (size_t)kind * d.max_tracks;
   const int32_t* sec = d.leg_sec + kind * LEG_SEC_STRIDE;
   const int32_t* list = d.leg_list + (size_t)kind * d.max_tracks;
+  const float4* bk0 = d.leg_bk + (size_t)(2 * kind) * d.max_tracks;
+  const float4* bk1 = d.leg_bk + (size_t)(2 * kind + 1) * d.max_tracks;
   unsigned long long* bestv = d.leg_best + (size_t)kind * d.max_tracks;
   const LegEnd A = load_end(ends, a);
   if (!A.cand) return;
@@ -178,6 +201,19 @@ __global__ void __launch_bounds__(128) k_leg_match(Dev d) {
   const float sig = kind == 0 ? 1.0f : -1.0f;
   const int sgn = ((sig * A.q) * d.kq > 0.0f) ? 1 : -1;
   const int base = ring > 0 ? (A.sector / ring) * ring : A.sector, l = A.sector - base;
+  // Conservative z window of the partners (same z side, so |z| orders like z up to the sign): a partner passes
+  // |tA + tB| <= dt_tol, |RA - RB| <= f Rm and theta <= theta_max, hence |mean slope| <= |tA| + dt_tol / 2 and
+  // arc <= theta_max RA / (1 - f / 2); zB - zA lies within that product plus leg_dz_max.  1 % and one bin of slack.
+  const float f2 = 0.5f * d.LP.leg_radius_frac;
+  const float thmax = kind == 0 ? d.LP.leg_max_turn : d.LP.leg_inner_max_turn;
+  int zb_lo = 0, zb_hi = LEG_NZB - 1;
+  if (f2 < 0.9f) {
+    const float reach = 1.01f * ((fabsf(A.t) + 0.5f * d.LP.leg_dzds_tol) * (thmax * A.R / (1.0f - f2)) + d.LP.leg_dz_max) + 1.0f;
+    const float az = fabsf(A.z);
+    zb_lo = max(0, leg_zbin(fmaxf(az - reach, 0.0f)) - 1);
+    zb_hi = min(LEG_NZB - 1, leg_zbin(az + reach) + 1);
+    if (!(reach == reach)) { zb_lo = 0; zb_hi = LEG_NZB - 1; }
+  }
   // sector offsets dsec = 0 .. ring-1 of the partner; jrot as in DESIGN.md D4
   const int nsec = ring > 0 ? ring : 1;
   unsigned long long best = LEG_NONE;
@@ -195,11 +231,19 @@ __global__ void __launch_bounds__(128) k_leg_match(Dev d) {
     }
     const int sb = ring > 0 ? base + (l + dsec) % ring : A.sector;
     if (sb >= d.n_sectors) continue;
-    const int b0 = sec[sb], b1 = sec[sb + 1];
+    const int b0 = sec[sb * LEG_NZB + zb_lo], b1 = sec[sb * LEG_NZB + zb_hi + 1];
     for (int pos = b0 + lane; pos < b1; pos += 32) {
       const int b = list[pos];
       if (b <= a) continue;
-      const LegEnd B = load_end(ends, b);
+      // the cheap cuts first, on the first 16 bytes of B's record (q/pT sign and slope sum), then the radius: the order of
+      // the cuts does not change which pairs pass all of them (D7)
+      const float4 b0v = bk0[pos];
+      if (!(A.q * b0v.w < 0.0f) || !(fabsf(A.t + b0v.z) <= d.LP.leg_dzds_tol)) continue;
+      const float4 b1v = bk1[pos];
+      if (!(fabsf(A.R - b1v.y) <= d.LP.leg_radius_frac * (0.5f * (A.R + b1v.y)))) continue;
+      LegEnd B;
+      B.z = b0v.x; B.s = b0v.y; B.t = b0v.z; B.q = b0v.w; B.c = b1v.x; B.R = b1v.y; B.xc = b1v.z; B.yc = b1v.w;
+      B.sector = sb; B.cand = 1;
       const float sc = leg_pair_score(d, A, B, jrot, sgn, sig, ca, sa);
       if (!(sc >= 0.0f)) continue;
       const unsigned long long sb64 = (unsigned long long)__float_as_uint(sc) << 32;  // score >= +0: bits order like values
@@ -289,16 +333,16 @@ void launch_legs(const Dev& d, Launch& L) {
   const int K = d.max_tracks;
   if (d.n > 0) cudaMemsetAsync(d.tags_out, 0, (size_t)d.n, L.st);
   if (d.n > 0 && K > 0) {
-    k_leg_reset<<<(max(K, 128) + 255) / 256, 256, 0, L.st>>>(d);
+    k_leg_reset<<<(max(K, 2 * LEG_SEC_STRIDE) + 255) / 256, 256, 0, L.st>>>(d);
     k_leg_ends<<<(K + 127) / 128, 128, 0, L.st>>>(d);
-    k_leg_offsets<<<2, 128, 0, L.st>>>(d);
+    k_leg_offsets<<<2, 1024, 0, L.st>>>(d);
     k_leg_scatter<<<dim3((K + 127) / 128, 2), 128, 0, L.st>>>(d);
     k_leg_match<<<dim3((K + 3) / 4, 2), 128, 0, L.st>>>(d);
     k_leg_link<<<(K + 255) / 256, 256, 0, L.st>>>(d);
     k_leg_tags<<<(K + 3) / 4, 128, 0, L.st>>>(d);
     L.count += 7;
   } else {
-    k_leg_reset<<<1, 256, 0, L.st>>>(d);
+    k_leg_reset<<<8, 256, 0, L.st>>>(d);
     L.count++;
   }
   k_leg_summary<<<1, 32, 0, L.st>>>(d);
