@@ -12,7 +12,7 @@ SO = os.path.join(_HERE, "libtpcca.so")
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-    "-fmad=false",  # decision arithmetic must not contract a*b+c
+    "-fmad=false",  # the compiler never fuses on its own: a fused multiply-add exists exactly where DESIGN.md section 3 states one
     "-Xcompiler", "-fPIC", "-shared", "--cudart", "static",
 ]
 
