@@ -84,7 +84,11 @@ bool transport(KF& k, float xnew, float kq, float max_sinphi) {
   const float cos0 = std::sqrt(fma32(-s0, s0, 1.0f));
   const float cos1 = std::sqrt(fma32(-s1, s1, 1.0f));
   const float csum = cos0 + cos1;
-  const float f = (s0 + s1) / csum;
+  // the three quotients by cos0, cos1 and their sum share ONE division: inv = 1 / (cos0 cos1 csum)
+  const float c01 = cos0 * cos1;
+  const float inv = 1.0f / (c01 * csum);
+  const float icsum = c01 * inv, icos0 = (cos1 * csum) * inv, icos1 = (cos0 * csum) * inv;
+  const float f = (s0 + s1) * icsum;
   const float dy = dx * f;
   float L = std::sqrt(fma32(dx, dx, dy * dy));
   if (dx < 0.0f) L = -L;
@@ -93,8 +97,8 @@ bool transport(KF& k, float xnew, float kq, float max_sinphi) {
   const float g = fma32(u2, fma32(u2, 0.075f, 0.16666667f), 1.0f);  // asin(u)/u = 1 + u^2/6 + 3u^4/40 + ...
   const float arc = L * g;
   // Jacobian (d g neglected): d f / d s0 and d f / d s1, then the chain rule through s1 = s0 + dx * kq * q
-  const float df_ds0 = (1.0f + (f * s0) / cos0) / csum;
-  const float df_ds1 = (1.0f + (f * s1) / cos1) / csum;
+  const float df_ds0 = fma32(f * s0, icos0, 1.0f) * icsum;
+  const float df_ds1 = fma32(f * s1, icos1, 1.0f) * icsum;
   const float ds1_dq = dx * kq;
   const float df_ds = df_ds0 + df_ds1;
   const float darc_df = (tl * g) * ((dx * dy) / L);  // d(z~)/df = t * g * dL/df, dL/df = dx*dy/L
