@@ -182,7 +182,10 @@ __device__ __forceinline__ bool kf_transport(KF& k, float xnew, float kq, float 
   const float c0 = sqrtf(fmaf(-s, s, 1.0f));
   const float c1 = sqrtf(fmaf(-s1, s1, 1.0f));
   const float cc = c0 + c1;
-  const float f = (s + s1) / cc;
+  const float c01 = c0 * c1;
+  const float inv = 1.0f / (c01 * cc);  // the one division shared by 1/cc, 1/c0, 1/c1
+  const float icc = c01 * inv, ic0 = (c1 * cc) * inv, ic1 = (c0 * cc) * inv;
+  const float f = (s + s1) * icc;
   const float dy = dx * f;
   float L = sqrtf(fmaf(dx, dx, dy * dy));
   if (dx < 0.0f) L = -L;
@@ -190,8 +193,8 @@ __device__ __forceinline__ bool kf_transport(KF& k, float xnew, float kq, float 
   const float u2 = u * u;
   const float g = fmaf(u2, fmaf(u2, 0.075f, 0.16666667f), 1.0f);
   const float dS = L * g;
-  const float fs0 = (1.0f + (f * s) / c0) / cc;
-  const float fs1 = (1.0f + (f * s1) / c1) / cc;
+  const float fs0 = fmaf(f * s, ic0, 1.0f) * icc;
+  const float fs1 = fmaf(f * s1, ic1, 1.0f) * icc;
   const float h = dx * kq;
   const float fss = fs0 + fs1;
   const float a02 = dx * fss;
@@ -239,8 +242,7 @@ __device__ __forceinline__ bool kf_transport(KF& k, float xnew, float kq, float 
 
 // One scalar measurement update of component with pre-update column (i0..i4), state value xi, variance v
 // (x_j <- fma(K_j, r, x_j), C_jl <- fma(-K_j, ci_l, C_jl), chi2 <- fma(r*r, w, chi2)).
-__device__ __forceinline__ void kf_update1(KF& k, float i0, float i1, float i2, float i3, float i4, float r, float S) {
-  const float w = 1.0f / S;
+__device__ __forceinline__ void kf_update1(KF& k, float i0, float i1, float i2, float i3, float i4, float r, float w) {
   const float K0 = i0 * w, K1 = i1 * w, K2 = i2 * w, K3 = i3 * w, K4 = i4 * w;
   k.y = fmaf(K0, r, k.y); k.z = fmaf(K1, r, k.z); k.s = fmaf(K2, r, k.s); k.t = fmaf(K3, r, k.t); k.q = fmaf(K4, r, k.q);
   k.c00 = fmaf(-K0, i0, k.c00);
@@ -252,10 +254,12 @@ __device__ __forceinline__ void kf_update1(KF& k, float i0, float i1, float i2, 
   k.chi2 = fmaf(r * r, w, k.chi2);
 }
 
-// Sequential scalar updates, y then z~.
-__device__ __forceinline__ void kf_update(KF& k, float ym, float zm, float sy2, float sz2) {
-  kf_update1(k, k.c00, k.c10, k.c20, k.c30, k.c40, ym - k.y, k.c00 + sy2);  // component 0: column (c00, c10, c20, c30, c40)
-  kf_update1(k, k.c10, k.c11, k.c21, k.c31, k.c41, zm - k.z, k.c11 + sz2);  // component 1: column (c10, c11, c21, c31, c41)
+// Sequential scalar updates, y then z~; w = 1/S of each.  wy: the caller's 1 / (c00 + sy2) if it already has it (the predicted
+// distance of a hit uses the same quotient), else a negative value.
+__device__ __forceinline__ void kf_update(KF& k, float ym, float zm, float sy2, float sz2, float wy = -1.0f) {
+  if (wy < 0.0f) wy = 1.0f / (k.c00 + sy2);
+  kf_update1(k, k.c00, k.c10, k.c20, k.c30, k.c40, ym - k.y, wy);                     // component 0: column (c00, c10, c20, c30, c40)
+  kf_update1(k, k.c10, k.c11, k.c21, k.c31, k.c41, zm - k.z, 1.0f / (k.c11 + sz2));  // component 1: column (c10, c11, c21, c31, c41)
 }
 
 // same-row key order (ord z, ord y, input index): true if a < b

@@ -257,7 +257,7 @@ __global__ void __launch_bounds__(64) k_merge_fit(Dev d) {
         const float dz = (pj.y - z_ref) - k.z;
         const float dist = fmaf(dz * dz, iz, (dy * dy) * iy);
         if (!(dist <= d.MP.fit_reject_cut)) continue;  // outlier for this pass
-        kf_update(k, pj.x, pj.y - z_ref, vy, vz);
+        kf_update(k, pj.x, pj.y - z_ref, vy, vz, iy);
         n_used++;
       }
     }

@@ -115,10 +115,12 @@ __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefe
 #ifndef SEARCH_UNROLL
 #define SEARCH_UNROLL 3
 #endif
-__device__ __forceinline__ int search_row(const Dev& d, const GridHdr& g, const KF& k, float z_ref, float2& pbest) {
+// wy_out = 1 / (c00 + sigma_y^2): the same quotient the update of the chosen hit starts with.
+__device__ __forceinline__ int search_row(const Dev& d, const GridHdr& g, const KF& k, float z_ref, float2& pbest, float& wy_out) {
   const float cut = d.P.pick_cut;
   const float vy = k.c00 + d.sy2, vz = k.c11 + d.sz2;
   const float iy = 1.0f / vy, iz = 1.0f / vz;
+  wy_out = iy;
   const float wy = sqrtf(cut * vy), wz = sqrtf(cut * vz);
   int y0, y1, z0, z1;
   const float zc = z_ref + k.z;  // search centre in frame coordinates (bin lookup only)
@@ -312,10 +314,11 @@ __global__ void __launch_bounds__(E_THREADS, E2_BLOCKS) k_tl_e2(Dev d) {
       continue;
     }
     float2 pb = make_float2(0.f, 0.f);
-    const int cand = search_row(d, g, k, z_ref, pb);
+    float wy;
+    const int cand = search_row(d, g, k, z_ref, pb, wy);
     rh[r] = cand;
     if (cand >= 0) {
-      kf_update(k, pb.x, pb.y - z_ref, d.sy2, d.sz2);
+      kf_update(k, pb.x, pb.y - z_ref, d.sy2, d.sz2, wy);
       gap = 0; top_row = r;
       sx = k.x; sy = k.y; sz = k.z; ss = k.s; st_ = k.t; sq = k.q;
     } else {
@@ -419,8 +422,10 @@ __global__ void __launch_bounds__(E_THREADS, E3_BLOCKS) k_tl_e3a(Dev d) {
       continue;
     }
     int cand;
+    float wy;
     if (cur >= 0) {  // existing hit: kept iff d <= reject_cut (no window), O5/E3
       const float iy = 1.0f / (k.c00 + d.sy2), iz = 1.0f / (k.c11 + d.sz2);
+      wy = iy;
       const float dy = pb.x - k.y;
       const float dz = (pb.y - z_ref) - k.z;
       const float dist = fmaf(dz * dz, iz, (dy * dy) * iy);
@@ -428,11 +433,11 @@ __global__ void __launch_bounds__(E_THREADS, E3_BLOCKS) k_tl_e3a(Dev d) {
     } else {  // gap row inside the range (rare): pick-up search
       n_search++;
       const GridHdr g = d.grid[sbase + r];
-      cand = search_row(d, g, k, z_ref, pb);
+      cand = search_row(d, g, k, z_ref, pb, wy);
     }
     if (cand != cur) rh[r] = cand;  // rejected hit -> -1, or the search result
     if (cand >= 0) {
-      kf_update(k, pb.x, pb.y - z_ref, d.sy2, d.sz2);
+      kf_update(k, pb.x, pb.y - z_ref, d.sy2, d.sz2, wy);
       gap = 0; inner_row = r; n_hits++;
       if (outer_row < 0) outer_row = r;
       ix = k.x; iy_ = k.y; iz_ = k.z; is = k.s; it = k.t; iq = k.q; ichi = k.chi2;
@@ -523,10 +528,11 @@ __global__ void __launch_bounds__(E_THREADS, E3B_BLOCKS) k_tl_e3b(Dev d) {
       continue;
     }
     float2 pb = make_float2(0.f, 0.f);
-    const int cand = search_row(d, g, k, z_ref, pb);
+    float wy;
+    const int cand = search_row(d, g, k, z_ref, pb, wy);
     rh[r] = cand;
     if (cand >= 0) {
-      kf_update(k, pb.x, pb.y - z_ref, d.sy2, d.sz2);
+      kf_update(k, pb.x, pb.y - z_ref, d.sy2, d.sz2, wy);
       gap = 0; inner_row = r; n_hits++;
       if (outer_row < 0) outer_row = r;
       ix = k.x; iy_ = k.y; iz_ = k.z; is = k.s; it = k.t; iq = k.q; ichi = k.chi2;
