@@ -50,6 +50,18 @@ def test_legs_parity_full_frame(row_x):
     assert (orc.leg_partner >= 0).sum() > 1000
 
 
+def test_legs_parity_23ms_time_frame(row_x):
+    """|z| up to 6e4 cm: z differences of nearby legs are still exact in fp32 (a few ulp of 4e-3 cm against
+    a 4 cm window), and the z bins of the candidate buckets saturate (everything beyond 4096 cm falls into the last bin) --
+    the links must not depend on that search structure."""
+    cfg = synth.config(5, scale=0.4, seed=23)
+    cfg["time_window_us"] = 23000.0
+    fr = synth.generate(cfg)
+    assert float(np.abs(fr.clusters["z"]).max()) > 5.0e4
+    t, orc = compare_legs(fr, row_x)
+    assert (orc.leg_partner >= 0).sum() > 200 and (orc.leg_partner_in >= 0).sum() > 200
+
+
 def test_legs_parity_hand_built_loopers(row_x):
     """The float64 helices of the oracle pins: one looper of each charge, three turns at a 12 cm pitch, a 45 MeV/c secondary
     circling inside the TPC -- all in one frame."""
