@@ -35,6 +35,13 @@ DEFAULT_LEG_PARAMS = dict(leg_min_qpt=4.0, leg_min_sinphi=0.5, leg_inner_min_sin
                           leg_inner_max_sector_gap=9, leg_max_turn=2.9, leg_inner_max_turn=5.0, leg_centre_frac=0.05, leg_centre_abs=1.5, leg_radius_frac=0.2,
                           leg_dz_max=4.0, leg_dzds_tol=0.1, tag_qpt_low=20.0, tag_qpt_leg=5.0, tag_sinphi=0.8, ring=18)
 TAG_LOW_PT, TAG_EXTRA_LEG, TAG_HIGH_INCLINATION = 1, 2, 4
+# DESIGN.md section 15 Table E defaults of the fit through both legs of a turn
+DEFAULT_LEG_FIT_PARAMS = dict(fit_rot_sinphi=0.5, fit_step_sinphi=0.7, fit_min_d=0.3, fit_reject_cut=30.0, shared_err_scale=2.0, ring=18)
+
+
+class _FitParams(C.Structure):
+    _fields_ = [("fit_rot_sinphi", C.c_float), ("fit_step_sinphi", C.c_float), ("fit_min_d", C.c_float), ("fit_reject_cut", C.c_float),
+                ("shared_err_scale", C.c_float), ("ring", C.c_int32)]
 
 
 class _LegParams(C.Structure):
@@ -136,6 +143,11 @@ def _load(opt: str = "-O2"):
         for name in ("orc_leg_partner", "orc_leg_partner_in", "orc_leg_first", "orc_cluster_tags"):
             getattr(lib, name).restype = C.c_void_p
             getattr(lib, name).argtypes = [C.c_void_p]
+        lib.orc_fit_legs.restype = C.c_int64
+        lib.orc_fit_legs.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_float, C.POINTER(_Params), C.c_void_p,
+                                     C.POINTER(_FitParams)]
+        lib.orc_leg_fits.restype = C.c_void_p
+        lib.orc_leg_fits.argtypes = [C.c_void_p]
         lib.orc_angle_upper.restype = C.c_float
         lib.orc_angle_upper.argtypes = [C.c_float, C.c_float]
         lib.orc_leg_end.argtypes = [C.c_int32, C.c_void_p, C.c_float, C.c_float, C.POINTER(_LegParams), C.c_void_p]
@@ -190,6 +202,7 @@ class OracleResult:
     leg_partner_in: np.ndarray = None  # merged track -> merged track joined through the inner region or -1
     leg_first: np.ndarray = None     # merged track: 1 first / only leg, 0 additional leg
     cluster_tags: np.ndarray = None  # uint8 per cluster: TAG_* bits (O13)
+    leg_fits: np.ndarray = None      # TRACK_DTYPE, one fit per pair of legs joined at a turning point (O14); with leg_fit=...
     time_sector: np.ndarray = None   # (n_tracks, 4): z_dca, z_shift, t0_us, dca_xy (O11); only with time=...
     time_merged: np.ndarray = None   # (n_merged, 4)
 
@@ -203,7 +216,7 @@ def _arr(ptr, n, dtype):
 
 def track(clusters: np.ndarray, sector_offsets: np.ndarray, row_x: np.ndarray, bz: float = 0.5,
           params: dict | None = None, brute: bool = False, opt: str = "-O2", merge: dict | bool | None = None,
-          time: dict | bool | None = None, legs: dict | bool | None = None) -> OracleResult:
+          time: dict | bool | None = None, legs: dict | bool | None = None, leg_fit: dict | bool | None = None) -> OracleResult:
     """Steps O1-O7 on one frame.  `clusters`: structured (x,y,z f32,row i32); returns input-index-space results.
     merge: True or a dict of DEFAULT_MERGE_PARAMS overrides -> also steps O8-O10 (sector-segment merger + final fit).
     legs: True or a dict of DEFAULT_LEG_PARAMS overrides -> also O12-O13 (looper legs, cluster tags); needs merge.
@@ -251,6 +264,14 @@ def track(clusters: np.ndarray, sector_offsets: np.ndarray, row_x: np.ndarray, b
             res.leg_partner_in = _arr(lib.orc_leg_partner_in(h), len(res.merged), np.int32)
             res.leg_first = _arr(lib.orc_leg_first(h), len(res.merged), np.uint8)
             res.cluster_tags = _arr(lib.orc_cluster_tags(h), n, np.uint8)
+        if leg_fit:
+            assert legs, "the pair fit needs the leg links"
+            fd = dict(DEFAULT_LEG_FIT_PARAMS)
+            if isinstance(leg_fit, dict):
+                fd.update(leg_fit)
+            fp = _FitParams(**fd)
+            nf = lib.orc_fit_legs(h, nr, rx.ctypes.data, bz, C.byref(cp), cl.ctypes.data, C.byref(fp))
+            res.leg_fits = _arr(lib.orc_leg_fits(h), nf, TRACK_DTYPE)
         if time:
             td = dict(DEFAULT_TIME_PARAMS)
             if isinstance(time, dict):

@@ -203,6 +203,7 @@ struct Result {
   std::vector<int32_t> leg_partner_in;           // merged track -> merged track joined through the inner region, or -1
   std::vector<uint8_t> leg_first;                // merged track: 1 = first (or only) leg, 0 = additional leg
   std::vector<uint8_t> cluster_tags;             // per cluster: TAG_* bits
+  std::vector<TrackRec> leg_fits;                // O14: one fit per pair of legs joined at a turning point
 };
 
 struct Sector {
@@ -874,6 +875,178 @@ void find_legs(Result* R, const Ctx& c, const LegParams& L) {
   }
 }
 
+// ---- O14: one fit through both legs of a turn ("the refit was tuned to enable arbitrary rotations for
+// following the full helix") ----
+// The filter runs in a frame that is turned in sector steps whenever |sin(phi)| grows beyond fit_rot_sinphi, so that the
+// track always points roughly along the frame's x axis -- also over the turning point, where no sector frame can describe
+// it.  A hit of sector S seen from frame F (beta = (S - F) sector angles): its position is rotated into the frame; the
+// pad row is no longer parallel to the frame's y axis, and the row coordinate of the track's crossing differs from the
+// track's y at the hit's x by the factor D = cos(beta) + sin(beta) tan(phi), so the hit is a measurement of y with the
+// error sigma_y * |D| (the dependence of D on the state is neglected, the z measurement is unchanged).
+struct FitParams {
+  float fit_rot_sinphi;   // turn the frame while |sin(phi)| exceeds this
+  float fit_step_sinphi;  // a step never takes |sin(phi)| beyond this: it stops there and the frame is turned
+  float fit_min_d;        // hits with |D| below this are not used (pad row nearly parallel to the track)
+  float fit_reject_cut, shared_err_scale;
+  int32_t ring;
+};
+
+struct ChainHit { int32_t h, sector; };
+
+// cos / sin of n sector angles by n rotations of (1, 0)
+inline void sector_cs(int n, float ca, float sa, float& cb, float& sb) {
+  cb = 1.0f; sb = 0.0f;
+  const float ss = (n >= 0) ? sa : -sa;
+  for (int i = 0; i < std::abs(n); i++) {
+    const float u = fma32(-sb, ss, cb * ca), v = fma32(cb, ss, sb * ca);
+    cb = u; sb = v;
+  }
+}
+
+// One pair: hits in trajectory order (first leg inner -> outer, second leg outer -> inner).  Returns false if a frame
+// change or a transport fails.
+bool fit_chain(const Ctx& c, const Result* R, const std::vector<ChainHit>& hits, float q0, const FitParams& F, float ca, float sa,
+               KF& k, int& frame, float& z_ref, int& n_used, int& n_turn) {
+  const Cl* cl = c.cl;
+  const Params& P = c.P;
+  const int n = (int)hits.size();
+  const int ring = F.ring;  // <= 0: the frame cannot be turned (a fit that needs it fails)
+  // start at the last hit, direction towards the one before it, in the last hit's sector frame
+  const Cl& hN = cl[hits[n - 1].h];
+  const Cl& hM = cl[hits[n - 2].h];
+  if (hits[n - 1].sector != hits[n - 2].sector) return false;
+  frame = hits[n - 1].sector;
+  z_ref = hN.z;
+  {
+    const float dx = hM.x - hN.x, dy = hM.y - hN.y, dz = hM.z - hN.z;
+    const float ds = std::sqrt(fma32(dx, dx, dy * dy));
+    k.x = hN.x;
+    k.p[0] = hN.y; k.p[1] = 0.0f; k.p[2] = dy / ds; k.p[3] = dz / ds; k.p[4] = q0;
+  }
+  n_turn = 0;
+  for (int pass = 0; pass < 3; pass++) {
+    reset_cov(k, P);
+    n_used = 0;
+    for (int j = 0; j < n; j++) {
+      const int idx = (pass == 1) ? j : n - 1 - j;
+      const Cl& h = cl[hits[idx].h];
+      // Frame policy: keep the track roughly along the frame's x axis.  Turn the frame (one sector step at a time) while
+      // |sin(phi)| > fit_rot_sinphi; if the way to the hit would take |sin(phi)| beyond fit_step_sinphi (the gap over the
+      // turning point, where no pad row was tracked), go only as far as |sin(phi)| = fit_step_sinphi, turn, and go on.
+      float cb = 1.0f, sb = 0.0f, X = 0.0f, Y = 0.0f;
+      bool reached = false;
+      for (int iter = 0; iter < 4 * ring + 1 && !reached; iter++) {
+        for (int step = 0; step < ring && std::fabs(k.p[2]) > F.fit_rot_sinphi; step++) {
+          const int sgn = k.p[2] > 0.0f ? 1 : -1;
+          if (!rotate_frame(k, ca, (float)sgn * sa, c.kq, 0.9999f)) return false;
+          frame = (frame / ring) * ring + ((frame % ring) + sgn + ring) % ring;
+          n_turn++;
+        }
+        int beta = 0;
+        if (ring > 0) {
+          beta = ((hits[idx].sector - frame) % ring + ring) % ring;
+          if (2 * beta > ring) beta -= ring;
+        } else if (hits[idx].sector != frame) return false;
+        sector_cs(beta, ca, sa, cb, sb);
+        X = fma32(-h.y, sb, h.x * cb); Y = fma32(h.x, sb, h.y * cb);  // the hit in the fit frame
+        const float kk = k.p[4] * c.kq;
+        const float s_at = fma32(X - k.x, kk, k.p[2]);
+        if (std::fabs(s_at) <= F.fit_step_sinphi) { reached = true; break; }
+        const float target = s_at > 0.0f ? F.fit_step_sinphi : -F.fit_step_sinphi;
+        const float dxp = (target - k.p[2]) / kk;
+        if (!((dxp > 0.0f) == (X - k.x > 0.0f)) || dxp == 0.0f) return false;
+        if (!transport(k, k.x + dxp, c.kq, P.max_sinphi)) return false;
+      }
+      if (!reached) return false;
+      if (!transport(k, X, c.kq, P.max_sinphi)) return false;
+      const float cphi = std::sqrt(fma32(-k.p[2], k.p[2], 1.0f));
+      const float D = fma32(sb, k.p[2] / cphi, cb);
+      if (!(std::fabs(D) >= F.fit_min_d)) continue;
+      const bool sh = R->shared[hits[idx].h] != 0;
+      const float ey = (sh ? P.sigma_y * F.shared_err_scale : P.sigma_y) * D;
+      const float ez = sh ? P.sigma_z * F.shared_err_scale : P.sigma_z;
+      const float vy = ey * ey, vz = ez * ez;
+      const float iy = 1.0f / (k.C[0] + vy), iz = 1.0f / (k.C[2] + vz);
+      const float dy = Y - k.p[0];
+      const float dz = (h.z - z_ref) - k.p[1];
+      const float d = fma32(dz * dz, iz, (dy * dy) * iy);
+      if (!(d <= F.fit_reject_cut)) continue;
+      update(k, Y, h.z - z_ref, vy, vz);
+      n_used++;
+    }
+  }
+  return true;
+}
+
+void fit_leg_pairs(Result* R, const Ctx& c, const FitParams& F) {
+  const Params& P = c.P;
+  const int nm = (int)R->merged.size();
+  const float th = P.tan_half_angle;
+  const float den = fma32(th, th, 1.0f);
+  const float ca = fma32(-th, th, 1.0f) / den, sa = (2.0f * th) / den;
+  R->leg_fits.clear();
+  auto chain_hits = [&](int m, bool reversed, std::vector<ChainHit>& out) {
+    std::vector<ChainHit> tmp;
+    for (int t = R->merged[m].pad[4]; t >= 0; t = R->link_next[t])
+      for (int32_t h : R->track_hits[t]) tmp.push_back({h, R->tracks[t].sector});
+    if (reversed) std::reverse(tmp.begin(), tmp.end());
+    out.insert(out.end(), tmp.begin(), tmp.end());
+  };
+  for (int a = 0; a < nm; a++) {
+    const int b = R->leg_partner[a];
+    if (b < a) continue;  // none, or the pair was done from its lower id
+    const float za = std::fabs(R->merged[a].z), zb = std::fabs(R->merged[b].z);
+    const bool a_first = (za < zb) || (za == zb);   // a < b: equal |z| -> the lower id
+    const int f = a_first ? a : b, g = a_first ? b : a;
+    std::vector<ChainHit> hits;
+    chain_hits(f, false, hits);
+    chain_hits(g, true, hits);
+    TrackRec tr;
+    std::memset(&tr, 0, sizeof(tr));
+    KF k;
+    k.x = 0; k.chi2 = 0;
+    for (int i = 0; i < 5; i++) k.p[i] = 0;
+    for (int i = 0; i < 15; i++) k.C[i] = 0;
+    int frame = 0, n_used = 0, n_turn = 0;
+    float z_ref = 0;
+    bool ok = fit_chain(c, R, hits, R->merged[g].qpt, F, ca, sa, k, frame, z_ref, n_used, n_turn);
+    // The filter arrives at the first leg's innermost hit running AGAINST that leg's direction of fit.  Report the state
+    // as the leg's own record does -- direction outward, frame of the innermost segment's sector: seen from the frame
+    // turned by half a ring the reversed direction has cos(phi) > 0 again (x, y, dz/ds and q/pT change sign, sin(phi) does
+    // not), then the frame is turned step by step to the sector's.
+    const int ring = F.ring;
+    if (ok && ring > 0 && ring % 2 == 0) {
+      static const float sg[5] = {-1.0f, 1.0f, 1.0f, -1.0f, -1.0f};
+      k.x = -k.x; k.p[0] = -k.p[0]; k.p[3] = -k.p[3]; k.p[4] = -k.p[4];
+      for (int i = 0; i < 5; i++)
+        for (int j = 0; j <= i; j++) k.C[tri(i, j)] = (sg[i] * sg[j]) * k.C[tri(i, j)];
+      frame = (frame / ring) * ring + ((frame % ring) + ring / 2) % ring;
+      const int target = R->merged[f].sector;
+      int dsec = ((target - frame) % ring + ring) % ring;
+      if (2 * dsec > ring) dsec -= ring;
+      const int sgn = dsec >= 0 ? 1 : -1;
+      for (int i = 0; i < std::abs(dsec) && ok; i++) {
+        ok = rotate_frame(k, ca, (float)sgn * sa, c.kq, 0.9999f);
+        frame = (frame / ring) * ring + ((frame % ring) + sgn + ring) % ring;
+      }
+      // the fitted point left the pad row by (fitted - measured y) * sin(beta): a last, tiny step back onto it
+      if (ok) ok = transport(k, c.cl[hits.front().h].x, c.kq, 0.9999f);
+    }
+    tr.sector = frame; tr.first_row = c.cl[hits.front().h].row; tr.last_row = c.cl[hits.back().h].row;
+    tr.n_hits = (int32_t)hits.size();
+    if (ok) {
+      tr.x = k.x; tr.y = k.p[0]; tr.z = k.p[1] + z_ref; tr.sinphi = k.p[2]; tr.dzds = k.p[3]; tr.qpt = k.p[4];
+      for (int i = 0; i < 15; i++) tr.cov[i] = k.C[i];
+      tr.chi2 = k.chi2;
+      tr.ndf = 2 * n_used - 5;
+    } else {
+      tr.ndf = -1;
+    }
+    tr.pad[0] = f; tr.pad[1] = g; tr.pad[2] = ok ? (int32_t)hits.size() - n_used : -1; tr.pad[3] = n_turn; tr.pad[4] = 0;
+    R->leg_fits.push_back(tr);
+  }
+}
+
 }  // namespace
 
 extern "C" {
@@ -1047,6 +1220,15 @@ float orc_leg_pair(int32_t sig, const float* a7, const float* b7, float bz, floa
   const LegEnd B = leg_end(sig, (int)b7[0], b7[1], b7[2], b7[3], b7[4], b7[5], b7[6], true, kq, x_last, *L);
   return leg_pair_score(A, B, kq, ca, sa, *L);
 }
+
+// O14 on a result of orc_track + orc_merge + orc_legs.  Returns the number of pair fits (= outer links).
+int64_t orc_fit_legs(void* r, int32_t n_rows, const float* row_x, float bz, const Params* P, const Cl* cl, const FitParams* F) {
+  Result* R = (Result*)r;
+  Ctx c = make_ctx(cl, row_x, n_rows, *P, bz, false);
+  fit_leg_pairs(R, c, *F);
+  return (int64_t)R->leg_fits.size();
+}
+const TrackRec* orc_leg_fits(void* r) { return ((Result*)r)->leg_fits.data(); }
 
 void orc_free(void* r) { delete (Result*)r; }
 int64_t orc_n_start(void* r) { return (int64_t)((Result*)r)->start_hits.size(); }
