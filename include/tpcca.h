@@ -244,6 +244,32 @@ int tpcca_find_legs(tpcca_handle* h, const tpcca_leg_params* lp, void* stream, i
                     int32_t* out_leg_partner_inner, uint8_t* out_leg_first, uint8_t* out_cluster_tags,
                     tpcca_leg_summary* out_summary);
 
+/* ---- One fit through both legs of a turn ("the refit was tuned to enable arbitrary rotations for following the
+ * full helix", Table E).  For every pair of merged tracks joined at an outer turning point by the
+ * last tpcca_find_legs, a three-pass Kalman fit over the hits of BOTH legs in trajectory order; the frame of the filter is
+ * turned in sector steps so that the track always points roughly along its x axis, and a hit seen from a turned frame
+ * enters with the error sigma_y * |cos(beta) + sin(beta) tan(phi)|. */
+typedef struct {
+  float fit_rot_sinphi;    /* turn the frame one sector step while |sin(phi)| exceeds this */
+  float fit_step_sinphi;   /* a transport never takes |sin(phi)| beyond this: it stops there and the frame is turned */
+  float fit_min_d;         /* hits whose pad row runs nearly along the track (|D| below this) are not used */
+  float fit_reject_cut;    /* 2-dof predicted distance above which a hit is left out of a pass */
+  float shared_err_scale;  /* sigma_y, sigma_z multiplier of shared clusters */
+  int32_t ring;            /* sectors per z side closing the ring; must be even (18) for the report in the first leg's frame */
+} tpcca_leg_fit_params;
+void tpcca_default_leg_fit_params(tpcca_leg_fit_params* p);
+
+/* Fit the pairs of the LAST tpcca_find_legs on this handle (whose out_leg_partner, and the outputs of the tpcca_merge and
+ * tpcca_track before it, must still be valid and unchanged); enqueued on `stream`, returns without waiting.
+ * out_fits: device, 16-byte aligned, sizeof(tpcca_out_header) + max_tracks * 128 bytes: header {n_tracks = pairs,
+ *   n_tracklets = fits that failed (ndf = -1), n_start_hits = 0, status}, then one tpcca_track_rec per pair in the order
+ *   of the pair's lower merged id: state at the innermost hit of the FIRST leg (smaller |z| of the inner end), in that
+ *   leg's innermost sector frame, direction outward -- comparable with the leg's own merged record --, first_row = its
+ *   row, last_row = the row of the other leg's innermost hit, n_hits of both legs, ndf = 2 * used - 5,
+ *   pad = {first leg, other leg, hits not used in the last pass (-1: failed), frame turns, 0}.
+ * TPCCA_ERR_ARGUMENT without a preceding tpcca_find_legs, for null / misaligned pointers or parameters out of range. */
+int tpcca_fit_legs(tpcca_handle* h, const tpcca_leg_fit_params* fp, void* stream, void* out_fits);
+
 /* Per-stage device times, averaged over the tpcca_track calls (at most the last 32) made since profiling
  * was switched on (CUDA events recorded on each call's stream; synchronises those events).  ms: host float[TPCCA_N_STAGES]. */
 enum { TPCCA_STAGE_GRID = 0, TPCCA_STAGE_NEIGHBOURS, TPCCA_STAGE_CLEAN_START, TPCCA_STAGE_TRACKLETS,

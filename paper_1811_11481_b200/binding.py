@@ -66,6 +66,11 @@ class LegParams(C.Structure):
 
 TAG_LOW_PT, TAG_EXTRA_LEG, TAG_HIGH_INCLINATION = 1, 2, 4
 
+
+class LegFitParams(C.Structure):
+    _fields_ = [("fit_rot_sinphi", C.c_float), ("fit_step_sinphi", C.c_float), ("fit_min_d", C.c_float),
+                ("fit_reject_cut", C.c_float), ("shared_err_scale", C.c_float), ("ring", C.c_int32)]
+
 _lib = None
 
 
@@ -93,6 +98,9 @@ def load():
         lib.tpcca_find_legs.restype = C.c_int
         lib.tpcca_find_legs.argtypes = [C.c_void_p, C.POINTER(LegParams), C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                         C.c_void_p, C.c_void_p]
+        lib.tpcca_default_leg_fit_params.argtypes = [C.POINTER(LegFitParams)]
+        lib.tpcca_fit_legs.restype = C.c_int
+        lib.tpcca_fit_legs.argtypes = [C.c_void_p, C.POINTER(LegFitParams), C.c_void_p, C.c_void_p]
         lib.tpcca_estimate_time.restype = C.c_int
         lib.tpcca_estimate_time.argtypes = [C.c_void_p, C.c_float, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p]
         lib.tpcca_wait.restype = C.c_int
@@ -115,6 +123,12 @@ def load():
         lib.tpcca_free.argtypes = [C.c_void_p]
         _lib = lib
     return _lib
+
+
+def default_leg_fit_params() -> LegFitParams:
+    p = LegFitParams()
+    load().tpcca_default_leg_fit_params(C.byref(p))
+    return p
 
 
 def default_leg_params() -> LegParams:
@@ -325,6 +339,25 @@ class Tracker:
                 self.out_leg_first[:nm].cpu().numpy().copy(), self.out_tags[:int(self.n)].cpu().numpy().copy(),
                 dict(n_links_outer=int(sm[0]), n_links_inner=int(sm[1]), n_tag_low_pt=int(sm[2]), n_tag_extra_leg=int(sm[3]),
                      n_tag_high_inclination=int(sm[4])))
+
+    # ---- one fit through both legs of every pair joined at a turning point (tpcca_fit_legs), after find_legs()
+    def fit_legs_enqueue(self, **params):
+        torch = self.torch
+        fp = default_leg_fit_params()
+        for k, v in params.items():
+            if not hasattr(fp, k):
+                raise TypeError(f"unknown leg fit parameter {k}")
+            setattr(fp, k, v)
+        if getattr(self, "out_leg_fits", None) is None:
+            self.out_leg_fits = torch.empty(16 + 128 * self.max_tracks, dtype=torch.uint8, device=self.device)
+        self._check(self.lib.tpcca_fit_legs(self.h, C.byref(fp), self._stream(), self.out_leg_fits.data_ptr()))
+
+    def fit_legs(self, **params) -> tuple:
+        """Returns (records TRACK_DTYPE[n_pairs], n_failed)."""
+        self.fit_legs_enqueue(**params)
+        h = self.out_leg_fits[:16].cpu().numpy().view(HEADER_DTYPE)[0]
+        n = int(h["n_tracks"])
+        return self.out_leg_fits[16:16 + 128 * n].cpu().numpy().view(TRACK_DTYPE).copy(), int(h["n_tracklets"])
 
     def estimate_time(self, vdrift: float = 2.58, z_max: float = 250.0, merged: bool = True):
         """tpcca_estimate_time: (n_tracks, 4) and, after merge(), (n_merged, 4) arrays of z_dca, z_shift, t0_us, dca_xy."""

@@ -32,6 +32,7 @@ struct tpcca_handle {
   // last tpcca_merge (for tpcca_estimate_time and tpcca_find_legs)
   void* last_merged;
   int32_t* last_track_merged;
+  int32_t* last_leg_partner;  // out_leg_partner of the last tpcca_find_legs (for tpcca_fit_legs)
   uint64_t seq_submit, seq_wait;
   // last call
   int64_t last_n;
@@ -269,6 +270,7 @@ static int track_impl(tpcca_handle* h, const tpcca_cluster* clusters, int64_t n,
   h->d.n = d.n; h->d.clusters = d.clusters; h->d.out_hdr = d.out_hdr; h->d.out_tracks = d.out_tracks; h->d.out_assign = out_assign;
   h->last_n = n;
   h->last_merged = nullptr;  // a new frame: the merged tracks of the previous one are gone
+  h->last_leg_partner = nullptr;
   const bool prof = h->profiling;
   cudaEvent_t* ev = h->ev[h->prof_calls % PROF_RING];
   // tpcca_set_debug(h, 1): synchronise after every stage and name the stage that faulted (debugging aid)
@@ -413,6 +415,7 @@ int tpcca_merge(tpcca_handle* h, const tpcca_merge_params* mp, void* stream, voi
   h->launches = L.count;
   h->last_merged = out_merged;
   h->last_track_merged = out_track_merged;
+  h->last_leg_partner = nullptr;
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) { set_err("merge launch failed: %s", cudaGetErrorString(e)); return TPCCA_ERR_CUDA; }
   return TPCCA_OK;
@@ -454,8 +457,42 @@ int tpcca_find_legs(tpcca_handle* h, const tpcca_leg_params* lp, void* stream, i
   Launch L{(cudaStream_t)stream, 0, nullptr};
   launch_legs(d, L);
   h->launches = L.count;
+  h->last_leg_partner = out_leg_partner;
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) { set_err("leg launch failed: %s", cudaGetErrorString(e)); return TPCCA_ERR_CUDA; }
+  return TPCCA_OK;
+}
+
+void tpcca_default_leg_fit_params(tpcca_leg_fit_params* p) {
+  if (!p) return;
+  memset(p, 0, sizeof(*p));
+  p->fit_rot_sinphi = 0.5f; p->fit_step_sinphi = 0.7f; p->fit_min_d = 0.3f; p->fit_reject_cut = 30.0f;
+  p->shared_err_scale = 2.0f; p->ring = 18;
+}
+
+int tpcca_fit_legs(tpcca_handle* h, const tpcca_leg_fit_params* fp, void* stream, void* out_fits) {
+  if (!h) { set_err("handle is null (not initialised)"); return TPCCA_ERR_NOT_INIT; }
+  if (!fp || !out_fits) { set_err("null fit parameters or output"); return TPCCA_ERR_ARGUMENT; }
+  if ((uintptr_t)out_fits & 15) { set_err("misaligned fit output"); return TPCCA_ERR_ARGUMENT; }
+  if (!h->d.out_hdr || !h->last_merged || !h->last_leg_partner) {
+    set_err("tpcca_fit_legs needs a tpcca_find_legs after the last tpcca_merge on this handle"); return TPCCA_ERR_ARGUMENT;
+  }
+  if (fp->ring < 0 || fp->ring > TPCCA_MAX_SECTORS || !(fp->fit_rot_sinphi > 0.0f) || !(fp->fit_rot_sinphi < 0.9f) ||
+      !(fp->fit_step_sinphi >= fp->fit_rot_sinphi) || !(fp->fit_step_sinphi < 0.95f) || !(fp->fit_min_d >= 0.0f) ||
+      !(fp->shared_err_scale > 0.0f)) {
+    set_err("fit parameters out of range"); return TPCCA_ERR_ARGUMENT;
+  }
+  Dev d = h->d;
+  d.FP = *fp;
+  d.merged_out = reinterpret_cast<tpcca_track_rec*>((char*)h->last_merged + sizeof(tpcca_out_header));
+  d.leg_partner_out = h->last_leg_partner;
+  d.fit_hdr = reinterpret_cast<tpcca_out_header*>(out_fits);
+  d.fit_out = reinterpret_cast<tpcca_track_rec*>((char*)out_fits + sizeof(tpcca_out_header));
+  Launch L{(cudaStream_t)stream, 0, nullptr};
+  launch_leg_fit(d, L);
+  h->launches = L.count;
+  const cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) { set_err("leg fit launch failed: %s", cudaGetErrorString(e)); return TPCCA_ERR_CUDA; }
   return TPCCA_OK;
 }
 

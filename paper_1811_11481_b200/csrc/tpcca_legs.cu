@@ -348,3 +348,216 @@ void launch_legs(const Dev& d, Launch& L) {
   k_leg_summary<<<1, 32, 0, L.st>>>(d);
   L.count++;
 }
+
+// ---------------------------------------------------------------- fit through both legs of a turn (O14)
+// One lane per pair.  The hits of a leg are the owned-hit lists of its sector segments (chain order, increasing row).
+#define FIT_MAX_SEGS 24
+struct FitSeg { int off, cnt, sector; };
+
+__device__ __forceinline__ int ring_add(int frame, int step, int ring) {
+  return (frame / ring) * ring + ((frame % ring) + step + ring) % ring;
+}
+
+// cos / sin of n sector angles by |n| rotations of (1, 0)
+__device__ __forceinline__ void sector_cs(int n, float ca, float sa, float& cb, float& sb) {
+  cb = 1.0f; sb = 0.0f;
+  const float ss = (n >= 0) ? sa : -sa;
+  for (int i = 0; i < abs(n); i++) {
+    const float u = fmaf(-sb, ss, cb * ca), v = fmaf(cb, ss, sb * ca);
+    cb = u; sb = v;
+  }
+}
+
+struct FitCtx {
+  KF k;
+  int frame, n_used, n_turn;
+  float z_ref;
+  bool ok;
+};
+
+// one hit of the trajectory (E3-E5 of DESIGN.md section 15)
+__device__ __forceinline__ void fit_hit(const Dev& d, FitCtx& c, float xh, float yh, float zh, int hsec, bool shared, float ca, float sa) {
+  if (!c.ok) return;
+  KF& k = c.k;
+  const int ring = d.FP.ring;
+  float cb = 1.0f, sb = 0.0f, X = 0.0f, Y = 0.0f;
+  bool reached = false;
+  for (int iter = 0; iter < 4 * ring + 1 && !reached; iter++) {
+    for (int step = 0; step < ring && fabsf(k.s) > d.FP.fit_rot_sinphi; step++) {
+      const int sgn = k.s > 0.0f ? 1 : -1;
+      if (!kf_rotate(k, ca, (float)sgn * sa, d.kq, 0.9999f)) { c.ok = false; return; }
+      c.frame = ring_add(c.frame, sgn, ring);
+      c.n_turn++;
+    }
+    int beta = 0;
+    if (ring > 0) {
+      beta = ((hsec - c.frame) % ring + ring) % ring;
+      if (2 * beta > ring) beta -= ring;
+    } else if (hsec != c.frame) { c.ok = false; return; }
+    sector_cs(beta, ca, sa, cb, sb);
+    X = fmaf(-yh, sb, xh * cb); Y = fmaf(xh, sb, yh * cb);
+    const float kk = k.q * d.kq;
+    const float s_at = fmaf(X - k.x, kk, k.s);
+    if (fabsf(s_at) <= d.FP.fit_step_sinphi) { reached = true; break; }
+    const float target = s_at > 0.0f ? d.FP.fit_step_sinphi : -d.FP.fit_step_sinphi;
+    const float dxp = (target - k.s) / kk;
+    if (!((dxp > 0.0f) == (X - k.x > 0.0f)) || dxp == 0.0f) { c.ok = false; return; }
+    if (!kf_transport(k, k.x + dxp, d.kq, d.P.max_sinphi)) { c.ok = false; return; }
+  }
+  if (!reached) { c.ok = false; return; }
+  if (!kf_transport(k, X, d.kq, d.P.max_sinphi)) { c.ok = false; return; }
+  const float cphi = sqrtf(fmaf(-k.s, k.s, 1.0f));
+  const float D = fmaf(sb, k.s / cphi, cb);
+  if (!(fabsf(D) >= d.FP.fit_min_d)) return;
+  const float ey = (shared ? d.P.sigma_y * d.FP.shared_err_scale : d.P.sigma_y) * D;
+  const float ez = shared ? d.P.sigma_z * d.FP.shared_err_scale : d.P.sigma_z;
+  const float vy = ey * ey, vz = ez * ez;
+  const float iy = 1.0f / (k.c00 + vy), iz = 1.0f / (k.c11 + vz);
+  const float dy = Y - k.y;
+  const float dz = (zh - c.z_ref) - k.z;
+  const float dist = fmaf(dz * dz, iz, (dy * dy) * iy);
+  if (!(dist <= d.FP.fit_reject_cut)) return;
+  kf_update(k, Y, zh - c.z_ref, vy, vz, iy);
+  c.n_used++;
+}
+
+__device__ __forceinline__ int leg_segments(const Dev& d, int m, FitSeg* segs) {
+  int n = 0;
+  for (int t = d.merged_out[m].pad[4]; t >= 0 && n < FIT_MAX_SEGS; t = d.m_next[t]) {
+    const int2 wl = d.w_list[d.track_w[t]];
+    segs[n].off = wl.x; segs[n].cnt = wl.y; segs[n].sector = d.out_tracks[t].sector;
+    n++;
+  }
+  return n;
+}
+
+__global__ void __launch_bounds__(64) k_leg_fit_flag(Dev d) {
+  const int a = blockIdx.x * blockDim.x + threadIdx.x;
+  if (a < d.cnt->n_merged) d.m_scan[a] = (d.leg_partner_out[a] > a) ? 1 : 0;
+}
+
+__global__ void __launch_bounds__(64) k_leg_fit(Dev d) {
+  const int a = blockIdx.x * blockDim.x + threadIdx.x;
+  const int nm = d.cnt->n_merged;
+  if (a >= nm) return;
+  const int b = d.leg_partner_out[a];
+  if (b <= a) return;
+  const int slot = d.m_scan[a];
+  const float za = fabsf(d.merged_out[a].z), zb = fabsf(d.merged_out[b].z);
+  const bool a_first = (za < zb) || (za == zb);
+  const int f = a_first ? a : b, g = a_first ? b : a;
+  FitSeg sf[FIT_MAX_SEGS], sg[FIT_MAX_SEGS];
+  const int nf = leg_segments(d, f, sf), ng = leg_segments(d, g, sg);
+  const Rot R = sector_rotation(d.tan_half_angle);
+  int n_total = 0;
+  for (int i = 0; i < nf; i++) n_total += sf[i].cnt;
+  for (int i = 0; i < ng; i++) n_total += sg[i].cnt;
+  FitCtx c;
+  c.ok = true; c.n_used = 0; c.n_turn = 0;
+  // start: the last hit of the trajectory = the innermost hit of g's innermost segment, direction towards the hit before it
+  const int jN = sg[0].off, jM = sg[0].off + 1;
+  const float2 pN = d.th_yz[jN], pM = d.th_yz[jM];
+  const float xN = d.row_x[d.th_row[jN]], xM = d.row_x[d.th_row[jM]];
+  c.frame = sg[0].sector;
+  c.z_ref = pN.y;
+  {
+    const float dx = xM - xN, dy = pM.x - pN.x, dz = pM.y - pN.y;
+    const float ds = sqrtf(fmaf(dx, dx, dy * dy));
+    c.k.x = xN;
+    c.k.y = pN.x; c.k.z = 0.0f; c.k.s = dy / ds; c.k.t = dz / ds; c.k.q = d.merged_out[g].qpt;
+    c.k.chi2 = 0.0f;
+  }
+  for (int pass = 0; pass < 3; pass++) {
+    kf_reset_cov(c.k, d.P.cov0);
+    c.n_used = 0;
+    if (pass == 1) {  // forward along the trajectory: f inner -> outer, then g outer -> inner
+      for (int si = 0; si < nf; si++)
+        for (int i = 0; i < sf[si].cnt; i++) {
+          const int j = sf[si].off + i;
+          const float2 p = d.th_yz[j];
+          fit_hit(d, c, d.row_x[d.th_row[j]], p.x, p.y, sf[si].sector, d.th_shared[j] != 0, R.ca, R.sa);
+        }
+      for (int si = ng - 1; si >= 0; si--)
+        for (int i = sg[si].cnt - 1; i >= 0; i--) {
+          const int j = sg[si].off + i;
+          const float2 p = d.th_yz[j];
+          fit_hit(d, c, d.row_x[d.th_row[j]], p.x, p.y, sg[si].sector, d.th_shared[j] != 0, R.ca, R.sa);
+        }
+    } else {          // backward: g inner -> outer, then f outer -> inner
+      for (int si = 0; si < ng; si++)
+        for (int i = 0; i < sg[si].cnt; i++) {
+          const int j = sg[si].off + i;
+          const float2 p = d.th_yz[j];
+          fit_hit(d, c, d.row_x[d.th_row[j]], p.x, p.y, sg[si].sector, d.th_shared[j] != 0, R.ca, R.sa);
+        }
+      for (int si = nf - 1; si >= 0; si--)
+        for (int i = sf[si].cnt - 1; i >= 0; i--) {
+          const int j = sf[si].off + i;
+          const float2 p = d.th_yz[j];
+          fit_hit(d, c, d.row_x[d.th_row[j]], p.x, p.y, sf[si].sector, d.th_shared[j] != 0, R.ca, R.sa);
+        }
+    }
+  }
+  // report in the first leg's innermost sector frame, direction outward (E7)
+  KF& k = c.k;
+  const int ring = d.FP.ring;
+  if (c.ok && ring > 0 && (ring & 1) == 0) {
+    k.x = -k.x; k.y = -k.y; k.t = -k.t; k.q = -k.q;
+    // sign pattern (-, +, +, -, -): an element changes sign iff exactly one of its indices is in {0, 3, 4}
+    k.c10 = -k.c10; k.c20 = -k.c20; k.c31 = -k.c31; k.c32 = -k.c32; k.c41 = -k.c41; k.c42 = -k.c42;
+    c.frame = ring_add(c.frame, ring / 2, ring);
+    const int target = d.merged_out[f].sector;
+    int dsec = ((target - c.frame) % ring + ring) % ring;
+    if (2 * dsec > ring) dsec -= ring;
+    const int sgn = dsec >= 0 ? 1 : -1;
+    for (int i = 0; i < abs(dsec) && c.ok; i++) {
+      c.ok = kf_rotate(k, R.ca, (float)sgn * R.sa, d.kq, 0.9999f);
+      c.frame = ring_add(c.frame, sgn, ring);
+    }
+    if (c.ok) c.ok = kf_transport(k, d.row_x[d.th_row[sf[0].off]], d.kq, 0.9999f);
+  }
+  tpcca_track_rec o;
+  memset(&o, 0, sizeof(o));
+  o.sector = c.frame; o.first_row = d.th_row[sf[0].off]; o.last_row = d.th_row[sg[0].off]; o.n_hits = n_total;
+  if (c.ok) {
+    o.x = k.x; o.y = k.y; o.z = k.z + c.z_ref; o.sinphi = k.s; o.dzds = k.t; o.qpt = k.q;
+    o.cov[0] = k.c00; o.cov[1] = k.c10; o.cov[2] = k.c11; o.cov[3] = k.c20; o.cov[4] = k.c21; o.cov[5] = k.c22;
+    o.cov[6] = k.c30; o.cov[7] = k.c31; o.cov[8] = k.c32; o.cov[9] = k.c33; o.cov[10] = k.c40; o.cov[11] = k.c41;
+    o.cov[12] = k.c42; o.cov[13] = k.c43; o.cov[14] = k.c44;
+    o.chi2 = k.chi2;
+    o.ndf = 2 * c.n_used - 5;
+  } else {
+    o.ndf = -1;
+    atomicAdd(&d.leg_summary[5], 1);
+  }
+  o.pad[0] = f; o.pad[1] = g; o.pad[2] = c.ok ? n_total - c.n_used : -1; o.pad[3] = c.n_turn; o.pad[4] = 0;
+  float4* dst = reinterpret_cast<float4*>(&d.fit_out[slot]);
+  const float4* src = reinterpret_cast<const float4*>(&o);
+#pragma unroll
+  for (int i = 0; i < 8; i++) dst[i] = src[i];
+}
+
+// header: pairs = total of the flag scan (0 without tracks), failed fits counted in leg_summary[5]
+__global__ void k_leg_fit_begin(Dev d) { d.leg_summary[5] = 0; }
+__global__ void k_leg_fit_header(Dev d, int have_scan) {
+  tpcca_out_header hd;
+  hd.n_tracks = have_scan ? d.m_scan[d.cnt->n_merged] : 0;
+  hd.n_tracklets = d.leg_summary[5]; hd.n_start_hits = 0; hd.status = d.cnt->status;
+  *d.fit_hdr = hd;
+}
+
+void launch_leg_fit(const Dev& d, Launch& L) {
+  const int K = d.max_tracks;
+  k_leg_fit_begin<<<1, 1, 0, L.st>>>(d);
+  L.count++;
+  const bool work = d.n > 0 && K > 0;
+  if (work) {
+    k_leg_fit_flag<<<(K + 63) / 64, 64, 0, L.st>>>(d);
+    L.count++;
+    launch_scan_i32(d.m_scan, &d.cnt->n_merged, K, d.scan_tmp, L);
+    k_leg_fit<<<(K + 63) / 64, 64, 0, L.st>>>(d);
+    L.count++;
+  }
+  k_leg_fit_header<<<1, 1, 0, L.st>>>(d, work ? 1 : 0);
+  L.count++;
+}

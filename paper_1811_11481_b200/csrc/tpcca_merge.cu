@@ -7,53 +7,6 @@
 
 #define M_NONE 0xffffffffffffffffull
 
-struct Rot {  // cos and sin of the sector angle from tan(10 deg) by the double-angle formulas
-  float ca, sa;
-};
-__device__ __forceinline__ Rot sector_rotation(float th) {
-  const float den = fmaf(th, th, 1.0f);
-  Rot r;
-  r.ca = fmaf(-th, th, 1.0f) / den;
-  r.sa = (2.0f * th) / den;
-  return r;
-}
-
-// Frame change by sgn * (sector angle): ss = sgn * sin.  false: |sin(phi)| leaves the allowed range (state unchanged).
-__device__ __forceinline__ bool kf_rotate(KF& k, float ca, float ss, float kq, float max_sinphi) {
-  const float s = k.s;
-  if (!(fabsf(s) <= max_sinphi)) return false;
-  const float cphi = sqrtf(fmaf(-s, s, 1.0f));
-  const float s1 = fmaf(s, ca, -(cphi * ss));
-  if (!(fabsf(s1) <= max_sinphi)) return false;
-  const float c1 = sqrtf(fmaf(-s1, s1, 1.0f));
-  const float rr = c1 / cphi;
-  const float ry = cphi / c1;
-  const float rz = -((k.t * ss) / c1);
-  const float rs = -((k.q * kq) * ss);
-  const float x = k.x, y = k.y;
-  k.x = fmaf(y, ss, x * ca);
-  k.y = fmaf(y, ca, -(x * ss));
-  k.s = s1;
-  // M = F C with F = diag(ry, 1, rr, 1, 1) + rz at (1,0) + rs at (2,0); C' = M F^T
-  const float m00 = ry * k.c00;
-  const float m10 = fmaf(rz, k.c00, k.c10), m11 = fmaf(rz, k.c10, k.c11);
-  const float m20 = fmaf(rs, k.c00, rr * k.c20), m21 = fmaf(rs, k.c10, rr * k.c21), m22 = fmaf(rs, k.c20, rr * k.c22);
-  const float m30 = k.c30, m31 = k.c31, m32 = k.c32;
-  const float m40 = k.c40, m41 = k.c41, m42 = k.c42;
-  k.c00 = m00 * ry;
-  k.c10 = m10 * ry; k.c11 = fmaf(rz, m10, m11);
-  k.c20 = m20 * ry; k.c21 = fmaf(rz, m20, m21); k.c22 = fmaf(rs, m20, m22 * rr);
-  k.c30 = m30 * ry; k.c31 = fmaf(rz, m30, m31); k.c32 = fmaf(rs, m30, m32 * rr);
-  k.c40 = m40 * ry; k.c41 = fmaf(rz, m40, m41); k.c42 = fmaf(rs, m40, m42 * rr);
-  return true;
-}
-
-__device__ __forceinline__ int ring_neighbour(int sector, int side, int ring) {
-  if (ring <= 0) return -1;
-  const int base = (sector / ring) * ring, l = sector - base;
-  return base + (l + side + ring) % ring;
-}
-
 // ---------------------------------------------------------------- (m0) reset, candidate buckets, shared flags of the lists
 // The inner ends are bucketed by (sector, first_row) with a counting sort (histogram -> scan -> scatter), so that the row
 // window of DESIGN.md B2 is ONE contiguous range of the sorted order.  Scratch: the per-slice arrays of the grid and
