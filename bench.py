@@ -290,6 +290,16 @@ def run_gpu(args):
     l1.record(stream)
     torch.cuda.synchronize()
     legs_ms = l0.elapsed_time(l1) / args.steps
+    # ---- one fit through both legs of every pair joined at a turning point (tpcca_fit_legs), timed on its own
+    leg_fits, leg_fit_failed = trk.fit_legs()
+    torch.cuda.synchronize()
+    k0, k1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    k0.record(stream)
+    for _ in range(args.steps):
+        trk.fit_legs_enqueue()
+    k1.record(stream)
+    torch.cuda.synchronize()
+    leg_fit_ms = k0.elapsed_time(k1) / args.steps
 
     # ---- end to end through the library's host calls (pinned host buffers, H2D + D2H inside the timed region)
     hc = torch.from_numpy(fr.clusters.view(np.uint8).reshape(-1)).pin_memory()
@@ -371,8 +381,18 @@ def run_gpu(args):
                   "per_particle": {"sector_tracks": {k: round(float(v), 5) for k, v in q_sec.items()},
                                    "merged_tracks": {k: round(float(v), 5) for k, v in q_mrg.items()},
                                    "merged_tracks_legs_joined": {k: round(float(v), 5) for k, v in q_leg.items()}}}
+    sigma_ratio = None
+    if len(leg_fits):
+        okf = leg_fits["pad"][:, 2] >= 0
+        c_fit = leg_fits["cov"][:, 14][okf]
+        c_leg = trk.merged()["cov"][:, 14][leg_fits["pad"][:, 0][okf]]
+        good = (c_fit > 0) & (c_leg > 0)
+        if good.any():
+            sigma_ratio = round(float(np.median(np.sqrt(c_fit[good] / c_leg[good]))), 4)
     legs_info = {"ms": legs_ms, "api": "tpcca_find_legs (after tpcca_merge, not part of `value`)", **leg_sum,
-                 "tagged_fraction_of_clusters": round(float((tags > 0).mean()), 5) if n else 0.0}
+                 "tagged_fraction_of_clusters": round(float((tags > 0).mean()), 5) if n else 0.0,
+                 "pair_fit": {"ms": leg_fit_ms, "api": "tpcca_fit_legs", "pairs": int(len(leg_fits)), "failed": int(leg_fit_failed),
+                              "median_sigma_qpt_ratio_to_first_leg": sigma_ratio}}
     # ---- roofline (algorithmic bytes of DESIGN.md section 7 x live device counters)
     peak, peak_src = peaks()
     T = hd["n_start_hits"]

@@ -24,7 +24,8 @@ def test_exports_every_declared_symbol(lib):
     names = set(re.findall(r"\b(tpcca_[a-z_]+)\s*\(", hdr))
     assert {"tpcca_init", "tpcca_track", "tpcca_free", "tpcca_track_host", "tpcca_get_intermediate", "tpcca_merge",
             "tpcca_track_host_async", "tpcca_wait", "tpcca_default_merge_params", "tpcca_get_kernel_ms",
-            "tpcca_estimate_time", "tpcca_find_legs", "tpcca_default_leg_params", "tpcca_debug_workspace_layout"} <= names
+            "tpcca_estimate_time", "tpcca_find_legs", "tpcca_default_leg_params", "tpcca_debug_workspace_layout",
+            "tpcca_fit_legs", "tpcca_default_leg_fit_params"} <= names
     for n in names:
         assert hasattr(lib, n), n
 

@@ -409,7 +409,7 @@ def _gaps_untouched(t, poison):
 @pytest.mark.parametrize("case", ["config2", "dense_noise", "tight_capacity", "loopers"])
 def test_no_kernel_writes_outside_its_arrays(row_x, case):
     """Bounds check of our own (compute-sanitizer is closed on the GPU pool): the workspace is filled with a pattern, the
-    whole chain track -> merge -> find_legs -> estimate_time runs, and the padding behind every one of the carved arrays,
+    whole chain track -> merge -> find_legs -> fit_legs -> estimate_time runs, and the padding behind every one of the carved arrays,
     the guard bands around the caller's output buffers and the unused tail of the outputs must be untouched."""
     import torch
     poison = 0xA5
@@ -430,6 +430,7 @@ def test_no_kernel_writes_outside_its_arrays(row_x, case):
     for name, nbytes in (("tracks", 16 + 128 * t.max_tracks), ("assign", 4 * fr.n), ("merged", 16 + 128 * t.max_tracks),
                          ("track_merged", 4 * max(1, t.max_tracks)), ("partner", 4 * max(1, t.max_tracks)),
                          ("partner_in", 4 * max(1, t.max_tracks)), ("first", max(1, t.max_tracks)), ("tags", fr.n), ("summary", 32),
+                         ("leg_fits", 16 + 128 * t.max_tracks),
                          ("time_s", 16 * max(1, t.max_tracks)), ("time_m", 16 * max(1, t.max_tracks))):
         full = torch.full((nbytes + 2 * G,), poison, dtype=torch.uint8, device="cuda")
         bufs[name] = (full, full[G:G + nbytes])
@@ -443,6 +444,8 @@ def test_no_kernel_writes_outside_its_arrays(row_x, case):
         assert t.lib.tpcca_merge(t.h, C.byref(mp), t._stream(), p("merged"), p("track_merged")) == 0
         assert t.lib.tpcca_find_legs(t.h, C.byref(lp), t._stream(), p("partner"), p("partner_in"), p("first"), p("tags"),
                                      p("summary")) == 0
+        fp = B.default_leg_fit_params()
+        assert t.lib.tpcca_fit_legs(t.h, C.byref(fp), t._stream(), p("leg_fits")) == 0
         assert t.lib.tpcca_estimate_time(t.h, 2.58, 250.0, t._stream(), p("time_s"), p("time_m")) == 0
     torch.cuda.synchronize()
     hd = bufs["tracks"][1][:16].cpu().numpy().view(B.HEADER_DTYPE)[0]
