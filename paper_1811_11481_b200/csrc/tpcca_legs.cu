@@ -351,7 +351,7 @@ void launch_legs(const Dev& d, Launch& L) {
 
 // ---------------------------------------------------------------- fit through both legs of a turn (O14)
 // One lane per pair.  The hits of a leg are the owned-hit lists of its sector segments (chain order, increasing row).
-#define FIT_MAX_SEGS 24
+#define FIT_MAX_SEGS 24  // sector segments per leg (as MERGE_MAX_SEGS: a merged chain grows in row, >= 10 rows per segment of 152)
 struct FitSeg { int off, cnt, sector; };
 
 __device__ __forceinline__ int ring_add(int frame, int step, int ring) {
