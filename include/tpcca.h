@@ -297,6 +297,39 @@ int tpcca_get_stats(tpcca_handle* h, int64_t* stats, void* stream);
 /* Kernels launched by the last tpcca_track / tpcca_track_host on this handle. */
 int tpcca_last_launch_count(tpcca_handle* h);
 
+/* ---- Link cleaner and start-hit finder that allocates nothing and needs no workspace (steps (c) and (d): PAPER.md:49, a
+ * link between neighbouring rows is kept only if both ends agree, and the hits where a chain of links begins are collected;
+ * DESIGN.md O3 / O4).
+ *
+ * For whom: callers that cannot obtain device memory at run time and therefore have no workspace to pass to tpcca_init --
+ * a component inside a process whose framework took all GPU memory for its own allocator at start-up, a monitoring task
+ * inspecting the links of a frame it does not own, or code in a real-time loop where cudaMalloc / cudaFree would
+ * synchronise the device under the frames being tracked on other streams.  This call makes no cudaMalloc, cudaFree or
+ * other allocating call: the scratch of its compaction (one counter and one int32 per 1024 clusters) is a fixed array
+ * built into the library image, 131,328 bytes of device memory that every GPU loading the library holds until the process
+ * exits.  Hence the hard limit n <= TPCCA_STATIC_MAX_CLUSTERS; a larger n returns TPCCA_ERR_ARGUMENT (text in
+ * tpcca_last_error) and nothing is written.
+ *
+ * link_up_raw / link_down_raw: device, int32[n], links before cleaning in any index space of [0, n), -1 (or any value
+ *   outside [0, n)) = no link -- e.g. TPCCA_LINK_UP_RAW / TPCCA_LINK_DOWN_RAW of tpcca_get_intermediate.
+ * out_link_up / out_link_down: device, int32[n]: the link where the partner points back, else -1.  Must not overlap the
+ *   inputs or each other.
+ * out_start_hits: device, int32[n] capacity: the clusters with an up link and no down link after cleaning, in ASCENDING
+ *   index (tpcca_track orders them by sector, row, z, y instead: same set, different order).
+ * out_n_start: device, one int32: how many.   All pointers 4-byte aligned; the caller owns every buffer.
+ * stream: a cudaStream_t of the CURRENT device; the work is enqueued and the call returns without waiting.
+ *
+ * Sharing: there is ONE scratch array per GPU and every call uses it, whatever the stream or thread.  Two calls on the same
+ * GPU that could run at the same time race on it and give wrong start hits: keep them on one stream, or order them with
+ * events.  Calls on different GPUs are independent.  The array keeps the previous call's contents; the one word that must
+ * be zero is cleared on `stream` at the start of every call.
+ * First call on a device: it looks up the device address of the array (cudaGetSymbolAddress, with that device current) and
+ * remembers it; this may load the CUDA module.  Make that first call during set-up, before any stream capture is begun.
+ * n == 0 is valid (*out_n_start = 0).  Returns 0, TPCCA_ERR_ARGUMENT or TPCCA_ERR_CUDA. */
+#define TPCCA_STATIC_MAX_CLUSTERS 33554432LL /* 2^25 */
+int tpcca_clean_links_static(const int32_t* link_up_raw, const int32_t* link_down_raw, int64_t n, void* stream,
+                             int32_t* out_link_up, int32_t* out_link_down, int32_t* out_start_hits, int32_t* out_n_start);
+
 const char* tpcca_last_error(void);
 void tpcca_free(tpcca_handle* h);
 

@@ -119,6 +119,9 @@ def load():
         lib.tpcca_get_stats.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
         lib.tpcca_last_launch_count.restype = C.c_int
         lib.tpcca_last_launch_count.argtypes = [C.c_void_p]
+        lib.tpcca_clean_links_static.restype = C.c_int
+        lib.tpcca_clean_links_static.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p,
+                                                 C.c_void_p, C.c_void_p]
         lib.tpcca_last_error.restype = C.c_char_p
         lib.tpcca_free.argtypes = [C.c_void_p]
         _lib = lib
@@ -151,6 +154,26 @@ def default_params() -> Params:
 
 class TpccaError(RuntimeError):
     pass
+
+
+STATIC_MAX_CLUSTERS = 1 << 25  # TPCCA_STATIC_MAX_CLUSTERS of include/tpcca.h
+
+
+def clean_links_static(link_up_raw, link_down_raw, n: int, out_link_up, out_link_down, out_start_hits, out_n_start,
+                       stream: int | None = None) -> None:
+    """tpcca_clean_links_static: mutual links and chain starts from raw links, for callers that cannot allocate device
+    memory (no workspace, no cudaMalloc inside: the scratch is a fixed array in the library, so n <= STATIC_MAX_CLUSTERS and
+    calls that overlap on one GPU race -- see include/tpcca.h).  All arguments are CUDA int32 tensors the caller made
+    (marshalling only); enqueued on `stream` (default: torch's current stream), returns without waiting."""
+    import torch
+    lib = load()
+    if stream is None:
+        stream = torch.cuda.current_stream().cuda_stream
+    ptr = lambda t: t.data_ptr() if t is not None and t.numel() else None
+    rc = lib.tpcca_clean_links_static(ptr(link_up_raw), ptr(link_down_raw), int(n), stream, ptr(out_link_up),
+                                      ptr(out_link_down), ptr(out_start_hits), ptr(out_n_start))
+    if rc != 0:
+        raise TpccaError(f"tpcca error {rc}: {lib.tpcca_last_error().decode()}")
 
 
 class Tracker:

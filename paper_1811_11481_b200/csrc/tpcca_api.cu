@@ -12,6 +12,9 @@
 static thread_local char g_err[512] = "";
 static void set_err(const char* fmt, const char* a = "", long long b = 0) { snprintf(g_err, sizeof(g_err), fmt, a, b); }
 
+// for entry points that live in other translation units (tpcca_static.cu)
+void tpcca_internal_set_err(const char* msg) { snprintf(g_err, sizeof(g_err), "%s", msg ? msg : ""); }
+
 #define PROF_RING 32
 #define MAX_LAYOUT 128
 struct tpcca_handle {
