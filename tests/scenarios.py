@@ -182,3 +182,43 @@ def helix_in_two_sectors(row_x, sector=3, side=+1, par=None, z_shift_b=0.0, drop
     cl = np.concatenate([parts[s] for s in sorted(parts)])
     fr = synth.Frame(cl, so, np.full(len(cl), -1, np.int32), np.zeros((0, 8)), n_sectors, "two_sector_helix")
     return fr, dict(rows_a=rows_a, rows_b=rows_b, y_a=ya, z_a=za, s_a=sa, sector_b=sector_b, par=par)
+
+
+# ---------------------------------------------------------------- round-3 scenarios (pins of tests/test_oracle_pins_r3.py)
+def displaced_hit_helix_z(row_x, row=120, dz=0.45):
+    """As displaced_hit_helix, but the hit is moved along z: its keep / reject distance on the inward pass is
+    dz^2 / (var(z~) predicted + sigma_z^2) -- the z variance of the filter, not a y term."""
+    rows, y, z = one_helix(row_x)
+    z = z.copy()
+    z[row] += dz
+    return mk(rows, y, z, row_x)
+
+
+def lone_row_helix(row_x, row=100, dy=0.0, dz=0.0, duplicate=False, dup_positions=None):
+    """A helix whose row `row` cannot be linked (two rows removed on either side of it: DESIGN.md A5 allows one skipped row)
+    and is therefore reached by the pick-up search only, from the chain below (E2) and again from the chain above (E3).
+    The cluster of that row is moved by (dy, dz); with `duplicate` it exists twice, bit for bit, at the array positions
+    `dup_positions` (default: appended).  Returns (clusters, positions of the lone row's cluster(s))."""
+    R = len(row_x)
+    rows = np.r_[np.arange(0, row - 2), [row], np.arange(row + 3, R)]
+    rows, y, z = one_helix(row_x, rows)
+    y, z = y.copy(), z.copy()
+    i = int(np.flatnonzero(rows == row)[0])
+    y[i] += dy
+    z[i] += dz
+    cl = mk(rows, y, z, row_x)
+    if not duplicate:
+        return cl, [i]
+    lone = cl[i:i + 1]
+    rest = np.delete(cl, i)
+    p, q = dup_positions if dup_positions is not None else (len(rest), len(rest) + 1)
+    out = np.insert(rest, min(p, len(rest)), lone)
+    out = np.insert(out, min(q, len(out)), lone)
+    pos = [int(k) for k in np.flatnonzero(out["row"] == row)]
+    return out, pos
+
+
+def window_triplet(row_x, dy=0.0, dz=0.0, row=50):
+    """Three clusters on a straight line through rows row-1, row, row+1 (cost 0), the outer two displaced by -/+ (dy, dz)."""
+    f = np.float32
+    return mk(np.array([row - 1, row, row + 1]), np.array([-dy, 0.0, dy], f), np.array([10.0 - dz, 10.0, 10.0 + dz], f), row_x)
