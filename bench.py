@@ -7,7 +7,8 @@ library's pipelined host call (tpcca_track_host_async / tpcca_wait: pinned host 
 the timed region, two frames in flight in ONE workspace).  `--gpus N` starts N ranks itself (torchrun
 re-exec) unless it already runs under torchrun; `--shard frames` (default, weak scaling: one frame per
 rank) or `--shard sectors` (one frame split into contiguous sector ranges, strong
-scaling).  `--config k` times another BASELINE.json config (parity-test cases; the bench line is config 5).
+scaling; tpcca_merge and the leg calls then run per rank WITHOUT an exchange of boundary segments, so for N > 2 the
+tracks crossing a rank boundary stay unmerged -- `config.merge.cuts_inside_a_side` counts those boundaries).  `--config k` times another BASELINE.json config (parity-test cases; the bench line is config 5).
 See DESIGN.md "Measurement".  `--impl reference` times the CPU oracle (the only reference this tier has).
 """
 from __future__ import annotations
@@ -123,6 +124,24 @@ class ClockSampler:
                 "source": "nvml" if self._nvml is not None else "nvidia-smi"}
 
 
+def host_cpu() -> dict:
+    """CPU model and core count of the box the oracle is timed on; the oracle itself is single-threaded."""
+    model = "unknown"
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.startswith("model name"):
+                    model = line.split(":", 1)[1].strip()
+                    break
+    except OSError:
+        pass
+    try:
+        usable = len(os.sched_getaffinity(0))
+    except AttributeError:
+        usable = os.cpu_count() or 0
+    return {"cpu_model": model, "host_cores": os.cpu_count() or 0, "host_cores_usable": usable}
+
+
 def oracle_timed(cfg: int, scale: float, seed: int, steps: int, warmup: int, fr=None):
     """The CPU oracle as it stands on `fr`, or on a bounded sample of the workload (config `cfg` at `scale`)."""
     import oracle
@@ -164,8 +183,12 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": WORKLOADS[args.config] + " (bounded sample)", "clusters_per_step": n},
-            "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "config": {"workload": WORKLOADS[args.config] + " (bounded sample)", "clusters_per_step": n,
+                       "sample_scale": scale,
+                       "note": ("a bounded sample of the workload, not the full frame the CUDA arm times: the ratio of the two "
+                                "arms compares clusters/s across different frame sizes" if scale != 1.0 else
+                                "the same frame the CUDA arm times")},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample, **host_cpu()},
             "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
     return 0
@@ -378,6 +401,8 @@ def run_gpu(args):
     al = np.where(am >= 0, leg_root[np.maximum(am, 0)], -1) if len(leg_partner) else am
     q_leg = score.score(al, fr.truth, one, mh["n_merged"])
     merge_info = {"ms": merge_ms, "api": "tpcca_merge (after the timed path, not part of `value`)", **mh,
+                  "cuts_inside_a_side": (distributed.cuts_inside_a_side(36, world, 18)
+                                         if args.shard == "sectors" else 0),
                   "per_particle": {"sector_tracks": {k: round(float(v), 5) for k, v in q_sec.items()},
                                    "merged_tracks": {k: round(float(v), 5) for k, v in q_mrg.items()},
                                    "merged_tracks_legs_joined": {k: round(float(v), 5) for k, v in q_leg.items()}}}
@@ -450,7 +475,7 @@ def run_gpu(args):
     cpu_baseline = None
     if world == 1 and not args.no_cpu_baseline:
         cv, ct, cn, ores = oracle_timed(cfg, 1.0, cfg, 1, 0, fr=fr)
-        cpu_baseline = {"value": cv, "unit": UNIT, "cores": 1, "kind": "oracle",
+        cpu_baseline = {"value": cv, "unit": UNIT, "cores": 1, "kind": "oracle", **host_cpu(),
                         "sample": f"one pass over the same config-{cfg} frame, {cn} clusters, {ct:.1f} s",
                         "quality": quality(ores.assignment, len(ores.tracks), fr),
                         "assignment_equals_cuda_path": bool(np.array_equal(ores.assignment, gpu_assignment))}

@@ -15,6 +15,11 @@
  * memory: all scratch lives in the caller-provided workspace.  All entry points return 0 on success
  * or a negative tpcca_status; tpcca_last_error() describes the last failure of the calling thread.
  * There is no CPU fallback: without a CUDA device tpcca_init fails.
+ *
+ * Streams: all calls on one handle share the handle's workspace, so the library runs them on the GPU in the order they were
+ * made even if each is given a different stream (every enqueueing call makes its stream wait for an event recorded at the end
+ * of the previous call on the handle; free when the stream is the same).  Calls on one handle from several host threads at
+ * once are not supported; different handles are independent.
  */
 #ifndef TPCCA_H
 #define TPCCA_H
@@ -40,7 +45,10 @@ enum {
   TPCCA_STAT_TRACKLET_OVERFLOW = 1, /* more start hits than max_tracklets: highest ids dropped */
   TPCCA_STAT_TRACK_OVERFLOW = 2,    /* more tracks than max_tracks: highest ids dropped */
   TPCCA_STAT_BAD_CLUSTER = 4,       /* a cluster with row outside [0,n_rows) or a non-finite y / z was ignored */
-  TPCCA_STAT_BIN_OVERFLOW = 8       /* internal grid capacity hit (never with the default sizing) */
+  TPCCA_STAT_BIN_OVERFLOW = 8,      /* internal grid capacity hit (never with the default sizing) */
+  TPCCA_STAT_CHAIN_TRUNCATED = 16   /* tpcca_merge / tpcca_fit_legs: a chain of more than 24 sector segments was fitted over its
+                                       first 24 only (impossible with the default cuts: every segment gains >= 8 rows of 152);
+                                       reported in the header of that call and of the later calls on the same frame */
 };
 
 /* Geometry (152 pad rows; 36 trapezoidal sectors). */
@@ -170,7 +178,8 @@ typedef struct {
   int32_t merge_row_back, merge_row_fwd; /* first_row(B) - last_row(A) in [-back, fwd] */
   float fit_reject_cut;        /* 2-dof predicted distance above which a hit is left out of a pass of the final fit */
   float shared_err_scale;      /* sigma_y, sigma_z multiplier of shared clusters in the final fit */
-  int32_t ring;                /* sectors per z side closing the ring (18); 0: no neighbours, nothing merges */
+  int32_t ring;                /* sectors per z side closing the ring (18); 0: no neighbours, nothing merges; 1 and values
+                                  above 64 are refused (a sector would be its own neighbour) */
 } tpcca_merge_params;
 void tpcca_default_merge_params(tpcca_merge_params* p);
 
@@ -222,7 +231,7 @@ typedef struct {
   float tag_qpt_low;          /* TAG_LOW_PT: |q/pT| of the merged track above this (20 = 50 MeV/c) */
   float tag_qpt_leg;          /* TAG_EXTRA_LEG: additional leg with |q/pT| above this (5 = 200 MeV/c) */
   float tag_sinphi;           /* TAG_HIGH_INCLINATION: local |sin(phi)| above this */
-  int32_t ring;               /* sectors per z side closing the ring (18); 0: partners in the same sector only */
+  int32_t ring;               /* sectors per z side closing the ring (18); 0: partners in the same sector only; 1 and > 64 refused */
 } tpcca_leg_params;
 void tpcca_default_leg_params(tpcca_leg_params* p);
 enum { TPCCA_TAG_LOW_PT = 1, TPCCA_TAG_EXTRA_LEG = 2, TPCCA_TAG_HIGH_INCLINATION = 4 };

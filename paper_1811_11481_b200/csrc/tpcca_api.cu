@@ -37,6 +37,12 @@ struct tpcca_handle {
   int32_t* last_track_merged;
   int32_t* last_leg_partner;  // out_leg_partner of the last tpcca_find_legs (for tpcca_fit_legs)
   uint64_t seq_submit, seq_wait;
+  // Everything above lives in ONE workspace, so the calls on a handle must run on the GPU in the order they were made, also
+  // when the caller passes a different stream each time: every entry point that enqueues work first makes its stream wait
+  // for ev_last (recorded at the end of the previous one), unless it is the same stream anyway.
+  cudaEvent_t ev_last;
+  cudaStream_t last_stream;
+  bool have_last;
   // last call
   int64_t last_n;
   int launches;
@@ -48,6 +54,18 @@ struct tpcca_handle {
 };
 
 static size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
+
+// Stream order across calls on one handle (see tpcca_handle::ev_last).
+static bool order_after_last(tpcca_handle* h, cudaStream_t st) {
+  if (!h->have_last || st == h->last_stream) return true;
+  const cudaError_t e = cudaStreamWaitEvent(st, h->ev_last, 0);
+  if (e != cudaSuccess) { set_err("cudaStreamWaitEvent failed: %s", cudaGetErrorString(e)); cudaGetLastError(); return false; }
+  return true;
+}
+static void mark_last(tpcca_handle* h, cudaStream_t st) {
+  if (cudaEventRecord(h->ev_last, st) == cudaSuccess) { h->last_stream = st; h->have_last = true; }
+  else cudaGetLastError();
+}
 
 // One pass computes the layout; with base != NULL it also assigns the pointers.
 static size_t carve(tpcca_handle* h, const tpcca_geometry* g, const tpcca_params* p, char* base) {
@@ -240,7 +258,8 @@ tpcca_handle* tpcca_init(const tpcca_geometry* g, float bz_tesla, const tpcca_pa
         tpcca_free(h);  // destroys the events created so far
         return nullptr;
       }
-  bool ok = cudaStreamCreateWithFlags(&h->st_in, cudaStreamNonBlocking) == cudaSuccess &&
+  bool ok = cudaEventCreateWithFlags(&h->ev_last, cudaEventDisableTiming) == cudaSuccess &&
+            cudaStreamCreateWithFlags(&h->st_in, cudaStreamNonBlocking) == cudaSuccess &&
             cudaStreamCreateWithFlags(&h->st_out, cudaStreamNonBlocking) == cudaSuccess &&
             cudaStreamCreateWithFlags(&h->st_rec, cudaStreamNonBlocking) == cudaSuccess;
   for (int sl = 0; sl < 2 && ok; sl++)
@@ -329,8 +348,10 @@ int tpcca_track(tpcca_handle* h, const tpcca_cluster* clusters, int64_t n, const
   int rc = check_call(h, clusters, n, sector_offsets, out_tracks, out_hit_assignment);
   if (rc) return rc;
   Launch L{(cudaStream_t)stream, 0, nullptr};
+  if (!order_after_last(h, L.st)) return TPCCA_ERR_CUDA;
   rc = track_impl(h, clusters, n, sector_offsets, L.st, out_tracks, out_hit_assignment, L);
   h->launches = L.count;
+  mark_last(h, L.st);
   return rc;
 }
 
@@ -348,16 +369,21 @@ int tpcca_track_host_async(tpcca_handle* h, const tpcca_cluster* clusters, int64
   cudaError_t e = cudaSuccess;
   if (n > 0) {
     // the kernels of the frame that used this slot last (two frames ago) read stage_clusters[sl]: they were waited for by
-    // tpcca_wait; the event keeps the order explicit for callers that switch streams between frames
+    // tpcca_wait; the event keeps that order explicit.  (Kernel-to-kernel order between frames on different streams is
+    // ev_last's job, below.)
     e = cudaStreamWaitEvent(h->st_in, h->ev_k[sl], 0);
     if (e == cudaSuccess) e = cudaMemcpyAsync(h->stage_clusters[sl], clusters, (size_t)n * 16, cudaMemcpyHostToDevice, h->st_in);
   }
   if (e == cudaSuccess) e = cudaEventRecord(h->ev_in[sl], h->st_in);
   if (e == cudaSuccess) e = cudaStreamWaitEvent(st, h->ev_in[sl], 0);
   if (e != cudaSuccess) { set_err("H2D copy failed: %s", cudaGetErrorString(e)); cudaGetLastError(); return TPCCA_ERR_CUDA; }
+  // the kernels of this frame reuse the workspace of the previous frame (and of any merge / legs call made on it), which
+  // may have been given another stream
+  if (!order_after_last(h, st)) return TPCCA_ERR_CUDA;
   rc = track_impl(h, reinterpret_cast<const tpcca_cluster*>(h->stage_clusters[sl]), n, sector_offsets, st,
                   h->stage_tracks[sl], h->stage_assign[sl], L);
   h->launches = L.count;
+  mark_last(h, st);
   if (rc) return rc;
   e = cudaEventRecord(h->ev_k[sl], st);
   if (e == cudaSuccess) e = cudaStreamWaitEvent(h->st_out, h->ev_k[sl], 0);
@@ -405,8 +431,9 @@ int tpcca_merge(tpcca_handle* h, const tpcca_merge_params* mp, void* stream, voi
   if (!mp || !out_merged || !out_track_merged) { set_err("null merge parameters or output"); return TPCCA_ERR_ARGUMENT; }
   if (((uintptr_t)out_merged & 15) || ((uintptr_t)out_track_merged & 3)) { set_err("misaligned merge output"); return TPCCA_ERR_ARGUMENT; }
   if (!h->d.out_hdr) { set_err("tpcca_merge needs a preceding tpcca_track on this handle"); return TPCCA_ERR_ARGUMENT; }
-  if (mp->ring < 0 || mp->merge_row_back < 0 || mp->merge_row_fwd < 0 || !(mp->shared_err_scale > 0)) {
-    set_err("merge parameters out of range"); return TPCCA_ERR_ARGUMENT;
+  if (mp->ring < 0 || mp->ring == 1 || mp->ring > TPCCA_MAX_SECTORS || mp->merge_row_back < 0 || mp->merge_row_fwd < 0 ||
+      !(mp->shared_err_scale > 0)) {
+    set_err("merge parameters out of range (ring must be 0 or 2..64: with ring 1 a sector is its own neighbour)"); return TPCCA_ERR_ARGUMENT;
   }
   Dev d = h->d;
   d.MP = *mp;
@@ -414,7 +441,9 @@ int tpcca_merge(tpcca_handle* h, const tpcca_merge_params* mp, void* stream, voi
   d.merged_out = reinterpret_cast<tpcca_track_rec*>((char*)out_merged + sizeof(tpcca_out_header));
   d.track_merged_out = out_track_merged;
   Launch L{(cudaStream_t)stream, 0, nullptr};
+  if (!order_after_last(h, L.st)) return TPCCA_ERR_CUDA;
   launch_merge(d, L);
+  mark_last(h, L.st);
   h->launches = L.count;
   h->last_merged = out_merged;
   h->last_track_merged = out_track_merged;
@@ -441,7 +470,7 @@ int tpcca_find_legs(tpcca_handle* h, const tpcca_leg_params* lp, void* stream, i
   if (!lp || !out_leg_partner || !out_leg_partner_inner || !out_leg_first || !out_cluster_tags || !out_summary) { set_err("null leg parameters or output"); return TPCCA_ERR_ARGUMENT; }
   if (((uintptr_t)out_leg_partner & 3) || ((uintptr_t)out_leg_partner_inner & 3) || ((uintptr_t)out_summary & 15)) { set_err("misaligned leg output"); return TPCCA_ERR_ARGUMENT; }
   if (!h->d.out_hdr || !h->last_merged) { set_err("tpcca_find_legs needs a tpcca_merge after the last tpcca_track on this handle"); return TPCCA_ERR_ARGUMENT; }
-  if (lp->ring < 0 || lp->leg_max_sector_gap < 0 || lp->leg_inner_max_sector_gap < 0 || !(lp->leg_max_turn > 0.0f) ||
+  if (lp->ring < 0 || lp->ring == 1 || lp->ring > TPCCA_MAX_SECTORS || lp->leg_max_sector_gap < 0 || lp->leg_inner_max_sector_gap < 0 || !(lp->leg_max_turn > 0.0f) ||
       !(lp->leg_max_turn < 3.14159f) || !(lp->leg_inner_max_turn > 0.0f) || !(lp->leg_inner_max_turn < 6.28318f) ||
       !(lp->leg_min_sinphi > 0.0f) || !(lp->leg_inner_min_sinphi > 0.0f) || !(lp->leg_min_qpt > 0.0f) || !(lp->leg_centre_abs >= 0.0f) || !(lp->leg_centre_frac >= 0.0f) ||
       !(lp->leg_centre_abs + lp->leg_centre_frac > 0.0f) || !(lp->leg_radius_frac > 0.0f) || !(lp->leg_dz_max > 0.0f) ||
@@ -458,7 +487,9 @@ int tpcca_find_legs(tpcca_handle* h, const tpcca_leg_params* lp, void* stream, i
   d.tags_out = out_cluster_tags;
   d.leg_summary_out = reinterpret_cast<int32_t*>(out_summary);
   Launch L{(cudaStream_t)stream, 0, nullptr};
+  if (!order_after_last(h, L.st)) return TPCCA_ERR_CUDA;
   launch_legs(d, L);
+  mark_last(h, L.st);
   h->launches = L.count;
   h->last_leg_partner = out_leg_partner;
   const cudaError_t e = cudaGetLastError();
@@ -492,7 +523,9 @@ int tpcca_fit_legs(tpcca_handle* h, const tpcca_leg_fit_params* fp, void* stream
   d.fit_hdr = reinterpret_cast<tpcca_out_header*>(out_fits);
   d.fit_out = reinterpret_cast<tpcca_track_rec*>((char*)out_fits + sizeof(tpcca_out_header));
   Launch L{(cudaStream_t)stream, 0, nullptr};
+  if (!order_after_last(h, L.st)) return TPCCA_ERR_CUDA;
   launch_leg_fit(d, L);
+  mark_last(h, L.st);
   h->launches = L.count;
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) { set_err("leg fit launch failed: %s", cudaGetErrorString(e)); return TPCCA_ERR_CUDA; }
@@ -509,7 +542,9 @@ int tpcca_estimate_time(tpcca_handle* h, float vdrift, float z_max, void* stream
   Dev d = h->d;
   if (out_merged) d.merged_out = reinterpret_cast<tpcca_track_rec*>((char*)h->last_merged + sizeof(tpcca_out_header));
   Launch L{(cudaStream_t)stream, 0, nullptr};
+  if (!order_after_last(h, L.st)) return TPCCA_ERR_CUDA;
   launch_time_estimate(d, vdrift, z_max, out_sector, out_merged, L);
+  mark_last(h, L.st);
   const cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) { set_err("time estimate launch failed: %s", cudaGetErrorString(e)); return TPCCA_ERR_CUDA; }
   return TPCCA_OK;
@@ -531,6 +566,7 @@ int tpcca_get_intermediate(tpcca_handle* h, int what, void* dst, size_t bytes, v
   // the sizes of the tracklet / track tables are data dependent: read the live counters (synchronises `stream`;
   // this is a parity / debugging interface, not part of the hot path)
   DevCounters c;
+  if (!order_after_last(h, (cudaStream_t)stream)) return TPCCA_ERR_CUDA;
   cudaError_t e = cudaMemcpyAsync(&c, d.cnt, sizeof(c), cudaMemcpyDeviceToHost, (cudaStream_t)stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);
   if (e != cudaSuccess) { set_err("counter copy failed: %s", cudaGetErrorString(e)); cudaGetLastError(); return TPCCA_ERR_CUDA; }
@@ -546,6 +582,7 @@ int tpcca_get_intermediate(tpcca_handle* h, int what, void* dst, size_t bytes, v
   if (bytes < need) { set_err("dst too small%s (need %lld bytes)", "", (long long)need); return TPCCA_ERR_ARGUMENT; }
   Launch L{(cudaStream_t)stream, 0, nullptr};
   launch_export(d, what, dst, L);
+  mark_last(h, L.st);
   e = cudaGetLastError();
   if (e != cudaSuccess) { set_err("export launch failed: %s", cudaGetErrorString(e)); return TPCCA_ERR_CUDA; }
   return TPCCA_OK;
@@ -565,7 +602,13 @@ int tpcca_set_profiling(tpcca_handle* h, int on) {
   h->have_ktimes = false;
   if (h->kprofiling && !h->kev[0])
     for (int i = 0; i < 2 * TPCCA_N_KERNELS; i++)
-      if (cudaEventCreate(&h->kev[i]) != cudaSuccess) { set_err("cudaEventCreate failed"); h->kprofiling = false; return TPCCA_ERR_CUDA; }
+      if (cudaEventCreate(&h->kev[i]) != cudaSuccess) {
+        // all or nothing: kev[0] != null must mean that every kernel event exists
+        cudaGetLastError();
+        h->kev[i] = nullptr;
+        for (int j = 0; j < i; j++) { cudaEventDestroy(h->kev[j]); h->kev[j] = nullptr; }
+        set_err("cudaEventCreate failed"); h->kprofiling = false; return TPCCA_ERR_CUDA;
+      }
   return TPCCA_OK;
 }
 
@@ -602,6 +645,7 @@ int tpcca_get_stats(tpcca_handle* h, int64_t* stats, void* stream) {
   if (!h) { set_err("handle is null (not initialised)"); return TPCCA_ERR_NOT_INIT; }
   if (!stats) { set_err("stats is null"); return TPCCA_ERR_ARGUMENT; }
   DevCounters c;
+  if (!order_after_last(h, (cudaStream_t)stream)) return TPCCA_ERR_CUDA;
   cudaError_t e = cudaMemcpyAsync(&c, h->d.cnt, sizeof(c), cudaMemcpyDeviceToHost, (cudaStream_t)stream);
   if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);
   if (e != cudaSuccess) { set_err("stats copy failed: %s", cudaGetErrorString(e)); cudaGetLastError(); return TPCCA_ERR_CUDA; }
@@ -630,6 +674,7 @@ void tpcca_free(tpcca_handle* h) {
   }
   for (int i = 0; i < 2 * TPCCA_N_KERNELS; i++)
     if (h->kev[i]) cudaEventDestroy(h->kev[i]);
+  if (h->ev_last) cudaEventDestroy(h->ev_last);
   if (h->st_in) cudaStreamDestroy(h->st_in);
   if (h->st_out) cudaStreamDestroy(h->st_out);
   if (h->st_rec) cudaStreamDestroy(h->st_rec);

@@ -298,6 +298,7 @@ __global__ void __launch_bounds__(128) k_leg_tags(Dev d) {
   if (t >= d.cnt->n_tracks) return;
   const tpcca_track_rec* T = &d.out_tracks[t];
   const int m = d.track_merged_out[t];
+  if (m < 0) return;  // a segment outside every chain (k_merge_reset's initial value): no merged record to read
   const float qm = fabsf(d.merged_out[m].qpt);
   int base = 0;
   if (qm > d.LP.tag_qpt_low) base |= 1;
@@ -423,11 +424,13 @@ __device__ __forceinline__ void fit_hit(const Dev& d, FitCtx& c, float xh, float
 
 __device__ __forceinline__ int leg_segments(const Dev& d, int m, FitSeg* segs) {
   int n = 0;
-  for (int t = d.merged_out[m].pad[4]; t >= 0 && n < FIT_MAX_SEGS; t = d.m_next[t]) {
+  int t = d.merged_out[m].pad[4];
+  for (; t >= 0 && n < FIT_MAX_SEGS; t = d.m_next[t]) {
     const int2 wl = d.w_list[d.track_w[t]];
     segs[n].off = wl.x; segs[n].cnt = wl.y; segs[n].sector = d.out_tracks[t].sector;
     n++;
   }
+  if (t >= 0) atomicOr(&d.cnt->status, TPCCA_STAT_CHAIN_TRUNCATED);
   return n;
 }
 

@@ -15,11 +15,13 @@ __global__ void __launch_bounds__(256) k_merge_reset(Dev d) {
   const int nt = d.cnt->n_tracks;
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i == 0) { d.cnt->n_merged = 0; d.cnt->n_links = 0; d.cnt->n_fit_failed = 0; }
-  if (i < 1024) d.ord[4 * 1024 + i] = 0;  // counting-sort scratch of the fit order (slot 4)
+  // counting-sort scratch of the fit order (slot 4): strided, the grid may be smaller than the slot (small capacities)
+  for (int j = i; j < 1024; j += gridDim.x * blockDim.x) d.ord[4 * 1024 + j] = 0;
   if (i <= d.n_slices) d.slice_nstart[i] = 0;
   if (i < nt) {
     d.m_best_out[i] = M_NONE; d.m_best_in[i] = M_NONE;
     d.m_next[i] = -1; d.m_prev[i] = -1;
+    d.track_merged_out[i] = -1;  // stays -1 only for a segment no head reaches (cannot happen for ring != 1; k_leg_tags checks)
   }
 }
 __global__ void __launch_bounds__(256) k_merge_count(Dev d) {
@@ -165,7 +167,9 @@ __global__ void __launch_bounds__(64) k_merge_fit(Dev d) {
   const tpcca_track_rec* tr = d.out_tracks;
   int segs[MERGE_MAX_SEGS];
   int n_seg = 0, n = 0;
-  for (int s = head; s >= 0 && n_seg < MERGE_MAX_SEGS; s = d.m_next[s]) { segs[n_seg++] = s; n += tr[s].n_hits; }
+  int s_rest = head;
+  for (; s_rest >= 0 && n_seg < MERGE_MAX_SEGS; s_rest = d.m_next[s_rest]) { segs[n_seg++] = s_rest; n += tr[s_rest].n_hits; }
+  if (s_rest >= 0) atomicOr(&d.cnt->status, TPCCA_STAT_CHAIN_TRUNCATED);  // never with the default cuts (>= 8 rows gained per segment)
   const int last = segs[n_seg - 1];
   const Rot R = sector_rotation(d.tan_half_angle);
   // start: chord of the two outermost hits of the outermost segment, q/pT of its record

@@ -7,6 +7,13 @@ on the farm).  Two ways to use N GPUs, both running the unchanged single-GPU lib
     shard_sectors(36, N, r); track ids become global by adding the exclusive scan of the per-rank track counts.
 The only communication is the timing / throughput reduction and, for the sector split, one all-gather of the
 per-rank track counts (4 bytes per rank).  This module holds index arithmetic only -- no tracking step.
+
+Limit of the sector split: tpcca_merge / tpcca_find_legs / tpcca_fit_legs run per rank on the rank's own sectors, and no
+boundary records are exchanged.  A track crossing from the last sector of one rank into the first sector of the next
+therefore stays two segments (and the ring closure 17 -> 0 is lost whenever a z side is spread over several ranks).  Only
+splits whose cuts all fall between the two z sides -- world == 2 for the 36-sector TPC -- give the whole-frame merged
+tracks; `cuts_inside_a_side` tells which case applies and bench.py reports it.  tpcca_track itself (assignment, sector
+tracks) is exact for every split.
 """
 from __future__ import annotations
 
@@ -45,6 +52,16 @@ def shard_sectors(n_sectors: int, world: int, rank: int) -> tuple[int, int]:
     b = (n_sectors * rank) // world
     e = (n_sectors * (rank + 1)) // world
     return b, e
+
+
+def cuts_inside_a_side(n_sectors: int, world: int, ring: int) -> int:
+    """How many rank boundaries of `shard_sectors` cut through a z side (a ring of `ring` sectors) instead of falling
+    between two sides.  0: the per-rank merger sees every pair of neighbouring sectors, so merged tracks equal the
+    whole-frame ones; > 0: segments meeting at those cuts (and at the ring closure of a divided side) stay unmerged."""
+    if ring <= 0 or world <= 1:
+        return 0
+    return sum(1 for r in range(1, world) if 0 < shard_sectors(n_sectors, world, r)[0] < n_sectors
+               and shard_sectors(n_sectors, world, r)[0] % ring != 0)
 
 
 def shard_frame(clusters: np.ndarray, sector_offsets: np.ndarray, world: int, rank: int):

@@ -66,3 +66,14 @@ def test_single_process_passthrough():
     assert np.concatenate([p[0] for p in parts]).tolist() == list(range(12))
     for cl, lso, lo in parts:
         assert lso[0] == 0 and lso[-1] == len(cl) and (np.diff(lso) >= 0).all()
+
+
+def test_cuts_inside_a_side_tells_when_the_per_rank_merger_is_incomplete():
+    """The sector split exchanges no boundary segments: only cuts between the two z sides keep the
+    merged tracks of the whole frame."""
+    assert [distributed.cuts_inside_a_side(36, n, 18) for n in (1, 2, 3, 4, 6, 8)] == [0, 0, 2, 2, 4, 6]
+    assert distributed.cuts_inside_a_side(36, 4, 9) == 0      # four rings of nine sectors: every cut on a ring boundary
+    assert distributed.cuts_inside_a_side(36, 4, 0) == 0      # ring 0: nothing merges anyway
+    for n in (2, 3, 4, 6, 8):                                 # brute force: a cut at sector b is harmless iff b % ring == 0
+        cuts = [distributed.shard_sectors(36, n, r)[0] for r in range(1, n)]
+        assert distributed.cuts_inside_a_side(36, n, 18) == sum(1 for b in cuts if b % 18)

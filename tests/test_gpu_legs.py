@@ -104,7 +104,7 @@ def test_legs_twice_and_argument_checks(row_x):
     assert t.lib.tpcca_find_legs(t.h, C.byref(lp), t._stream(), pa.data_ptr() + 2, *args[1:]) == -1
     assert t.lib.tpcca_find_legs(t.h, C.byref(lp), t._stream(), *args[:4], sm.data_ptr() + 4) == -1
     assert t.lib.tpcca_find_legs(t.h, C.byref(lp), t._stream(), args[0], None, *args[2:]) == -1
-    for field, bad in (("leg_max_turn", 3.2), ("leg_inner_max_turn", 6.3), ("leg_min_sinphi", 0.0), ("leg_dz_max", 0.0), ("ring", -1)):
+    for field, bad in (("leg_max_turn", 3.2), ("leg_inner_max_turn", 6.3), ("leg_min_sinphi", 0.0), ("leg_dz_max", 0.0), ("ring", -1), ("ring", 1), ("ring", 65)):
         q = B.default_leg_params()
         setattr(q, field, bad)
         assert t.lib.tpcca_find_legs(t.h, C.byref(q), t._stream(), *args) == -1, field
@@ -118,3 +118,16 @@ def test_legs_twice_and_argument_checks(row_x):
     t.merge()
     p, pi_, f, g, s = t.find_legs()
     assert len(p) == 0 and len(pi_) == 0 and len(g) == 0 and not any(s.values())
+
+
+@pytest.mark.parametrize("seed", [1, 3])
+def test_low_pt_tag_threshold_between_segment_and_merged_curvature(row_x, seed):
+    """tests/test_oracle_pins_r3.py::test_low_pt_tag_follows_the_merged_tracks_curvature on the GPU."""
+    from tests import scenarios
+    par = dict(x0=85.0, y0=4.0, z0=25.0, sinphi0=0.12, tanl=0.5, qpt=-4.5, bz=0.5)
+    with np.errstate(invalid="ignore"):
+        fr, info = scenarios.helix_in_two_sectors(row_x, rng=np.random.default_rng(seed), par=par)
+    base = oracle.track(fr.clusters, fr.sector_offsets, row_x, merge=True, legs=True)
+    thr = 0.5 * (abs(float(base.tracks["qpt"][0])) + abs(float(base.merged["qpt"][0])))
+    t, orc = compare_legs(fr, row_x, legs=dict(tag_qpt_low=thr))
+    assert ((orc.cluster_tags & 1) != 0).sum() in (0, int((orc.assignment >= 0).sum()))

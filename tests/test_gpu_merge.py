@@ -116,8 +116,10 @@ def test_merge_argument_checks(row_x):
     assert t.lib.tpcca_merge(t.h, None, t._stream(), om.data_ptr(), tm.data_ptr()) == -1
     assert t.lib.tpcca_merge(t.h, C.byref(mp), t._stream(), om.data_ptr() + 4, tm.data_ptr()) == -1
     assert t.lib.tpcca_merge(None, C.byref(mp), t._stream(), om.data_ptr(), tm.data_ptr()) == -2
-    mp.ring = -1
-    assert t.lib.tpcca_merge(t.h, C.byref(mp), t._stream(), om.data_ptr(), tm.data_ptr()) == -1
+    for bad_ring in (-1, 1, 65):  # ring 1: a sector would be its own neighbour (self links, chains without a head)
+        mp.ring = bad_ring
+        assert t.lib.tpcca_merge(t.h, C.byref(mp), t._stream(), om.data_ptr(), tm.data_ptr()) == -1, bad_ring
+    assert b"ring" in t.lib.tpcca_last_error()
     # an empty frame merges to nothing
     empty = synth.Frame(np.zeros(0, synth.CLUSTER_DTYPE), np.zeros(37, np.int32), np.zeros(0, np.int32), np.zeros((0, 8)), 36, "e")
     run_gpu(empty, row_x, t)

@@ -286,9 +286,50 @@ def test_parity_hand_built_scenarios(row_x):
         for margin in (3.0, 0.0, 60.0):
             cases.append((scenarios.edge_helix(row_x, inward)[0], dict(edge_margin=margin)))
     cases.append((scenarios.e3_gap_above_start(row_x), dict(reject_cut=4.0)))
+    # round 3 (tests/test_oracle_pins_r3.py): z-displaced seed hit either side of its float64 distance 7.93, duplicates and
+    # displaced clusters in a row only the pick-up search reaches (either side of pick_cut, per axis), an inward stop inside
+    # the seed, the inclusive minimum hit counts, the quality step of the selector weight
+    for rc in (8.16, 7.69):
+        cases.append((scenarios.displaced_hit_helix_z(row_x), dict(reject_cut=rc)))
+    for pos in (None, (0, 1), (0, 200), (70, 10)):
+        cases.append((scenarios.lone_row_helix(row_x, duplicate=True, dup_positions=pos)[0], None))
+    for kw in (dict(dz=0.55), dict(dz=0.66), dict(dy=0.38), dict(dy=0.50)):
+        cases.append((scenarios.lone_row_helix(row_x, **kw)[0], None))
+    cases.append((scenarios.edge_helix(row_x, inward=True, decoy_step=1)[0], dict(edge_margin=0.5)))
+    full = scenarios.mk(*scenarios.one_helix(row_x), row_x)
+    for kw in (dict(min_seed_hits=150), dict(min_tracklet_hits=152), dict(min_track_hits=152)):
+        cases.append((full, kw))
+    for dy in (0.035, 0.05):
+        cases.append((scenarios.equal_length_crossing(row_x, "A", False, dy=dy)[0], None))
     for cl, params in cases:
         t, orc, exact = compare(scenarios.frame(cl), row_x, params=params)
         assert len(orc.tracks) >= 1 and exact
+
+
+def test_parity_minimum_hit_counts_one_above(row_x):
+    """One more than the frame has: no tracklet (seed / tracklet minimum) or no track (track minimum), on both sides."""
+    from tests import scenarios
+    full = scenarios.mk(*scenarios.one_helix(row_x), row_x)
+    for kw, n_valid in ((dict(min_seed_hits=151), 0), (dict(min_tracklet_hits=153), 0), (dict(min_track_hits=153), 1)):
+        t, orc, exact = compare(scenarios.frame(full), row_x, params=kw)
+        assert len(orc.tracks) == 0 and t.header()["n_tracklets"] == n_valid, kw
+
+
+def test_parity_unequal_neighbour_windows(row_x):
+    """nbr_dydx != nbr_dzdx (tests/test_oracle_pins_r3.py: brute-force triplets with a narrow y and a wide z window)."""
+    from tests import scenarios
+    kw = dict(nbr_dydx=0.25, nbr_margin_y=0.2, nbr_dzdx=2.5, nbr_margin_z=1.5)
+    fr = synth.generate(synth.config(1, scale=0.02, seed=13), noise_frac=0.4)
+    compare(fr, row_x, params=kw)
+    compare(synth.generate(synth.config(2, scale=0.1, seed=14)), row_x, params=kw)
+    for k2 in (dict(nbr_dydx=0.3), dict(nbr_dzdx=0.3)):
+        for dy, dz in ((0.9, 0.0), (0.0, 1.2)):
+            fr = scenarios.frame(scenarios.window_triplet(row_x, dy, dz))
+            import oracle
+            orc = oracle.track(fr.clusters, fr.sector_offsets, row_x, params=k2)
+            t = run_gpu(fr, row_x, **k2)
+            assert np.array_equal(t.intermediate(B.LINK_UP_RAW), orc.link_up_raw)
+            assert np.array_equal(t.intermediate(B.LINK_DOWN_RAW), orc.link_down_raw)
 
 
 def test_parity_exact_cost_ties(row_x):
@@ -362,6 +403,52 @@ def test_pipelined_host_call(row_x):
     t.wait()
     t.track_host(bufs[1][0], frs[1].n, frs[1].sector_offsets, bufs[1][1], bufs[1][2])
     assert np.array_equal(bufs[1][2].numpy(), ref[1][0])
+
+
+def test_calls_on_one_handle_keep_their_order_across_streams(row_x):
+    """All calls on a handle share one workspace.  Frames submitted alternately on two streams, with tpcca_merge and
+    tpcca_get_intermediate on a third, must still give the single-stream results: the library orders them itself
+    (include/tpcca.h "Streams")."""
+    import torch
+    frs = [synth.generate(synth.config(2, scale=0.25, seed=81)), synth.generate(synth.config(3, scale=0.2, seed=82))]
+    nmax = max(f.n for f in frs)
+    t = B.Tracker(row_x, max_clusters=nmax, max_tracklets=max(1024, nmax // 4))
+    ref = []
+    for fr in frs:
+        run_gpu(fr, row_x, t)
+        t.merge()
+        t.torch.cuda.synchronize()
+        ref.append((t.assignment(), t.tracks().tobytes(), t.merged().tobytes(), t.intermediate(B.START_HITS)))
+    bufs = [(torch.from_numpy(fr.clusters.view(np.uint8).reshape(-1).copy()).pin_memory(),
+             torch.empty(16 + 128 * t.max_tracks, dtype=torch.uint8).pin_memory(),
+             torch.empty(fr.n, dtype=torch.int32).pin_memory()) for fr in frs]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()]
+    torch.cuda.synchronize()
+    for rep in range(3):
+        # two frames in flight, each on its own stream, no host synchronisation in between
+        for i in (0, 1):
+            with torch.cuda.stream(streams[i]):
+                t.track_host_async(bufs[i][0], frs[i].n, frs[i].sector_offsets, bufs[i][1], bufs[i][2])
+        t.wait()
+        t.wait()
+        for i in (0, 1):
+            nt = int(bufs[i][1][:16].numpy().view(B.HEADER_DTYPE)["n_tracks"][0])
+            assert np.array_equal(bufs[i][2].numpy(), ref[i][0]), (rep, i)
+            assert bufs[i][1][16:16 + 128 * nt].numpy().tobytes() == ref[i][1], (rep, i)
+        # device-resident frame on one stream, merge and an intermediate on others, again without waiting in between
+        i = rep % 2
+        dev = t.upload(frs[i].clusters)
+        sh = torch.full((len(ref[i][3]) + 4,), -1, dtype=torch.int32, device="cuda")
+        torch.cuda.synchronize()
+        with torch.cuda.stream(streams[0]):
+            t.track(dev, frs[i].n, frs[i].sector_offsets)
+        with torch.cuda.stream(streams[1]):
+            t.merge()
+        t._check(t.lib.tpcca_get_intermediate(t.h, B.START_HITS, sh.data_ptr(), sh.numel() * 4, streams[2].cuda_stream))
+        torch.cuda.synchronize()
+        assert np.array_equal(t.assignment(), ref[i][0]) and t.tracks().tobytes() == ref[i][1], rep
+        assert t.merged().tobytes() == ref[i][2], rep
+        assert np.array_equal(sh.cpu().numpy()[:len(ref[i][3])], ref[i][3]), rep
 
 
 @pytest.mark.parametrize("world", [2, 3])

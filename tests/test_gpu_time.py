@@ -77,3 +77,18 @@ def test_time_estimate_argument_checks(row_x):
     run_gpu(fr, row_x, t)  # a new frame invalidates the merged tracks
     assert f(t.h, 2.58, 250.0, t._stream(), out.data_ptr(), out.data_ptr()) == -1
     torch.cuda.synchronize()
+
+
+def test_merged_track_clamp_uses_every_segment(row_x):
+    """tests/test_oracle_pins_r3.py::test_merged_track_is_shifted_inside_the_volume_by_all_its_clusters on the GPU: the largest
+    z of a two-sector track lies in its outer segment and fixes the shift of the merged track."""
+    from tests import scenarios
+    par = dict(x0=85.0, y0=4.0, z0=175.0, sinphi0=0.12, tanl=1.1, qpt=-1.1, bz=0.5)
+    with np.errstate(invalid="ignore"):
+        fr, info = scenarios.helix_in_two_sectors(row_x, par=par)
+    orc = oracle.track(fr.clusters, fr.sector_offsets, row_x, merge=True, time=True)
+    t = run_gpu(fr, row_x)
+    t.merge()
+    check_time(t, orc, float(np.abs(fr.clusters["z"]).max()))
+    ts, tm = t.estimate_time()
+    assert len(tm) == 1 and tm[0, 1] == np.float32(fr.clusters["z"].max()) - np.float32(250.0) and tm[0, 1] > ts[0, 1]
