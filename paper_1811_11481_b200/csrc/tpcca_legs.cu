@@ -439,13 +439,28 @@ __global__ void __launch_bounds__(64) k_leg_fit_flag(Dev d) {
   if (a < d.cnt->n_merged) d.m_scan[a] = (d.leg_partner_out[a] > a) ? 1 : 0;
 }
 
-__global__ void __launch_bounds__(64) k_leg_fit(Dev d) {
+// The pairs are compacted (leg_list[slot] = lower merged id, slot = rank of the pair in id order = its output record) and
+// fitted longest first (m_order: slots by decreasing hit count), so that a warp holds 32 pairs of about the same length
+// instead of the few merged tracks in 32 that have a partner.  leg_list / m_order are free here: the first is rebuilt by
+// every tpcca_find_legs, the second by every tpcca_merge.
+__global__ void __launch_bounds__(64) k_leg_fit_list(Dev d) {
   const int a = blockIdx.x * blockDim.x + threadIdx.x;
   const int nm = d.cnt->n_merged;
+  if (a == 0) d.leg_summary[6] = d.m_scan[nm];  // number of pairs, read by the order kernels
   if (a >= nm) return;
   const int b = d.leg_partner_out[a];
   if (b <= a) return;
   const int slot = d.m_scan[a];
+  d.leg_list[slot] = a;
+  d.leg_list[(size_t)d.max_tracks + slot] = (d.merged_out[a].n_hits + d.merged_out[b].n_hits) >> 1;  // sort key, clamped by the sort
+}
+
+__global__ void __launch_bounds__(64) k_leg_fit(Dev d) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p >= d.leg_summary[6]) return;
+  const int slot = d.m_order[p];
+  const int a = d.leg_list[slot];
+  const int b = d.leg_partner_out[a];
   const float za = fabsf(d.merged_out[a].z), zb = fabsf(d.merged_out[b].z);
   const bool a_first = (za < zb) || (za == zb);
   const int f = a_first ? a : b, g = a_first ? b : a;
@@ -541,7 +556,10 @@ __global__ void __launch_bounds__(64) k_leg_fit(Dev d) {
 }
 
 // header: pairs = total of the flag scan (0 without tracks), failed fits counted in leg_summary[5]
-__global__ void k_leg_fit_begin(Dev d) { d.leg_summary[5] = 0; }
+__global__ void __launch_bounds__(1024) k_leg_fit_begin(Dev d) {
+  if (threadIdx.x == 0) { d.leg_summary[5] = 0; d.leg_summary[6] = 0; }
+  d.ord[4 * 1024 + threadIdx.x] = 0;  // counting-sort scratch of the pair order (slot 4: the merged fit is through with it)
+}
 __global__ void k_leg_fit_header(Dev d, int have_scan) {
   tpcca_out_header hd;
   hd.n_tracks = have_scan ? d.m_scan[d.cnt->n_merged] : 0;
@@ -551,14 +569,17 @@ __global__ void k_leg_fit_header(Dev d, int have_scan) {
 
 void launch_leg_fit(const Dev& d, Launch& L) {
   const int K = d.max_tracks;
-  k_leg_fit_begin<<<1, 1, 0, L.st>>>(d);
+  k_leg_fit_begin<<<1, 1024, 0, L.st>>>(d);
   L.count++;
   const bool work = d.n > 0 && K > 0;
   if (work) {
     k_leg_fit_flag<<<(K + 63) / 64, 64, 0, L.st>>>(d);
     L.count++;
     launch_scan_i32(d.m_scan, &d.cnt->n_merged, K, d.scan_tmp, L);
-    k_leg_fit<<<(K + 63) / 64, 64, 0, L.st>>>(d);
+    k_leg_fit_list<<<(K + 63) / 64, 64, 0, L.st>>>(d);
+    L.count++;
+    launch_order_desc(d, 4, d.leg_list + (size_t)K, &d.leg_summary[6], K, d.m_order, L);
+    k_leg_fit<<<(K / 2 + 63) / 64, 64, 0, L.st>>>(d);  // at most K / 2 pairs
     L.count++;
   }
   k_leg_fit_header<<<1, 1, 0, L.st>>>(d, work ? 1 : 0);
